@@ -1,0 +1,118 @@
+/*
+ * lwe_oracle.h -- ORACLE. Test infrastructure, not the product.
+ *
+ * A plain, slow, obviously-correct CPU restatement of what the hot path of
+ * arxiv/paper_2606_01211 ("GPU Acceleration of Learning With Errors KEMs Using
+ * OpenACC") computes, in the Regev-style form BASELINE.json fixes.  It is the
+ * definition written out: one `% q` after every multiply-add, byte-oriented
+ * FIPS-197 AES, no tables shared with, and no code shared with, the CUDA path
+ * under paper_2606_01211_b200/.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may call it.
+ *
+ * Citations: P:Lnnn = /root/reference/PAPER.md line nnn; S8(c) Ok = SURVEY.md
+ * section 8(c) definition Ok; BJ = BASELINE.json.  DESIGN.md section 3 lists every
+ * reading taken where the paper is silent.
+ *
+ * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): FIPS-197 App. B / C.1 and
+ * SP 800-38A F.5.1 known answers, 64-bit carry in the counter, an independent
+ * AES (python `cryptography`/OpenSSL), closed-form CBD pmf, exhaustive rounding,
+ * brute force with python big integers, linearity, unit-vector / one-hot
+ * special cases, the noise identity  v - U^T s - mu*floor(q/2) = e^T R  and
+ * decaps(encaps(mu)) == mu.  No function here is "parity unpinned"; the
+ * conventions O3-O6 (seed->key, tags, bit order) are fixed by SURVEY 8(c) /
+ * DESIGN.md and implemented twice, independently, here and in CUDA.
+ *
+ * All vectors hold canonical representatives in [0, q) as uint16_t (S13).
+ * q in (1, 65536].  Everything is integer arithmetic.
+ */
+#ifndef LWE_ORACLE_H
+#define LWE_ORACLE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Object tags of O3: which seeded object a stream belongs to. */
+enum { ORC_TAG_A = 1, ORC_TAG_S = 2, ORC_TAG_E = 3, ORC_TAG_R = 4, ORC_TAG_MU = 5 };
+
+/* O1. AES-128 block cipher, FIPS-197 (10 rounds). P:L154 (AES-based generator),
+ * BJ north_star (1) (AES-128-CTR). */
+void orc_aes128_encrypt_block(const uint8_t key[16], const uint8_t in[16], uint8_t out[16]);
+
+/* O2. CTR keystream, SP 800-38A: block j = AES_key((iv + j) mod 2^128), iv and the
+ * sum being 128-bit big-endian integers; out[x] = byte (byte_offset + x) of the
+ * concatenated blocks. P:L154-156 ("identical sequences", "one sub-seed per output
+ * element"); BJ north_star ("counter-indexed so any stream offset is reproducible"). */
+void orc_ctr_bytes(const uint8_t key[16], const uint8_t iv[16],
+                   uint64_t byte_offset, size_t nbytes, uint8_t *out);
+
+/* O3. key(seed) = LE64(seed) || 0^8 ; iv(tag, attempt, inst) =
+ * BE64(tag*2^56 + attempt*2^32 + inst) || 0^8.  P:L154 (64-bit master seed). */
+void orc_seed_key(uint64_t seed, uint8_t key[16]);
+void orc_object_iv(uint32_t tag, uint32_t attempt, uint32_t inst, uint8_t iv[16]);
+
+/* O4. Uniform mod q by rejection, element t in [first, first+count):
+ * for attempt a = 0,1,..: c = LE16(bytes [2t,2t+1] of KS(key(seed), iv(tag,a,inst)));
+ * T = q*floor(65536/q); accept iff c < T; value c mod q.  BJ configs[2]. */
+void orc_sample_uniform(uint16_t *out, uint64_t first, uint64_t count,
+                        uint64_t seed, uint32_t tag, uint32_t inst, uint32_t q);
+
+/* O5. Centred binomial eta in [1,8], element t: w = LE16(bytes [2t,2t+1] of
+ * KS(key(seed), iv(tag,0,inst))); x = popcount(w & M) - popcount((w>>8) & M),
+ * M = 2^eta - 1; stored as x mod q.  P:L70, P:L170, P:L320 (FIPS 203 CBD). */
+void orc_sample_cbd(uint16_t *out, uint64_t first, uint64_t count,
+                    uint64_t seed, uint32_t tag, uint32_t inst, uint32_t q, uint32_t eta);
+
+/* O5 on one 16-bit stream word (what orc_sample_cbd applies to every word). */
+uint16_t orc_cbd_from_word(uint32_t w, uint32_t q, uint32_t eta);
+
+/* O6. Bits [first_bit, first_bit+nbits) of KS(key(seed), iv(tag,0,inst)), bit t =
+ * (byte floor(t/8) >> (t mod 8)) & 1, written packed LSB-first starting at bit 0
+ * of out[0].  P:L78 Alg.4 l.1; BJ configs (binary R, message bits). */
+void orc_sample_bits(uint8_t *out, uint64_t first_bit, uint64_t nbits,
+                     uint64_t seed, uint32_t tag, uint32_t inst);
+
+/* O7. KeyGen: b_i = (sum_{j<n} A[i*n+j]*s[j] + e[i]) mod q, 0 <= i < m.
+ * P:L60 eq.(1). */
+void orc_keygen(const uint16_t *A, const uint16_t *s, const uint16_t *e, uint16_t *b,
+                uint32_t m, uint32_t n, uint32_t q);
+
+/* O8. Encaps, all k bits at once (intra-operation batching):
+ * U[j*k+c] = (sum_{i<m} A[i*n+j]*R_ic) mod q ;
+ * v[c]     = (sum_{i<m} b[i]*R_ic + mu_c*floor(q/2)) mod q ;
+ * R_ic = bit (i*k+c) of Rbits, mu_c = bit c of mubits (LSB-first packing). */
+void orc_encaps(const uint16_t *A, const uint16_t *b, const uint8_t *Rbits,
+                const uint8_t *mubits, uint16_t *U, uint16_t *v,
+                uint32_t m, uint32_t n, uint32_t k, uint32_t q);
+
+/* O8 restricted to chosen rows of U (used at sizes where the full contraction is
+ * impractical on a CPU): Urows[r*k+c] = U[rows[r]*k+c]. */
+void orc_encaps_rows(const uint16_t *A, const uint8_t *Rbits, const uint32_t *rows,
+                     uint32_t nrows, uint16_t *Urows,
+                     uint32_t m, uint32_t n, uint32_t k, uint32_t q);
+
+/* O8, v only. */
+void orc_encaps_v(const uint16_t *b, const uint8_t *Rbits, const uint8_t *mubits,
+                  uint16_t *v, uint32_t m, uint32_t k, uint32_t q);
+
+/* O9. Decaps: d_c = (v[c] - sum_{j<n} U[j*k+c]*s[j]) mod q in [0,q);
+ * bit_c = floor((4*d_c + q) / (2q)) mod 2; packed LSB-first into mubits_out[k/8].
+ * If d_out != NULL it receives d_c.  P:L174; P:L68 ("decoding threshold"). */
+void orc_decaps(const uint16_t *U, const uint16_t *v, const uint16_t *s,
+                uint8_t *mubits_out, uint16_t *d_out,
+                uint32_t n, uint32_t k, uint32_t q);
+
+/* O9 rounding on one value d in [0,q): floor((4d + q)/(2q)) mod 2
+ * (= 1 iff q/4 <= d < 3q/4). */
+uint32_t orc_round_bit(uint32_t d, uint32_t q);
+
+/* Number of OpenMP threads the loops above will use (1 if built without OpenMP). */
+int orc_num_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LWE_ORACLE_H */

@@ -1,0 +1,176 @@
+"""ctypes wrapper around liblwe_oracle.so (ORACLE -- test infrastructure).
+
+Argument marshalling only: numpy arrays in, numpy arrays out.  All arithmetic
+is in lwe_oracle.c.  Names follow SURVEY.md 8(c) (O1..O9).
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+TAG_A, TAG_S, TAG_E, TAG_R, TAG_MU = 1, 2, 3, 4, 5
+
+__all__ = [
+    "TAG_A", "TAG_S", "TAG_E", "TAG_R", "TAG_MU",
+    "aes128_encrypt_block", "ctr_bytes", "seed_key", "object_iv",
+    "sample_uniform", "sample_cbd", "sample_bits",
+    "keygen", "encaps", "encaps_rows", "encaps_v", "decaps", "num_threads",
+    "cbd_from_word", "round_bit",
+]
+
+_lib = None
+
+
+def _L():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(str(_build.build()))
+        u8p, u16p, u32p = C.POINTER(C.c_uint8), C.POINTER(C.c_uint16), C.POINTER(C.c_uint32)
+        u32, u64, sz = C.c_uint32, C.c_uint64, C.c_size_t
+        lib.orc_aes128_encrypt_block.argtypes = [u8p, u8p, u8p]
+        lib.orc_ctr_bytes.argtypes = [u8p, u8p, u64, sz, u8p]
+        lib.orc_seed_key.argtypes = [u64, u8p]
+        lib.orc_object_iv.argtypes = [u32, u32, u32, u8p]
+        lib.orc_sample_uniform.argtypes = [u16p, u64, u64, u64, u32, u32, u32]
+        lib.orc_sample_cbd.argtypes = [u16p, u64, u64, u64, u32, u32, u32, u32]
+        lib.orc_sample_bits.argtypes = [u8p, u64, u64, u64, u32, u32]
+        lib.orc_keygen.argtypes = [u16p, u16p, u16p, u16p, u32, u32, u32]
+        lib.orc_encaps.argtypes = [u16p, u16p, u8p, u8p, u16p, u16p, u32, u32, u32, u32]
+        lib.orc_encaps_rows.argtypes = [u16p, u8p, u32p, u32, u16p, u32, u32, u32, u32]
+        lib.orc_encaps_v.argtypes = [u16p, u8p, u8p, u16p, u32, u32, u32]
+        lib.orc_decaps.argtypes = [u16p, u16p, u16p, u8p, u16p, u32, u32, u32]
+        lib.orc_num_threads.restype = C.c_int
+        lib.orc_cbd_from_word.argtypes = [u32, u32, u32]
+        lib.orc_cbd_from_word.restype = C.c_uint16
+        lib.orc_round_bit.argtypes = [u32, u32]
+        lib.orc_round_bit.restype = C.c_uint32
+        for f in ("orc_aes128_encrypt_block", "orc_ctr_bytes", "orc_seed_key", "orc_object_iv",
+                  "orc_sample_uniform", "orc_sample_cbd", "orc_sample_bits", "orc_keygen",
+                  "orc_encaps", "orc_encaps_rows", "orc_encaps_v", "orc_decaps"):
+            getattr(lib, f).restype = None
+        _lib = lib
+    return _lib
+
+
+def _p(a, ct):
+    return a.ctypes.data_as(C.POINTER(ct))
+
+
+def _u8(x, n=None):
+    a = np.ascontiguousarray(np.frombuffer(bytes(x), dtype=np.uint8) if isinstance(x, (bytes, bytearray)) else x,
+                             dtype=np.uint8)
+    if n is not None and a.size != n:
+        raise ValueError(f"expected {n} bytes, got {a.size}")
+    return a
+
+
+def _u16(x):
+    return np.ascontiguousarray(x, dtype=np.uint16)
+
+
+def aes128_encrypt_block(key, block) -> bytes:
+    k, b = _u8(key, 16), _u8(block, 16)
+    out = np.zeros(16, np.uint8)
+    _L().orc_aes128_encrypt_block(_p(k, C.c_uint8), _p(b, C.c_uint8), _p(out, C.c_uint8))
+    return out.tobytes()
+
+
+def ctr_bytes(key, iv, byte_offset: int, nbytes: int) -> np.ndarray:
+    k, v = _u8(key, 16), _u8(iv, 16)
+    out = np.zeros(nbytes, np.uint8)
+    _L().orc_ctr_bytes(_p(k, C.c_uint8), _p(v, C.c_uint8), byte_offset, nbytes, _p(out, C.c_uint8))
+    return out
+
+
+def seed_key(seed: int) -> bytes:
+    out = np.zeros(16, np.uint8)
+    _L().orc_seed_key(seed, _p(out, C.c_uint8))
+    return out.tobytes()
+
+
+def object_iv(tag: int, attempt: int, inst: int) -> bytes:
+    out = np.zeros(16, np.uint8)
+    _L().orc_object_iv(tag, attempt, inst, _p(out, C.c_uint8))
+    return out.tobytes()
+
+
+def sample_uniform(first: int, count: int, seed: int, tag: int, inst: int, q: int) -> np.ndarray:
+    out = np.zeros(count, np.uint16)
+    _L().orc_sample_uniform(_p(out, C.c_uint16), first, count, seed, tag, inst, q)
+    return out
+
+
+def sample_cbd(first: int, count: int, seed: int, tag: int, inst: int, q: int, eta: int) -> np.ndarray:
+    out = np.zeros(count, np.uint16)
+    _L().orc_sample_cbd(_p(out, C.c_uint16), first, count, seed, tag, inst, q, eta)
+    return out
+
+
+def sample_bits(first_bit: int, nbits: int, seed: int, tag: int, inst: int) -> np.ndarray:
+    out = np.zeros((nbits + 7) // 8, np.uint8)
+    _L().orc_sample_bits(_p(out, C.c_uint8), first_bit, nbits, seed, tag, inst)
+    return out
+
+
+def keygen(A, s, e, q: int) -> np.ndarray:
+    A, s, e = _u16(A), _u16(s), _u16(e)
+    m, n = A.shape
+    assert s.shape == (n,) and e.shape == (m,)
+    b = np.zeros(m, np.uint16)
+    _L().orc_keygen(_p(A, C.c_uint16), _p(s, C.c_uint16), _p(e, C.c_uint16), _p(b, C.c_uint16), m, n, q)
+    return b
+
+
+def encaps(A, b, Rbits, mubits, k: int, q: int):
+    A, b, Rbits, mubits = _u16(A), _u16(b), _u8(Rbits), _u8(mubits)
+    m, n = A.shape
+    assert b.shape == (m,) and Rbits.size == m * k // 8 and mubits.size == k // 8
+    U = np.zeros((n, k), np.uint16)
+    v = np.zeros(k, np.uint16)
+    _L().orc_encaps(_p(A, C.c_uint16), _p(b, C.c_uint16), _p(Rbits, C.c_uint8), _p(mubits, C.c_uint8),
+                    _p(U, C.c_uint16), _p(v, C.c_uint16), m, n, k, q)
+    return U, v
+
+
+def encaps_rows(A, Rbits, rows, k: int, q: int) -> np.ndarray:
+    A, Rbits = _u16(A), _u8(Rbits)
+    rows = np.ascontiguousarray(rows, dtype=np.uint32)
+    m, n = A.shape
+    out = np.zeros((rows.size, k), np.uint16)
+    _L().orc_encaps_rows(_p(A, C.c_uint16), _p(Rbits, C.c_uint8), _p(rows, C.c_uint32), rows.size,
+                         _p(out, C.c_uint16), m, n, k, q)
+    return out
+
+
+def encaps_v(b, Rbits, mubits, k: int, q: int) -> np.ndarray:
+    b, Rbits, mubits = _u16(b), _u8(Rbits), _u8(mubits)
+    v = np.zeros(k, np.uint16)
+    _L().orc_encaps_v(_p(b, C.c_uint16), _p(Rbits, C.c_uint8), _p(mubits, C.c_uint8), _p(v, C.c_uint16),
+                      b.size, k, q)
+    return v
+
+
+def decaps(U, v, s, q: int, return_d: bool = False):
+    U, v, s = _u16(U), _u16(v), _u16(s)
+    n, k = U.shape
+    assert v.shape == (k,) and s.shape == (n,)
+    out = np.zeros(k // 8, np.uint8)
+    d = np.zeros(k, np.uint16)
+    _L().orc_decaps(_p(U, C.c_uint16), _p(v, C.c_uint16), _p(s, C.c_uint16), _p(out, C.c_uint8),
+                    _p(d, C.c_uint16), n, k, q)
+    return (out, d) if return_d else out
+
+
+def cbd_from_word(w: int, q: int, eta: int) -> int:
+    return int(_L().orc_cbd_from_word(w, q, eta))
+
+
+def round_bit(d: int, q: int) -> int:
+    return int(_L().orc_round_bit(d, q))
+
+
+def num_threads() -> int:
+    return int(_L().orc_num_threads())
