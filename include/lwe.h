@@ -1,0 +1,156 @@
+/*
+ * lwe.h -- C ABI of liblwe_b200: the data-parallel core of the plain-LWE KEM of
+ * arxiv/paper_2606_01211, written for one NVIDIA B200 (sm_100a).
+ *
+ * Citations: P:Lnnn = PAPER.md line nnn; BJ = BASELINE.json; S8(x) = SURVEY.md
+ * section 8(x); DESIGN.md section 3 = the readings taken where the paper is silent.
+ *
+ * Notation (S8): A in Z_q^{m x n} row-major uint16; s in Z_q^n; e, b in Z_q^m;
+ * R in {0,1}^{m x k}; mu in {0,1}^k; U in Z_q^{n x k} row-major uint16; v in Z_q^k.
+ * All vectors hold canonical representatives in [0, q).  Everything is integer
+ * arithmetic; results are exact, so they do not depend on launch geometry.
+ *
+ * Conventions for every entry point
+ *  - Pointers named d_* are DEVICE pointers (device of the context), caller-owned;
+ *    h_* are HOST pointers (pinned memory recommended).  The library never frees or
+ *    keeps them beyond the stream work it enqueues.  Inputs are never modified.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *    Calls with d_* arguments only ENQUEUE work and return; they never synchronise
+ *    the host (the paper's goal of removing sync points).
+ *  - The context owns one workspace sized at creation from (m, k, max_batch); no
+ *    call allocates ("allocate once").  A context must not be used from two
+ *    streams at the same time.
+ *  - Return value: LWE_OK or a negative lwe_status.  Arguments are validated before
+ *    anything is launched: on an error nothing has been written.  No C++ exception
+ *    crosses the ABI; nothing aborts.
+ *  - Alignment: every d_* / h_* pointer must be 16-byte aligned (LWE_ERR_ALIGN).
+ *  - There is no CPU fallback and no other backend: a device that is not compute
+ *    capability 10.x gives LWE_ERR_UNSUPPORTED at lwe_create.
+ */
+#ifndef LWE_B200_H
+#define LWE_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    LWE_OK = 0,
+    LWE_ERR_PARAM = -1,       /* a size / modulus / range argument is invalid          */
+    LWE_ERR_ALIGN = -2,       /* a pointer or offset violates the alignment contract    */
+    LWE_ERR_NULLPTR = -3,     /* a required pointer is NULL                             */
+    LWE_ERR_CUDA = -4,        /* the CUDA runtime reported an error (see lwe_last_cuda_error) */
+    LWE_ERR_UNSUPPORTED = -5  /* not an sm_100 device, or a variant that is not built   */
+} lwe_status;
+
+/* Object tags of the seeded streams (S8(c) O3). */
+enum { LWE_TAG_A = 1, LWE_TAG_S = 2, LWE_TAG_E = 3, LWE_TAG_R = 4, LWE_TAG_MU = 5 };
+
+/* Problem shape.  n, m multiples of 8 (one AES block = 8 elements); k multiple of 8;
+ * q in (1, 65536]; eta in [1, 8]; max_batch >= 1 = the largest `batch` any call
+ * will pass (number of independent instances sharing one A, BJ configs[3]). */
+typedef struct {
+    uint32_t n, m, k, q, eta, max_batch;
+} lwe_params;
+
+typedef struct lwe_ctx lwe_ctx; /* opaque: tables, workspace, TMA descriptors */
+
+/* Create / destroy a context on CUDA device `device`.  Allocates the workspace
+ * (m*k*max_batch bytes for the expanded R operand + small accumulators). */
+int lwe_create(lwe_ctx **ctx, const lwe_params *p, int device);
+void lwe_destroy(lwe_ctx *ctx);
+
+const char *lwe_strerror(int code);
+/* cudaError_t of the last LWE_ERR_CUDA on this context (0 if none). */
+int lwe_last_cuda_error(const lwe_ctx *ctx);
+/* Number of kernels this context has launched since creation (bench's gpu_launches). */
+uint64_t lwe_launch_count(const lwe_ctx *ctx);
+
+/* ---- a1: device-resident AES-128-CTR stream --------------------------------------
+ * d_out[x] = byte (byte_offset + x) of KS(key, iv), 0 <= x < nbytes, where block j of
+ * KS is AES-128_key((iv + j) mod 2^128), iv and the sum being 128-bit big-endian
+ * integers (SP 800-38A CTR; equals `openssl aes-128-ctr` keystream).  Any offset is
+ * reproducible: the result is a pure function of (key, iv, byte position).
+ * P:L154-156 (device RNG, identical sequences on every GPU, one sub-seed per output
+ * element); BJ north_star (1).  key, iv: HOST pointers, read before returning.
+ * byte_offset and nbytes are arbitrary; d_out needs 16-byte alignment. */
+int lwe_rng_fill(lwe_ctx *ctx, void *d_out, size_t nbytes, const uint8_t key[16],
+                 const uint8_t iv[16], uint64_t byte_offset, void *stream);
+
+/* ---- a2: samplers over the seeded streams (S8(c) O3-O6) --------------------------
+ * Stream of object (seed, tag, attempt, inst): key = LE64(seed) || 0^8,
+ * iv = BE64(tag*2^56 + attempt*2^32 + inst) || 0^8.  P:L154 (64-bit master seed).
+ * Each call fills n_inst consecutive instances inst0 .. inst0+n_inst-1:
+ * d_out[t][x] for instance inst0+t, element first+x; rows are `count` elements apart.
+ *
+ * uniform: element e: for attempt a = 0,1,..: c = LE16(stream bytes [2e, 2e+1] of
+ *   attempt a); T = q*floor(65536/q); accept iff c < T; value c mod q.  Exactly
+ *   uniform and O(1) random access.  BJ configs[2] ("uniform mod q by rejection").
+ * cbd: w = LE16(stream bytes [2e,2e+1], attempt 0); x = popcount(w & M) -
+ *   popcount((w >> 8) & M), M = 2^eta - 1; stored as x mod q.  P:L70.
+ * bits: bit t of the stream = (byte floor(t/8) >> (t mod 8)) & 1; output packed the
+ *   same way, ceil(nbits/8) bytes per instance, unused top bits zero.  first_bit must
+ *   be a multiple of 8 (LWE_ERR_ALIGN).  P:L78 Alg.4 l.1; BJ configs (binary R).
+ * `first` must be a multiple of 8 for uniform/cbd (one AES block = 8 elements). */
+int lwe_sample_uniform(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count,
+                       uint64_t seed, uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream);
+int lwe_sample_cbd(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count,
+                   uint64_t seed, uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream);
+int lwe_sample_bits(lwe_ctx *ctx, uint8_t *d_out, uint64_t first_bit, uint64_t nbits,
+                    uint64_t seed, uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream);
+
+/* ---- a3 / a3': KeyGen ------------------------------------------------------------
+ * d_b[t][i] = ( sum_{j<n} A[i][j] * d_s[t][j] + d_e[t][i] ) mod q,  0 <= t < batch.
+ * P:L60 eq.(1).  d_A: m x n row-major, read once per instance group,
+ * streamed from HBM.  d_A == NULL: A is never read; every element is regenerated
+ * inside the kernel from (seed_A, LWE_TAG_A, inst 0) exactly as lwe_sample_uniform
+ * would produce it (the paper's on-demand A).  batch <= max_batch. */
+int lwe_keygen(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
+               const uint16_t *d_s /*[batch][n]*/, const uint16_t *d_e /*[batch][m]*/,
+               uint16_t *d_b /*[batch][m]*/, uint32_t batch, void *stream);
+
+/* ---- a4 + a5: Encaps, all k bits of an instance in one contraction -----------------
+ * d_U[t][j][c] = ( sum_{i<m} A[i][j] * R_t[i][c] ) mod q
+ * d_v[t][c]    = ( sum_{i<m} d_b[t][i] * R_t[i][c] + mu_t[c]*floor(q/2) ) mod q
+ * with R_t[i][c] = bit (i*k + c) of d_Rbits[t] and mu_t[c] = bit c of d_mubits[t]
+ * (LSB-first).  Intra-operation batching, P:L130 item 3.
+ * Runs as a u8 x u8 -> s32 tensor-core GEMM (tcgen05 kind::i8) over the byte planes
+ * of A with a mod-q recombine epilogue; shapes the tensor path does not cover
+ * (k % 16 != 0) use a CUDA-core kernel with identical results.
+ * d_A == NULL (regenerate from seed_A) returns LWE_ERR_UNSUPPORTED in this build. */
+int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
+               const uint16_t *d_b /*[batch][m]*/, const uint8_t *d_Rbits /*[batch][m*k/8]*/,
+               const uint8_t *d_mubits /*[batch][k/8]*/, uint16_t *d_U /*[batch][n][k]*/,
+               uint16_t *d_v /*[batch][k]*/, uint32_t batch, void *stream);
+
+/* ---- a6: Decaps ------------------------------------------------------------------
+ * d = ( d_v[t][c] - sum_{j<n} d_U[t][j][c] * d_s[t][j] ) mod q in [0,q);
+ * bit = floor((4d + q) / (2q)) mod 2  (1 iff q/4 <= d < 3q/4); packed LSB-first into
+ * d_mubits_out[t][k/8].  P:L174 ("mu = v - s.u (mod q)"), P:L68 (decoding threshold). */
+int lwe_decaps(lwe_ctx *ctx, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
+               uint8_t *d_mubits_out /*[batch][k/8]*/, uint32_t batch, void *stream);
+
+/* ---- end-to-end with HOST buffers -----------------------------------------------
+ * One full pass keygen -> encaps -> decaps for `batch` instances whose per-instance
+ * inputs live in host memory: copies h_s, h_e, h_Rbits, h_mubits to the device,
+ * runs the three steps against the device-resident public matrix d_A (or seed_A if
+ * d_A == NULL, keygen only), copies h_b, h_v, h_mubits_out (and h_U if not NULL) back,
+ * and returns after synchronising `stream`.  Layouts as in the calls above. */
+int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
+                 const uint16_t *h_s, const uint16_t *h_e, const uint8_t *h_Rbits,
+                 const uint8_t *h_mubits, uint16_t *h_b, uint16_t *h_U /* may be NULL */,
+                 uint16_t *h_v, uint8_t *h_mubits_out, uint32_t batch, void *stream);
+
+/* ---- tuning / test hooks (no new semantics) ----------------------------------------
+ * LWE_OPT_ENCAPS_PATH: 0 = auto, 1 = force CUDA-core kernel, 2 = force tcgen05 GEMM
+ *                      (LWE_ERR_UNSUPPORTED at call time if the shape does not fit). */
+enum { LWE_OPT_ENCAPS_PATH = 1 };
+int lwe_set_option(lwe_ctx *ctx, int option, int64_t value);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LWE_B200_H */

@@ -1,0 +1,167 @@
+"""Thin ctypes face of liblwe_b200.so -- argument marshalling only.
+
+Same names as include/lwe.h.  Every step of the path runs in the library's CUDA
+kernels; PyTorch appears only as the owner of device memory and streams.  There is
+no fallback: if the library is missing or the device is not sm_100, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import torch
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "lib" / "liblwe_b200.so"
+
+LWE_OK = 0
+ERRORS = {-1: "LWE_ERR_PARAM", -2: "LWE_ERR_ALIGN", -3: "LWE_ERR_NULLPTR", -4: "LWE_ERR_CUDA",
+          -5: "LWE_ERR_UNSUPPORTED"}
+TAG_A, TAG_S, TAG_E, TAG_R, TAG_MU = 1, 2, 3, 4, 5
+OPT_ENCAPS_PATH = 1
+
+EXPORTS = [
+    "lwe_create", "lwe_destroy", "lwe_strerror", "lwe_last_cuda_error", "lwe_launch_count",
+    "lwe_rng_fill", "lwe_sample_uniform", "lwe_sample_cbd", "lwe_sample_bits",
+    "lwe_keygen", "lwe_encaps", "lwe_decaps", "lwe_kem_host", "lwe_set_option",
+]
+
+
+class LweError(RuntimeError):
+    def __init__(self, code: int, where: str, detail: str = ""):
+        self.code = code
+        super().__init__(f"{where}: {ERRORS.get(code, code)} {detail}".strip())
+
+
+class lwe_params(C.Structure):
+    _fields_ = [(x, C.c_uint32) for x in ("n", "m", "k", "q", "eta", "max_batch")]
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen the in-tree library (no compute); raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2606_01211_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(str(LIB_PATH))
+    vp, u64, u32, sz = C.c_void_p, C.c_uint64, C.c_uint32, C.c_size_t
+    lib.lwe_create.argtypes = [C.POINTER(vp), C.POINTER(lwe_params), C.c_int]
+    lib.lwe_destroy.argtypes = [vp]
+    lib.lwe_destroy.restype = None
+    lib.lwe_strerror.argtypes = [C.c_int]
+    lib.lwe_strerror.restype = C.c_char_p
+    lib.lwe_last_cuda_error.argtypes = [vp]
+    lib.lwe_launch_count.argtypes = [vp]
+    lib.lwe_launch_count.restype = u64
+    lib.lwe_set_option.argtypes = [vp, C.c_int, C.c_int64]
+    lib.lwe_rng_fill.argtypes = [vp, vp, sz, C.c_char_p, C.c_char_p, u64, vp]
+    for f in (lib.lwe_sample_uniform, lib.lwe_sample_cbd, lib.lwe_sample_bits):
+        f.argtypes = [vp, vp, u64, u64, u64, u32, u32, u32, vp]
+    lib.lwe_keygen.argtypes = [vp, vp, u64, vp, vp, vp, u32, vp]
+    lib.lwe_encaps.argtypes = [vp, vp, u64, vp, vp, vp, vp, vp, u32, vp]
+    lib.lwe_decaps.argtypes = [vp, vp, vp, vp, vp, u32, vp]
+    lib.lwe_kem_host.argtypes = [vp, vp, u64, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
+    _lib = lib
+    return lib
+
+
+def _ptr(t) -> int | None:
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    return t.data_ptr()
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+class Context:
+    """RAII wrapper of lwe_ctx.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, n: int, m: int, k: int, q: int, eta: int, max_batch: int = 1, device: int = 0):
+        self._h = C.c_void_p()
+        self._lib = load_library()
+        self.params = lwe_params(n, m, k, q, eta, max_batch)
+        self.device = device
+        rc = self._lib.lwe_create(C.byref(self._h), C.byref(self.params), device)
+        if rc != LWE_OK:
+            self._h = C.c_void_p()
+            raise LweError(rc, "lwe_create")
+
+    # -- plumbing
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self._lib.lwe_destroy(self._h)
+            self._h = C.c_void_p()
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def _check(self, rc: int, where: str):
+        if rc != LWE_OK:
+            detail = ""
+            if rc == -4:
+                detail = f"(cudaError {self._lib.lwe_last_cuda_error(self._h)})"
+            raise LweError(rc, where, detail)
+
+    def launch_count(self) -> int:
+        return int(self._lib.lwe_launch_count(self._h))
+
+    def set_option(self, option: int, value: int):
+        self._check(self._lib.lwe_set_option(self._h, option, value), "lwe_set_option")
+
+    # -- a1 / a2
+    def rng_fill(self, d_out, nbytes: int, key: bytes, iv: bytes, byte_offset: int = 0, stream=None):
+        assert len(key) == 16 and len(iv) == 16
+        self._check(self._lib.lwe_rng_fill(self._h, _ptr(d_out), nbytes, key, iv, byte_offset, _stream(stream)),
+                    "lwe_rng_fill")
+
+    def sample_uniform(self, d_out, first: int, count: int, seed: int, tag: int, inst0: int = 0, n_inst: int = 1,
+                       stream=None):
+        self._check(self._lib.lwe_sample_uniform(self._h, _ptr(d_out), first, count, seed, tag, inst0, n_inst,
+                                                 _stream(stream)), "lwe_sample_uniform")
+
+    def sample_cbd(self, d_out, first: int, count: int, seed: int, tag: int, inst0: int = 0, n_inst: int = 1,
+                   stream=None):
+        self._check(self._lib.lwe_sample_cbd(self._h, _ptr(d_out), first, count, seed, tag, inst0, n_inst,
+                                             _stream(stream)), "lwe_sample_cbd")
+
+    def sample_bits(self, d_out, first_bit: int, nbits: int, seed: int, tag: int, inst0: int = 0, n_inst: int = 1,
+                    stream=None):
+        self._check(self._lib.lwe_sample_bits(self._h, _ptr(d_out), first_bit, nbits, seed, tag, inst0, n_inst,
+                                              _stream(stream)), "lwe_sample_bits")
+
+    # -- a3..a6
+    def keygen(self, d_A, seed_A: int, d_s, d_e, d_b, batch: int = 1, stream=None):
+        self._check(self._lib.lwe_keygen(self._h, _ptr(d_A), seed_A, _ptr(d_s), _ptr(d_e), _ptr(d_b), batch,
+                                         _stream(stream)), "lwe_keygen")
+
+    def encaps(self, d_A, seed_A: int, d_b, d_Rbits, d_mubits, d_U, d_v, batch: int = 1, stream=None):
+        self._check(self._lib.lwe_encaps(self._h, _ptr(d_A), seed_A, _ptr(d_b), _ptr(d_Rbits), _ptr(d_mubits),
+                                         _ptr(d_U), _ptr(d_v), batch, _stream(stream)), "lwe_encaps")
+
+    def decaps(self, d_U, d_v, d_s, d_mubits_out, batch: int = 1, stream=None):
+        self._check(self._lib.lwe_decaps(self._h, _ptr(d_U), _ptr(d_v), _ptr(d_s), _ptr(d_mubits_out), batch,
+                                         _stream(stream)), "lwe_decaps")
+
+    def kem_host(self, d_A, seed_A: int, h_s, h_e, h_Rbits, h_mubits, h_b, h_U, h_v, h_mubits_out, batch: int = 1,
+                 stream=None):
+        self._check(self._lib.lwe_kem_host(self._h, _ptr(d_A), seed_A, _ptr(h_s), _ptr(h_e), _ptr(h_Rbits),
+                                           _ptr(h_mubits), _ptr(h_b), _ptr(h_U), _ptr(h_v), _ptr(h_mubits_out),
+                                           batch, _stream(stream)), "lwe_kem_host")

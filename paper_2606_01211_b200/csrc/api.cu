@@ -1,0 +1,306 @@
+// api.cu -- the C ABI of include/lwe.h: argument validation, context and workspace
+// management, and stream-ordered dispatch to the kernels.  No arithmetic of the method
+// happens on the host.
+#include <new>
+#include <string.h>
+
+#include "lwe_internal.cuh"
+
+using namespace lwe;
+
+struct lwe_ctx {
+    Ctx c;
+};
+
+namespace {
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+bool is_pow2(uint32_t x) { return x && !(x & (x - 1)); }
+
+ModQ make_modq(uint32_t q)
+{
+    ModQ mq;
+    mq.q = q;
+    mq.mu = (uint32_t)((1ull << 32) / q);
+    mq.T = q * (65536u / q);
+    mq.half = q / 2;
+    mq.pow2 = is_pow2(q) ? 1u : 0u;
+    mq.mask = q - 1;
+    return mq;
+}
+
+template <class T>
+cudaError_t dev_alloc(T **p, size_t count)
+{
+    return cudaMalloc(reinterpret_cast<void **>(p), count * sizeof(T) ? count * sizeof(T) : 16);
+}
+
+void free_all(Ctx *c)
+{
+    cudaFree(c->d_te0); cudaFree(c->d_Rexp); cudaFree(c->d_vacc); cudaFree(c->d_dacc); cudaFree(c->d_counters);
+    cudaFree(c->d_hs); cudaFree(c->d_he); cudaFree(c->d_hb); cudaFree(c->d_hU); cudaFree(c->d_hv);
+    cudaFree(c->d_hR); cudaFree(c->d_hmu); cudaFree(c->d_hmuout);
+}
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+#define CHECK_CTX(ctx) do { if (!(ctx)) return LWE_ERR_NULLPTR; } while (0)
+#define REQUIRE_PTR(p) do { if (!(p)) return LWE_ERR_NULLPTR; } while (0)
+#define REQUIRE_ALIGNED(p) do { if (!aligned16(p)) return LWE_ERR_ALIGN; } while (0)
+#define LAUNCH(c, expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { (c)->last_cuda_error = (int)_e; return LWE_ERR_CUDA; } } while (0)
+
+}  // namespace
+
+extern "C" {
+
+const char *lwe_strerror(int code)
+{
+    switch (code) {
+    case LWE_OK: return "ok";
+    case LWE_ERR_PARAM: return "invalid parameter";
+    case LWE_ERR_ALIGN: return "pointer or offset not aligned as the contract requires";
+    case LWE_ERR_NULLPTR: return "required pointer is NULL";
+    case LWE_ERR_CUDA: return "CUDA runtime error (see lwe_last_cuda_error)";
+    case LWE_ERR_UNSUPPORTED: return "unsupported device or variant";
+    default: return "unknown error code";
+    }
+}
+
+int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
+{
+    if (!out || !p) return LWE_ERR_NULLPTR;
+    *out = nullptr;
+    if (p->n == 0 || p->m == 0 || p->k == 0 || p->n % 8 || p->m % 8 || p->k % 8) return LWE_ERR_PARAM;
+    if (p->q < 2 || p->q > 65536 || p->eta < 1 || p->eta > 8 || p->max_batch < 1) return LWE_ERR_PARAM;
+    if (p->k > 2048 || p->n > (1u << 20) || p->m > (1u << 20)) return LWE_ERR_PARAM;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return LWE_ERR_UNSUPPORTED;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return LWE_ERR_CUDA;
+    if (prop.major != 10) return LWE_ERR_UNSUPPORTED;          // sm_100a only: no fallback, no other backend
+
+    DeviceGuard guard(device);
+    if (!guard.ok) return LWE_ERR_CUDA;
+
+    lwe_ctx *h = new (std::nothrow) lwe_ctx();
+    if (!h) return LWE_ERR_CUDA;
+    Ctx *c = &h->c;
+    memset(c, 0, sizeof(*c));
+    c->p = *p;
+    c->mq = make_modq(p->q);
+    c->device = device;
+    c->sm_count = prop.multiProcessorCount;
+
+    const size_t B = p->max_batch, n = p->n, m = p->m, k = p->k;
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+    ok(dev_alloc(&c->d_te0, 256));
+    ok(dev_alloc(&c->d_Rexp, m * k * B));
+    ok(dev_alloc(&c->d_vacc, k * B));
+    ok(dev_alloc(&c->d_dacc, k * B));
+    ok(dev_alloc(&c->d_counters, 8 + 2 * B));
+    ok(dev_alloc(&c->d_hs, B * n)); ok(dev_alloc(&c->d_he, B * m)); ok(dev_alloc(&c->d_hb, B * m));
+    ok(dev_alloc(&c->d_hU, B * n * k)); ok(dev_alloc(&c->d_hv, B * k));
+    ok(dev_alloc(&c->d_hR, B * m * k / 8)); ok(dev_alloc(&c->d_hmu, B * k / 8)); ok(dev_alloc(&c->d_hmuout, B * k / 8));
+    if (e == cudaSuccess) {
+        uint32_t te0[256];
+        aes_te0_host(te0);
+        ok(cudaMemcpy(c->d_te0, te0, sizeof(te0), cudaMemcpyHostToDevice));
+        ok(cudaMemset(c->d_vacc, 0, k * B * sizeof(unsigned long long)));
+        ok(cudaMemset(c->d_dacc, 0, k * B * sizeof(unsigned long long)));
+        ok(cudaMemset(c->d_counters, 0, (8 + 2 * B) * sizeof(unsigned int)));
+    }
+    if (e != cudaSuccess) {
+        free_all(c);
+        delete h;
+        return LWE_ERR_CUDA;
+    }
+    // TMA descriptor encoder, resolved through the runtime (no link-time libcuda dependency)
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPointByVersion("cuTensorMapEncodeTiled", &fn, 12000, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+        c->encode_tiled = fn;
+    cudaGetLastError();
+    *out = h;
+    return LWE_OK;
+}
+
+void lwe_destroy(lwe_ctx *ctx)
+{
+    if (!ctx) return;
+    DeviceGuard guard(ctx->c.device);
+    cudaDeviceSynchronize();
+    free_all(&ctx->c);
+    delete ctx;
+}
+
+int lwe_last_cuda_error(const lwe_ctx *ctx) { return ctx ? ctx->c.last_cuda_error : 0; }
+uint64_t lwe_launch_count(const lwe_ctx *ctx) { return ctx ? ctx->c.launches : 0; }
+
+int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
+{
+    CHECK_CTX(ctx);
+    if (option == LWE_OPT_ENCAPS_PATH) {
+        if (value < 0 || value > 2) return LWE_ERR_PARAM;
+        ctx->c.encaps_path = (int)value;
+        return LWE_OK;
+    }
+    return LWE_ERR_PARAM;
+}
+
+int lwe_rng_fill(lwe_ctx *ctx, void *d_out, size_t nbytes, const uint8_t key[16], const uint8_t iv[16],
+                 uint64_t byte_offset, void *stream)
+{
+    CHECK_CTX(ctx);
+    REQUIRE_PTR(key); REQUIRE_PTR(iv);
+    if (nbytes == 0) return LWE_OK;
+    REQUIRE_PTR(d_out); REQUIRE_ALIGNED(d_out);
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    AesKey k;
+    aes128_expand_key_host(key, &k);
+    uint64_t hi = 0, lo = 0;
+    for (int i = 0; i < 8; i++) { hi = (hi << 8) | iv[i]; lo = (lo << 8) | iv[8 + i]; }
+    LAUNCH(c, launch_rng_fill(c, (uint8_t *)d_out, nbytes, k, hi, lo, byte_offset, (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+static int sampler_args(lwe_ctx *ctx, const void *d_out, uint64_t first, uint64_t count, uint32_t tag,
+                        uint32_t inst0, uint32_t n_inst)
+{
+    CHECK_CTX(ctx);
+    if (tag == 0 || tag > 255) return LWE_ERR_PARAM;
+    if ((uint64_t)inst0 + n_inst > (1ull << 32)) return LWE_ERR_PARAM;
+    if (first % 8) return LWE_ERR_ALIGN;
+    if (count == 0 || n_inst == 0) return LWE_OK;
+    REQUIRE_PTR(d_out); REQUIRE_ALIGNED(d_out);
+    return LWE_OK;
+}
+
+int lwe_sample_uniform(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count, uint64_t seed,
+                       uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream)
+{
+    int rc = sampler_args(ctx, d_out, first, count, tag, inst0, n_inst);
+    if (rc != LWE_OK || count == 0 || n_inst == 0) return rc;
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_sample_uniform(c, d_out, first, count, seed_key_host(seed), tag, inst0, n_inst, (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+int lwe_sample_cbd(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count, uint64_t seed,
+                   uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream)
+{
+    int rc = sampler_args(ctx, d_out, first, count, tag, inst0, n_inst);
+    if (rc != LWE_OK || count == 0 || n_inst == 0) return rc;
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_sample_cbd(c, d_out, first, count, seed_key_host(seed), tag, inst0, n_inst, (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+int lwe_sample_bits(lwe_ctx *ctx, uint8_t *d_out, uint64_t first_bit, uint64_t nbits, uint64_t seed,
+                    uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream)
+{
+    int rc = sampler_args(ctx, d_out, first_bit, nbits, tag, inst0, n_inst);
+    if (rc != LWE_OK || nbits == 0 || n_inst == 0) return rc;
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_sample_bits(c, d_out, first_bit, nbits, seed_key_host(seed), tag, inst0, n_inst, (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+int lwe_keygen(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_t *d_s, const uint16_t *d_e,
+               uint16_t *d_b, uint32_t batch, void *stream)
+{
+    CHECK_CTX(ctx);
+    Ctx *c = &ctx->c;
+    if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
+    REQUIRE_PTR(d_s); REQUIRE_PTR(d_e); REQUIRE_PTR(d_b);
+    REQUIRE_ALIGNED(d_A); REQUIRE_ALIGNED(d_s); REQUIRE_ALIGNED(d_e); REQUIRE_ALIGNED(d_b);
+    DeviceGuard guard(c->device);
+    if (d_A) LAUNCH(c, launch_keygen_stored(c, d_A, d_s, d_e, d_b, batch, (cudaStream_t)stream));
+    else LAUNCH(c, launch_keygen_regen(c, seed_key_host(seed_A), d_s, d_e, d_b, batch, (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_t *d_b, const uint8_t *d_Rbits,
+               const uint8_t *d_mubits, uint16_t *d_U, uint16_t *d_v, uint32_t batch, void *stream)
+{
+    (void)seed_A;
+    CHECK_CTX(ctx);
+    Ctx *c = &ctx->c;
+    if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
+    if (!d_A) return LWE_ERR_UNSUPPORTED;                     // regenerated-A encaps: not in this build
+    REQUIRE_PTR(d_b); REQUIRE_PTR(d_Rbits); REQUIRE_PTR(d_mubits); REQUIRE_PTR(d_U); REQUIRE_PTR(d_v);
+    REQUIRE_ALIGNED(d_A); REQUIRE_ALIGNED(d_b); REQUIRE_ALIGNED(d_Rbits); REQUIRE_ALIGNED(d_mubits);
+    REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v);
+    bool tc = encaps_tc_supported(c, batch);
+    if (c->encaps_path == 1) tc = false;
+    if (c->encaps_path == 2 && !tc) return LWE_ERR_UNSUPPORTED;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    LAUNCH(c, launch_expand_R_and_v(c, d_b, d_Rbits, d_mubits, d_v, batch, tc, st));
+    if (tc) LAUNCH(c, launch_encaps_tc(c, d_A, d_U, batch, st));
+    else LAUNCH(c, launch_encaps_simt(c, d_A, d_Rbits, d_U, batch, st));
+    return LWE_OK;
+}
+
+int lwe_decaps(lwe_ctx *ctx, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
+               uint8_t *d_mubits_out, uint32_t batch, void *stream)
+{
+    CHECK_CTX(ctx);
+    Ctx *c = &ctx->c;
+    if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
+    REQUIRE_PTR(d_U); REQUIRE_PTR(d_v); REQUIRE_PTR(d_s); REQUIRE_PTR(d_mubits_out);
+    REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v); REQUIRE_ALIGNED(d_s); REQUIRE_ALIGNED(d_mubits_out);
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_decaps(c, d_U, d_v, d_s, d_mubits_out, batch, (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_t *h_s, const uint16_t *h_e,
+                 const uint8_t *h_Rbits, const uint8_t *h_mubits, uint16_t *h_b, uint16_t *h_U, uint16_t *h_v,
+                 uint8_t *h_mubits_out, uint32_t batch, void *stream)
+{
+    CHECK_CTX(ctx);
+    Ctx *c = &ctx->c;
+    if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
+    if (!d_A) return LWE_ERR_UNSUPPORTED;
+    REQUIRE_PTR(h_s); REQUIRE_PTR(h_e); REQUIRE_PTR(h_Rbits); REQUIRE_PTR(h_mubits);
+    REQUIRE_PTR(h_b); REQUIRE_PTR(h_v); REQUIRE_PTR(h_mubits_out);
+    REQUIRE_ALIGNED(d_A);
+    const size_t B = batch, n = c->p.n, m = c->p.m, k = c->p.k;
+    cudaStream_t st = (cudaStream_t)stream;
+    DeviceGuard guard(c->device);
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hs, h_s, B * n * 2, cudaMemcpyHostToDevice, st));
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_he, h_e, B * m * 2, cudaMemcpyHostToDevice, st));
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hR, h_Rbits, B * m * k / 8, cudaMemcpyHostToDevice, st));
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hmu, h_mubits, B * k / 8, cudaMemcpyHostToDevice, st));
+    int rc = lwe_keygen(ctx, d_A, seed_A, c->d_hs, c->d_he, c->d_hb, batch, stream);
+    if (rc != LWE_OK) return rc;
+    rc = lwe_encaps(ctx, d_A, seed_A, c->d_hb, c->d_hR, c->d_hmu, c->d_hU, c->d_hv, batch, stream);
+    if (rc != LWE_OK) return rc;
+    rc = lwe_decaps(ctx, c->d_hU, c->d_hv, c->d_hs, c->d_hmuout, batch, stream);
+    if (rc != LWE_OK) return rc;
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_b, c->d_hb, B * m * 2, cudaMemcpyDeviceToHost, st));
+    if (h_U) LWE_CUDA_TRY(c, cudaMemcpyAsync(h_U, c->d_hU, B * n * k * 2, cudaMemcpyDeviceToHost, st));
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_v, c->d_hv, B * k * 2, cudaMemcpyDeviceToHost, st));
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_mubits_out, c->d_hmuout, B * k / 8, cudaMemcpyDeviceToHost, st));
+    LWE_CUDA_TRY(c, cudaStreamSynchronize(st));
+    return LWE_OK;
+}
+
+}  // extern "C"

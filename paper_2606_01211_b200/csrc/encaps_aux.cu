@@ -1,0 +1,131 @@
+// encaps_aux.cu -- the small parts of Encaps (S8(a) a4/a5):
+//   * expand_R_and_v: one pass over the packed bits of R that (i) writes them as the
+//     u8 {0,1} B-operand of the tensor-core GEMM, laid out [i][t*k + c] so that one
+//     256-column GEMM tile is one instance, and (ii) accumulates
+//     v_c = sum_i b_i R_ic + mu_c floor(q/2) mod q  (BJ north_star) on the fly,
+//     so that R's bits are read from HBM once.
+//   * encaps_simt: CUDA-core U = A^T R for shapes the tensor path does not take
+//     (k % 16 != 0, tiny n) and as an in-library cross-check of the tcgen05 kernel.
+#include "lwe_internal.cuh"
+
+namespace lwe {
+
+constexpr int kAuxThreads = 256;
+
+// grid (row_splits, batch).  Thread = (row slot, column byte): 8 columns of one row.
+__global__ void __launch_bounds__(kAuxThreads)
+expand_R_and_v_kernel(const uint16_t *__restrict__ b, const uint8_t *__restrict__ Rbits,
+                      const uint8_t *__restrict__ mubits, uint8_t *__restrict__ Rexp, uint16_t *__restrict__ v,
+                      unsigned long long *__restrict__ acc, unsigned int *__restrict__ tickets,
+                      uint32_t m, uint32_t k, uint32_t ld_exp, bool write_Rexp, ModQ mq)
+{
+    __shared__ uint32_t sLast;
+    const uint32_t t = blockIdx.y;
+    const uint32_t kb = k / 8;                           // bytes of R bits per row
+    const uint32_t rows_per_iter = kAuxThreads / kb;     // >= 1 (k <= 2048)
+    const uint32_t rslot = threadIdx.x / kb, cb = threadIdx.x % kb;
+    const bool active = rslot < rows_per_iter;
+    const uint8_t *Rt = Rbits + (size_t)t * m * kb;
+    const uint16_t *bt = b + (size_t)t * m;
+
+    uint32_t a[8];                                       // sum_i b_i R_ic <= 65535 * 65536 < 2^32
+#pragma unroll
+    for (int x = 0; x < 8; x++) a[x] = 0;
+    if (active) {
+        for (uint32_t i = blockIdx.x * rows_per_iter + rslot; i < m; i += gridDim.x * rows_per_iter) {
+            uint32_t r = __ldg(Rt + (size_t)i * kb + cb);
+            uint32_t bi = __ldg(bt + i);
+            if (write_Rexp) {
+                // bit x of r -> byte x of the 8-byte output
+                uint32_t lo = (r & 1u) | ((r & 2u) << 7) | ((r & 4u) << 14) | ((r & 8u) << 21);
+                uint32_t hi = ((r >> 4) & 1u) | ((r & 0x20u) << 3) | ((r & 0x40u) << 10) | ((r & 0x80u) << 17);
+                *reinterpret_cast<uint2 *>(Rexp + (size_t)i * ld_exp + (size_t)t * k + 8 * cb) = make_uint2(lo, hi);
+            }
+#pragma unroll
+            for (int x = 0; x < 8; x++) a[x] += ((r >> x) & 1u) ? bi : 0u;
+        }
+#pragma unroll
+        for (int x = 0; x < 8; x++)
+            if (a[x]) atomicAdd(acc + (size_t)t * k + 8 * cb + x, (unsigned long long)a[x]);
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) sLast = (atomicAdd(tickets + t, 1u) == gridDim.x - 1) ? 1u : 0u;
+    __syncthreads();
+    if (!sLast) return;
+    __threadfence();
+    for (uint32_t c = threadIdx.x; c < k; c += kAuxThreads) {
+        unsigned long long sum = __ldcg(acc + (size_t)t * k + c);
+        acc[(size_t)t * k + c] = 0;
+        uint32_t mu = (mubits[(size_t)t * kb + c / 8] >> (c % 8)) & 1u;
+        v[(size_t)t * k + c] = (uint16_t)mod_u64(sum + (unsigned long long)mu * mq.half, mq);
+    }
+    if (threadIdx.x == 0) tickets[t] = 0;
+}
+
+cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_Rbits, const uint8_t *d_mubits,
+                                  uint16_t *d_v, uint32_t batch, bool write_Rexp, cudaStream_t st)
+{
+    const uint32_t m = c->p.m, k = c->p.k;
+    const uint32_t rows_per_iter = kAuxThreads / (k / 8);
+    uint32_t splits = (uint32_t)((8 * c->sm_count + batch - 1) / batch);
+    uint32_t max_splits = (m + rows_per_iter - 1) / rows_per_iter;
+    if (splits > max_splits) splits = max_splits;
+    if (splits < 1) splits = 1;
+    dim3 grid(splits, batch);
+    expand_R_and_v_kernel<<<grid, kAuxThreads, 0, st>>>(d_b, d_Rbits, d_mubits, c->d_Rexp, d_v, c->d_vacc,
+                                                        c->d_counters + 8 + c->p.max_batch, m, k,
+                                                        batch * k, write_Rexp, c->mq);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ CUDA-core U = A^T R
+// grid (ceil(n/32), k/8, batch), block 32 x 8: thread (x, y) owns U[j = 32*bx + x][8 columns of
+// byte by] over the row range y, y+8, ...; the 8 row-slices are summed through shared memory.
+__global__ void __launch_bounds__(256)
+encaps_simt_kernel(const uint16_t *__restrict__ A, const uint8_t *__restrict__ Rbits, uint16_t *__restrict__ U,
+                   uint32_t m, uint32_t n, uint32_t k, ModQ mq)
+{
+    __shared__ uint32_t sAcc[8][32][8];
+    const uint32_t t = blockIdx.z, cb = blockIdx.y, kb = k / 8;
+    const uint32_t j = blockIdx.x * 32 + threadIdx.x;
+    const uint8_t *Rt = Rbits + (size_t)t * m * kb;
+    uint32_t a[8];
+#pragma unroll
+    for (int x = 0; x < 8; x++) a[x] = 0;
+    if (j < n) {
+        for (uint32_t i = threadIdx.y; i < m; i += 8) {
+            uint32_t aij = __ldg(A + (size_t)i * n + j);
+            uint32_t r = __ldg(Rt + (size_t)i * kb + cb);
+#pragma unroll
+            for (int x = 0; x < 8; x++) a[x] += ((r >> x) & 1u) ? aij : 0u;   // <= 65535 * 65536 < 2^32
+        }
+    }
+#pragma unroll
+    for (int x = 0; x < 8; x++) sAcc[threadIdx.y][threadIdx.x][x] = a[x];
+    __syncthreads();
+    if (threadIdx.y == 0 && j < n) {
+        uint32_t o[8];
+#pragma unroll
+        for (int x = 0; x < 8; x++) {
+            unsigned long long sum = 0;
+            for (int y = 0; y < 8; y++) sum += sAcc[y][threadIdx.x][x];
+            o[x] = mod_u64(sum, mq);
+        }
+        uint4 pk = make_uint4(o[0] | (o[1] << 16), o[2] | (o[3] << 16), o[4] | (o[5] << 16), o[6] | (o[7] << 16));
+        *reinterpret_cast<uint4 *>(U + ((size_t)t * n + j) * k + 8 * cb) = pk;
+    }
+}
+
+cudaError_t launch_encaps_simt(Ctx *c, const uint16_t *d_A, const uint8_t *d_Rbits, uint16_t *d_U,
+                               uint32_t batch, cudaStream_t st)
+{
+    const uint32_t m = c->p.m, n = c->p.n, k = c->p.k;
+    dim3 grid((n + 31) / 32, k / 8, batch), block(32, 8);
+    encaps_simt_kernel<<<grid, block, 0, st>>>(d_A, d_Rbits, d_U, m, n, k, c->mq);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace lwe

@@ -1,0 +1,335 @@
+// encaps_tc.cu -- a4: U = A^T R mod q as a tcgen05 kind::i8 GEMM (BJ north_star (3);
+// the bit-batched contraction of P:L136-148).
+//
+// Formulation.  The little-endian uint16 matrix A (m x n) is read, unchanged, as a
+// uint8 matrix A8 (m x 2n): byte-column 2j is the low byte plane of column j, 2j+1 the
+// high plane.  One GEMM  D[2n x N] = A8^T . Rexp  (u8 x u8 -> s32, N = batch*k, K = m)
+// therefore yields acc_lo in even rows and acc_hi in odd rows with no split pass, and
+//   U[j][c] = (D[2j][c] + 256*D[2j+1][c]) mod q.
+// Bounds (m <= 65536): D <= 255*m < 2^31; D_lo + 256*D_hi <= 65535*m < 2^32.
+//
+// Operand major-ness.  The contraction index i is the SLOW axis of both A8 (row-major
+// m x 2n) and Rexp (m x N): both operands are "MN-major".  tcgen05 accepts MN-major
+// 8-bit operands (instruction-descriptor bits 15/16), and the canonical MN-major
+// SWIZZLE_128B shared-memory layout (rows of 128 bytes along M/N, 8 K-rows per 1 KB
+// atom) is exactly what a TMA box {128 bytes, K rows} with CU_TENSOR_MAP_SWIZZLE_128B
+// writes -- so A is consumed in place: no transpose, no plane split, no second copy.
+//
+// Kernel shape (v1): persistent, one CTA per SM, cta_group::1, tile 128 (byte-rows
+// of D = 64 columns of A) x 256 (= one instance when k = 256) x K_TILE 128 per stage,
+// 4-stage TMA->smem ring, two 256-column TMEM accumulators so the epilogue of tile t
+// overlaps the main loop of tile t+1.
+//   warp 0 : TMA producer (1 lane)      warp 1 : TMEM alloc + MMA issuer (1 lane)
+//   warps 2-5 : epilogue, one TMEM lane quarter each: tcgen05.ld -> pair lo/hi lanes by
+//               shuffle -> mod q -> 32-byte stores into U[t][j][c]
+#include "lwe_internal.cuh"
+
+namespace lwe {
+
+namespace {
+
+constexpr uint32_t kTileM = 128;      // bytes of A8 row = 64 u16 columns of A
+constexpr uint32_t kTileN = 256;
+constexpr uint32_t kTileK = 128;      // rows of A / R per pipeline stage
+constexpr uint32_t kStages = 4;
+constexpr uint32_t kUmmaK = 32;       // K per tcgen05.mma for 8-bit operands
+constexpr uint32_t kBytesA = kTileM * kTileK;              // 16 KB
+constexpr uint32_t kBytesBHalf = 128 * kTileK;             // 16 KB per 128-column half
+constexpr uint32_t kBytesStage = kBytesA + 2 * kBytesBHalf; // 48 KB
+constexpr uint32_t kThreads = 192;
+constexpr uint32_t kTmemCols = 512;
+constexpr uint32_t kSmemBytes = kStages * kBytesStage + 1024 /*align*/ + 256 /*barriers*/;
+
+// ---- PTX wrappers ---------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    // Watchdog: a protocol bug (wrong tx byte count, lost arrive) must surface as a launch
+    // error, not as a hung GPU.  ~4 s at 2 GHz; only evaluated on the slow path.
+    uint32_t done;
+    long long t0 = 0;
+    for (;;) {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        if (done) break;
+        long long now = clock64();
+        if (t0 == 0) t0 = now;
+        else if (now - t0 > 8000000000ll) __trap();
+    }
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int32_t c0, int32_t c1)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void umma_i8(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_32x32b_x32(uint32_t taddr, uint32_t (&r)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+        "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// Shared-memory matrix descriptor, MN-major, SWIZZLE_128B (sm_100 format, version 1):
+// [0,14) start>>4 | [16,30) LBO>>4 (stride between 128-byte MN atoms) |
+// [32,46) SBO>>4 (stride between 8-row K groups) | [46,48) version=1 | [61,64) layout=2.
+__device__ __forceinline__ uint64_t make_desc_mn_sw128(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3ffffu) >> 4);
+    d |= (uint64_t)((lbo_bytes >> 4) & 0x3fffu) << 16;
+    d |= (uint64_t)((sbo_bytes >> 4) & 0x3fffu) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)2 << 61;
+    return d;
+}
+
+// Instruction descriptor for kind::i8: D = s32 (c_format 2 at [4,6)), A = B = u8 (format 0),
+// A and B MN-major (bits 15, 16), N>>3 at [17,23), M>>4 at [24,29).
+constexpr uint32_t kInstrDesc = (2u << 4) | (1u << 15) | (1u << 16) | ((kTileN >> 3) << 17) | ((kTileM >> 4) << 24);
+
+struct TileSched {
+    uint32_t m_tiles, n_tiles, total;
+    __device__ __forceinline__ void coords(uint32_t t, uint32_t &mt, uint32_t &nt) const
+    {
+        // groups of 8 n-tiles; inside a group n varies fastest, then m: CTAs running at the
+        // same time share A strips (L2) and the group's R panels stay L2-resident.
+        const uint32_t g = 8;
+        uint32_t per_group = m_tiles * g;
+        uint32_t grp = t / per_group, r = t - grp * per_group;
+        uint32_t width = (n_tiles - grp * g) < g ? (n_tiles - grp * g) : g;
+        mt = r / width;
+        nt = grp * g + (r - mt * width);
+    }
+};
+
+__global__ void __launch_bounds__(kThreads, 1)
+encaps_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
+                 uint16_t *__restrict__ U, uint32_t m, uint32_t n, uint32_t k, uint32_t ncols_total, ModQ mq)
+{
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = smem_u32(smem_raw);
+    const uint32_t base = (raw + 1023u) & ~1023u;                 // SWIZZLE_128B atoms need 1 KB alignment
+    const uint32_t bars = base + kStages * kBytesStage;           // barrier block (8-byte aligned)
+    // barrier layout: full[kStages], empty[kStages], tmem_full[2], tmem_empty[2], then the TMEM base word
+    auto full_bar = [&](uint32_t s) { return bars + 8 * s; };
+    auto empty_bar = [&](uint32_t s) { return bars + 8 * (kStages + s); };
+    auto tfull_bar = [&](uint32_t a) { return bars + 8 * (2 * kStages + a); };
+    auto tempty_bar = [&](uint32_t a) { return bars + 8 * (2 * kStages + 2 + a); };
+    const uint32_t tmem_slot = bars + 8 * (2 * kStages + 4);
+    volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
+
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    TileSched sched;
+    sched.m_tiles = (2 * n + kTileM - 1) / kTileM;
+    sched.n_tiles = (ncols_total + kTileN - 1) / kTileN;
+    sched.total = sched.m_tiles * sched.n_tiles;
+    const uint32_t k_blocks = (m + kTileK - 1) / kTileK;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapR) : "memory");
+        for (uint32_t s = 0; s < kStages; s++) {
+            mbar_init(full_bar(s), 1);
+            mbar_init(empty_bar(s), 1);
+        }
+        for (uint32_t a = 0; a < 2; a++) {
+            mbar_init(tfull_bar(a), 1);
+            mbar_init(tempty_bar(a), 4);                            // one arrival per epilogue warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) tmem_alloc(tmem_slot, kTmemCols);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        if (lane == 0) {
+            uint32_t stage = 0, phase = 0;
+            for (uint32_t t = blockIdx.x; t < sched.total; t += gridDim.x) {
+                uint32_t mt, nt;
+                sched.coords(t, mt, nt);
+                const int32_t a_col = (int32_t)(mt * kTileM), r_col = (int32_t)(nt * kTileN);
+                for (uint32_t kb = 0; kb < k_blocks; kb++) {
+                    mbar_wait(empty_bar(stage), phase ^ 1);
+                    const uint32_t sa = base + stage * kBytesStage;
+                    mbar_expect_tx(full_bar(stage), kBytesStage);
+                    const int32_t row = (int32_t)(kb * kTileK);
+                    tma_load_2d(sa, &mapA, full_bar(stage), a_col, row);
+                    tma_load_2d(sa + kBytesA, &mapR, full_bar(stage), r_col, row);
+                    tma_load_2d(sa + kBytesA + kBytesBHalf, &mapR, full_bar(stage), r_col + 128, row);
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer =====================
+        if (lane == 0) {
+            uint32_t stage = 0, phase = 0, it = 0;
+            for (uint32_t t = blockIdx.x; t < sched.total; t += gridDim.x, it++) {
+                const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
+                mbar_wait(tempty_bar(acc), acc_phase ^ 1);          // epilogue has drained this accumulator
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + acc * kTileN;
+                for (uint32_t kb = 0; kb < k_blocks; kb++) {
+                    mbar_wait(full_bar(stage), phase);
+                    tc_fence_after();
+                    const uint32_t sa = base + stage * kBytesStage;
+                    const uint32_t sb = sa + kBytesA;
+#pragma unroll
+                    for (uint32_t ks = 0; ks < kTileK / kUmmaK; ks++) {
+                        // K step = 32 rows of 128 bytes = 4 KB in both operands
+                        uint64_t adesc = make_desc_mn_sw128(sa + ks * kUmmaK * 128, 0, 1024);
+                        uint64_t bdesc = make_desc_mn_sw128(sb + ks * kUmmaK * 128, kBytesBHalf, 1024);
+                        umma_i8(d_tmem, adesc, bdesc, kInstrDesc, (kb | ks) ? 1u : 0u);
+                    }
+                    umma_commit(empty_bar(stage));                  // smem slot free once these MMAs retire
+                    if (kb == k_blocks - 1) umma_commit(tfull_bar(acc));
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else {
+        // ===================== epilogue (warps 2..5) =====================
+        const uint32_t quarter = warp & 3;                          // TMEM lanes 32*quarter .. +31
+        uint32_t it = 0;
+        for (uint32_t t = blockIdx.x; t < sched.total; t += gridDim.x, it++) {
+            uint32_t mt, nt;
+            sched.coords(t, mt, nt);
+            const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
+            mbar_wait(tfull_bar(acc), acc_phase);
+            tc_fence_after();
+            const uint32_t brow = mt * kTileM + quarter * 32 + lane;   // byte-row of D
+            const uint32_t j = brow >> 1;                             // column of A / row of U
+            const bool odd = lane & 1;
+            const uint32_t taddr = tmem_base + ((quarter * 32) << 16) + acc * kTileN;
+#pragma unroll 1
+            for (uint32_t cb = 0; cb < kTileN; cb += 32) {
+                uint32_t r[32];
+                tmem_ld_32x32b_x32(taddr + cb, r);
+                tmem_ld_wait();
+                uint32_t o[16];
+#pragma unroll
+                for (int x = 0; x < 16; x++) {
+                    uint32_t send = odd ? r[x] : r[16 + x];
+                    uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 1);
+                    uint32_t val = odd ? (recv + (r[16 + x] << 8)) : (r[x] + (recv << 8));
+                    o[x] = mq.pow2 ? (val & mq.mask) : mod_u32(val, mq);
+                }
+                const uint32_t col = nt * kTileN + cb + (odd ? 16u : 0u);   // first of my 16 columns
+                if (j < n && col < ncols_total) {
+                    const uint32_t inst = col / k, c = col - inst * k;
+                    uint4 *dst = reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c);
+                    dst[0] = make_uint4(o[0] | (o[1] << 16), o[2] | (o[3] << 16), o[4] | (o[5] << 16), o[6] | (o[7] << 16));
+                    dst[1] = make_uint4(o[8] | (o[9] << 16), o[10] | (o[11] << 16), o[12] | (o[13] << 16), o[14] | (o[15] << 16));
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty_bar(acc));
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem_base, kTmemCols);
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// u8 matrix [rows][width] row-major, box {128 bytes, kTileK rows}, SWIZZLE_128B, OOB -> 0
+bool make_map_u8(const Ctx *c, CUtensorMap *map, const void *ptr, uint64_t width, uint64_t rows)
+{
+    if (!c->encode_tiled) return false;
+    cuuint64_t dims[2] = {width, rows};
+    cuuint64_t strides[1] = {width};
+    cuuint32_t box[2] = {128, kTileK};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = ((EncodeTiledFn)c->encode_tiled)(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(ptr), dims,
+                                                  strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+bool encaps_tc_supported(const Ctx *c, uint32_t batch)
+{
+    const lwe_params &p = c->p;
+    return c->encode_tiled != nullptr && p.k % 16 == 0 && p.m <= 65536 && (2ull * p.n) % 16 == 0 &&
+           ((uint64_t)batch * p.k) % 16 == 0;
+}
+
+cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st)
+{
+    const lwe_params &p = c->p;
+    const uint32_t ncols = batch * p.k;
+    CUtensorMap mapA, mapR;
+    if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, p.m)) return cudaErrorInvalidValue;
+    if (!make_map_u8(c, &mapR, c->d_Rexp, ncols, p.m)) return cudaErrorInvalidValue;
+    cudaError_t err = cudaFuncSetAttribute(encaps_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (err != cudaSuccess) return err;
+    const uint32_t tiles = ((2 * p.n + kTileM - 1) / kTileM) * ((ncols + kTileN - 1) / kTileN);
+    uint32_t grid = tiles < (uint32_t)c->sm_count ? tiles : (uint32_t)c->sm_count;
+    encaps_tc_kernel<<<grid, kThreads, kSmemBytes, st>>>(mapA, mapR, d_U, p.m, p.n, p.k, ncols, c->mq);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace lwe

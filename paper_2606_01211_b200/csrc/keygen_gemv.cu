@@ -1,0 +1,176 @@
+// keygen_gemv.cu -- a3 / a3': b = A s + e mod q (eq.(1)).
+//
+// HBM-bound: A (2mn bytes) is read exactly once, 16 bytes per thread per load, fully
+// coalesced; everything else is noise.  The paper's kernel gives one thread a whole
+// row -- on B200 that is an uncoalesced stream; here a TEAM of threads
+// (a warp for short rows, the whole CTA for long ones) owns a row, so that the
+// work items are small (no tail) and each load instruction covers 512 B..4 KB of
+// one row.
+//
+// Arithmetic: s is split into bytes once per CTA and kept in shared memory packed
+// for dp2a: word p = s_lo[2p] | s_lo[2p+1]<<8 | s_hi[2p]<<16 | s_hi[2p+1]<<24.  One A
+// word holds two u16 elements, so
+//     acc_lo = dp2a.lo(Aword, sword, acc_lo)   (+= a0*s_lo0 + a1*s_lo1)
+//     acc_hi = dp2a.hi(Aword, sword, acc_hi)   (+= a0*s_hi0 + a1*s_hi1)
+// costs one instruction per element with no unpacking of A.  A.s = acc_lo + 256*acc_hi.
+// Each dp2a adds < 2^25, so u32 accumulators are flushed into u64 every 128 steps
+// (exact for any q); for q | 2^32 wrap-around is already exact and the flush is moot.
+#include "aes_ctr.cuh"
+
+namespace lwe {
+
+constexpr int kGemvThreads = 256;
+constexpr int kFlushEvery = 32;          // uint4 loads between flushes: 32*4 = 128 dp2a per accumulator
+
+__device__ __forceinline__ uint4 ldg_stream(const uint4 *p)
+{
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ void dot8(uint4 a, uint4 sw, uint32_t &lo, uint32_t &hi)
+{
+    lo = __dp2a_lo(a.x, sw.x, lo); hi = __dp2a_hi(a.x, sw.x, hi);
+    lo = __dp2a_lo(a.y, sw.y, lo); hi = __dp2a_hi(a.y, sw.y, hi);
+    lo = __dp2a_lo(a.z, sw.z, lo); hi = __dp2a_hi(a.z, sw.z, hi);
+    lo = __dp2a_lo(a.w, sw.w, lo); hi = __dp2a_hi(a.w, sw.w, hi);
+}
+
+// pack s (n u16) into the dp2a operand layout in shared memory
+__device__ __forceinline__ void pack_s_to_smem(uint32_t *sS, const uint16_t *__restrict__ s, uint32_t n)
+{
+    const uint32_t *s32 = reinterpret_cast<const uint32_t *>(s);
+    for (uint32_t p = threadIdx.x; p < n / 2; p += blockDim.x) {
+        uint32_t w = __ldg(s32 + p);                    // s[2p] | s[2p+1] << 16
+        sS[p] = __byte_perm(w, 0, 0x3120);              // (b0, b2, b1, b3)
+    }
+    __syncthreads();
+}
+
+template <int TPR>   // threads per row team: 32 (a warp) or kGemvThreads (the CTA)
+__device__ __forceinline__ uint64_t team_reduce(uint64_t v, uint64_t *sRed)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (TPR == 32) return v;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();                                    // previous row's readers are done
+    if (lane == 0) sRed[warp] = v;
+    __syncthreads();
+    uint64_t t = 0;
+#pragma unroll
+    for (int w = 0; w < kGemvThreads / 32; w++) t += sRed[w];
+    return t;
+}
+
+// kRegen = false: A streamed from HBM.  kRegen = true: A never read, every 16-byte
+// chunk (8 elements) is one AES-CTR block of object (seed_A, LWE_TAG_A, inst 0)
+// (+ rejection attempts), S8(c) O4 -- the paper's on-demand A.
+template <int TPR, bool kRegen>
+__global__ void __launch_bounds__(kGemvThreads)
+keygen_gemv_kernel(const uint16_t *__restrict__ A, AesKey key, const uint32_t *__restrict__ te0,
+                   const uint16_t *__restrict__ s, const uint16_t *__restrict__ e, uint16_t *__restrict__ b,
+                   uint32_t m, uint32_t n, uint32_t batch, ModQ mq)
+{
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    uint32_t *sS = reinterpret_cast<uint32_t *>(smem_raw);                // n/2 words
+    uint64_t *sRed = reinterpret_cast<uint64_t *>(smem_raw + 2 * (size_t)n);  // 8 u64
+    const uint32_t *sTl = nullptr;
+    if (kRegen) {
+        uint32_t *sT = reinterpret_cast<uint32_t *>(smem_raw + 2 * (size_t)n + 64);
+        aes_table_to_smem(sT, te0);
+        sTl = sT + (threadIdx.x & 31);
+    }
+
+    constexpr int kTeams = kGemvThreads / TPR;
+    const uint32_t team = threadIdx.x / TPR, tl = threadIdx.x % TPR;
+    const uint32_t chunks = n / 8;                       // 16-byte chunks per row
+    const uint32_t row0 = blockIdx.x * kTeams + team;
+    const uint32_t row_step = gridDim.x * kTeams;
+    const uint4 *sS4 = reinterpret_cast<const uint4 *>(sS);
+
+    for (uint32_t t = 0; t < batch; t++) {
+        if (t) __syncthreads();
+        pack_s_to_smem(sS, s + (size_t)t * n, n);
+        // rows are visited team-uniformly; TPR == CTA needs every thread in the loop
+        for (uint32_t i = row0; i < m; i += row_step) {
+            uint64_t sum_lo = 0, sum_hi = 0;
+            uint32_t lo = 0, hi = 0;
+            const uint4 *Arow = reinterpret_cast<const uint4 *>(A + (size_t)i * n);
+            uint32_t since = 0;
+            for (uint32_t c0 = tl; c0 < chunks; c0 += 4 * TPR) {
+                uint4 a[4];
+#pragma unroll
+                for (int u = 0; u < 4; u++) {
+                    uint32_t c = c0 + u * TPR;
+                    if (c < chunks) {
+                        if (kRegen) a[u] = uniform_block(key, sTl, mq, LWE_TAG_A, 0, (uint64_t)i * chunks + c);
+                        else a[u] = ldg_stream(Arow + c);
+                    } else {
+                        a[u] = make_uint4(0, 0, 0, 0);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; u++) {
+                    uint32_t c = c0 + u * TPR;
+                    uint4 sw = (c < chunks) ? sS4[c] : make_uint4(0, 0, 0, 0);
+                    dot8(a[u], sw, lo, hi);
+                }
+                since += 4;
+                if (!mq.pow2 && since >= kFlushEvery) {
+                    sum_lo += lo; sum_hi += hi; lo = 0; hi = 0; since = 0;
+                }
+            }
+            uint64_t total;
+            if (mq.pow2) total = (uint64_t)(lo + (hi << 8));              // exact mod 2^32, q | 2^32
+            else total = (sum_lo + lo) + ((sum_hi + hi) << 8);
+            total = team_reduce<TPR>(total, sRed);
+            if (tl == 0) {
+                uint32_t ei = e[(size_t)t * m + i];
+                uint32_t r = mq.pow2 ? (((uint32_t)total + ei) & mq.mask) : mod_u64(total + ei, mq);
+                b[(size_t)t * m + i] = (uint16_t)r;
+            }
+        }
+    }
+}
+
+template <int TPR, bool kRegen>
+static cudaError_t launch_gemv(Ctx *c, const uint16_t *d_A, const AesKey &key, const uint16_t *d_s,
+                               const uint16_t *d_e, uint16_t *d_b, uint32_t batch, cudaStream_t st)
+{
+    const uint32_t n = c->p.n, m = c->p.m;
+    size_t smem = 2 * (size_t)n + 64 + (kRegen ? kAesTableBytes : 0);
+    auto kern = keygen_gemv_kernel<TPR, kRegen>;
+    cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return err;
+    int per_sm = 0;
+    err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kGemvThreads, smem);
+    if (err != cudaSuccess) return err;
+    if (per_sm < 1) per_sm = 1;
+    constexpr int kTeams = kGemvThreads / TPR;
+    uint32_t grid = (uint32_t)(c->sm_count * per_sm);
+    uint32_t need = (m + kTeams - 1) / kTeams;
+    if (grid > need) grid = need;
+    kern<<<grid, kGemvThreads, smem, st>>>(d_A, key, c->d_te0, d_s, d_e, d_b, m, n, batch, c->mq);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_keygen_stored(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, const uint16_t *d_e,
+                                 uint16_t *d_b, uint32_t batch, cudaStream_t st)
+{
+    AesKey none = {};
+    if (c->p.n >= 4096) return launch_gemv<kGemvThreads, false>(c, d_A, none, d_s, d_e, d_b, batch, st);
+    return launch_gemv<32, false>(c, d_A, none, d_s, d_e, d_b, batch, st);
+}
+
+cudaError_t launch_keygen_regen(Ctx *c, const AesKey &key, const uint16_t *d_s, const uint16_t *d_e,
+                                uint16_t *d_b, uint32_t batch, cudaStream_t st)
+{
+    if (c->p.n >= 4096) return launch_gemv<kGemvThreads, true>(c, nullptr, key, d_s, d_e, d_b, batch, st);
+    return launch_gemv<32, true>(c, nullptr, key, d_s, d_e, d_b, batch, st);
+}
+
+}  // namespace lwe

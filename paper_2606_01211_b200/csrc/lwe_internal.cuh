@@ -1,0 +1,125 @@
+// lwe_internal.cuh -- shared declarations of the CUDA path (context, launch helpers,
+// modular arithmetic).  Product code: shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/lwe.h"
+
+namespace lwe {
+
+// ---------------------------------------------------------------------------------
+// AES-128 round keys in the word convention the kernels use: word c of a 16-byte
+// block is its bytes 4c..4c+3 loaded little-endian.
+struct AesKey {
+    uint32_t rk[44];
+};
+
+// Identifies one seeded stream family: key(seed) plus the upper 64 bits of the counter
+// without the attempt / instance fields (S8(c) O3).
+struct StreamId {
+    AesKey key;
+    uint32_t tag;
+};
+
+// mod-q helper constants.  mu = floor(2^32 / q) (exact 2^32/q for powers of two, which
+// then needs q < 2^32: q = 65536 gives 65536).
+struct ModQ {
+    uint32_t q;
+    uint32_t mu;        // floor(2^32 / q)
+    uint32_t T;         // q * floor(65536 / q): rejection threshold of the uniform sampler
+    uint32_t half;      // floor(q / 2)
+    uint32_t pow2;      // 1 if q is a power of two
+    uint32_t mask;      // q - 1 when pow2
+};
+
+__host__ __device__ __forceinline__ uint32_t mod_u32(uint32_t x, const ModQ &mq)
+{
+#ifdef __CUDA_ARCH__
+    uint32_t qhat = __umulhi(x, mq.mu);
+#else
+    uint32_t qhat = (uint32_t)(((uint64_t)x * mq.mu) >> 32);
+#endif
+    uint32_t r = x - qhat * mq.q;          // in [0, 3q): Barrett with mu = floor(2^32/q)
+    if (r >= mq.q) r -= mq.q;
+    if (r >= mq.q) r -= mq.q;
+    return r;
+}
+
+__host__ __device__ __forceinline__ uint32_t mod_u64(uint64_t x, const ModQ &mq)
+{
+    // x = hi*2^32 + lo; reduce hi first so that the combination fits 64 bits, then one
+    // 64-bit remainder.  Only used once per output element, never in an inner loop.
+    return (uint32_t)(x % (uint64_t)mq.q);
+}
+
+// ---------------------------------------------------------------------------------
+struct Ctx {
+    lwe_params p;
+    ModQ mq;
+    int device;
+    int sm_count;
+    int last_cuda_error;
+    uint64_t launches;
+    int encaps_path;                  // LWE_OPT_ENCAPS_PATH
+
+    // device tables
+    uint32_t *d_te0;                  // 256-entry AES T-table (word = 2S | S<<8 | S<<16 | 3S<<24)
+
+    // workspace (allocated once in lwe_create)
+    uint8_t *d_Rexp;                  // [m][max_batch*k] u8 in {0,1}: B operand of the encaps GEMM
+    unsigned long long *d_vacc;       // [max_batch*k] u64 partial sums of b^T R
+    unsigned long long *d_dacc;       // [max_batch*k] u64 partial sums of U^T s
+    unsigned int *d_counters;         // [8 + max_batch] self-resetting "last block" tickets
+    // staging for lwe_kem_host
+    uint16_t *d_hs, *d_he, *d_hb, *d_hU, *d_hv;
+    uint8_t *d_hR, *d_hmu, *d_hmuout;
+
+    // driver entry point for TMA descriptors (resolved at create; no link-time libcuda)
+    void *encode_tiled;
+};
+
+#define LWE_CUDA_TRY(ctx, expr)                                   \
+    do {                                                          \
+        cudaError_t _e = (expr);                                  \
+        if (_e != cudaSuccess) {                                  \
+            (ctx)->last_cuda_error = (int)_e;                     \
+            return LWE_ERR_CUDA;                                  \
+        }                                                         \
+    } while (0)
+
+// host-side key expansion (FIPS-197 5.2) into the kernels' word convention
+void aes128_expand_key_host(const uint8_t key[16], AesKey *out);
+void aes_te0_host(uint32_t te0[256]);
+AesKey seed_key_host(uint64_t seed);
+
+// kernel launchers (each returns a cudaError_t from the launch) --------------------
+cudaError_t launch_rng_fill(Ctx *c, uint8_t *d_out, size_t nbytes, const AesKey &key,
+                            uint64_t iv_hi, uint64_t iv_lo, uint64_t byte_offset, cudaStream_t st);
+cudaError_t launch_sample_uniform(Ctx *c, uint16_t *d_out, uint64_t first, uint64_t count,
+                                  const AesKey &key, uint32_t tag, uint32_t inst0, uint32_t n_inst,
+                                  cudaStream_t st);
+cudaError_t launch_sample_cbd(Ctx *c, uint16_t *d_out, uint64_t first, uint64_t count,
+                              const AesKey &key, uint32_t tag, uint32_t inst0, uint32_t n_inst,
+                              cudaStream_t st);
+cudaError_t launch_sample_bits(Ctx *c, uint8_t *d_out, uint64_t first_bit, uint64_t nbits,
+                               const AesKey &key, uint32_t tag, uint32_t inst0, uint32_t n_inst,
+                               cudaStream_t st);
+cudaError_t launch_keygen_stored(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, const uint16_t *d_e,
+                                 uint16_t *d_b, uint32_t batch, cudaStream_t st);
+cudaError_t launch_keygen_regen(Ctx *c, const AesKey &key, const uint16_t *d_s, const uint16_t *d_e,
+                                uint16_t *d_b, uint32_t batch, cudaStream_t st);
+cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_Rbits,
+                                  const uint8_t *d_mubits, uint16_t *d_v, uint32_t batch,
+                                  bool write_Rexp, cudaStream_t st);
+cudaError_t launch_encaps_simt(Ctx *c, const uint16_t *d_A, const uint8_t *d_Rbits, uint16_t *d_U,
+                               uint32_t batch, cudaStream_t st);
+bool encaps_tc_supported(const Ctx *c, uint32_t batch);
+cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st);
+cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
+                          uint8_t *d_out, uint32_t batch, cudaStream_t st);
+
+}  // namespace lwe

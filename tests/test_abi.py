@@ -1,0 +1,72 @@
+"""The C-ABI library builds for sm_100a, loads without a GPU and exports every entry
+point include/lwe.h declares; the binding mirrors them.  No compute calls here."""
+import ctypes
+import re
+from pathlib import Path
+
+import pytest
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+def declared_functions():
+    text = (ROOT / "include" / "lwe.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(lwe_[a-z0-9_]+)\s*\(", text)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_01211_b200 import build
+    path = build.build()
+    return ctypes.CDLL(str(path))
+
+
+def test_header_declares_the_north_star_calls():
+    names = declared_functions()
+    for required in ("lwe_keygen", "lwe_encaps", "lwe_decaps", "lwe_rng_fill", "lwe_create", "lwe_destroy"):
+        assert required in names
+
+
+def test_library_exports_every_declared_symbol(lib):
+    for name in declared_functions():
+        assert hasattr(lib, name), f"{name} declared in include/lwe.h but not exported"
+
+
+def test_binding_lists_the_same_entry_points():
+    from paper_2606_01211_b200 import binding
+    assert sorted(binding.EXPORTS) == declared_functions()
+
+
+def test_strerror_and_null_handling_without_a_gpu(lib):
+    lib.lwe_strerror.restype = ctypes.c_char_p
+    assert lib.lwe_strerror(0) == b"ok"
+    for code in (-1, -2, -3, -4, -5):
+        assert lib.lwe_strerror(code)
+    assert lib.lwe_create(None, None, 0) == -3            # LWE_ERR_NULLPTR, nothing touched
+    lib.lwe_destroy(None)                                 # no-op
+    lib.lwe_launch_count.restype = ctypes.c_uint64
+    assert lib.lwe_launch_count(None) == 0
+
+
+def test_no_cuda_device_is_reported_not_faked(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_2606_01211_b200 import binding
+    with pytest.raises(binding.LweError) as ei:
+        binding.Context(256, 512, 256, 65536, 4)
+    assert ei.value.code in (-5, -4)                      # unsupported: there is no CPU fallback
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = ROOT / "paper_2606_01211_b200"
+    for p in list(pkg.rglob("*.py")) + list(pkg.rglob("*.cu")) + list(pkg.rglob("*.cuh")) + [ROOT / "include" / "lwe.h"]:
+        text = p.read_text()
+        assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), p
+        assert "lwe_oracle" not in text and "orc_" not in text, p
+    for p in (ROOT / "oracle").glob("*"):
+        if p.suffix in (".py", ".c", ".h"):
+            text = p.read_text()
+            assert not re.search(r"^\s*(from|import)\s+paper_2606_01211_b200\b", text, flags=re.M), p
+            assert "#include \"../paper" not in text and "lwe_internal" not in text and "lwe.h" not in text, p

@@ -1,0 +1,219 @@
+"""GPU parity, a3-a6: keygen (stored and regenerated A), encaps (tcgen05 GEMM and
+CUDA-core path), decaps -- bit-exact against the oracle on the same seeded inputs,
+through the C ABI.  Sizes span several tiles and ragged tails; full configs are
+checked on sampled rows plus invariants that hold at any size."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle as O  # noqa: E402
+from paper_2606_01211_b200 import workloads as W  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def H():
+    import gpu_helpers
+    return gpu_helpers
+
+
+def B():
+    import paper_2606_01211_b200.binding as b
+    return b
+
+
+# ---------------------------------------------------------------- keygen
+
+KEYGEN_SHAPES = [  # (m, n, q, batch)
+    (512, 256, 65536, 1), (2048, 1024, 65536, 1), (264, 4096, 65521, 1), (136, 4104, 65521, 2),
+    (1000, 40, 65521, 3), (8, 8, 17, 1), (304, 8192, 65536, 2), (96, 16392, 65521, 1), (520, 2056, 3329, 1),
+]
+
+
+@pytest.mark.parametrize("m,n,q,batch", KEYGEN_SHAPES)
+def test_keygen_stored_matches_oracle(H, m, n, q, batch):
+    A = W.random_u16((m, n), q, 1)
+    s = W.random_u16((batch, n), q, 2)
+    e = W.random_u16((batch, m), q, 3)
+    with B().Context(n, m, 256, q, 4, batch) as c:
+        b = H.dev_empty_u16(batch, m)
+        c.keygen(H.dev(A), 0, H.dev(s), H.dev(e), b, batch)
+        got = H.host_u16(b)
+    for t in range(batch):
+        assert np.array_equal(got[t], O.keygen(A, s[t], e[t], q)), (m, n, q, t)
+
+
+def test_keygen_extreme_values(H):
+    # every product and every partial sum at its maximum (P9)
+    for q in (65536, 65521):
+        m, n = 64, 32768
+        A = np.full((m, n), q - 1, np.uint16)
+        s = np.full((1, n), q - 1, np.uint16)
+        e = np.full((1, m), q - 1, np.uint16)
+        with B().Context(n, m, 256, q, 4, 1) as c:
+            b = H.dev_empty_u16(1, m)
+            c.keygen(H.dev(A), 0, H.dev(s), H.dev(e), b, 1)
+            assert np.all(H.host_u16(b) == (n * (q - 1) * (q - 1) + (q - 1)) % q)
+
+
+@pytest.mark.parametrize("m,n,q,seed", [(512, 256, 65536, 1), (264, 4096, 65521, 3), (72, 1032, 40000, 9),
+                                         (2048, 1024, 65536, 2)])
+def test_keygen_regenerated_A_equals_stored_and_oracle(H, m, n, q, seed):
+    # P11: A never stored; must equal the oracle's A drawn from the same seed
+    A = O.sample_uniform(0, m * n, seed, O.TAG_A, 0, q).reshape(m, n)
+    s = W.random_u16((2, n), q, 5)
+    e = W.random_u16((2, m), q, 6)
+    with B().Context(n, m, 256, q, 4, 2) as c:
+        b1, b2 = H.dev_empty_u16(2, m), H.dev_empty_u16(2, m)
+        dA = H.dev_empty_u16(m, n)
+        c.sample_uniform(dA, 0, m * n, seed, W.TAG_A)
+        assert np.array_equal(H.host_u16(dA), A)
+        c.keygen(dA, 0, H.dev(s), H.dev(e), b1, 2)
+        c.keygen(None, seed, H.dev(s), H.dev(e), b2, 2)
+        g1, g2 = H.host_u16(b1), H.host_u16(b2)
+    assert np.array_equal(g1, g2)
+    for t in range(2):
+        assert np.array_equal(g2[t], O.keygen(A, s[t], e[t], q))
+
+
+# ---------------------------------------------------------------- encaps
+
+ENCAPS_SHAPES = [  # (m, n, k, q, batch)
+    (512, 256, 256, 65536, 1),        # C1
+    (640, 192, 256, 65521, 2),        # several K blocks, 3 M tiles, prime q
+    (200, 72, 256, 65521, 3),         # ragged K tail (200 = 128 + 72), ragged M tile (144 bytes)
+    (136, 64, 128, 65536, 3),         # k = 128: N tile straddles instances, ragged N tail (384 cols)
+    (128, 64, 16, 17, 2),             # 32 columns in total
+    (2048, 1024, 256, 65536, 1),      # C2
+]
+
+
+def run_encaps(H, path, m, n, k, q, batch, A, b, Rbits, mubits):
+    with B().Context(n, m, k, q, 4, batch) as c:
+        c.set_option(B().OPT_ENCAPS_PATH, path)
+        U, v = H.dev_empty_u16(batch, n, k), H.dev_empty_u16(batch, k)
+        U.fill_(-1)
+        c.encaps(H.dev(A), 0, H.dev(b), H.dev(Rbits), H.dev(mubits), U, v, batch)
+        return H.host_u16(U), H.host_u16(v)
+
+
+@pytest.mark.parametrize("path", [2, 1], ids=["tcgen05", "simt"])
+@pytest.mark.parametrize("m,n,k,q,batch", ENCAPS_SHAPES)
+def test_encaps_matches_oracle(H, path, m, n, k, q, batch):
+    A = W.random_u16((m, n), q, 21)
+    b = W.random_u16((batch, m), q, 22)
+    Rbits = W.random_bytes(batch * m * k // 8, 23).reshape(batch, -1)
+    mubits = W.random_bytes(batch * k // 8, 24).reshape(batch, -1)
+    U, v = run_encaps(H, path, m, n, k, q, batch, A, b, Rbits, mubits)
+    for t in range(batch):
+        Uo, vo = O.encaps(A, b[t], Rbits[t], mubits[t], k, q)
+        assert np.array_equal(v[t], vo), ("v", t)
+        bad = np.argwhere(U[t] != Uo)
+        assert bad.size == 0, (f"U mismatch inst {t}: {len(bad)} entries, first {bad[:5].tolist()}, "
+                               f"got {U[t][tuple(bad[0])]} want {Uo[tuple(bad[0])]}")
+
+
+@pytest.mark.parametrize("path", [2, 1], ids=["tcgen05", "simt"])
+def test_encaps_extreme_accumulators(H, path):
+    # P9: A = q-1 (or 65535), R = all ones, m = 65536 -> both byte-plane accumulators and the
+    # recombined 32-bit value hit their bounds exactly
+    for q in (65536, 65521):
+        m, n, k = 65536, 64, 256
+        A = np.full((m, n), q - 1, np.uint16)
+        b = np.full((1, m), q - 1, np.uint16)
+        Rbits = np.full((1, m * k // 8), 0xFF, np.uint8)
+        mubits = np.full((1, k // 8), 0xFF, np.uint8)
+        U, v = run_encaps(H, path, m, n, k, q, 1, A, b, Rbits, mubits)
+        assert np.all(U == (m * (q - 1)) % q)
+        assert np.all(v == (m * (q - 1) + q // 2) % q)
+
+
+def test_encaps_one_hot_R_picks_a_row_of_A(H):
+    m, n, k, q = 256, 128, 256, 65521
+    A = W.random_u16((m, n), q, 31)
+    b = W.random_u16((1, m), q, 32)
+    R = np.zeros((m, k), np.uint8)
+    R[77, 200] = 1
+    R[5, 0] = 1
+    Rbits = np.packbits(R.ravel(), bitorder="little")[None, :]
+    mubits = np.zeros((1, k // 8), np.uint8)
+    U, v = run_encaps(H, 2, m, n, k, q, 1, A, b, Rbits, mubits)
+    assert np.array_equal(U[0][:, 200], A[77]) and np.array_equal(U[0][:, 0], A[5])
+    assert int(v[0][200]) == int(b[0][77]) and int(v[0][0]) == int(b[0][5])
+    U[0][:, 200] = 0
+    U[0][:, 0] = 0
+    assert not U.any()
+
+
+# ---------------------------------------------------------------- decaps
+
+@pytest.mark.parametrize("n,k,q,batch", [(256, 256, 65536, 1), (1000, 256, 65521, 3), (64, 8, 17, 2),
+                                          (4096, 128, 65521, 2), (8192, 256, 65536, 4)])
+def test_decaps_matches_oracle(H, n, k, q, batch):
+    U = W.random_u16((batch, n, k), q, 41)
+    v = W.random_u16((batch, k), q, 42)
+    s = W.random_u16((batch, n), q, 43)
+    with B().Context(n, 8, k, q, 4, batch) as c:
+        out = H.dev_empty_u8(batch, k // 8)
+        for _ in range(2):                               # second call: workspace was left clean
+            out.fill_(0xEE)
+            c.decaps(H.dev(U), H.dev(v), H.dev(s), out, batch)
+            got = H.host_u8(out)
+            for t in range(batch):
+                assert np.array_equal(got[t], O.decaps(U[t], v[t], s[t], q)), (n, k, q, t)
+
+
+def test_decaps_rounding_boundaries(H):
+    # U = 0 so d = v: sweep v over the decision boundaries (P10)
+    for q in (65536, 65521):
+        k, n = 256, 8
+        edges = [0, 1, q // 4 - 1, q // 4, q // 4 + 1, q // 2, 3 * q // 4 - 1, 3 * q // 4, 3 * q // 4 + 1, q - 1]
+        v = np.array([(edges * 26)[:k]], np.uint16)
+        U = np.zeros((1, n, k), np.uint16)
+        s = W.random_u16((1, n), q, 1)
+        with B().Context(n, 8, k, q, 4, 1) as c:
+            out = H.dev_empty_u8(1, k // 8)
+            c.decaps(H.dev(U), H.dev(v), H.dev(s), out, 1)
+            got = H.unpack_bits(H.host_u8(out)[0], k)
+        want = np.array([1 if (4 * int(d) >= q and 4 * int(d) < 3 * q) else 0 for d in v[0]])
+        assert np.array_equal(got, want)
+
+
+# ---------------------------------------------------------------- whole path from seeds
+
+def gpu_kem_from_seed(H, c, w, n, m, batch, dA):
+    k = w.k
+    s, e, b = H.dev_empty_u16(batch, n), H.dev_empty_u16(batch, m), H.dev_empty_u16(batch, m)
+    Rbits, mubits = H.dev_empty_u8(batch, m * k // 8), H.dev_empty_u8(batch, k // 8)
+    U, v, out = H.dev_empty_u16(batch, n, k), H.dev_empty_u16(batch, k), H.dev_empty_u8(batch, k // 8)
+    c.sample_uniform(s, 0, n, w.seed, W.TAG_S, 0, batch)
+    c.sample_cbd(e, 0, m, w.seed, W.TAG_E, 0, batch)
+    c.sample_bits(Rbits, 0, m * k, w.seed, W.TAG_R, 0, batch)
+    c.sample_bits(mubits, 0, k, w.seed, W.TAG_MU, 0, batch)
+    c.keygen(dA, 0, s, e, b, batch)
+    c.encaps(dA, 0, b, Rbits, mubits, U, v, batch)
+    c.decaps(U, v, s, out, batch)
+    return dict(s=H.host_u16(s), e=H.host_u16(e), b=H.host_u16(b), Rbits=H.host_u8(Rbits),
+                mubits=H.host_u8(mubits), U=H.host_u16(U), v=H.host_u16(v), out=H.host_u8(out))
+
+
+@pytest.mark.parametrize("w,n,m,batch", [(W.C1, None, None, 1), (W.C2, None, None, 1), (W.C3, 512, 1024, 1),
+                                          (W.C4, 256, 512, 4)])
+def test_full_path_small_matches_oracle_everywhere(H, w, n, m, batch):
+    n, m = n or w.n, m or w.m
+    with H.make_ctx(w, n=n, m=m, max_batch=batch) as c:
+        dA = H.dev_empty_u16(m, n)
+        c.sample_uniform(dA, 0, m * n, w.seed, W.TAG_A)
+        g = gpu_kem_from_seed(H, c, w, n, m, batch, dA)
+        A = H.host_u16(dA)
+    for t in range(batch):
+        oi = H.OracleInstance(w, t, n, m)
+        assert np.array_equal(A, oi.A)
+        assert np.array_equal(g["s"][t], oi.s) and np.array_equal(g["e"][t], oi.e)
+        assert np.array_equal(g["Rbits"][t], oi.Rbits) and np.array_equal(g["mubits"][t], oi.mubits)
+        b = O.keygen(oi.A, oi.s, oi.e, w.q)
+        assert np.array_equal(g["b"][t], b)
+        U, v = O.encaps(oi.A, b, oi.Rbits, oi.mubits, w.k, w.q)
+        assert np.array_equal(g["U"][t], U) and np.array_equal(g["v"][t], v)
+        assert np.array_equal(g["out"][t], O.decaps(U, v, oi.s, w.q))
+        assert np.array_equal(g["out"][t], oi.mubits)                # every bit recovered
