@@ -144,11 +144,27 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
                  const uint8_t *h_mubits, uint16_t *h_b, uint16_t *h_U /* may be NULL */,
                  uint16_t *h_v, uint8_t *h_mubits_out, uint32_t batch, void *stream);
 
-/* ---- tuning / test hooks (no new semantics) ----------------------------------------
+/* ---- tuning / test / measurement hooks (no new semantics) --------------------------
  * LWE_OPT_ENCAPS_PATH: 0 = auto, 1 = force CUDA-core kernel, 2 = force tcgen05 GEMM
- *                      (LWE_ERR_UNSUPPORTED at call time if the shape does not fit). */
-enum { LWE_OPT_ENCAPS_PATH = 1 };
+ *                      (LWE_ERR_UNSUPPORTED at call time if the shape does not fit).
+ * LWE_OPT_PROFILE:     1 = bracket every kernel launch with a CUDA event pair on the
+ *                      stream it is launched on (at most 8192 launches are kept between
+ *                      resets; later ones are simply not timed); 0 = off (default). */
+enum { LWE_OPT_ENCAPS_PATH = 1, LWE_OPT_PROFILE = 2 };
 int lwe_set_option(lwe_ctx *ctx, int option, int64_t value);
+
+/* Kernel ids for lwe_profile_read (one per __global__ function of the library). */
+enum {
+    LWE_K_RNG_FILL = 0, LWE_K_SAMPLE_UNIFORM = 1, LWE_K_SAMPLE_CBD = 2, LWE_K_SAMPLE_BITS = 3,
+    LWE_K_KEYGEN_STORED = 4, LWE_K_KEYGEN_REGEN = 5, LWE_K_EXPAND_R_V = 6, LWE_K_ENCAPS_TC = 7,
+    LWE_K_ENCAPS_SIMT = 8, LWE_K_DECAPS = 9, LWE_K_COUNT = 10
+};
+/* Sum of the device durations (milliseconds, CUDA events) and the number of timed launches
+ * of kernel `kernel_id` since the last reset.  Waits for the recorded events to complete
+ * (host synchronisation: call it outside any timed region).  h_total_ms / h_launches: HOST
+ * pointers, either may be NULL.  lwe_profile_reset forgets all recorded pairs. */
+int lwe_profile_read(lwe_ctx *ctx, int kernel_id, double *h_total_ms, uint64_t *h_launches);
+int lwe_profile_reset(lwe_ctx *ctx);
 
 #ifdef __cplusplus
 }

@@ -19,11 +19,15 @@ ERRORS = {-1: "LWE_ERR_PARAM", -2: "LWE_ERR_ALIGN", -3: "LWE_ERR_NULLPTR", -4: "
           -5: "LWE_ERR_UNSUPPORTED"}
 TAG_A, TAG_S, TAG_E, TAG_R, TAG_MU = 1, 2, 3, 4, 5
 OPT_ENCAPS_PATH = 1
+OPT_PROFILE = 2
+KERNELS = ["rng_fill", "sample_uniform", "sample_cbd", "sample_bits", "keygen_stored", "keygen_regen",
+           "expand_R_v", "encaps_tc", "encaps_simt", "decaps"]
 
 EXPORTS = [
     "lwe_create", "lwe_destroy", "lwe_strerror", "lwe_last_cuda_error", "lwe_launch_count",
     "lwe_rng_fill", "lwe_sample_uniform", "lwe_sample_cbd", "lwe_sample_bits",
     "lwe_keygen", "lwe_encaps", "lwe_decaps", "lwe_kem_host", "lwe_set_option",
+    "lwe_profile_read", "lwe_profile_reset",
 ]
 
 
@@ -59,6 +63,8 @@ def load_library() -> C.CDLL:
     lib.lwe_launch_count.argtypes = [vp]
     lib.lwe_launch_count.restype = u64
     lib.lwe_set_option.argtypes = [vp, C.c_int, C.c_int64]
+    lib.lwe_profile_read.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(u64)]
+    lib.lwe_profile_reset.argtypes = [vp]
     lib.lwe_rng_fill.argtypes = [vp, vp, sz, C.c_char_p, C.c_char_p, u64, vp]
     for f in (lib.lwe_sample_uniform, lib.lwe_sample_cbd, lib.lwe_sample_bits):
         f.argtypes = [vp, vp, u64, u64, u64, u32, u32, u32, vp]
@@ -125,6 +131,19 @@ class Context:
 
     def set_option(self, option: int, value: int):
         self._check(self._lib.lwe_set_option(self._h, option, value), "lwe_set_option")
+
+    def profile_reset(self):
+        self._check(self._lib.lwe_profile_reset(self._h), "lwe_profile_reset")
+
+    def profile_read(self) -> dict:
+        """{kernel name: (total device ms, timed launches)} since the last reset (synchronises)"""
+        out = {}
+        for kid, name in enumerate(KERNELS):
+            ms, cnt = C.c_double(0), C.c_uint64(0)
+            self._check(self._lib.lwe_profile_read(self._h, kid, C.byref(ms), C.byref(cnt)), "lwe_profile_read")
+            if cnt.value:
+                out[name] = (ms.value, int(cnt.value))
+        return out
 
     # -- a1 / a2
     def rng_fill(self, d_out, nbytes: int, key: bytes, iv: bytes, byte_offset: int = 0, stream=None):

@@ -41,6 +41,14 @@ void free_all(Ctx *c)
     cudaFree(c->d_te0); cudaFree(c->d_Rexp); cudaFree(c->d_vacc); cudaFree(c->d_dacc); cudaFree(c->d_counters);
     cudaFree(c->d_hs); cudaFree(c->d_he); cudaFree(c->d_hb); cudaFree(c->d_hU); cudaFree(c->d_hv);
     cudaFree(c->d_hR); cudaFree(c->d_hmu); cudaFree(c->d_hmuout);
+    if (c->ev) {
+        for (int i = 0; i < 2 * kMaxProfEvents; i++)
+            if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+        delete[] c->ev;
+        c->ev = nullptr;
+    }
+    delete[] c->ev_kernel;
+    c->ev_kernel = nullptr;
 }
 
 struct DeviceGuard {
@@ -157,7 +165,48 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
         ctx->c.encaps_path = (int)value;
         return LWE_OK;
     }
+    if (option == LWE_OPT_PROFILE) {
+        Ctx *c = &ctx->c;
+        if (value != 0 && value != 1) return LWE_ERR_PARAM;
+        if (value && !c->ev) {
+            DeviceGuard guard(c->device);
+            c->ev = new (std::nothrow) cudaEvent_t[2 * kMaxProfEvents]();
+            c->ev_kernel = new (std::nothrow) uint8_t[kMaxProfEvents]();
+            if (!c->ev || !c->ev_kernel) return LWE_ERR_CUDA;
+            for (int i = 0; i < 2 * kMaxProfEvents; i++) LWE_CUDA_TRY(c, cudaEventCreate(&c->ev[i]));
+        }
+        c->profile = (int)value;
+        return LWE_OK;
+    }
     return LWE_ERR_PARAM;
+}
+
+int lwe_profile_reset(lwe_ctx *ctx)
+{
+    CHECK_CTX(ctx);
+    ctx->c.n_ev = 0;
+    return LWE_OK;
+}
+
+int lwe_profile_read(lwe_ctx *ctx, int kernel_id, double *h_total_ms, uint64_t *h_launches)
+{
+    CHECK_CTX(ctx);
+    if (kernel_id < 0 || kernel_id >= LWE_K_COUNT) return LWE_ERR_PARAM;
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    double total = 0.0;
+    uint64_t count = 0;
+    for (int i = 0; i < c->n_ev; i++) {
+        if (c->ev_kernel[i] != kernel_id) continue;
+        LWE_CUDA_TRY(c, cudaEventSynchronize(c->ev[2 * i + 1]));
+        float ms = 0.f;
+        LWE_CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev[2 * i], c->ev[2 * i + 1]));
+        total += ms;
+        count++;
+    }
+    if (h_total_ms) *h_total_ms = total;
+    if (h_launches) *h_launches = count;
+    return LWE_OK;
 }
 
 int lwe_rng_fill(lwe_ctx *ctx, void *d_out, size_t nbytes, const uint8_t key[16], const uint8_t iv[16],

@@ -80,6 +80,7 @@ cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, cons
     if (splits > max_splits) splits = max_splits;
     if (splits < 1) splits = 1;
     dim3 grid(splits, batch);
+    ProfScope prof(c, LWE_K_DECAPS, st);
     decaps_kernel<<<grid, kDecThreads, 0, st>>>(d_U, d_v, d_s, d_out, c->d_dacc, c->d_counters + 8, n, k, c->mq);
     c->launches++;
     return cudaGetLastError();

@@ -73,6 +73,7 @@ cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_
     if (splits > max_splits) splits = max_splits;
     if (splits < 1) splits = 1;
     dim3 grid(splits, batch);
+    ProfScope prof(c, LWE_K_EXPAND_R_V, st);
     expand_R_and_v_kernel<<<grid, kAuxThreads, 0, st>>>(d_b, d_Rbits, d_mubits, c->d_Rexp, d_v, c->d_vacc,
                                                         c->d_counters + 8 + c->p.max_batch, m, k,
                                                         batch * k, write_Rexp, c->mq);
@@ -123,6 +124,7 @@ cudaError_t launch_encaps_simt(Ctx *c, const uint16_t *d_A, const uint8_t *d_Rbi
 {
     const uint32_t m = c->p.m, n = c->p.n, k = c->p.k;
     dim3 grid((n + 31) / 32, k / 8, batch), block(32, 8);
+    ProfScope prof(c, LWE_K_ENCAPS_SIMT, st);
     encaps_simt_kernel<<<grid, block, 0, st>>>(d_A, d_Rbits, d_U, m, n, k, c->mq);
     c->launches++;
     return cudaGetLastError();

@@ -327,6 +327,7 @@ cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_
     if (err != cudaSuccess) return err;
     const uint32_t tiles = ((2 * p.n + kTileM - 1) / kTileM) * ((ncols + kTileN - 1) / kTileN);
     uint32_t grid = tiles < (uint32_t)c->sm_count ? tiles : (uint32_t)c->sm_count;
+    ProfScope prof(c, LWE_K_ENCAPS_TC, st);
     encaps_tc_kernel<<<grid, kThreads, kSmemBytes, st>>>(mapA, mapR, d_U, p.m, p.n, p.k, ncols, c->mq);
     c->launches++;
     return cudaGetLastError();

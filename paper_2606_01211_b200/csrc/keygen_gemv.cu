@@ -153,6 +153,7 @@ static cudaError_t launch_gemv(Ctx *c, const uint16_t *d_A, const AesKey &key, c
     uint32_t grid = (uint32_t)(c->sm_count * per_sm);
     uint32_t need = (m + kTeams - 1) / kTeams;
     if (grid > need) grid = need;
+    ProfScope prof(c, kRegen ? LWE_K_KEYGEN_REGEN : LWE_K_KEYGEN_STORED, st);
     kern<<<grid, kGemvThreads, smem, st>>>(d_A, key, c->d_te0, d_s, d_e, d_b, m, n, batch, c->mq);
     c->launches++;
     return cudaGetLastError();

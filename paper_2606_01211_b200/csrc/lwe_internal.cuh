@@ -80,6 +80,32 @@ struct Ctx {
 
     // driver entry point for TMA descriptors (resolved at create; no link-time libcuda)
     void *encode_tiled;
+
+    // per-kernel device timing (LWE_OPT_PROFILE): event pairs recorded around launches
+    int profile;
+    int n_ev;                                              // pairs used so far
+    cudaEvent_t *ev;                                       // [2 * kMaxProfEvents], created lazily
+    uint8_t *ev_kernel;                                    // kernel id of each pair
+};
+
+constexpr int kMaxProfEvents = 8192;
+
+// Brackets one kernel launch with CUDA events on the launching stream when profiling is on.
+struct ProfScope {
+    Ctx *c;
+    cudaStream_t st;
+    int slot;
+    ProfScope(Ctx *c_, int kernel_id, cudaStream_t st_) : c(c_), st(st_), slot(-1)
+    {
+        if (!c->profile || !c->ev || c->n_ev >= kMaxProfEvents) return;
+        slot = c->n_ev++;
+        c->ev_kernel[slot] = (uint8_t)kernel_id;
+        cudaEventRecord(c->ev[2 * slot], st);
+    }
+    ~ProfScope()
+    {
+        if (slot >= 0) cudaEventRecord(c->ev[2 * slot + 1], st);
+    }
 };
 
 #define LWE_CUDA_TRY(ctx, expr)                                   \
