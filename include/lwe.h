@@ -104,8 +104,9 @@ int lwe_sample_bits(lwe_ctx *ctx, uint8_t *d_out, uint64_t first_bit, uint64_t n
 
 /* ---- a3 / a3': KeyGen ------------------------------------------------------------
  * d_b[t][i] = ( sum_{j<n} A[i][j] * d_s[t][j] + d_e[t][i] ) mod q,  0 <= t < batch.
- * P:L60 eq.(1).  d_A: m x n row-major, read once per instance group,
- * streamed from HBM.  d_A == NULL: A is never read; every element is regenerated
+ * P:L60 eq.(1).  d_A: m x n row-major, streamed from HBM: once per call for
+ * batch >= 2 (all instances in one tensor-core GEMM, "many concurrent key
+ * exchanges"), as one HBM-bound GEMV for batch 1.  d_A == NULL: A is never read; every element is regenerated
  * inside the kernel from (seed_A, LWE_TAG_A, inst 0) exactly as lwe_sample_uniform
  * would produce it (the paper's on-demand A).  batch <= max_batch. */
 int lwe_keygen(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
@@ -149,15 +150,20 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
  *                      (LWE_ERR_UNSUPPORTED at call time if the shape does not fit).
  * LWE_OPT_PROFILE:     1 = bracket every kernel launch with a CUDA event pair on the
  *                      stream it is launched on (at most 8192 launches are kept between
- *                      resets; later ones are simply not timed); 0 = off (default). */
-enum { LWE_OPT_ENCAPS_PATH = 1, LWE_OPT_PROFILE = 2 };
+ *                      resets; later ones are simply not timed); 0 = off (default).
+ * LWE_OPT_GEMV_VARIANT: keygen GEMV launch shape, 0 = auto; 1/2 = a warp per row with 4/8 loads in
+ *                      flight per lane; 3/4 = a CTA per row with 4/2 loads per thread.  Same result.
+ * LWE_OPT_KEYGEN_PATH: stored-A keygen, 0 = auto (GEMV for batch 1, tensor-core skinny GEMM that reads A
+ *                      once for batch >= 2), 1 = force one GEMV per instance, 2 = force the tcgen05 GEMM
+ *                      (LWE_ERR_UNSUPPORTED if n > 32768 or 4*batch > 256). */
+enum { LWE_OPT_ENCAPS_PATH = 1, LWE_OPT_PROFILE = 2, LWE_OPT_GEMV_VARIANT = 3, LWE_OPT_KEYGEN_PATH = 4 };
 int lwe_set_option(lwe_ctx *ctx, int option, int64_t value);
 
 /* Kernel ids for lwe_profile_read (one per __global__ function of the library). */
 enum {
     LWE_K_RNG_FILL = 0, LWE_K_SAMPLE_UNIFORM = 1, LWE_K_SAMPLE_CBD = 2, LWE_K_SAMPLE_BITS = 3,
     LWE_K_KEYGEN_STORED = 4, LWE_K_KEYGEN_REGEN = 5, LWE_K_EXPAND_R_V = 6, LWE_K_ENCAPS_TC = 7,
-    LWE_K_ENCAPS_SIMT = 8, LWE_K_DECAPS = 9, LWE_K_COUNT = 10
+    LWE_K_ENCAPS_SIMT = 8, LWE_K_DECAPS = 9, LWE_K_KEYGEN_PREP = 10, LWE_K_KEYGEN_TC = 11, LWE_K_COUNT = 12
 };
 /* Sum of the device durations (milliseconds, CUDA events) and the number of timed launches
  * of kernel `kernel_id` since the last reset.  Waits for the recorded events to complete

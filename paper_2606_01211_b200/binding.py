@@ -20,8 +20,10 @@ ERRORS = {-1: "LWE_ERR_PARAM", -2: "LWE_ERR_ALIGN", -3: "LWE_ERR_NULLPTR", -4: "
 TAG_A, TAG_S, TAG_E, TAG_R, TAG_MU = 1, 2, 3, 4, 5
 OPT_ENCAPS_PATH = 1
 OPT_PROFILE = 2
+OPT_GEMV_VARIANT = 3
+OPT_KEYGEN_PATH = 4
 KERNELS = ["rng_fill", "sample_uniform", "sample_cbd", "sample_bits", "keygen_stored", "keygen_regen",
-           "expand_R_v", "encaps_tc", "encaps_simt", "decaps"]
+           "expand_R_v", "encaps_tc", "encaps_simt", "decaps", "keygen_prep", "keygen_tc"]
 
 EXPORTS = [
     "lwe_create", "lwe_destroy", "lwe_strerror", "lwe_last_cuda_error", "lwe_launch_count",

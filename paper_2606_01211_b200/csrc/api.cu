@@ -38,6 +38,7 @@ cudaError_t dev_alloc(T **p, size_t count)
 
 void free_all(Ctx *c)
 {
+    cudaFree(c->d_Sx);
     cudaFree(c->d_te0); cudaFree(c->d_Rexp); cudaFree(c->d_vacc); cudaFree(c->d_dacc); cudaFree(c->d_counters);
     cudaFree(c->d_hs); cudaFree(c->d_he); cudaFree(c->d_hb); cudaFree(c->d_hU); cudaFree(c->d_hv);
     cudaFree(c->d_hR); cudaFree(c->d_hmu); cudaFree(c->d_hmuout);
@@ -115,6 +116,7 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
     auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
     ok(dev_alloc(&c->d_te0, 256));
     ok(dev_alloc(&c->d_Rexp, m * k * B));
+    if (p->n <= 32768 && 4 * B <= 256) ok(dev_alloc(&c->d_Sx, keygen_tc_workspace_bytes(*p)));
     ok(dev_alloc(&c->d_vacc, k * B));
     ok(dev_alloc(&c->d_dacc, k * B));
     ok(dev_alloc(&c->d_counters, 8 + 2 * B));
@@ -163,6 +165,16 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
     if (option == LWE_OPT_ENCAPS_PATH) {
         if (value < 0 || value > 2) return LWE_ERR_PARAM;
         ctx->c.encaps_path = (int)value;
+        return LWE_OK;
+    }
+    if (option == LWE_OPT_KEYGEN_PATH) {
+        if (value < 0 || value > 2) return LWE_ERR_PARAM;
+        ctx->c.keygen_path = (int)value;
+        return LWE_OK;
+    }
+    if (option == LWE_OPT_GEMV_VARIANT) {
+        if (value < 0 || value > 4) return LWE_ERR_PARAM;
+        ctx->c.gemv_variant = (int)value;
         return LWE_OK;
     }
     if (option == LWE_OPT_PROFILE) {
@@ -279,8 +291,11 @@ int lwe_keygen(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_
     if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
     REQUIRE_PTR(d_s); REQUIRE_PTR(d_e); REQUIRE_PTR(d_b);
     REQUIRE_ALIGNED(d_A); REQUIRE_ALIGNED(d_s); REQUIRE_ALIGNED(d_e); REQUIRE_ALIGNED(d_b);
+    bool tcp = d_A && keygen_tc_supported(c, batch) && (c->keygen_path == 2 || (c->keygen_path == 0 && batch >= 2));
+    if (d_A && c->keygen_path == 2 && !tcp) return LWE_ERR_UNSUPPORTED;
     DeviceGuard guard(c->device);
-    if (d_A) LAUNCH(c, launch_keygen_stored(c, d_A, d_s, d_e, d_b, batch, (cudaStream_t)stream));
+    if (tcp) LAUNCH(c, launch_keygen_tc(c, d_A, d_s, d_e, d_b, batch, (cudaStream_t)stream));
+    else if (d_A) LAUNCH(c, launch_keygen_stored(c, d_A, d_s, d_e, d_b, batch, (cudaStream_t)stream));
     else LAUNCH(c, launch_keygen_regen(c, seed_key_host(seed_A), d_s, d_e, d_b, batch, (cudaStream_t)stream));
     return LWE_OK;
 }

@@ -42,9 +42,17 @@ decaps_kernel(const uint16_t *__restrict__ U, const uint16_t *__restrict__ v, co
             a[6] += (unsigned long long)((u.w & 0xffffu) * sj);
             a[7] += (unsigned long long)((u.w >> 16) * sj);
         }
+    }
+    // sum the row slots of the CTA in shared memory, then one atomic per column per CTA
+    __shared__ unsigned long long sCol[kDecThreads * 8];
 #pragma unroll
-        for (int x = 0; x < 8; x++)
-            if (a[x]) atomicAdd(acc + (size_t)t * k + 8 * cg + x, a[x]);
+    for (int x = 0; x < 8; x++) sCol[x * kDecThreads + threadIdx.x] = a[x];      // inactive threads hold zeros
+    __syncthreads();
+    for (uint32_t c = threadIdx.x; c < k; c += kDecThreads) {
+        const uint32_t ccg = c >> 3, x = c & 7;
+        unsigned long long sum = 0;
+        for (uint32_t rs = 0; rs < rows_per_iter; rs++) sum += sCol[x * kDecThreads + rs * tpr + ccg];
+        if (sum) atomicAdd(acc + (size_t)t * k + c, sum);
     }
     __threadfence();
     __syncthreads();
@@ -76,7 +84,7 @@ cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, cons
     const uint32_t n = c->p.n, k = c->p.k;
     const uint32_t rows_per_iter = kDecThreads / (k / 8);
     uint32_t splits = (uint32_t)((4 * c->sm_count + batch - 1) / batch);
-    uint32_t max_splits = (n + rows_per_iter - 1) / rows_per_iter;
+    uint32_t max_splits = (n + 4 * rows_per_iter - 1) / (4 * rows_per_iter);       // >= 4 row groups per CTA
     if (splits > max_splits) splits = max_splits;
     if (splits < 1) splits = 1;
     dim3 grid(splits, batch);

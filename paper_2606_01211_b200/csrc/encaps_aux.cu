@@ -36,17 +36,26 @@ expand_R_and_v_kernel(const uint16_t *__restrict__ b, const uint8_t *__restrict_
             uint32_t r = __ldg(Rt + (size_t)i * kb + cb);
             uint32_t bi = __ldg(bt + i);
             if (write_Rexp) {
-                // bit x of r -> byte x of the 8-byte output
-                uint32_t lo = (r & 1u) | ((r & 2u) << 7) | ((r & 4u) << 14) | ((r & 8u) << 21);
-                uint32_t hi = ((r >> 4) & 1u) | ((r & 0x20u) << 3) | ((r & 0x40u) << 10) | ((r & 0x80u) << 17);
+                // bit x of r -> byte x of the 8-byte output: (nibble * 0x00204081) & 0x01010101
+                uint32_t lo = ((r & 0xfu) * 0x00204081u) & 0x01010101u;
+                uint32_t hi = ((r >> 4) * 0x00204081u) & 0x01010101u;
                 *reinterpret_cast<uint2 *>(Rexp + (size_t)i * ld_exp + (size_t)t * k + 8 * cb) = make_uint2(lo, hi);
             }
 #pragma unroll
             for (int x = 0; x < 8; x++) a[x] += ((r >> x) & 1u) ? bi : 0u;
         }
+    }
+    // Block-level sum over the row slots (a CTA's total still fits 32 bits: <= 65535 * m), then
+    // ONE atomic per column per CTA instead of one per thread.
+    __shared__ uint32_t sCol[kAuxThreads * 8];
 #pragma unroll
-        for (int x = 0; x < 8; x++)
-            if (a[x]) atomicAdd(acc + (size_t)t * k + 8 * cb + x, (unsigned long long)a[x]);
+    for (int x = 0; x < 8; x++) sCol[x * kAuxThreads + threadIdx.x] = active ? a[x] : 0u;
+    __syncthreads();
+    for (uint32_t c = threadIdx.x; c < k; c += kAuxThreads) {
+        const uint32_t ccb = c >> 3, x = c & 7;
+        uint32_t sum = 0;
+        for (uint32_t rs = 0; rs < rows_per_iter; rs++) sum += sCol[x * kAuxThreads + rs * kb + ccb];
+        if (sum) atomicAdd(acc + (size_t)t * k + c, (unsigned long long)sum);
     }
     __threadfence();
     __syncthreads();
@@ -68,8 +77,8 @@ cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_
 {
     const uint32_t m = c->p.m, k = c->p.k;
     const uint32_t rows_per_iter = kAuxThreads / (k / 8);
-    uint32_t splits = (uint32_t)((8 * c->sm_count + batch - 1) / batch);
-    uint32_t max_splits = (m + rows_per_iter - 1) / rows_per_iter;
+    uint32_t splits = (uint32_t)((4 * c->sm_count + batch - 1) / batch);
+    uint32_t max_splits = (m + 4 * rows_per_iter - 1) / (4 * rows_per_iter);   // >= 4 row groups per CTA
     if (splits > max_splits) splits = max_splits;
     if (splits < 1) splits = 1;
     dim3 grid(splits, batch);

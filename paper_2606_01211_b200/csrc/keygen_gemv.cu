@@ -68,7 +68,7 @@ __device__ __forceinline__ uint64_t team_reduce(uint64_t v, uint64_t *sRed)
 // kRegen = false: A streamed from HBM.  kRegen = true: A never read, every 16-byte
 // chunk (8 elements) is one AES-CTR block of object (seed_A, LWE_TAG_A, inst 0)
 // (+ rejection attempts), S8(c) O4 -- the paper's on-demand A.
-template <int TPR, bool kRegen>
+template <int TPR, bool kRegen, int UNR>
 __global__ void __launch_bounds__(kGemvThreads)
 keygen_gemv_kernel(const uint16_t *__restrict__ A, AesKey key, const uint32_t *__restrict__ te0,
                    const uint16_t *__restrict__ s, const uint16_t *__restrict__ e, uint16_t *__restrict__ b,
@@ -100,10 +100,10 @@ keygen_gemv_kernel(const uint16_t *__restrict__ A, AesKey key, const uint32_t *_
             uint32_t lo = 0, hi = 0;
             const uint4 *Arow = reinterpret_cast<const uint4 *>(A + (size_t)i * n);
             uint32_t since = 0;
-            for (uint32_t c0 = tl; c0 < chunks; c0 += 4 * TPR) {
-                uint4 a[4];
+            for (uint32_t c0 = tl; c0 < chunks; c0 += UNR * TPR) {
+                uint4 a[UNR];
 #pragma unroll
-                for (int u = 0; u < 4; u++) {
+                for (int u = 0; u < UNR; u++) {
                     uint32_t c = c0 + u * TPR;
                     if (c < chunks) {
                         if (kRegen) a[u] = uniform_block(key, sTl, mq, LWE_TAG_A, 0, (uint64_t)i * chunks + c);
@@ -113,12 +113,12 @@ keygen_gemv_kernel(const uint16_t *__restrict__ A, AesKey key, const uint32_t *_
                     }
                 }
 #pragma unroll
-                for (int u = 0; u < 4; u++) {
+                for (int u = 0; u < UNR; u++) {
                     uint32_t c = c0 + u * TPR;
                     uint4 sw = (c < chunks) ? sS4[c] : make_uint4(0, 0, 0, 0);
                     dot8(a[u], sw, lo, hi);
                 }
-                since += 4;
+                since += UNR;
                 if (!mq.pow2 && since >= kFlushEvery) {
                     sum_lo += lo; sum_hi += hi; lo = 0; hi = 0; since = 0;
                 }
@@ -136,19 +136,26 @@ keygen_gemv_kernel(const uint16_t *__restrict__ A, AesKey key, const uint32_t *_
     }
 }
 
-template <int TPR, bool kRegen>
+template <int TPR, bool kRegen, int UNR>
 static cudaError_t launch_gemv(Ctx *c, const uint16_t *d_A, const AesKey &key, const uint16_t *d_s,
                                const uint16_t *d_e, uint16_t *d_b, uint32_t batch, cudaStream_t st)
 {
     const uint32_t n = c->p.n, m = c->p.m;
     size_t smem = 2 * (size_t)n + 64 + (kRegen ? kAesTableBytes : 0);
-    auto kern = keygen_gemv_kernel<TPR, kRegen>;
-    cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    int per_sm = 0;
-    err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kGemvThreads, smem);
-    if (err != cudaSuccess) return err;
-    if (per_sm < 1) per_sm = 1;
+    auto kern = keygen_gemv_kernel<TPR, kRegen, UNR>;
+    // attribute + occupancy are queried once per (instantiation, smem size): host calls, not per launch
+    static size_t cached_smem = 0;
+    static int cached_per_sm = 0;
+    if (cached_smem != smem) {
+        cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (err != cudaSuccess) return err;
+        int q = 0;
+        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&q, kern, kGemvThreads, smem);
+        if (err != cudaSuccess) return err;
+        cached_per_sm = q < 1 ? 1 : q;
+        cached_smem = smem;
+    }
+    const int per_sm = cached_per_sm;
     constexpr int kTeams = kGemvThreads / TPR;
     uint32_t grid = (uint32_t)(c->sm_count * per_sm);
     uint32_t need = (m + kTeams - 1) / kTeams;
@@ -163,15 +170,21 @@ cudaError_t launch_keygen_stored(Ctx *c, const uint16_t *d_A, const uint16_t *d_
                                  uint16_t *d_b, uint32_t batch, cudaStream_t st)
 {
     AesKey none = {};
-    if (c->p.n >= 4096) return launch_gemv<kGemvThreads, false>(c, d_A, none, d_s, d_e, d_b, batch, st);
-    return launch_gemv<32, false>(c, d_A, none, d_s, d_e, d_b, batch, st);
+    int v = c->gemv_variant;
+    if (v == 0) v = (c->p.n >= 2048) ? 2 : 1;          // measured on B200: a warp per row, 8 x 16 B in flight per lane
+    switch (v) {
+    case 1: return launch_gemv<32, false, 4>(c, d_A, none, d_s, d_e, d_b, batch, st);
+    case 2: return launch_gemv<32, false, 8>(c, d_A, none, d_s, d_e, d_b, batch, st);
+    case 4: return launch_gemv<kGemvThreads, false, 2>(c, d_A, none, d_s, d_e, d_b, batch, st);
+    default: return launch_gemv<kGemvThreads, false, 4>(c, d_A, none, d_s, d_e, d_b, batch, st);
+    }
 }
 
 cudaError_t launch_keygen_regen(Ctx *c, const AesKey &key, const uint16_t *d_s, const uint16_t *d_e,
                                 uint16_t *d_b, uint32_t batch, cudaStream_t st)
 {
-    if (c->p.n >= 4096) return launch_gemv<kGemvThreads, true>(c, nullptr, key, d_s, d_e, d_b, batch, st);
-    return launch_gemv<32, true>(c, nullptr, key, d_s, d_e, d_b, batch, st);
+    if (c->p.n >= 4096) return launch_gemv<kGemvThreads, true, 4>(c, nullptr, key, d_s, d_e, d_b, batch, st);
+    return launch_gemv<32, true, 4>(c, nullptr, key, d_s, d_e, d_b, batch, st);
 }
 
 }  // namespace lwe

@@ -65,12 +65,15 @@ struct Ctx {
     int last_cuda_error;
     uint64_t launches;
     int encaps_path;                  // LWE_OPT_ENCAPS_PATH
+    int gemv_variant;                 // LWE_OPT_GEMV_VARIANT
+    int keygen_path;                  // LWE_OPT_KEYGEN_PATH
 
     // device tables
     uint32_t *d_te0;                  // 256-entry AES T-table (word = 2S | S<<8 | S<<16 | 3S<<24)
 
     // workspace (allocated once in lwe_create)
     uint8_t *d_Rexp;                  // [m][max_batch*k] u8 in {0,1}: B operand of the encaps GEMM
+    uint8_t *d_Sx;                    // [4*max_batch rounded to 16][2n] u8: B operand of the batched keygen GEMM
     unsigned long long *d_vacc;       // [max_batch*k] u64 partial sums of b^T R
     unsigned long long *d_dacc;       // [max_batch*k] u64 partial sums of U^T s
     unsigned int *d_counters;         // [8 + max_batch] self-resetting "last block" tickets
@@ -136,6 +139,10 @@ cudaError_t launch_sample_bits(Ctx *c, uint8_t *d_out, uint64_t first_bit, uint6
                                cudaStream_t st);
 cudaError_t launch_keygen_stored(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, const uint16_t *d_e,
                                  uint16_t *d_b, uint32_t batch, cudaStream_t st);
+size_t keygen_tc_workspace_bytes(const lwe_params &p);
+bool keygen_tc_supported(const Ctx *c, uint32_t batch);
+cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, const uint16_t *d_e, uint16_t *d_b,
+                             uint32_t batch, cudaStream_t st);
 cudaError_t launch_keygen_regen(Ctx *c, const AesKey &key, const uint16_t *d_s, const uint16_t *d_e,
                                 uint16_t *d_b, uint32_t batch, cudaStream_t st);
 cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_Rbits,

@@ -43,6 +43,47 @@ def test_keygen_stored_matches_oracle(H, m, n, q, batch):
         assert np.array_equal(got[t], O.keygen(A, s[t], e[t], q)), (m, n, q, t)
 
 
+KEYGEN_TC_SHAPES = [  # (m, n, q, batch): forced tcgen05 skinny GEMM (reads A once for the whole batch)
+    (512, 256, 65536, 1), (512, 256, 65536, 4), (264, 4096, 65521, 5), (136, 4104, 65521, 2), (1000, 40, 65521, 3),
+    (8, 8, 17, 1), (2048, 1024, 65536, 32), (640, 520, 3329, 33), (384, 1024, 65521, 64), (16384, 8192, 65536, 32),
+]
+
+
+@pytest.mark.parametrize("m,n,q,batch", KEYGEN_TC_SHAPES)
+def test_keygen_tensor_core_batched_matches_oracle_and_gemv(H, m, n, q, batch):
+    A = W.random_u16((m, n), q, 11)
+    s = W.random_u16((batch, n), q, 12)
+    e = W.random_u16((batch, m), q, 13)
+    with B().Context(n, m, 256, q, 4, batch) as c:
+        dA, ds, de = H.dev(A), H.dev(s), H.dev(e)
+        b_tc, b_gemv = H.dev_empty_u16(batch, m), H.dev_empty_u16(batch, m)
+        b_tc.fill_(-1)
+        c.set_option(B().OPT_KEYGEN_PATH, 2)
+        c.keygen(dA, 0, ds, de, b_tc, batch)
+        c.set_option(B().OPT_KEYGEN_PATH, 1)
+        c.keygen(dA, 0, ds, de, b_gemv, batch)
+        g_tc, g_gemv = H.host_u16(b_tc), H.host_u16(b_gemv)
+    assert np.array_equal(g_tc, g_gemv)
+    check = range(batch) if m * n <= (1 << 22) else (0, batch // 2, batch - 1)   # the oracle is slow: sample instances
+    for t in check:
+        assert np.array_equal(g_tc[t], O.keygen(A, s[t], e[t], q)), (m, n, q, t)
+
+
+def test_keygen_tensor_core_extreme_values(H):
+    # every byte product and all four plane accumulators at their maxima (n = 32768 is the path's limit)
+    for q in (65536, 65521):
+        m, n, batch = 128, 32768, 2
+        A = np.full((m, n), 0xFFFF if q == 65536 else q - 1, np.uint16)
+        s = np.full((batch, n), 0xFFFF if q == 65536 else q - 1, np.uint16)
+        e = np.full((batch, m), q - 1, np.uint16)
+        with B().Context(n, m, 256, q, 4, batch) as c:
+            b = H.dev_empty_u16(batch, m)
+            c.set_option(B().OPT_KEYGEN_PATH, 2)
+            c.keygen(H.dev(A), 0, H.dev(s), H.dev(e), b, batch)
+            a0 = int(A[0, 0])
+            assert np.all(H.host_u16(b) == (n * a0 * a0 + (q - 1)) % q)
+
+
 def test_keygen_extreme_values(H):
     # every product and every partial sum at its maximum (P9)
     for q in (65536, 65521):
