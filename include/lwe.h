@@ -146,8 +146,10 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
                  uint16_t *h_v, uint8_t *h_mubits_out, uint32_t batch, void *stream);
 
 /* ---- tuning / test / measurement hooks (no new semantics) --------------------------
- * LWE_OPT_ENCAPS_PATH: 0 = auto, 1 = force CUDA-core kernel, 2 = force tcgen05 GEMM
- *                      (LWE_ERR_UNSUPPORTED at call time if the shape does not fit).
+ * LWE_OPT_ENCAPS_PATH: 0 = auto (tcgen05 GEMM on CTA pairs where the shape fits, else CUDA cores),
+ *                      1 = force the CUDA-core kernel, 2 = force the single-CTA tcgen05 GEMM
+ *                      (cta_group::1), 3 = force the CTA-pair tcgen05 GEMM (cta_group::2);
+ *                      2 / 3 give LWE_ERR_UNSUPPORTED at call time if the shape does not fit.
  * LWE_OPT_PROFILE:     1 = bracket every kernel launch with a CUDA event pair on the
  *                      stream it is launched on (at most 8192 launches are kept between
  *                      resets; later ones are simply not timed); 0 = off (default).

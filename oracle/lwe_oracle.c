@@ -241,6 +241,29 @@ void orc_sample_uniform(uint16_t *out, uint64_t first, uint64_t count,
     }
 }
 
+/* O4 on the elements first, first+stride, first+2*stride, ...: element by element, straight from
+ * the definition (one stream word per attempt).  Used to draw a COLUMN of the row-major A
+ * (first = j, stride = n) at sizes where A itself is too big to draw on a CPU. */
+void orc_sample_uniform_strided(uint16_t *out, uint64_t first, uint64_t stride, uint64_t count,
+                                uint64_t seed, uint32_t tag, uint32_t inst, uint32_t q)
+{
+    uint8_t key[16], rk[176];
+    sbox_init();
+    orc_seed_key(seed, key);
+    aes128_expand_key(key, rk);
+    const uint32_t T = q * (65536u / q);
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (uint64_t r = 0; r < count; r++) {
+        const uint64_t t = first + r * stride;
+        uint32_t c = stream_word16(rk, tag, 0, inst, t);
+        for (uint32_t attempt = 1; c >= T; attempt++)
+            c = stream_word16(rk, tag, attempt, inst, t);
+        out[r] = (uint16_t)(c % q);
+    }
+}
+
 /* ------------------------------------------------------------------ O5: CBD */
 
 static int popcount16(unsigned w)

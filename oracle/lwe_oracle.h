@@ -60,6 +60,11 @@ void orc_object_iv(uint32_t tag, uint32_t attempt, uint32_t inst, uint8_t iv[16]
 void orc_sample_uniform(uint16_t *out, uint64_t first, uint64_t count,
                         uint64_t seed, uint32_t tag, uint32_t inst, uint32_t q);
 
+/* O4 on elements first + r*stride, 0 <= r < count (e.g. column j of the row-major m x n matrix A:
+ * first = j, stride = n, count = m).  Same values orc_sample_uniform gives at those positions. */
+void orc_sample_uniform_strided(uint16_t *out, uint64_t first, uint64_t stride, uint64_t count,
+                                uint64_t seed, uint32_t tag, uint32_t inst, uint32_t q);
+
 /* O5. Centred binomial eta in [1,8], element t: w = LE16(bytes [2t,2t+1] of
  * KS(key(seed), iv(tag,0,inst))); x = popcount(w & M) - popcount((w>>8) & M),
  * M = 2^eta - 1; stored as x mod q.  P:L70, P:L170, P:L320 (FIPS 203 CBD). */

@@ -16,7 +16,7 @@ TAG_A, TAG_S, TAG_E, TAG_R, TAG_MU = 1, 2, 3, 4, 5
 __all__ = [
     "TAG_A", "TAG_S", "TAG_E", "TAG_R", "TAG_MU",
     "aes128_encrypt_block", "ctr_bytes", "seed_key", "object_iv",
-    "sample_uniform", "sample_cbd", "sample_bits",
+    "sample_uniform", "sample_uniform_strided", "sample_cbd", "sample_bits",
     "keygen", "encaps", "encaps_rows", "encaps_v", "decaps", "num_threads",
     "cbd_from_word", "round_bit",
 ]
@@ -35,6 +35,7 @@ def _L():
         lib.orc_seed_key.argtypes = [u64, u8p]
         lib.orc_object_iv.argtypes = [u32, u32, u32, u8p]
         lib.orc_sample_uniform.argtypes = [u16p, u64, u64, u64, u32, u32, u32]
+        lib.orc_sample_uniform_strided.argtypes = [u16p, u64, u64, u64, u64, u32, u32, u32]
         lib.orc_sample_cbd.argtypes = [u16p, u64, u64, u64, u32, u32, u32, u32]
         lib.orc_sample_bits.argtypes = [u8p, u64, u64, u64, u32, u32]
         lib.orc_keygen.argtypes = [u16p, u16p, u16p, u16p, u32, u32, u32]
@@ -48,7 +49,7 @@ def _L():
         lib.orc_round_bit.argtypes = [u32, u32]
         lib.orc_round_bit.restype = C.c_uint32
         for f in ("orc_aes128_encrypt_block", "orc_ctr_bytes", "orc_seed_key", "orc_object_iv",
-                  "orc_sample_uniform", "orc_sample_cbd", "orc_sample_bits", "orc_keygen",
+                  "orc_sample_uniform", "orc_sample_uniform_strided", "orc_sample_cbd", "orc_sample_bits", "orc_keygen",
                   "orc_encaps", "orc_encaps_rows", "orc_encaps_v", "orc_decaps"):
             getattr(lib, f).restype = None
         _lib = lib
@@ -100,6 +101,12 @@ def object_iv(tag: int, attempt: int, inst: int) -> bytes:
 def sample_uniform(first: int, count: int, seed: int, tag: int, inst: int, q: int) -> np.ndarray:
     out = np.zeros(count, np.uint16)
     _L().orc_sample_uniform(_p(out, C.c_uint16), first, count, seed, tag, inst, q)
+    return out
+
+
+def sample_uniform_strided(first: int, stride: int, count: int, seed: int, tag: int, inst: int, q: int) -> np.ndarray:
+    out = np.zeros(count, np.uint16)
+    _L().orc_sample_uniform_strided(_p(out, C.c_uint16), first, stride, count, seed, tag, inst, q)
     return out
 
 

@@ -163,7 +163,7 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
 {
     CHECK_CTX(ctx);
     if (option == LWE_OPT_ENCAPS_PATH) {
-        if (value < 0 || value > 2) return LWE_ERR_PARAM;
+        if (value < 0 || value > 3) return LWE_ERR_PARAM;
         ctx->c.encaps_path = (int)value;
         return LWE_OK;
     }
@@ -313,11 +313,15 @@ int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_
     REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v);
     bool tc = encaps_tc_supported(c, batch);
     if (c->encaps_path == 1) tc = false;
-    if (c->encaps_path == 2 && !tc) return LWE_ERR_UNSUPPORTED;
+    if (c->encaps_path >= 2 && !tc) return LWE_ERR_UNSUPPORTED;
+    // CTA pairs (cta_group::2) by default; path 2 keeps the single-CTA kernel selectable
+    const bool pair = tc && c->encaps_path != 2 && encaps_tc2_supported(c, batch);
+    if (c->encaps_path == 3 && !pair) return LWE_ERR_UNSUPPORTED;
     DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
     LAUNCH(c, launch_expand_R_and_v(c, d_b, d_Rbits, d_mubits, d_v, batch, tc, st));
-    if (tc) LAUNCH(c, launch_encaps_tc(c, d_A, d_U, batch, st));
+    if (pair) LAUNCH(c, launch_encaps_tc2(c, d_A, d_U, batch, st));
+    else if (tc) LAUNCH(c, launch_encaps_tc(c, d_A, d_U, batch, st));
     else LAUNCH(c, launch_encaps_simt(c, d_A, d_Rbits, d_U, batch, st));
     return LWE_OK;
 }

@@ -1,0 +1,225 @@
+// encaps_tc2.cu -- a4 on CTA pairs: the same GEMM as encaps_tc.cu (D[2n x N] = A8^T . Rexp,
+// u8 x u8 -> s32, U = (D_even + 256 D_odd) mod q, BJ north_star (3)) issued as
+// tcgen05.mma.cta_group::2.
+//
+// Why a second kernel.  With cta_group::1 every SM stages its own copy of the 256-column R tile:
+// per 128-deep K block 16 KB of A and 32 KB of R cross L2 -> shared memory, and the tensor pipe
+// reads 96 B/clk of shared memory while TMA writes another 96 B/clk.  A CTA pair on one TPC splits
+// the N dimension of the B operand between its two SMs (each loads 128 of the 256 columns) while
+// each keeps its own 128 rows of A: 32 KB per K block and SM instead of 48 KB, i.e. one third less
+// L2->SM and shared-memory traffic for the same MMA rate.  ncu on the cta_group::1 kernel showed the
+// tensor pipe 84 % active with DRAM at 20 %: the feed, not HBM, was the limit.
+//
+// Shape.  Persistent, grid = SM count, clusters of 2.  Pair tile: 256 byte-rows of D (= 128 columns
+// of A) x 256 columns (= one instance at k = 256); each CTA owns 128 byte-rows, accumulated in its
+// own TMEM (two 256-column accumulators, so the epilogue of tile t overlaps the MMAs of tile t+1).
+// K block 128, 6-stage ring of 32 KB.
+//   warp 0 : TMA producer (both CTAs; completion bytes of both land on the LEADER's full barrier)
+//   warp 1 : TMEM alloc (both CTAs) + MMA issuer (leader CTA only, one lane)
+//   warps 2-5 : epilogue on the CTA's own TMEM lanes, as in encaps_tc.cu
+// Barriers: full[s] lives on the leader (1 arrival + 64 KB of transaction bytes); empty[s] and
+// tmem_full[a] exist in both CTAs and are signalled by multicast tcgen05.commit; tmem_empty[a]
+// lives on the leader and collects the 8 epilogue warps of the pair.
+#include "tc_common.cuh"
+
+namespace lwe {
+
+namespace {
+
+using namespace tc;
+
+constexpr uint32_t kCtaM = 128;                  // byte-rows of D per CTA
+constexpr uint32_t kPairM = 2 * kCtaM;           // per pair
+constexpr uint32_t kTileN = 256;
+constexpr uint32_t kHalfN = kTileN / 2;          // columns of R staged by each CTA
+constexpr uint32_t kTileK = 128;
+constexpr uint32_t kStages = 6;
+constexpr uint32_t kBytesA = kCtaM * kTileK;     // 16 KB
+constexpr uint32_t kBytesB = kHalfN * kTileK;    // 16 KB
+constexpr uint32_t kBytesStage = kBytesA + kBytesB;
+constexpr uint32_t kThreads = 192;
+constexpr uint32_t kTmemCols = 512;
+constexpr uint32_t kSmemBytes = kStages * kBytesStage + 1024 /*align*/ + 256 /*barriers*/;
+
+constexpr uint32_t kInstrDesc = instr_desc_u8(kPairM, kTileN, true, true);
+
+struct PairSched {
+    uint32_t m_tiles, n_tiles, total;
+    __device__ __forceinline__ void coords(uint32_t t, uint32_t &mt, uint32_t &nt) const
+    {
+        // groups of 8 n-tiles, n fastest inside a group: pairs running together share A strips and
+        // the group's R panels stay in L2 (same order as the cta_group::1 kernel)
+        const uint32_t g = 8;
+        uint32_t per_group = m_tiles * g;
+        uint32_t grp = t / per_group, r = t - grp * per_group;
+        uint32_t width = (n_tiles - grp * g) < g ? (n_tiles - grp * g) : g;
+        mt = r / width;
+        nt = grp * g + (r - mt * width);
+    }
+};
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
+                  uint16_t *__restrict__ U, uint32_t m, uint32_t n, uint32_t k, uint32_t ncols_total, ModQ mq)
+{
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = smem_u32(smem_raw);
+    const uint32_t base = (raw + 1023u) & ~1023u;
+    const uint32_t bars = base + kStages * kBytesStage;
+    auto full_bar = [&](uint32_t s) { return bars + 8 * s; };
+    auto empty_bar = [&](uint32_t s) { return bars + 8 * (kStages + s); };
+    auto tfull_bar = [&](uint32_t a) { return bars + 8 * (2 * kStages + a); };
+    auto tempty_bar = [&](uint32_t a) { return bars + 8 * (2 * kStages + 2 + a); };
+    const uint32_t tmem_slot = bars + 8 * (2 * kStages + 4);
+    volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
+
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();                     // 0 = leader
+    const uint32_t pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+
+    PairSched sched;
+    sched.m_tiles = (2 * n + kPairM - 1) / kPairM;
+    sched.n_tiles = (ncols_total + kTileN - 1) / kTileN;
+    sched.total = sched.m_tiles * sched.n_tiles;
+    const uint32_t k_blocks = (m + kTileK - 1) / kTileK;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapR) : "memory");
+        for (uint32_t s = 0; s < kStages; s++) {
+            mbar_init(full_bar(s), 1);                            // the leader's expect_tx arrival
+            mbar_init(empty_bar(s), 1);                           // one multicast commit
+        }
+        for (uint32_t a = 0; a < 2; a++) {
+            mbar_init(tfull_bar(a), 1);
+            mbar_init(tempty_bar(a), 8);                          // 4 epilogue warps of each CTA
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) tmem_alloc_pair(tmem_slot, kTmemCols);
+    tc_fence_before();
+    cluster_sync_all();                                           // barriers of BOTH CTAs are initialised
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===================== TMA producer (both CTAs) =====================
+        if (lane == 0) {
+            uint32_t stage = 0, phase = 0;
+            for (uint32_t t = pair; t < sched.total; t += n_pairs) {
+                uint32_t mt, nt;
+                sched.coords(t, mt, nt);
+                const int32_t a_col = (int32_t)(mt * kPairM + rank * kCtaM);
+                const int32_t r_col = (int32_t)(nt * kTileN + rank * kHalfN);
+                for (uint32_t kb = 0; kb < k_blocks; kb++) {
+                    mbar_wait(empty_bar(stage), phase ^ 1);
+                    const uint32_t sa = base + stage * kBytesStage;
+                    const uint32_t lead_full = map_to_cta(full_bar(stage), 0);
+                    if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * kBytesStage);   // both CTAs' bytes
+                    const int32_t row = (int32_t)(kb * kTileK);
+                    tma_load_2d_pair(sa, &mapA, lead_full, a_col, row);
+                    tma_load_2d_pair(sa + kBytesA, &mapR, lead_full, r_col, row);
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer (leader CTA) =====================
+        if (rank == 0 && lane == 0) {
+            uint32_t stage = 0, phase = 0, it = 0;
+            for (uint32_t t = pair; t < sched.total; t += n_pairs, it++) {
+                const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
+                mbar_wait(tempty_bar(acc), acc_phase ^ 1);          // both epilogues drained this accumulator
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + acc * kTileN;
+                for (uint32_t kb = 0; kb < k_blocks; kb++) {
+                    mbar_wait(full_bar(stage), phase);
+                    tc_fence_after();
+                    const uint32_t sa = base + stage * kBytesStage;
+                    const uint32_t sb = sa + kBytesA;
+#pragma unroll
+                    for (uint32_t ks = 0; ks < kTileK / kUmmaK; ks++) {
+                        uint64_t adesc = make_desc_mn_sw128(sa + ks * kUmmaK * 128, 0, 1024);
+                        uint64_t bdesc = make_desc_mn_sw128(sb + ks * kUmmaK * 128, 0, 1024);
+                        umma_i8_pair(d_tmem, adesc, bdesc, kInstrDesc, (kb | ks) ? 1u : 0u);
+                    }
+                    umma_commit_pair(empty_bar(stage), 0x3);        // frees the slot in both CTAs
+                    if (kb == k_blocks - 1) umma_commit_pair(tfull_bar(acc), 0x3);
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else {
+        // ===================== epilogue (warps 2..5, both CTAs) =====================
+        const uint32_t quarter = warp & 3;
+        const uint32_t lead_tempty0 = map_to_cta(tempty_bar(0), 0), lead_tempty1 = map_to_cta(tempty_bar(1), 0);
+        uint32_t it = 0;
+        for (uint32_t t = pair; t < sched.total; t += n_pairs, it++) {
+            uint32_t mt, nt;
+            sched.coords(t, mt, nt);
+            const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
+            mbar_wait(tfull_bar(acc), acc_phase);
+            tc_fence_after();
+            const uint32_t brow = mt * kPairM + rank * kCtaM + quarter * 32 + lane;   // byte-row of D
+            const uint32_t j = brow >> 1;
+            const bool odd = lane & 1;
+            const uint32_t taddr = tmem_base + ((quarter * 32) << 16) + acc * kTileN;
+#pragma unroll 1
+            for (uint32_t cb = 0; cb < kTileN; cb += 32) {
+                uint32_t r[32];
+                tmem_ld_32x32b_x32(taddr + cb, r);
+                tmem_ld_wait();
+                uint32_t o[16];
+#pragma unroll
+                for (int x = 0; x < 16; x++) {
+                    uint32_t send = odd ? r[x] : r[16 + x];
+                    uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 1);
+                    uint32_t val = odd ? (recv + (r[16 + x] << 8)) : (r[x] + (recv << 8));
+                    o[x] = mq.pow2 ? (val & mq.mask) : mod_u32(val, mq);
+                }
+                const uint32_t col = nt * kTileN + cb + (odd ? 16u : 0u);
+                if (j < n && col < ncols_total) {
+                    const uint32_t inst = col / k, c = col - inst * k;
+                    uint4 *dst = reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c);
+                    dst[0] = make_uint4(o[0] | (o[1] << 16), o[2] | (o[3] << 16), o[4] | (o[5] << 16), o[6] | (o[7] << 16));
+                    dst[1] = make_uint4(o[8] | (o[9] << 16), o[10] | (o[11] << 16), o[12] | (o[13] << 16), o[14] | (o[15] << 16));
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(acc ? lead_tempty1 : lead_tempty0);
+        }
+    }
+
+    // no CTA of the pair may leave (or free TMEM) while its partner can still signal it or read its smem
+    tc_fence_before();
+    cluster_sync_all();
+    if (warp == 1) tmem_dealloc_pair(tmem_base, kTmemCols);
+}
+
+}  // namespace
+
+bool encaps_tc2_supported(const Ctx *c, uint32_t batch)
+{
+    return encaps_tc_supported(c, batch) && c->sm_count >= 2;
+}
+
+cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st)
+{
+    const lwe_params &p = c->p;
+    const uint32_t ncols = batch * p.k;
+    CUtensorMap mapA, mapR;
+    if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, p.m, kTileK)) return cudaErrorInvalidValue;
+    if (!make_map_u8(c, &mapR, c->d_Rexp, ncols, p.m, kTileK)) return cudaErrorInvalidValue;
+    cudaError_t err = cudaFuncSetAttribute(encaps_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (err != cudaSuccess) return err;
+    const uint32_t tiles = ((2 * p.n + kPairM - 1) / kPairM) * ((ncols + kTileN - 1) / kTileN);
+    uint32_t pairs = (uint32_t)c->sm_count / 2;
+    if (pairs > tiles) pairs = tiles;
+    ProfScope prof(c, LWE_K_ENCAPS_TC, st);
+    encaps_tc2_kernel<<<2 * pairs, kThreads, kSmemBytes, st>>>(mapA, mapR, d_U, p.m, p.n, p.k, ncols, c->mq);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace lwe

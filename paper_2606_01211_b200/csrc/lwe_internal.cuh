@@ -152,6 +152,8 @@ cudaError_t launch_encaps_simt(Ctx *c, const uint16_t *d_A, const uint8_t *d_Rbi
                                uint32_t batch, cudaStream_t st);
 bool encaps_tc_supported(const Ctx *c, uint32_t batch);
 cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st);
+bool encaps_tc2_supported(const Ctx *c, uint32_t batch);
+cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st);
 cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
                           uint8_t *d_out, uint32_t batch, cudaStream_t st);
 

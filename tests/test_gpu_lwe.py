@@ -126,6 +126,8 @@ ENCAPS_SHAPES = [  # (m, n, k, q, batch)
     (136, 64, 128, 65536, 3),         # k = 128: N tile straddles instances, ragged N tail (384 cols)
     (128, 64, 16, 17, 2),             # 32 columns in total
     (2048, 1024, 256, 65536, 1),      # C2
+    (1160, 456, 256, 65521, 5),       # 10 K blocks (> ring depth) with a tail, 4 pair tiles (last ragged), 5 N tiles
+    (384, 1280, 256, 65536, 2),       # 10 pair tiles x 2: more tiles than a wave of small grids, both accumulators reused
 ]
 
 
@@ -138,7 +140,10 @@ def run_encaps(H, path, m, n, k, q, batch, A, b, Rbits, mubits):
         return H.host_u16(U), H.host_u16(v)
 
 
-@pytest.mark.parametrize("path", [2, 1], ids=["tcgen05", "simt"])
+ENCAPS_PATHS = dict(argvalues=[3, 2, 1], ids=["tcgen05_pair", "tcgen05", "simt"])
+
+
+@pytest.mark.parametrize("path", **ENCAPS_PATHS)
 @pytest.mark.parametrize("m,n,k,q,batch", ENCAPS_SHAPES)
 def test_encaps_matches_oracle(H, path, m, n, k, q, batch):
     A = W.random_u16((m, n), q, 21)
@@ -154,7 +159,7 @@ def test_encaps_matches_oracle(H, path, m, n, k, q, batch):
                                f"got {U[t][tuple(bad[0])]} want {Uo[tuple(bad[0])]}")
 
 
-@pytest.mark.parametrize("path", [2, 1], ids=["tcgen05", "simt"])
+@pytest.mark.parametrize("path", **ENCAPS_PATHS)
 def test_encaps_extreme_accumulators(H, path):
     # P9: A = q-1 (or 65535), R = all ones, m = 65536 -> both byte-plane accumulators and the
     # recombined 32-bit value hit their bounds exactly
@@ -169,7 +174,8 @@ def test_encaps_extreme_accumulators(H, path):
         assert np.all(v == (m * (q - 1) + q // 2) % q)
 
 
-def test_encaps_one_hot_R_picks_a_row_of_A(H):
+@pytest.mark.parametrize("path", [3, 2], ids=["tcgen05_pair", "tcgen05"])
+def test_encaps_one_hot_R_picks_a_row_of_A(H, path):
     m, n, k, q = 256, 128, 256, 65521
     A = W.random_u16((m, n), q, 31)
     b = W.random_u16((1, m), q, 32)
@@ -178,7 +184,7 @@ def test_encaps_one_hot_R_picks_a_row_of_A(H):
     R[5, 0] = 1
     Rbits = np.packbits(R.ravel(), bitorder="little")[None, :]
     mubits = np.zeros((1, k // 8), np.uint8)
-    U, v = run_encaps(H, 2, m, n, k, q, 1, A, b, Rbits, mubits)
+    U, v = run_encaps(H, path, m, n, k, q, 1, A, b, Rbits, mubits)
     assert np.array_equal(U[0][:, 200], A[77]) and np.array_equal(U[0][:, 0], A[5])
     assert int(v[0][200]) == int(b[0][77]) and int(v[0][0]) == int(b[0][5])
     U[0][:, 200] = 0
