@@ -157,8 +157,11 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
  *                      flight per lane; 3/4 = a CTA per row with 4/2 loads per thread.  Same result.
  * LWE_OPT_KEYGEN_PATH: stored-A keygen, 0 = auto (GEMV for batch 1, tensor-core skinny GEMM that reads A
  *                      once for batch >= 2), 1 = force one GEMV per instance, 2 = force the tcgen05 GEMM
- *                      (LWE_ERR_UNSUPPORTED if n > 32768 or 4*batch > 256). */
-enum { LWE_OPT_ENCAPS_PATH = 1, LWE_OPT_PROFILE = 2, LWE_OPT_GEMV_VARIANT = 3, LWE_OPT_KEYGEN_PATH = 4 };
+ *                      (LWE_ERR_UNSUPPORTED if n > 32768 or 4*batch > 256).
+ * LWE_OPT_TUNE:        launch-shape knob of the tensor-core kernels for measurements (tile order, L2
+ *                      eviction policy of the operand streams, ring depth); 0 = default.  Same result
+ *                      for every value. */
+enum { LWE_OPT_ENCAPS_PATH = 1, LWE_OPT_PROFILE = 2, LWE_OPT_GEMV_VARIANT = 3, LWE_OPT_KEYGEN_PATH = 4, LWE_OPT_TUNE = 5 };
 int lwe_set_option(lwe_ctx *ctx, int option, int64_t value);
 
 /* Kernel ids for lwe_profile_read (one per __global__ function of the library). */

@@ -22,6 +22,7 @@ OPT_ENCAPS_PATH = 1
 OPT_PROFILE = 2
 OPT_GEMV_VARIANT = 3
 OPT_KEYGEN_PATH = 4
+OPT_TUNE = 5
 KERNELS = ["rng_fill", "sample_uniform", "sample_cbd", "sample_bits", "keygen_stored", "keygen_regen",
            "expand_R_v", "encaps_tc", "encaps_simt", "decaps", "keygen_prep", "keygen_tc"]
 

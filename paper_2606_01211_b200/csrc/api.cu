@@ -177,6 +177,11 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
         ctx->c.gemv_variant = (int)value;
         return LWE_OK;
     }
+    if (option == LWE_OPT_TUNE) {
+        if (value < 0 || value > 0xffff) return LWE_ERR_PARAM;
+        ctx->c.tune = (int)value;
+        return LWE_OK;
+    }
     if (option == LWE_OPT_PROFILE) {
         Ctx *c = &ctx->c;
         if (value != 0 && value != 1) return LWE_ERR_PARAM;

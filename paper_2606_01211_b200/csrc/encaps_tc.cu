@@ -74,7 +74,7 @@ encaps_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     const uint32_t tmem_slot = bars + 8 * (2 * kStages + 4);
     volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
 
-    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;   // warp-uniform
 
     TileSched sched;
     sched.m_tiles = (2 * n + kTileM - 1) / kTileM;
@@ -101,51 +101,55 @@ encaps_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
+    // warp-convergent role loops, one elected lane around the issue (see encaps_tc2.cu)
     if (warp == 0) {
         // ===================== TMA producer =====================
-        if (lane == 0) {
-            uint32_t stage = 0, phase = 0;
-            for (uint32_t t = blockIdx.x; t < sched.total; t += gridDim.x) {
-                uint32_t mt, nt;
-                sched.coords(t, mt, nt);
-                const int32_t a_col = (int32_t)(mt * kTileM), r_col = (int32_t)(nt * kTileN);
-                for (uint32_t kb = 0; kb < k_blocks; kb++) {
-                    mbar_wait(empty_bar(stage), phase ^ 1);
-                    const uint32_t sa = base + stage * kBytesStage;
+        uint32_t stage = 0, phase = 0;
+        for (uint32_t t = blockIdx.x; t < sched.total; t += gridDim.x) {
+            uint32_t mt, nt;
+            sched.coords(t, mt, nt);
+            const int32_t a_col = (int32_t)(mt * kTileM), r_col = (int32_t)(nt * kTileN);
+            for (uint32_t kb = 0; kb < k_blocks; kb++) {
+                mbar_wait(empty_bar(stage), phase ^ 1);
+                const uint32_t sa = base + stage * kBytesStage;
+                const int32_t row = (int32_t)(kb * kTileK);
+                if (elect_one()) {
                     mbar_expect_tx(full_bar(stage), kBytesStage);
-                    const int32_t row = (int32_t)(kb * kTileK);
                     tma_load_2d(sa, &mapA, full_bar(stage), a_col, row);
                     tma_load_2d(sa + kBytesA, &mapR, full_bar(stage), r_col, row);
                     tma_load_2d(sa + kBytesA + kBytesBHalf, &mapR, full_bar(stage), r_col + 128, row);
-                    if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
+                __syncwarp();
+                if (++stage == kStages) { stage = 0; phase ^= 1; }
             }
         }
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
-        if (lane == 0) {
-            uint32_t stage = 0, phase = 0, it = 0;
-            for (uint32_t t = blockIdx.x; t < sched.total; t += gridDim.x, it++) {
-                const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
-                mbar_wait(tempty_bar(acc), acc_phase ^ 1);          // epilogue has drained this accumulator
+        uint32_t stage = 0, phase = 0, it = 0;
+        for (uint32_t t = blockIdx.x; t < sched.total; t += gridDim.x, it++) {
+            const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
+            mbar_wait(tempty_bar(acc), acc_phase ^ 1);          // epilogue has drained this accumulator
+            tc_fence_after();
+            const uint32_t d_tmem = tmem_base + acc * kTileN;
+            for (uint32_t kb = 0; kb < k_blocks; kb++) {
+                mbar_wait(full_bar(stage), phase);
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + acc * kTileN;
-                for (uint32_t kb = 0; kb < k_blocks; kb++) {
-                    mbar_wait(full_bar(stage), phase);
-                    tc_fence_after();
-                    const uint32_t sa = base + stage * kBytesStage;
-                    const uint32_t sb = sa + kBytesA;
+                const uint32_t sa = base + stage * kBytesStage;
+                if (elect_one()) {
+                    // K step = 32 rows of 128 bytes = 4 KB in both operands: one add on the address field
+                    uint64_t adesc = make_desc_mn_sw128(sa, 0, 1024);
+                    uint64_t bdesc = make_desc_mn_sw128(sa + kBytesA, kBytesBHalf, 1024);
 #pragma unroll
                     for (uint32_t ks = 0; ks < kTileK / kUmmaK; ks++) {
-                        // K step = 32 rows of 128 bytes = 4 KB in both operands
-                        uint64_t adesc = make_desc_mn_sw128(sa + ks * kUmmaK * 128, 0, 1024);
-                        uint64_t bdesc = make_desc_mn_sw128(sb + ks * kUmmaK * 128, kBytesBHalf, 1024);
                         umma_i8(d_tmem, adesc, bdesc, kInstrDesc, (kb | ks) ? 1u : 0u);
+                        adesc += (kUmmaK * 128) >> 4;
+                        bdesc += (kUmmaK * 128) >> 4;
                     }
                     umma_commit(empty_bar(stage));                  // smem slot free once these MMAs retire
                     if (kb == k_blocks - 1) umma_commit(tfull_bar(acc));
-                    if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
+                __syncwarp();
+                if (++stage == kStages) { stage = 0; phase ^= 1; }
             }
         }
     } else {

@@ -32,24 +32,17 @@ constexpr uint32_t kCtaM = 128;                  // byte-rows of D per CTA
 constexpr uint32_t kPairM = 2 * kCtaM;           // per pair
 constexpr uint32_t kTileN = 256;
 constexpr uint32_t kHalfN = kTileN / 2;          // columns of R staged by each CTA
-constexpr uint32_t kTileK = 128;
-constexpr uint32_t kStages = 6;
-constexpr uint32_t kBytesA = kCtaM * kTileK;     // 16 KB
-constexpr uint32_t kBytesB = kHalfN * kTileK;    // 16 KB
-constexpr uint32_t kBytesStage = kBytesA + kBytesB;
 constexpr uint32_t kThreads = 192;
 constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kSmemBytes = kStages * kBytesStage + 1024 /*align*/ + 256 /*barriers*/;
 
 constexpr uint32_t kInstrDesc = instr_desc_u8(kPairM, kTileN, true, true);
 
 struct PairSched {
-    uint32_t m_tiles, n_tiles, total;
+    uint32_t m_tiles, n_tiles, total, g;
     __device__ __forceinline__ void coords(uint32_t t, uint32_t &mt, uint32_t &nt) const
     {
-        // groups of 8 n-tiles, n fastest inside a group: pairs running together share A strips and
+        // groups of g n-tiles, n fastest inside a group: pairs running together share A strips and
         // the group's R panels stay in L2 (same order as the cta_group::1 kernel)
-        const uint32_t g = 8;
         uint32_t per_group = m_tiles * g;
         uint32_t grp = t / per_group, r = t - grp * per_group;
         uint32_t width = (n_tiles - grp * g) < g ? (n_tiles - grp * g) : g;
@@ -58,10 +51,40 @@ struct PairSched {
     }
 };
 
+// L2 eviction policy for a TMA stream: 0 = normal, 1 = evict_first, 2 = evict_last
+__device__ __forceinline__ uint64_t l2_policy(uint32_t kind)
+{
+    uint64_t pol;
+    if (kind == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    else if (kind == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void tma_load_2d_pair_hint(uint32_t dst, const CUtensorMap *map, uint32_t cluster_bar,
+                                                      int32_t c0, int32_t c1, uint64_t pol)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%3, %4}], [%2], %5;"
+        ::"r"(dst), "l"(map), "r"(cluster_bar), "r"(c0), "r"(c1), "l"(pol) : "memory");
+}
+
+template <uint32_t kStages, uint32_t kTileK>
+struct PairCfg {
+    static constexpr uint32_t kBytesA = kCtaM * kTileK;
+    static constexpr uint32_t kBytesB = kHalfN * kTileK;
+    static constexpr uint32_t kBytesStage = kBytesA + kBytesB;
+    static constexpr uint32_t kSmemBytes = kStages * kBytesStage + 1024 /*align*/ + 256 /*barriers*/;
+};
+
+template <uint32_t kStages, uint32_t kTileK>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
-                  uint16_t *__restrict__ U, uint32_t m, uint32_t n, uint32_t k, uint32_t ncols_total, ModQ mq)
+                  uint16_t *__restrict__ U, uint32_t m, uint32_t n, uint32_t k, uint32_t ncols_total, ModQ mq,
+                  uint32_t group_w, uint32_t polA_kind, uint32_t polR_kind)
 {
+    using Cfg = PairCfg<kStages, kTileK>;
+    constexpr uint32_t kBytesA = Cfg::kBytesA, kBytesStage = Cfg::kBytesStage;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t base = (raw + 1023u) & ~1023u;
@@ -73,11 +96,12 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
     const uint32_t tmem_slot = bars + 8 * (2 * kStages + 4);
     volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
 
-    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;   // warp-uniform
     const uint32_t rank = cluster_ctarank();                     // 0 = leader
     const uint32_t pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
 
     PairSched sched;
+    sched.g = group_w;
     sched.m_tiles = (2 * n + kPairM - 1) / kPairM;
     sched.n_tiles = (ncols_total + kTileN - 1) / kTileN;
     sched.total = sched.m_tiles * sched.n_tiles;
@@ -102,30 +126,37 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
+    // The producer and MMA roles run WARP-CONVERGENT loops and elect one lane only around the
+    // instructions that must be issued once: inside a divergent `if (lane == 0)` region the compiler
+    // cannot keep descriptors and barrier addresses in uniform registers and wraps every TMA / MMA /
+    // commit in an ELECT + R2UR + vote loop (~130 SASS instructions per K block, which made the
+    // issuing thread, not the tensor pipe, the bottleneck: ncu source page, profiles/r1b_*).
     if (warp == 0) {
         // ===================== TMA producer (both CTAs) =====================
-        if (lane == 0) {
-            uint32_t stage = 0, phase = 0;
-            for (uint32_t t = pair; t < sched.total; t += n_pairs) {
-                uint32_t mt, nt;
-                sched.coords(t, mt, nt);
-                const int32_t a_col = (int32_t)(mt * kPairM + rank * kCtaM);
-                const int32_t r_col = (int32_t)(nt * kTileN + rank * kHalfN);
-                for (uint32_t kb = 0; kb < k_blocks; kb++) {
-                    mbar_wait(empty_bar(stage), phase ^ 1);
-                    const uint32_t sa = base + stage * kBytesStage;
-                    const uint32_t lead_full = map_to_cta(full_bar(stage), 0);
+        uint32_t stage = 0, phase = 0;
+        const uint64_t polA = l2_policy(polA_kind), polR = l2_policy(polR_kind);
+        for (uint32_t t = pair; t < sched.total; t += n_pairs) {
+            uint32_t mt, nt;
+            sched.coords(t, mt, nt);
+            const int32_t a_col = (int32_t)(mt * kPairM + rank * kCtaM);
+            const int32_t r_col = (int32_t)(nt * kTileN + rank * kHalfN);
+            for (uint32_t kb = 0; kb < k_blocks; kb++) {
+                mbar_wait(empty_bar(stage), phase ^ 1);
+                const uint32_t sa = base + stage * kBytesStage;
+                const uint32_t lead_full = map_to_cta(full_bar(stage), 0);
+                const int32_t row = (int32_t)(kb * kTileK);
+                if (elect_one()) {
                     if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * kBytesStage);   // both CTAs' bytes
-                    const int32_t row = (int32_t)(kb * kTileK);
-                    tma_load_2d_pair(sa, &mapA, lead_full, a_col, row);
-                    tma_load_2d_pair(sa + kBytesA, &mapR, lead_full, r_col, row);
-                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                    tma_load_2d_pair_hint(sa, &mapA, lead_full, a_col, row, polA);
+                    tma_load_2d_pair_hint(sa + kBytesA, &mapR, lead_full, r_col, row, polR);
                 }
+                __syncwarp();
+                if (++stage == kStages) { stage = 0; phase ^= 1; }
             }
         }
     } else if (warp == 1) {
         // ===================== MMA issuer (leader CTA) =====================
-        if (rank == 0 && lane == 0) {
+        if (rank == 0) {
             uint32_t stage = 0, phase = 0, it = 0;
             for (uint32_t t = pair; t < sched.total; t += n_pairs, it++) {
                 const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
@@ -136,15 +167,20 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                     mbar_wait(full_bar(stage), phase);
                     tc_fence_after();
                     const uint32_t sa = base + stage * kBytesStage;
-                    const uint32_t sb = sa + kBytesA;
+                    if (elect_one()) {
+                        // descriptors differ only in the 14-bit start-address field: one add per MMA
+                        uint64_t adesc = make_desc_mn_sw128(sa, 0, 1024);
+                        uint64_t bdesc = make_desc_mn_sw128(sa + kBytesA, 0, 1024);
 #pragma unroll
-                    for (uint32_t ks = 0; ks < kTileK / kUmmaK; ks++) {
-                        uint64_t adesc = make_desc_mn_sw128(sa + ks * kUmmaK * 128, 0, 1024);
-                        uint64_t bdesc = make_desc_mn_sw128(sb + ks * kUmmaK * 128, 0, 1024);
-                        umma_i8_pair(d_tmem, adesc, bdesc, kInstrDesc, (kb | ks) ? 1u : 0u);
+                        for (uint32_t ks = 0; ks < kTileK / kUmmaK; ks++) {
+                            umma_i8_pair(d_tmem, adesc, bdesc, kInstrDesc, (kb | ks) ? 1u : 0u);
+                            adesc += (kUmmaK * 128) >> 4;
+                            bdesc += (kUmmaK * 128) >> 4;
+                        }
+                        umma_commit_pair(empty_bar(stage), 0x3);    // frees the slot in both CTAs
+                        if (kb == k_blocks - 1) umma_commit_pair(tfull_bar(acc), 0x3);
                     }
-                    umma_commit_pair(empty_bar(stage), 0x3);        // frees the slot in both CTAs
-                    if (kb == k_blocks - 1) umma_commit_pair(tfull_bar(acc), 0x3);
+                    __syncwarp();
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
             }
@@ -204,22 +240,40 @@ bool encaps_tc2_supported(const Ctx *c, uint32_t batch)
     return encaps_tc_supported(c, batch) && c->sm_count >= 2;
 }
 
-cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st)
+template <uint32_t kStages, uint32_t kTileK>
+static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st)
 {
+    using Cfg = PairCfg<kStages, kTileK>;
     const lwe_params &p = c->p;
     const uint32_t ncols = batch * p.k;
     CUtensorMap mapA, mapR;
     if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, p.m, kTileK)) return cudaErrorInvalidValue;
     if (!make_map_u8(c, &mapR, c->d_Rexp, ncols, p.m, kTileK)) return cudaErrorInvalidValue;
-    cudaError_t err = cudaFuncSetAttribute(encaps_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    auto kern = encaps_tc2_kernel<kStages, kTileK>;
+    cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes);
     if (err != cudaSuccess) return err;
     const uint32_t tiles = ((2 * p.n + kPairM - 1) / kPairM) * ((ncols + kTileN - 1) / kTileN);
     uint32_t pairs = (uint32_t)c->sm_count / 2;
     if (pairs > tiles) pairs = tiles;
+    // LWE_OPT_TUNE (experiments only): bits 0-3 log2 of the n-tile group width (0 = default 8),
+    // bits 4-5 / 6-7 L2 policy of the A / R streams, bits 8-9 ring variant
+    const uint32_t tune = (uint32_t)c->tune;
+    const uint32_t gw = (tune & 15u) ? (1u << ((tune & 15u) - 1)) : 8u;
     ProfScope prof(c, LWE_K_ENCAPS_TC, st);
-    encaps_tc2_kernel<<<2 * pairs, kThreads, kSmemBytes, st>>>(mapA, mapR, d_U, p.m, p.n, p.k, ncols, c->mq);
+    kern<<<2 * pairs, kThreads, Cfg::kSmemBytes, st>>>(mapA, mapR, d_U, p.m, p.n, p.k, ncols, c->mq, gw,
+                                                       (tune >> 4) & 3u, (tune >> 6) & 3u);
     c->launches++;
     return cudaGetLastError();
+}
+
+cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st)
+{
+    switch ((c->tune >> 8) & 3) {
+    case 1: return launch_pair<7, 128>(c, d_A, d_U, batch, st);
+    case 2: return launch_pair<12, 64>(c, d_A, d_U, batch, st);
+    case 3: return launch_pair<3, 256>(c, d_A, d_U, batch, st);
+    default: return launch_pair<6, 128>(c, d_A, d_U, batch, st);
+    }
 }
 
 }  // namespace lwe

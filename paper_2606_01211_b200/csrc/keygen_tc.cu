@@ -71,7 +71,7 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     const uint32_t tmem_slot = bars + 8 * (2 * kMaxStages + 4);
     volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
 
-    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;   // warp-uniform
     const uint32_t strips = (m + kTileM - 1) / kTileM;
     const uint32_t k_blocks = (2 * n + kTileK - 1) / kTileK;
     const uint32_t acc_cols = (N <= 32) ? 32 : (N <= 64) ? 64 : (N <= 128) ? 128 : 256;   // per accumulator
@@ -96,47 +96,51 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
+    // warp-convergent role loops, one elected lane around the issue (see encaps_tc2.cu)
     if (warp == 0) {
-        if (lane == 0) {
-            uint32_t stage = 0, phase = 0;
-            for (uint32_t t = blockIdx.x; t < strips; t += gridDim.x) {
-                const int32_t row0 = (int32_t)(t * kTileM);
-                for (uint32_t kb = 0; kb < k_blocks; kb++) {
-                    mbar_wait(empty_bar(stage), phase ^ 1);
-                    const uint32_t sa = base + stage * bytes_stage;
+        uint32_t stage = 0, phase = 0;
+        for (uint32_t t = blockIdx.x; t < strips; t += gridDim.x) {
+            const int32_t row0 = (int32_t)(t * kTileM);
+            for (uint32_t kb = 0; kb < k_blocks; kb++) {
+                mbar_wait(empty_bar(stage), phase ^ 1);
+                const uint32_t sa = base + stage * bytes_stage;
+                const int32_t k0 = (int32_t)(kb * kTileK);
+                if (elect_one()) {
                     mbar_expect_tx(full_bar(stage), bytes_stage);
-                    const int32_t k0 = (int32_t)(kb * kTileK);
                     tma_load_2d(sa, &mapA, full_bar(stage), k0, row0);          // 128 rows x 128 bytes of k'
                     tma_load_2d(sa + kBytesA, &mapS, full_bar(stage), k0, 0);   // N rows x 128 bytes of k'
-                    if (++stage == stages) { stage = 0; phase ^= 1; }
                 }
+                __syncwarp();
+                if (++stage == stages) { stage = 0; phase ^= 1; }
             }
         }
     } else if (warp == 1) {
-        if (lane == 0) {
-            const uint32_t idesc = instr_desc_u8(kTileM, N, false, false);      // both operands K-major
-            uint32_t stage = 0, phase = 0, it = 0;
-            for (uint32_t t = blockIdx.x; t < strips; t += gridDim.x, it++) {
-                const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
-                mbar_wait(tempty_bar(acc), acc_phase ^ 1);
+        const uint32_t idesc = instr_desc_u8(kTileM, N, false, false);      // both operands K-major
+        uint32_t stage = 0, phase = 0, it = 0;
+        for (uint32_t t = blockIdx.x; t < strips; t += gridDim.x, it++) {
+            const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
+            mbar_wait(tempty_bar(acc), acc_phase ^ 1);
+            tc_fence_after();
+            const uint32_t d_tmem = tmem_base + acc * acc_cols;
+            for (uint32_t kb = 0; kb < k_blocks; kb++) {
+                mbar_wait(full_bar(stage), phase);
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + acc * acc_cols;
-                for (uint32_t kb = 0; kb < k_blocks; kb++) {
-                    mbar_wait(full_bar(stage), phase);
-                    tc_fence_after();
-                    const uint32_t sa = base + stage * bytes_stage;
-                    const uint32_t sb = sa + kBytesA;
+                const uint32_t sa = base + stage * bytes_stage;
+                if (elect_one()) {
+                    // a K step is 32 bytes along the 128-byte swizzled row: advance the start address
+                    uint64_t adesc = make_desc_k_sw128(sa, 1024);
+                    uint64_t bdesc = make_desc_k_sw128(sa + kBytesA, 1024);
 #pragma unroll
                     for (uint32_t ks = 0; ks < kTileK / kUmmaK; ks++) {
-                        // a K step is 32 bytes along the 128-byte swizzled row: advance the start address
-                        uint64_t adesc = make_desc_k_sw128(sa + ks * kUmmaK, 1024);
-                        uint64_t bdesc = make_desc_k_sw128(sb + ks * kUmmaK, 1024);
                         umma_i8(d_tmem, adesc, bdesc, idesc, (kb | ks) ? 1u : 0u);
+                        adesc += kUmmaK >> 4;
+                        bdesc += kUmmaK >> 4;
                     }
                     umma_commit(empty_bar(stage));
                     if (kb == k_blocks - 1) umma_commit(tfull_bar(acc));
-                    if (++stage == stages) { stage = 0; phase ^= 1; }
                 }
+                __syncwarp();
+                if (++stage == stages) { stage = 0; phase ^= 1; }
             }
         }
     } else {

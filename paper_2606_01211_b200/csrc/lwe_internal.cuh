@@ -67,6 +67,7 @@ struct Ctx {
     int encaps_path;                  // LWE_OPT_ENCAPS_PATH
     int gemv_variant;                 // LWE_OPT_GEMV_VARIANT
     int keygen_path;                  // LWE_OPT_KEYGEN_PATH
+    int tune;                         // LWE_OPT_TUNE: launch-shape experiments, no semantic effect
 
     // device tables
     uint32_t *d_te0;                  // 256-entry AES T-table (word = 2S | S<<8 | S<<16 | 3S<<24)

@@ -42,6 +42,28 @@ def test_p4_any_subrange_equals_slice():
         assert np.array_equal(O.sample_uniform(first, count, 3, O.TAG_A, 0, 65521), full[first:first + count])
 
 
+@pytest.mark.parametrize("q", [65536, 65521, 40000, 17])
+def test_p4_strided_draw_is_the_openssl_stream_at_those_positions(q):
+    # a column of a row-major matrix: elements first + r*stride, re-derived through OpenSSL with an
+    # independent walk over the attempt streams (not through orc_sample_uniform)
+    first, stride, count = 5, 37, 700
+    pos = first + stride * np.arange(count)
+    N = int(pos[-1]) + 1
+    T = q * (65536 // q)
+    want = np.zeros(count, np.uint32)
+    pending = np.arange(count)
+    a = 0
+    while pending.size:
+        c = words(7, O.TAG_A, a, 0, N)[pos[pending]]
+        ok = c < T
+        want[pending[ok]] = c[ok] % q
+        pending = pending[~ok]
+        a += 1
+    got = O.sample_uniform_strided(first, stride, count, 7, O.TAG_A, 0, q)
+    assert np.array_equal(got, want)
+    assert np.array_equal(got, O.sample_uniform(0, N, 7, O.TAG_A, 0, q)[pos])
+
+
 @pytest.mark.parametrize("q", [3, 17, 251, 40000, 65521])
 def test_p4_rejection_follows_attempt_streams(q):
     N = 1 << 15
