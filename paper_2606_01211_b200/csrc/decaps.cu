@@ -12,6 +12,28 @@ namespace lwe {
 
 constexpr int kDecThreads = 256;
 
+__device__ __forceinline__ uint4 ldg_stream16(const uint4 *p)
+{
+    uint4 r;                                             // not volatile: read-only data, free to hoist
+    asm("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+        : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
+// acc += x * y with a 32 x 32 -> 64 bit multiply-add (one IMAD.WIDE)
+__device__ __forceinline__ void mad_wide(unsigned long long &acc, uint32_t x, uint32_t y)
+{
+    asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc) : "r"(x), "r"(y));
+}
+
+__device__ __forceinline__ void accumulate_row(unsigned long long (&a)[8], const uint4 &u, uint32_t sj)
+{
+    mad_wide(a[0], u.x & 0xffffu, sj); mad_wide(a[1], u.x >> 16, sj);
+    mad_wide(a[2], u.y & 0xffffu, sj); mad_wide(a[3], u.y >> 16, sj);
+    mad_wide(a[4], u.z & 0xffffu, sj); mad_wide(a[5], u.z >> 16, sj);
+    mad_wide(a[6], u.w & 0xffffu, sj); mad_wide(a[7], u.w >> 16, sj);
+}
+
 __global__ void __launch_bounds__(kDecThreads)
 decaps_kernel(const uint16_t *__restrict__ U, const uint16_t *__restrict__ v, const uint16_t *__restrict__ s,
               uint8_t *__restrict__ out, unsigned long long *__restrict__ acc, unsigned int *__restrict__ tickets,
@@ -30,18 +52,27 @@ decaps_kernel(const uint16_t *__restrict__ U, const uint16_t *__restrict__ v, co
 #pragma unroll
     for (int x = 0; x < 8; x++) a[x] = 0;
     if (active) {
-        for (uint32_t j = blockIdx.x * rows_per_iter + rslot; j < n; j += gridDim.x * rows_per_iter) {
-            uint4 u = __ldg(reinterpret_cast<const uint4 *>(Ut + (size_t)j * k) + cg);
-            uint32_t sj = __ldg(st + j);
-            a[0] += (unsigned long long)((u.x & 0xffffu) * sj);
-            a[1] += (unsigned long long)((u.x >> 16) * sj);
-            a[2] += (unsigned long long)((u.y & 0xffffu) * sj);
-            a[3] += (unsigned long long)((u.y >> 16) * sj);
-            a[4] += (unsigned long long)((u.z & 0xffffu) * sj);
-            a[5] += (unsigned long long)((u.z >> 16) * sj);
-            a[6] += (unsigned long long)((u.w & 0xffffu) * sj);
-            a[7] += (unsigned long long)((u.w >> 16) * sj);
+        // a CTA streams one contiguous range of rows; 4 independent 16-byte loads in flight per thread:
+        // the pass is HBM-bound (2nk bytes of U)
+        constexpr int kUnroll = 4;
+        const uint32_t per_cta = ((n + gridDim.x - 1) / gridDim.x + rows_per_iter - 1) / rows_per_iter * rows_per_iter;
+        const uint32_t jbeg = blockIdx.x * per_cta, jend = min(n, jbeg + per_cta);
+        const size_t row_u4 = k / 8;                      // uint4 per row
+        uint32_t j = jbeg + rslot;
+        const uint4 *up = reinterpret_cast<const uint4 *>(Ut) + (size_t)j * row_u4 + cg;
+        const size_t ustep = (size_t)rows_per_iter * row_u4;
+        for (; j + (kUnroll - 1) * rows_per_iter < jend; j += kUnroll * rows_per_iter, up += kUnroll * ustep) {
+            uint4 u[kUnroll];
+            uint32_t sj[kUnroll];
+#pragma unroll
+            for (int r = 0; r < kUnroll; r++) {
+                u[r] = ldg_stream16(up + r * ustep);
+                sj[r] = __ldg(st + j + r * rows_per_iter);
+            }
+#pragma unroll
+            for (int r = 0; r < kUnroll; r++) accumulate_row(a, u[r], sj[r]);
         }
+        for (; j < jend; j += rows_per_iter, up += ustep) accumulate_row(a, ldg_stream16(up), __ldg(st + j));
     }
     // sum the row slots of the CTA in shared memory, then one atomic per column per CTA
     __shared__ unsigned long long sCol[kDecThreads * 8];
@@ -60,20 +91,24 @@ decaps_kernel(const uint16_t *__restrict__ U, const uint16_t *__restrict__ v, co
     __syncthreads();
     if (!sLast) return;
     __threadfence();
-    // finalize: k columns, 8 per thread-iteration -> one output byte
-    for (uint32_t byte = threadIdx.x; byte < k / 8; byte += kDecThreads) {
-        uint32_t bits = 0;
-        for (uint32_t x = 0; x < 8; x++) {
-            uint32_t c = 8 * byte + x;
+    // finalize: one column per thread, a warp's 32 decisions packed by ballot (4 output bytes)
+    for (uint32_t c0 = 0; c0 < k; c0 += kDecThreads) {
+        const uint32_t c = c0 + threadIdx.x;
+        uint32_t bit = 0;
+        if (c < k) {
             unsigned long long sum = __ldcg(acc + (size_t)t * k + c);
             acc[(size_t)t * k + c] = 0;
             uint32_t us = mod_u64(sum, mq);
             uint32_t d = (uint32_t)v[(size_t)t * k + c] + mq.q - us;
             if (d >= mq.q) d -= mq.q;
-            uint32_t bit = (uint32_t)(((4ull * d + mq.q) / (2ull * mq.q)) & 1ull);
-            bits |= bit << x;
+            bit = (4u * d + mq.q) / (2u * mq.q) & 1u;            // d < q <= 65536: fits 32 bits
         }
-        out[(size_t)t * (k / 8) + byte] = (uint8_t)bits;
+        const uint32_t word = __ballot_sync(0xffffffffu, bit);
+        if ((threadIdx.x & 31) == 0) {
+            const uint32_t cw = c0 + (threadIdx.x & ~31u);          // first column of this warp
+            for (uint32_t by = 0; by < 4 && cw + 8 * by < k; by++)
+                out[(size_t)t * (k / 8) + cw / 8 + by] = (uint8_t)(word >> (8 * by));
+        }
     }
     if (threadIdx.x == 0) tickets[t] = 0;
 }
@@ -83,7 +118,7 @@ cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, cons
 {
     const uint32_t n = c->p.n, k = c->p.k;
     const uint32_t rows_per_iter = kDecThreads / (k / 8);
-    uint32_t splits = (uint32_t)((4 * c->sm_count + batch - 1) / batch);
+    uint32_t splits = (uint32_t)((8 * c->sm_count + batch - 1) / batch);
     uint32_t max_splits = (n + 4 * rows_per_iter - 1) / (4 * rows_per_iter);       // >= 4 row groups per CTA
     if (splits > max_splits) splits = max_splits;
     if (splits < 1) splits = 1;

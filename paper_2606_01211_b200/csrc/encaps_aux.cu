@@ -72,17 +72,120 @@ expand_R_and_v_kernel(const uint16_t *__restrict__ b, const uint8_t *__restrict_
     if (threadIdx.x == 0) tickets[t] = 0;
 }
 
+// Fast path for k = 32 * 2^j: a thread owns one 32-bit word of R bits (32 columns) of a row, so a warp
+// reads 128 contiguous bytes of bits and writes 32-byte pieces that tile whole 128-byte lines of Rexp
+// (HBM-bound: 1 bit in, 1 byte out).  Its 32 column sums sit in registers over all the rows it visits;
+// lanes and warps holding the same word column meet in shared memory, CTAs in the u64 global
+// accumulators, and the last CTA of the instance (ticket) reduces mod q and writes v.
+template <bool kWriteRexp>
+__global__ void __launch_bounds__(kAuxThreads)
+expand_R_and_v_w32_kernel(const uint16_t *__restrict__ b, const uint8_t *__restrict__ Rbits,
+                          const uint8_t *__restrict__ mubits, uint8_t *__restrict__ Rexp, uint16_t *__restrict__ v,
+                          unsigned long long *__restrict__ acc, unsigned int *__restrict__ tickets,
+                          uint32_t m, uint32_t k, uint32_t ld_exp, ModQ mq)
+{
+    __shared__ uint32_t sLast;
+    extern __shared__ uint32_t sSum[];                        // k column sums of this CTA (<= 65535 * m < 2^32)
+    const uint32_t t = blockIdx.y;
+    const uint32_t wpr = k / 32;                              // words per row, a power of two <= 64
+    const uint32_t w = threadIdx.x & (wpr - 1);               // my word column
+    const uint32_t rows_per_iter = kAuxThreads / wpr;
+    const uint32_t rslot = threadIdx.x / wpr;
+    const uint32_t *Rt = reinterpret_cast<const uint32_t *>(Rbits + (size_t)t * m * (k / 8));
+    const uint16_t *bt = b + (size_t)t * m;
+    for (uint32_t c = threadIdx.x; c < k; c += kAuxThreads) sSum[c] = 0;
+    __syncthreads();
+
+    uint32_t a[32];                                           // <= 65535 * rows visited (<= 65536) < 2^32
+#pragma unroll
+    for (int x = 0; x < 32; x++) a[x] = 0;
+    constexpr int kUnroll = 4;
+    // a CTA streams one contiguous range of rows
+    const uint32_t step = rows_per_iter;
+    const uint32_t per_cta = ((m + gridDim.x - 1) / gridDim.x + rows_per_iter - 1) / rows_per_iter * rows_per_iter;
+    const uint32_t ibeg = blockIdx.x * per_cta, iend = min(m, ibeg + per_cta);
+    for (uint32_t i0 = ibeg + rslot; i0 < iend; i0 += kUnroll * step) {
+        uint32_t r[kUnroll], bi[kUnroll];
+#pragma unroll
+        for (int u = 0; u < kUnroll; u++) {
+            const uint32_t i = i0 + u * step;
+            r[u] = (i < iend) ? __ldg(Rt + (size_t)i * wpr + w) : 0u;
+            bi[u] = (i < iend) ? (uint32_t)__ldg(bt + i) : 0u;
+        }
+#pragma unroll
+        for (int u = 0; u < kUnroll; u++) {
+            const uint32_t i = i0 + u * step;
+            if (kWriteRexp && i < iend) {
+                // bit x of a nibble -> byte x of a word: (nibble * 0x00204081) & 0x01010101
+                uint32_t o[8];
+#pragma unroll
+                for (int h = 0; h < 8; h++) o[h] = (((r[u] >> (4 * h)) & 0xfu) * 0x00204081u) & 0x01010101u;
+                uint4 *dst = reinterpret_cast<uint4 *>(Rexp + (size_t)i * ld_exp + (size_t)t * k + 32 * w);
+                dst[0] = make_uint4(o[0], o[1], o[2], o[3]);
+                dst[1] = make_uint4(o[4], o[5], o[6], o[7]);
+            }
+#pragma unroll
+            for (int x = 0; x < 32; x++)
+                if (r[u] & (1u << x)) a[x] += bi[u];           // bit test into a predicate + predicated add
+        }
+    }
+    // lanes of a warp that hold the same word column (lane mod wpr) first meet by shuffle
+    for (uint32_t off = wpr; off < 32; off <<= 1) {
+#pragma unroll
+        for (int x = 0; x < 32; x++) a[x] += __shfl_xor_sync(0xffffffffu, a[x], off);
+    }
+    if ((threadIdx.x & 31) < wpr || wpr >= 32) {
+#pragma unroll
+        for (int x = 0; x < 32; x++)
+            if (a[x]) atomicAdd(&sSum[32 * w + x], a[x]);
+    }
+    __syncthreads();
+    for (uint32_t c = threadIdx.x; c < k; c += kAuxThreads)
+        if (sSum[c]) atomicAdd(acc + (size_t)t * k + c, (unsigned long long)sSum[c]);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) sLast = (atomicAdd(tickets + t, 1u) == gridDim.x - 1) ? 1u : 0u;
+    __syncthreads();
+    if (!sLast) return;
+    __threadfence();
+    for (uint32_t c = threadIdx.x; c < k; c += kAuxThreads) {
+        unsigned long long sum = __ldcg(acc + (size_t)t * k + c);
+        acc[(size_t)t * k + c] = 0;
+        uint32_t mu = (mubits[(size_t)t * (k / 8) + c / 8] >> (c % 8)) & 1u;
+        v[(size_t)t * k + c] = (uint16_t)mod_u64(sum + (unsigned long long)mu * mq.half, mq);
+    }
+    if (threadIdx.x == 0) tickets[t] = 0;
+}
+
 cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_Rbits, const uint8_t *d_mubits,
                                   uint16_t *d_v, uint32_t batch, bool write_Rexp, cudaStream_t st)
 {
     const uint32_t m = c->p.m, k = c->p.k;
+    ProfScope prof(c, LWE_K_EXPAND_R_V, st);
+    const uint32_t wpr = k / 32;
+    if (k % 32 == 0 && (wpr & (wpr - 1)) == 0 && wpr <= 64) {
+        const uint32_t rows_per_iter = kAuxThreads / wpr;
+        uint32_t splits = (uint32_t)((4 * c->sm_count + batch - 1) / batch);
+        uint32_t max_splits = (m + 4 * rows_per_iter - 1) / (4 * rows_per_iter);   // >= 4 rows per thread
+        if (splits > max_splits) splits = max_splits;
+        if (splits < 1) splits = 1;
+        dim3 grid(splits, batch);
+        const size_t smem = (size_t)k * sizeof(uint32_t);
+        if (write_Rexp)
+            expand_R_and_v_w32_kernel<true><<<grid, kAuxThreads, smem, st>>>(
+                d_b, d_Rbits, d_mubits, c->d_Rexp, d_v, c->d_vacc, c->d_counters + 8 + c->p.max_batch, m, k, batch * k, c->mq);
+        else
+            expand_R_and_v_w32_kernel<false><<<grid, kAuxThreads, smem, st>>>(
+                d_b, d_Rbits, d_mubits, c->d_Rexp, d_v, c->d_vacc, c->d_counters + 8 + c->p.max_batch, m, k, batch * k, c->mq);
+        c->launches++;
+        return cudaGetLastError();
+    }
     const uint32_t rows_per_iter = kAuxThreads / (k / 8);
     uint32_t splits = (uint32_t)((4 * c->sm_count + batch - 1) / batch);
     uint32_t max_splits = (m + 4 * rows_per_iter - 1) / (4 * rows_per_iter);   // >= 4 row groups per CTA
     if (splits > max_splits) splits = max_splits;
     if (splits < 1) splits = 1;
     dim3 grid(splits, batch);
-    ProfScope prof(c, LWE_K_EXPAND_R_V, st);
     expand_R_and_v_kernel<<<grid, kAuxThreads, 0, st>>>(d_b, d_Rbits, d_mubits, c->d_Rexp, d_v, c->d_vacc,
                                                         c->d_counters + 8 + c->p.max_batch, m, k,
                                                         batch * k, write_Rexp, c->mq);
