@@ -59,7 +59,8 @@ typedef struct {
 typedef struct lwe_ctx lwe_ctx; /* opaque: tables, workspace, TMA descriptors */
 
 /* Create / destroy a context on CUDA device `device`.  Allocates the workspace
- * (m*k*max_batch bytes for the expanded R operand + small accumulators). */
+ * (m*k*max_batch bytes for the expanded R operand, one row panel of A of at most
+ * 64 MiB for the regenerated-A encaps, small accumulators, lwe_kem_host staging). */
 int lwe_create(lwe_ctx **ctx, const lwe_params *p, int device);
 void lwe_destroy(lwe_ctx *ctx);
 
@@ -121,7 +122,11 @@ int lwe_keygen(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
  * Runs as a u8 x u8 -> s32 tensor-core GEMM (tcgen05 kind::i8) over the byte planes
  * of A with a mod-q recombine epilogue; shapes the tensor path does not cover
  * (k % 16 != 0) use a CUDA-core kernel with identical results.
- * d_A == NULL (regenerate from seed_A) returns LWE_ERR_UNSUPPORTED in this build. */
+ * d_A == NULL: A is never read and never held in full: it is regenerated from
+ * (seed_A, LWE_TAG_A, inst 0) one ROW PANEL at a time (rows of A are contiguous ranges
+ * of the counter-indexed stream; a panel is <= 64 MiB of context workspace) and the
+ * contraction is accumulated over the panels -- same U, bit for bit (
+ * BJ configs[4] "stored and regenerated"). */
 int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
                const uint16_t *d_b /*[batch][m]*/, const uint8_t *d_Rbits /*[batch][m*k/8]*/,
                const uint8_t *d_mubits /*[batch][k/8]*/, uint16_t *d_U /*[batch][n][k]*/,
@@ -137,8 +142,8 @@ int lwe_decaps(lwe_ctx *ctx, const uint16_t *d_U, const uint16_t *d_v, const uin
 /* ---- end-to-end with HOST buffers -----------------------------------------------
  * One full pass keygen -> encaps -> decaps for `batch` instances whose per-instance
  * inputs live in host memory: copies h_s, h_e, h_Rbits, h_mubits to the device,
- * runs the three steps against the device-resident public matrix d_A (or seed_A if
- * d_A == NULL, keygen only), copies h_b, h_v, h_mubits_out (and h_U if not NULL) back,
+ * runs the three steps against the device-resident public matrix d_A (or A regenerated
+ * from seed_A if d_A == NULL), copies h_b, h_v, h_mubits_out (and h_U if not NULL) back,
  * and returns after synchronising `stream`.  Layouts as in the calls above. */
 int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
                  const uint16_t *h_s, const uint16_t *h_e, const uint8_t *h_Rbits,
@@ -160,8 +165,12 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
  *                      (LWE_ERR_UNSUPPORTED if n > 32768 or 4*batch > 256).
  * LWE_OPT_TUNE:        launch-shape knob of the tensor-core kernels for measurements (tile order, L2
  *                      eviction policy of the operand streams, ring depth); 0 = default.  Same result
- *                      for every value. */
-enum { LWE_OPT_ENCAPS_PATH = 1, LWE_OPT_PROFILE = 2, LWE_OPT_GEMV_VARIANT = 3, LWE_OPT_KEYGEN_PATH = 4, LWE_OPT_TUNE = 5 };
+ *                      for every value.
+ * LWE_OPT_PANEL_ROWS:  rows of A regenerated per panel by lwe_encaps(d_A == NULL): a multiple of 8 in
+ *                      [8, default]; 0 = default (<= 64 MiB of A per panel, a multiple of 128 rows).  Same
+ *                      result for every value (tests use it to cross many panels at small sizes). */
+enum { LWE_OPT_ENCAPS_PATH = 1, LWE_OPT_PROFILE = 2, LWE_OPT_GEMV_VARIANT = 3, LWE_OPT_KEYGEN_PATH = 4, LWE_OPT_TUNE = 5,
+       LWE_OPT_PANEL_ROWS = 6 };
 int lwe_set_option(lwe_ctx *ctx, int option, int64_t value);
 
 /* Kernel ids for lwe_profile_read (one per __global__ function of the library). */

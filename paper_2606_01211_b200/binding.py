@@ -23,6 +23,7 @@ OPT_PROFILE = 2
 OPT_GEMV_VARIANT = 3
 OPT_KEYGEN_PATH = 4
 OPT_TUNE = 5
+OPT_PANEL_ROWS = 6
 KERNELS = ["rng_fill", "sample_uniform", "sample_cbd", "sample_bits", "keygen_stored", "keygen_regen",
            "expand_R_v", "encaps_tc", "encaps_simt", "decaps", "keygen_prep", "keygen_tc"]
 

@@ -39,9 +39,18 @@ cudaError_t dev_alloc(T **p, size_t count)
 void free_all(Ctx *c)
 {
     cudaFree(c->d_Sx);
+    cudaFree(c->d_Apanel);
     cudaFree(c->d_te0); cudaFree(c->d_Rexp); cudaFree(c->d_vacc); cudaFree(c->d_dacc); cudaFree(c->d_counters);
     cudaFree(c->d_hs); cudaFree(c->d_he); cudaFree(c->d_hb); cudaFree(c->d_hU); cudaFree(c->d_hv);
     cudaFree(c->d_hR); cudaFree(c->d_hmu); cudaFree(c->d_hmuout);
+    if (c->s_in) cudaStreamDestroy(c->s_in);
+    if (c->s_out) cudaStreamDestroy(c->s_out);
+    if (c->ev_entry) cudaEventDestroy(c->ev_entry);
+    if (c->ev_out) cudaEventDestroy(c->ev_out);
+    for (int i = 0; i < kHostChunks; i++) {
+        if (c->ev_in[i]) cudaEventDestroy(c->ev_in[i]);
+        if (c->ev_done[i]) cudaEventDestroy(c->ev_done[i]);
+    }
     if (c->ev) {
         for (int i = 0; i < 2 * kMaxProfEvents; i++)
             if (c->ev[i]) cudaEventDestroy(c->ev[i]);
@@ -117,12 +126,28 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
     ok(dev_alloc(&c->d_te0, 256));
     ok(dev_alloc(&c->d_Rexp, m * k * B));
     if (p->n <= 32768 && 4 * B <= 256) ok(dev_alloc(&c->d_Sx, keygen_tc_workspace_bytes(*p)));
+    {
+        // row panel of a regenerated A: <= 64 MiB, a multiple of 128 rows (one K block of the GEMM), >= 128
+        size_t rows = ((size_t)64 << 20) / (2 * n) / 128 * 128;
+        if (rows < 128) rows = 128;
+        if (rows > m) rows = m;
+        c->panel_rows = c->panel_rows_alloc = (uint32_t)rows;
+        ok(dev_alloc(&c->d_Apanel, rows * n));
+    }
     ok(dev_alloc(&c->d_vacc, k * B));
     ok(dev_alloc(&c->d_dacc, k * B));
     ok(dev_alloc(&c->d_counters, 8 + 2 * B));
     ok(dev_alloc(&c->d_hs, B * n)); ok(dev_alloc(&c->d_he, B * m)); ok(dev_alloc(&c->d_hb, B * m));
     ok(dev_alloc(&c->d_hU, B * n * k)); ok(dev_alloc(&c->d_hv, B * k));
     ok(dev_alloc(&c->d_hR, B * m * k / 8)); ok(dev_alloc(&c->d_hmu, B * k / 8)); ok(dev_alloc(&c->d_hmuout, B * k / 8));
+    ok(cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
+    ok(cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
+    ok(cudaEventCreateWithFlags(&c->ev_entry, cudaEventDisableTiming));
+    ok(cudaEventCreateWithFlags(&c->ev_out, cudaEventDisableTiming));
+    for (int i = 0; i < kHostChunks; i++) {
+        ok(cudaEventCreateWithFlags(&c->ev_in[i], cudaEventDisableTiming));
+        ok(cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming));
+    }
     if (e == cudaSuccess) {
         uint32_t te0[256];
         aes_te0_host(te0);
@@ -180,6 +205,13 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
     if (option == LWE_OPT_TUNE) {
         if (value < 0 || value > 0xffff) return LWE_ERR_PARAM;
         ctx->c.tune = (int)value;
+        return LWE_OK;
+    }
+    if (option == LWE_OPT_PANEL_ROWS) {
+        Ctx *c = &ctx->c;
+        if (value == 0) { c->panel_rows = c->panel_rows_alloc; return LWE_OK; }
+        if (value < 8 || value % 8 || value > (int64_t)c->panel_rows_alloc) return LWE_ERR_PARAM;
+        c->panel_rows = (uint32_t)value;
         return LWE_OK;
     }
     if (option == LWE_OPT_PROFILE) {
@@ -308,11 +340,9 @@ int lwe_keygen(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_
 int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_t *d_b, const uint8_t *d_Rbits,
                const uint8_t *d_mubits, uint16_t *d_U, uint16_t *d_v, uint32_t batch, void *stream)
 {
-    (void)seed_A;
     CHECK_CTX(ctx);
     Ctx *c = &ctx->c;
     if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
-    if (!d_A) return LWE_ERR_UNSUPPORTED;                     // regenerated-A encaps: not in this build
     REQUIRE_PTR(d_b); REQUIRE_PTR(d_Rbits); REQUIRE_PTR(d_mubits); REQUIRE_PTR(d_U); REQUIRE_PTR(d_v);
     REQUIRE_ALIGNED(d_A); REQUIRE_ALIGNED(d_b); REQUIRE_ALIGNED(d_Rbits); REQUIRE_ALIGNED(d_mubits);
     REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v);
@@ -325,9 +355,24 @@ int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_
     DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
     LAUNCH(c, launch_expand_R_and_v(c, d_b, d_Rbits, d_mubits, d_v, batch, tc, st));
-    if (pair) LAUNCH(c, launch_encaps_tc2(c, d_A, d_U, batch, st));
-    else if (tc) LAUNCH(c, launch_encaps_tc(c, d_A, d_U, batch, st));
-    else LAUNCH(c, launch_encaps_simt(c, d_A, d_Rbits, d_U, batch, st));
+    // Stored A: one pass over all m rows.  d_A == NULL: A is regenerated from seed_A one row panel at a
+    // time into the context's panel buffer (rows of A are contiguous ranges of the counter-indexed
+    // stream) and the contraction is accumulated over the panels; A is never held in full.
+    const uint32_t m = c->p.m, step = d_A ? m : c->panel_rows;
+    const AesKey keyA = d_A ? AesKey() : seed_key_host(seed_A);
+    for (uint32_t row0 = 0; row0 < m; row0 += step) {
+        const uint32_t rows = (m - row0 < step) ? (m - row0) : step;
+        const uint16_t *panel = d_A;
+        if (!d_A) {
+            LAUNCH(c, launch_sample_uniform(c, c->d_Apanel, (uint64_t)row0 * c->p.n, (uint64_t)rows * c->p.n, keyA,
+                                            LWE_TAG_A, 0, 1, st));
+            panel = c->d_Apanel;
+        }
+        const bool acc = row0 != 0;
+        if (pair) LAUNCH(c, launch_encaps_tc2(c, panel, d_U, batch, row0, rows, acc, st));
+        else if (tc) LAUNCH(c, launch_encaps_tc(c, panel, d_U, batch, row0, rows, acc, st));
+        else LAUNCH(c, launch_encaps_simt(c, panel, d_Rbits, d_U, batch, row0, rows, acc, st));
+    }
     return LWE_OK;
 }
 
@@ -351,27 +396,64 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint1
     CHECK_CTX(ctx);
     Ctx *c = &ctx->c;
     if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
-    if (!d_A) return LWE_ERR_UNSUPPORTED;
     REQUIRE_PTR(h_s); REQUIRE_PTR(h_e); REQUIRE_PTR(h_Rbits); REQUIRE_PTR(h_mubits);
     REQUIRE_PTR(h_b); REQUIRE_PTR(h_v); REQUIRE_PTR(h_mubits_out);
     REQUIRE_ALIGNED(d_A);
-    const size_t B = batch, n = c->p.n, m = c->p.m, k = c->p.k;
+    const size_t n = c->p.n, m = c->p.m, k = c->p.k;
     cudaStream_t st = (cudaStream_t)stream;
     DeviceGuard guard(c->device);
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hs, h_s, B * n * 2, cudaMemcpyHostToDevice, st));
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_he, h_e, B * m * 2, cudaMemcpyHostToDevice, st));
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hR, h_Rbits, B * m * k / 8, cudaMemcpyHostToDevice, st));
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hmu, h_mubits, B * k / 8, cudaMemcpyHostToDevice, st));
-    int rc = lwe_keygen(ctx, d_A, seed_A, c->d_hs, c->d_he, c->d_hb, batch, stream);
-    if (rc != LWE_OK) return rc;
-    rc = lwe_encaps(ctx, d_A, seed_A, c->d_hb, c->d_hR, c->d_hmu, c->d_hU, c->d_hv, batch, stream);
-    if (rc != LWE_OK) return rc;
-    rc = lwe_decaps(ctx, c->d_hU, c->d_hv, c->d_hs, c->d_hmuout, batch, stream);
-    if (rc != LWE_OK) return rc;
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_b, c->d_hb, B * m * 2, cudaMemcpyDeviceToHost, st));
-    if (h_U) LWE_CUDA_TRY(c, cudaMemcpyAsync(h_U, c->d_hU, B * n * k * 2, cudaMemcpyDeviceToHost, st));
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_v, c->d_hv, B * k * 2, cudaMemcpyDeviceToHost, st));
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_mubits_out, c->d_hmuout, B * k / 8, cudaMemcpyDeviceToHost, st));
+    // Software pipeline over chunks of instances: the copy-in stream runs ahead of the compute stream (the
+    // caller's), the copy-out stream behind it, so that the PCIe transfers of the ciphertexts (U dominates:
+    // 2nk bytes per instance) overlap the GEMM of the following chunks.  Chunks of >= 4 instances keep the
+    // tensor-core GEMM's tile count above one wave.
+    uint32_t nchunks = batch / 4;
+    if (nchunks > (uint32_t)kHostChunks) nchunks = kHostChunks;
+    if (nchunks < 1) nchunks = 1;
+    uint32_t per = (batch + nchunks - 1) / nchunks;
+    // every chunk must start on a 16-byte boundary of each staging buffer (the packed-bit rows are the
+    // narrow ones: k/8 bytes of mu, m*k/8 bytes of R per instance); otherwise one chunk
+    if (((size_t)per * (k / 8)) % 16 || ((size_t)per * (m * k / 8)) % 16) per = batch;
+    LWE_CUDA_TRY(c, cudaEventRecord(c->ev_entry, st));
+    LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_in, c->ev_entry, 0));      // staging buffers are free again
+    LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_out, c->ev_entry, 0));
+    uint32_t ci = 0;
+    for (uint32_t t0 = 0; t0 < batch; t0 += per, ci++) {
+        const size_t g = (batch - t0 < per) ? (batch - t0) : per;
+        LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hs + t0 * n, h_s + t0 * n, g * n * 2, cudaMemcpyHostToDevice, c->s_in));
+        LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_he + t0 * m, h_e + t0 * m, g * m * 2, cudaMemcpyHostToDevice, c->s_in));
+        LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hR + t0 * (m * k / 8), h_Rbits + t0 * (m * k / 8), g * m * k / 8,
+                                        cudaMemcpyHostToDevice, c->s_in));
+        LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hmu + t0 * (k / 8), h_mubits + t0 * (k / 8), g * k / 8,
+                                        cudaMemcpyHostToDevice, c->s_in));
+        LWE_CUDA_TRY(c, cudaEventRecord(c->ev_in[ci], c->s_in));
+    }
+    ci = 0;
+    for (uint32_t t0 = 0; t0 < batch; t0 += per, ci++) {
+        const uint32_t g = (batch - t0 < per) ? (batch - t0) : per;
+        LWE_CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_in[ci], 0));
+        int rc = lwe_keygen(ctx, d_A, seed_A, c->d_hs + t0 * n, c->d_he + t0 * m, c->d_hb + t0 * m, g, stream);
+        if (rc == LWE_OK)
+            rc = lwe_encaps(ctx, d_A, seed_A, c->d_hb + t0 * m, c->d_hR + t0 * (m * k / 8), c->d_hmu + t0 * (k / 8),
+                            c->d_hU + t0 * n * k, c->d_hv + t0 * k, g, stream);
+        if (rc == LWE_OK)
+            rc = lwe_decaps(ctx, c->d_hU + t0 * n * k, c->d_hv + t0 * k, c->d_hs + t0 * n, c->d_hmuout + t0 * (k / 8), g,
+                            stream);
+        if (rc != LWE_OK) {
+            cudaStreamSynchronize(c->s_in); cudaStreamSynchronize(st); cudaStreamSynchronize(c->s_out);
+            return rc;
+        }
+        LWE_CUDA_TRY(c, cudaEventRecord(c->ev_done[ci], st));
+        LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_out, c->ev_done[ci], 0));
+        LWE_CUDA_TRY(c, cudaMemcpyAsync(h_b + t0 * m, c->d_hb + t0 * m, (size_t)g * m * 2, cudaMemcpyDeviceToHost, c->s_out));
+        if (h_U)
+            LWE_CUDA_TRY(c, cudaMemcpyAsync(h_U + t0 * n * k, c->d_hU + t0 * n * k, (size_t)g * n * k * 2,
+                                            cudaMemcpyDeviceToHost, c->s_out));
+        LWE_CUDA_TRY(c, cudaMemcpyAsync(h_v + t0 * k, c->d_hv + t0 * k, (size_t)g * k * 2, cudaMemcpyDeviceToHost, c->s_out));
+        LWE_CUDA_TRY(c, cudaMemcpyAsync(h_mubits_out + t0 * (k / 8), c->d_hmuout + t0 * (k / 8), (size_t)g * k / 8,
+                                        cudaMemcpyDeviceToHost, c->s_out));
+    }
+    LWE_CUDA_TRY(c, cudaEventRecord(c->ev_out, c->s_out));
+    LWE_CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_out, 0));            // the caller's stream sees the whole call
     LWE_CUDA_TRY(c, cudaStreamSynchronize(st));
     return LWE_OK;
 }

@@ -196,19 +196,21 @@ cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_
 // ------------------------------------------------------------------ CUDA-core U = A^T R
 // grid (ceil(n/32), k/8, batch), block 32 x 8: thread (x, y) owns U[j = 32*bx + x][8 columns of
 // byte by] over the row range y, y+8, ...; the 8 row-slices are summed through shared memory.
+// A holds rows [row0, row0 + rows) of the m-row matrix (the whole of it when row0 = 0, rows = m);
+// accumulate: add the residues already in U (row panels of a regenerated A, see tc_common.cuh).
 __global__ void __launch_bounds__(256)
 encaps_simt_kernel(const uint16_t *__restrict__ A, const uint8_t *__restrict__ Rbits, uint16_t *__restrict__ U,
-                   uint32_t m, uint32_t n, uint32_t k, ModQ mq)
+                   uint32_t m, uint32_t n, uint32_t k, uint32_t row0, uint32_t rows, bool accumulate, ModQ mq)
 {
     __shared__ uint32_t sAcc[8][32][8];
     const uint32_t t = blockIdx.z, cb = blockIdx.y, kb = k / 8;
     const uint32_t j = blockIdx.x * 32 + threadIdx.x;
-    const uint8_t *Rt = Rbits + (size_t)t * m * kb;
+    const uint8_t *Rt = Rbits + ((size_t)t * m + row0) * kb;
     uint32_t a[8];
 #pragma unroll
     for (int x = 0; x < 8; x++) a[x] = 0;
     if (j < n) {
-        for (uint32_t i = threadIdx.y; i < m; i += 8) {
+        for (uint32_t i = threadIdx.y; i < rows; i += 8) {
             uint32_t aij = __ldg(A + (size_t)i * n + j);
             uint32_t r = __ldg(Rt + (size_t)i * kb + cb);
 #pragma unroll
@@ -226,18 +228,27 @@ encaps_simt_kernel(const uint16_t *__restrict__ A, const uint8_t *__restrict__ R
             for (int y = 0; y < 8; y++) sum += sAcc[y][threadIdx.x][x];
             o[x] = mod_u64(sum, mq);
         }
-        uint4 pk = make_uint4(o[0] | (o[1] << 16), o[2] | (o[3] << 16), o[4] | (o[5] << 16), o[6] | (o[7] << 16));
-        *reinterpret_cast<uint4 *>(U + ((size_t)t * n + j) * k + 8 * cb) = pk;
+        uint4 *dst = reinterpret_cast<uint4 *>(U + ((size_t)t * n + j) * k + 8 * cb);
+        if (accumulate) {
+            const uint4 p = *dst;
+            const uint32_t old[4] = {p.x, p.y, p.z, p.w};
+#pragma unroll
+            for (int x = 0; x < 8; x++) {
+                uint32_t val = o[x] + ((x & 1) ? (old[x >> 1] >> 16) : (old[x >> 1] & 0xffffu));
+                o[x] = val >= mq.q ? val - mq.q : val;
+            }
+        }
+        *dst = make_uint4(o[0] | (o[1] << 16), o[2] | (o[3] << 16), o[4] | (o[5] << 16), o[6] | (o[7] << 16));
     }
 }
 
 cudaError_t launch_encaps_simt(Ctx *c, const uint16_t *d_A, const uint8_t *d_Rbits, uint16_t *d_U,
-                               uint32_t batch, cudaStream_t st)
+                               uint32_t batch, uint32_t row0, uint32_t rows, bool accumulate, cudaStream_t st)
 {
     const uint32_t m = c->p.m, n = c->p.n, k = c->p.k;
     dim3 grid((n + 31) / 32, k / 8, batch), block(32, 8);
     ProfScope prof(c, LWE_K_ENCAPS_SIMT, st);
-    encaps_simt_kernel<<<grid, block, 0, st>>>(d_A, d_Rbits, d_U, m, n, k, c->mq);
+    encaps_simt_kernel<<<grid, block, 0, st>>>(d_A, d_Rbits, d_U, m, n, k, row0, rows, accumulate, c->mq);
     c->launches++;
     return cudaGetLastError();
 }

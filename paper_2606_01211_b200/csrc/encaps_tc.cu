@@ -58,6 +58,7 @@ struct TileSched {
     }
 };
 
+template <bool kAccum>
 __global__ void __launch_bounds__(kThreads, 1)
 encaps_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
                  uint16_t *__restrict__ U, uint32_t m, uint32_t n, uint32_t k, uint32_t ncols_total, ModQ mq)
@@ -182,9 +183,7 @@ encaps_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
                 const uint32_t col = nt * kTileN + cb + (odd ? 16u : 0u);   // first of my 16 columns
                 if (j < n && col < ncols_total) {
                     const uint32_t inst = col / k, c = col - inst * k;
-                    uint4 *dst = reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c);
-                    dst[0] = make_uint4(o[0] | (o[1] << 16), o[2] | (o[3] << 16), o[4] | (o[5] << 16), o[6] | (o[7] << 16));
-                    dst[1] = make_uint4(o[8] | (o[9] << 16), o[10] | (o[11] << 16), o[12] | (o[13] << 16), o[14] | (o[15] << 16));
+                    store_u16x16<kAccum>(reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c), o, mq);
                 }
             }
             tc_fence_before();
@@ -207,19 +206,22 @@ bool encaps_tc_supported(const Ctx *c, uint32_t batch)
            ((uint64_t)batch * p.k) % 16 == 0;
 }
 
-cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st)
+cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0, uint32_t rows,
+                             bool accumulate, cudaStream_t st)
 {
     const lwe_params &p = c->p;
     const uint32_t ncols = batch * p.k;
     CUtensorMap mapA, mapR;
-    if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, p.m, kTileK)) return cudaErrorInvalidValue;
-    if (!make_map_u8(c, &mapR, c->d_Rexp, ncols, p.m, kTileK)) return cudaErrorInvalidValue;
-    cudaError_t err = cudaFuncSetAttribute(encaps_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    // d_A holds rows [row0, row0 + rows) of A (the whole matrix when row0 = 0, rows = m)
+    if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, rows, kTileK)) return cudaErrorInvalidValue;
+    if (!make_map_u8(c, &mapR, c->d_Rexp + (size_t)row0 * ncols, ncols, rows, kTileK)) return cudaErrorInvalidValue;
+    auto kern = accumulate ? encaps_tc_kernel<true> : encaps_tc_kernel<false>;
+    cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
     if (err != cudaSuccess) return err;
     const uint32_t tiles = ((2 * p.n + kTileM - 1) / kTileM) * ((ncols + kTileN - 1) / kTileN);
     uint32_t grid = tiles < (uint32_t)c->sm_count ? tiles : (uint32_t)c->sm_count;
     ProfScope prof(c, LWE_K_ENCAPS_TC, st);
-    encaps_tc_kernel<<<grid, kThreads, kSmemBytes, st>>>(mapA, mapR, d_U, p.m, p.n, p.k, ncols, c->mq);
+    kern<<<grid, kThreads, kSmemBytes, st>>>(mapA, mapR, d_U, rows, p.n, p.k, ncols, c->mq);
     c->launches++;
     return cudaGetLastError();
 }

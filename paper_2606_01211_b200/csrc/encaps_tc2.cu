@@ -77,7 +77,7 @@ struct PairCfg {
     static constexpr uint32_t kSmemBytes = kStages * kBytesStage + 1024 /*align*/ + 256 /*barriers*/;
 };
 
-template <uint32_t kStages, uint32_t kTileK>
+template <uint32_t kStages, uint32_t kTileK, bool kAccum>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
                   uint16_t *__restrict__ U, uint32_t m, uint32_t n, uint32_t k, uint32_t ncols_total, ModQ mq,
@@ -216,9 +216,7 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 const uint32_t col = nt * kTileN + cb + (odd ? 16u : 0u);
                 if (j < n && col < ncols_total) {
                     const uint32_t inst = col / k, c = col - inst * k;
-                    uint4 *dst = reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c);
-                    dst[0] = make_uint4(o[0] | (o[1] << 16), o[2] | (o[3] << 16), o[4] | (o[5] << 16), o[6] | (o[7] << 16));
-                    dst[1] = make_uint4(o[8] | (o[9] << 16), o[10] | (o[11] << 16), o[12] | (o[13] << 16), o[14] | (o[15] << 16));
+                    store_u16x16<kAccum>(reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c), o, mq);
                 }
             }
             tc_fence_before();
@@ -240,16 +238,18 @@ bool encaps_tc2_supported(const Ctx *c, uint32_t batch)
     return encaps_tc_supported(c, batch) && c->sm_count >= 2;
 }
 
-template <uint32_t kStages, uint32_t kTileK>
-static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st)
+template <uint32_t kStages, uint32_t kTileK, bool kAccum>
+static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0, uint32_t rows,
+                               cudaStream_t st)
 {
     using Cfg = PairCfg<kStages, kTileK>;
     const lwe_params &p = c->p;
     const uint32_t ncols = batch * p.k;
     CUtensorMap mapA, mapR;
-    if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, p.m, kTileK)) return cudaErrorInvalidValue;
-    if (!make_map_u8(c, &mapR, c->d_Rexp, ncols, p.m, kTileK)) return cudaErrorInvalidValue;
-    auto kern = encaps_tc2_kernel<kStages, kTileK>;
+    // d_A holds rows [row0, row0 + rows) of A; the matching rows of the expanded R follow from row0
+    if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, rows, kTileK)) return cudaErrorInvalidValue;
+    if (!make_map_u8(c, &mapR, c->d_Rexp + (size_t)row0 * ncols, ncols, rows, kTileK)) return cudaErrorInvalidValue;
+    auto kern = encaps_tc2_kernel<kStages, kTileK, kAccum>;
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes);
     if (err != cudaSuccess) return err;
     const uint32_t tiles = ((2 * p.n + kPairM - 1) / kPairM) * ((ncols + kTileN - 1) / kTileN);
@@ -260,19 +260,21 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint3
     const uint32_t tune = (uint32_t)c->tune;
     const uint32_t gw = (tune & 15u) ? (1u << ((tune & 15u) - 1)) : 8u;
     ProfScope prof(c, LWE_K_ENCAPS_TC, st);
-    kern<<<2 * pairs, kThreads, Cfg::kSmemBytes, st>>>(mapA, mapR, d_U, p.m, p.n, p.k, ncols, c->mq, gw,
+    kern<<<2 * pairs, kThreads, Cfg::kSmemBytes, st>>>(mapA, mapR, d_U, rows, p.n, p.k, ncols, c->mq, gw,
                                                        (tune >> 4) & 3u, (tune >> 6) & 3u);
     c->launches++;
     return cudaGetLastError();
 }
 
-cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st)
+cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0, uint32_t rows,
+                              bool accumulate, cudaStream_t st)
 {
+    if (accumulate) return launch_pair<6, 128, true>(c, d_A, d_U, batch, row0, rows, st);
     switch ((c->tune >> 8) & 3) {
-    case 1: return launch_pair<7, 128>(c, d_A, d_U, batch, st);
-    case 2: return launch_pair<12, 64>(c, d_A, d_U, batch, st);
-    case 3: return launch_pair<3, 256>(c, d_A, d_U, batch, st);
-    default: return launch_pair<6, 128>(c, d_A, d_U, batch, st);
+    case 1: return launch_pair<7, 128, false>(c, d_A, d_U, batch, row0, rows, st);
+    case 2: return launch_pair<12, 64, false>(c, d_A, d_U, batch, row0, rows, st);
+    case 3: return launch_pair<3, 256, false>(c, d_A, d_U, batch, row0, rows, st);
+    default: return launch_pair<6, 128, false>(c, d_A, d_U, batch, row0, rows, st);
     }
 }
 

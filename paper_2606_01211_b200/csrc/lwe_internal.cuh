@@ -57,6 +57,8 @@ __host__ __device__ __forceinline__ uint32_t mod_u64(uint64_t x, const ModQ &mq)
 }
 
 // ---------------------------------------------------------------------------------
+constexpr int kHostChunks = 8;        // lwe_kem_host splits a batch into at most this many chunks
+
 struct Ctx {
     lwe_params p;
     ModQ mq;
@@ -75,12 +77,19 @@ struct Ctx {
     // workspace (allocated once in lwe_create)
     uint8_t *d_Rexp;                  // [m][max_batch*k] u8 in {0,1}: B operand of the encaps GEMM
     uint8_t *d_Sx;                    // [4*max_batch rounded to 16][2n] u8: B operand of the batched keygen GEMM
+    uint16_t *d_Apanel;               // [panel_rows][n]: one row panel of a regenerated A (encaps with d_A == NULL)
+    uint32_t panel_rows;              // rows per panel in use (LWE_OPT_PANEL_ROWS), <= panel_rows_alloc
+    uint32_t panel_rows_alloc;        // multiple of 128 (or m if smaller): panel_rows_alloc * n * 2 <= ~64 MiB
     unsigned long long *d_vacc;       // [max_batch*k] u64 partial sums of b^T R
     unsigned long long *d_dacc;       // [max_batch*k] u64 partial sums of U^T s
     unsigned int *d_counters;         // [8 + max_batch] self-resetting "last block" tickets
     // staging for lwe_kem_host
     uint16_t *d_hs, *d_he, *d_hb, *d_hU, *d_hv;
     uint8_t *d_hR, *d_hmu, *d_hmuout;
+    // lwe_kem_host pipeline: copy-in / copy-out streams and the events that order them against the
+    // caller's compute stream, one pair per chunk of instances
+    cudaStream_t s_in, s_out;
+    cudaEvent_t ev_entry, ev_out, ev_in[kHostChunks], ev_done[kHostChunks];
 
     // driver entry point for TMA descriptors (resolved at create; no link-time libcuda)
     void *encode_tiled;
@@ -149,12 +158,17 @@ cudaError_t launch_keygen_regen(Ctx *c, const AesKey &key, const uint16_t *d_s, 
 cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_Rbits,
                                   const uint8_t *d_mubits, uint16_t *d_v, uint32_t batch,
                                   bool write_Rexp, cudaStream_t st);
+// The three U = A^T R kernels take a ROW PANEL of A: d_A holds rows [row0, row0 + rows) of the m-row matrix
+// (row0 = 0, rows = m for a stored A); accumulate = add the residues already in d_U (panels after the first
+// when A is regenerated panel by panel).
 cudaError_t launch_encaps_simt(Ctx *c, const uint16_t *d_A, const uint8_t *d_Rbits, uint16_t *d_U,
-                               uint32_t batch, cudaStream_t st);
+                               uint32_t batch, uint32_t row0, uint32_t rows, bool accumulate, cudaStream_t st);
 bool encaps_tc_supported(const Ctx *c, uint32_t batch);
-cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st);
+cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0,
+                             uint32_t rows, bool accumulate, cudaStream_t st);
 bool encaps_tc2_supported(const Ctx *c, uint32_t batch);
-cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, cudaStream_t st);
+cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0,
+                              uint32_t rows, bool accumulate, cudaStream_t st);
 cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
                           uint8_t *d_out, uint32_t batch, cudaStream_t st);
 

@@ -196,6 +196,25 @@ __host__ __device__ constexpr uint32_t instr_desc_u8(uint32_t M, uint32_t N, boo
            ((M >> 4) << 24);
 }
 
+// Epilogue store of 16 consecutive columns of one row of U (two 16-byte stores).  kAccum: add the residues
+// already stored there (mod q) -- used when the contraction over the rows of A is split into panels
+// (A regenerated panel by panel, encaps with d_A == NULL): a sum of residues mod q is the residue of the sum.
+template <bool kAccum>
+__device__ __forceinline__ void store_u16x16(uint4 *dst, uint32_t (&o)[16], const ModQ &mq)
+{
+    if (kAccum) {
+        const uint4 p0 = dst[0], p1 = dst[1];
+        const uint32_t old[8] = {p0.x, p0.y, p0.z, p0.w, p1.x, p1.y, p1.z, p1.w};
+#pragma unroll
+        for (int x = 0; x < 16; x++) {
+            uint32_t val = o[x] + ((x & 1) ? (old[x >> 1] >> 16) : (old[x >> 1] & 0xffffu));   // < 2q
+            o[x] = mq.pow2 ? (val & mq.mask) : (val >= mq.q ? val - mq.q : val);
+        }
+    }
+    dst[0] = make_uint4(o[0] | (o[1] << 16), o[2] | (o[3] << 16), o[4] | (o[5] << 16), o[6] | (o[7] << 16));
+    dst[1] = make_uint4(o[8] | (o[9] << 16), o[10] | (o[11] << 16), o[12] | (o[13] << 16), o[14] | (o[15] << 16));
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);

@@ -112,8 +112,8 @@ def test_c4_bench_configuration_sampled_rows_and_invariants(H):
 
 
 def test_c5_stored_and_regenerated_sampled_rows_columns_and_key_recovery(H):
-    """C5 (n=32768, m=65536, A = 4 GiB): A stored on the device and regenerated inside the keygen
-    kernel give the same b; the oracle recomputes 64 sampled rows of b (a row of A is a contiguous
+    """C5 (n=32768, m=65536, A = 4 GiB): A stored on the device and regenerated (inside the keygen kernel;
+    panel by panel for encaps) give the same b and the same U, v; the oracle recomputes 64 sampled rows of b (a row of A is a contiguous
     stream range) and 64 sampled rows of U x all 256 columns (row j of U needs column j of A, drawn
     by counter index: m AES blocks); the noise identity over all columns and full key recovery close
     the rest (BJ configs[4])."""
@@ -129,6 +129,11 @@ def test_c5_stored_and_regenerated_sampled_rows_columns_and_key_recovery(H):
         g = device_kem(H, c, w, 0, 1, dA, regen_too=True)
         torch.cuda.synchronize()
         assert torch.equal(g["b"], g["b_regen"]), "stored A and regenerated A disagree (P11)"
+        U_regen, v_regen = H.dev_empty_u16(1, n, k), H.dev_empty_u16(1, k)
+        c.encaps(None, w.seed, g["b"], g["Rbits"], g["mubits"], U_regen, v_regen, 1)   # 64 panels of 1024 rows
+        torch.cuda.synchronize()
+        assert torch.equal(g["U"], U_regen) and torch.equal(g["v"], v_regen), "encaps: stored vs regenerated A (P11)"
+        del U_regen
         b, U, v, out = H.host_u16(g["b"])[0], H.host_u16(g["U"])[0], H.host_u16(g["v"])[0], H.host_u8(g["out"])[0]
         s_g, e_g, R_g, mu_g = H.host_u16(g["s"])[0], H.host_u16(g["e"])[0], H.host_u8(g["Rbits"])[0], H.host_u8(g["mubits"])[0]
         A_dev_rows = H.host_u16(dA[torch.from_numpy(brows).cuda()])

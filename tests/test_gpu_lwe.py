@@ -192,6 +192,37 @@ def test_encaps_one_hot_R_picks_a_row_of_A(H, path):
     assert not U.any()
 
 
+@pytest.mark.parametrize("path", **ENCAPS_PATHS)
+@pytest.mark.parametrize("m,n,k,q,batch,seed,panel", [
+    (512, 256, 256, 65536, 1, 1, 0),        # C1: a single panel (default panel >= m)
+    (512, 256, 256, 65536, 2, 1, 128),      # 4 full panels, accumulate across them
+    (1160, 456, 256, 65521, 3, 3, 384),     # prime q (rejection sampling inside the panels), ragged last panel (8 rows)
+    (200, 72, 128, 40000, 3, 9, 72),        # panels that are not a multiple of the K block, ragged tail (56 rows)
+    (2048, 1024, 256, 65536, 1, 2, 1024),   # C2 in two panels
+])
+def test_encaps_regenerated_A_equals_stored_and_oracle(H, path, m, n, k, q, batch, seed, panel):
+    """BJ configs[4] / S8(c) P11: lwe_encaps(d_A = NULL) regenerates A from its seed one row panel at a time and
+    accumulates U over the panels; the result equals the stored-A path and the oracle (whose A is its own draw
+    from the same seed) bit for bit, whatever the panel height."""
+    A = O.sample_uniform(0, m * n, seed, O.TAG_A, 0, q).reshape(m, n)
+    b = W.random_u16((batch, m), q, 22)
+    Rbits = W.random_bytes(batch * m * k // 8, 23).reshape(batch, -1)
+    mubits = W.random_bytes(batch * k // 8, 24).reshape(batch, -1)
+    with B().Context(n, m, k, q, 4, batch) as c:
+        c.set_option(B().OPT_ENCAPS_PATH, path)
+        c.set_option(B().OPT_PANEL_ROWS, panel)
+        U, v = H.dev_empty_u16(batch, n, k), H.dev_empty_u16(batch, k)
+        U.fill_(-1)
+        c.encaps(None, seed, H.dev(b), H.dev(Rbits), H.dev(mubits), U, v, batch)
+        Ug, vg = H.host_u16(U), H.host_u16(v)
+    Us, vs = run_encaps(H, path, m, n, k, q, batch, A, b, Rbits, mubits)
+    assert np.array_equal(Ug, Us) and np.array_equal(vg, vs)
+    for t in range(batch):
+        Uo, vo = O.encaps(A, b[t], Rbits[t], mubits[t], k, q)
+        assert np.array_equal(vg[t], vo), ("v", t)
+        assert np.array_equal(Ug[t], Uo), ("U", t)
+
+
 # ---------------------------------------------------------------- decaps
 
 @pytest.mark.parametrize("n,k,q,batch", [(256, 256, 65536, 1), (1000, 256, 65521, 3), (64, 8, 17, 2),
@@ -264,3 +295,45 @@ def test_full_path_small_matches_oracle_everywhere(H, w, n, m, batch):
         assert np.array_equal(g["U"][t], U) and np.array_equal(g["v"][t], v)
         assert np.array_equal(g["out"][t], O.decaps(U, v, oi.s, w.q))
         assert np.array_equal(g["out"][t], oi.mubits)                # every bit recovered
+
+
+# ---------------------------------------------------------------- end to end with host buffers
+
+@pytest.mark.parametrize("n,m,k,q,batch,regen", [
+    (256, 512, 256, 65536, 1, False),      # one chunk
+    (192, 384, 256, 65521, 9, False),      # two chunks of 5 + 4 instances, prime q
+    (128, 264, 256, 65536, 32, False),     # eight chunks of 4 (the shape of bench.py's e2e leg), ragged K tail
+    (64, 128, 8, 17, 9, False),            # packed-bit rows narrower than 16 bytes: falls back to one chunk
+    (192, 384, 256, 65536, 9, True),       # A regenerated from its seed for keygen and encaps
+])
+def test_kem_host_pipeline_matches_oracle(H, n, m, k, q, batch, regen):
+    """lwe_kem_host (the e2e call bench.py times): pinned host buffers in, chunked copy/compute/copy-out
+    pipeline inside, every output compared with the oracle per instance."""
+    import torch
+    seed = 11
+    A = O.sample_uniform(0, m * n, seed, O.TAG_A, 0, q).reshape(m, n)
+    s, e = W.random_u16((batch, n), q, 51), W.random_u16((batch, m), 5, 52)
+    Rbits = W.random_bytes(batch * m * k // 8, 53).reshape(batch, -1)
+    mubits = W.random_bytes(batch * k // 8, 54).reshape(batch, -1)
+
+    def pinned(a):
+        t = torch.from_numpy(a.view(np.int16) if a.dtype == np.uint16 else a).pin_memory()
+        return t
+
+    h_s, h_e, h_R, h_mu = pinned(s), pinned(e), pinned(Rbits), pinned(mubits)
+    h_b = torch.zeros(batch, m, dtype=torch.int16).pin_memory()
+    h_U = torch.zeros(batch, n, k, dtype=torch.int16).pin_memory()
+    h_v = torch.zeros(batch, k, dtype=torch.int16).pin_memory()
+    h_out = torch.zeros(batch, k // 8, dtype=torch.uint8).pin_memory()
+    with B().Context(n, m, k, q, 4, batch) as c:
+        dA = None if regen else H.dev(A)
+        for _ in range(2):                                     # twice: the staging buffers are reused safely
+            c.kem_host(dA, seed, h_s, h_e, h_R, h_mu, h_b, h_U, h_v, h_out, batch)
+    gb, gU, gv, gout = (h_b.numpy().view(np.uint16), h_U.numpy().view(np.uint16), h_v.numpy().view(np.uint16),
+                        h_out.numpy())
+    for t in range(batch):
+        b = O.keygen(A, s[t], e[t], q)
+        U, v = O.encaps(A, b, Rbits[t], mubits[t], k, q)
+        assert np.array_equal(gb[t], b), ("b", t)
+        assert np.array_equal(gU[t], U) and np.array_equal(gv[t], v), ("U/v", t)
+        assert np.array_equal(gout[t], O.decaps(U, v, s[t], q)), ("mu'", t)
