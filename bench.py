@@ -335,17 +335,29 @@ def run_ours(args):
     for _ in range(args.warmup):
         job.step()
     ok = job.all_bits_recovered()
-    ctx.set_option(job.B.OPT_PROFILE, 1)
+    # the dominant kernel (encaps GEMM) is timed INSIDE the headline region: one CUDA-event pair per launch on the
+    # launching stream, nothing around the other kernels
+    ctx.set_option(job.B.OPT_PROFILE, 2 + job.B.KERNELS.index("encaps_tc"))
     ctx.profile_reset()
     launches0 = ctx.launch_count()
     with ClockSampler(local) as clk:
         ms_total = timed(job.step, args.steps, world)
     launches = ctx.launch_count() - launches0
-    prof = ctx.profile_read()
+    gemm_ms, gemm_cnt = ctx.profile_read().get("encaps_tc", (0.0, 0))
     ctx.set_option(job.B.OPT_PROFILE, 0)
     ok = ok and job.all_bits_recovered()
     ms_step, units = reduce_over_ranks(ms_total / args.steps, Bt)
     value = units / (ms_step * 1e-3)
+
+    # ---- the same K steps again with an event pair around every launch (LWE_OPT_PROFILE): per-kernel device
+    # times and shares.  A separate pass: the event records cost ~4 % of a step, so the headline region above
+    # runs without them; the shares are taken against THIS pass's own step time.
+    ctx.set_option(job.B.OPT_PROFILE, 1)
+    ctx.profile_reset()
+    ms_prof_total = timed(job.step, args.steps, world)
+    prof = ctx.profile_read()
+    ctx.set_option(job.B.OPT_PROFILE, 0)
+    ms_prof_step = ms_prof_total / args.steps
 
     # ---- end to end through lwe_kem_host (pinned host buffers, copies inside the timed region)
     job.make_host()
@@ -363,11 +375,11 @@ def run_ours(args):
 
     # ---- per-kernel shares inside the timed step (CUDA events on the launching stream)
     per_kernel = {name: {"ms_per_launch": ms / cnt, "launches_per_step": cnt / args.steps,
-                         "share_of_step": (ms / args.steps) / ms_step}
+                         "share_of_step": (ms / args.steps) / ms_prof_step}
                   for name, (ms, cnt) in prof.items()}
 
     # dominant kernel: the encaps contraction on the int8 tensor pipe
-    tc = per_kernel.get("encaps_tc")
+    tc = {"ms_per_launch": gemm_ms / gemm_cnt} if gemm_cnt else None      # from the headline region itself
     int8_ops = 4.0 * m * n * k * Bt                       # two byte planes x 2 ops per MAC
     int8_peak_sus = 2.0 * peaks["bf16_tflops_sustained"]  # nominal int8 : bf16 = 4.5 : 2.25 PFLOP/s dense
     int8_peak_burst = 2.0 * peaks["bf16_tflops"]
@@ -405,6 +417,11 @@ def run_ours(args):
     side["decaps_B32"] = {"ms": t2, "per_s": Bt * 1e3 / t2, "GOPs": w.ops_decaps() / (t2 * 1e-3) / 1e9,
                           "GBps": 2.0 * n * k * Bt / (t2 * 1e-3) / 1e9}
     side["kem_per_s_encaps_plus_decaps_only_B32"] = Bt * 1e3 / (t + t2)
+    # N3: decaps with the FO re-encryption check (decrypt + re-encrypt + compare on the device, Alg. 5 without hashes)
+    okflags = torch.empty(Bt, dtype=torch.uint8, device="cuda")
+    t3 = time_call(lambda: ctx.decaps_fo(job.A, job.b, job.U, job.v, job.s, job.Rbits, job.out, okflags, Bt))
+    side["decaps_fo_B32"] = {"ms": t3, "per_s": Bt * 1e3 / t3, "all_accepted": bool(okflags.all().item()),
+                             "kem_per_s_encaps_plus_fo_decaps_B32": Bt * 1e3 / (t + t3)}
     buf = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
     t = time_call(lambda: ctx.rng_fill(buf, buf.numel(), bytes(16), bytes(16), 0), reps=5)
     side["rng_fill_1GiB"] = {"ms": t, "GBps": buf.numel() / (t * 1e-3) / 1e9}
@@ -426,9 +443,12 @@ def run_ours(args):
                 "ms_per_step": ms_e2e, "api": "lwe_kem_host (pinned host buffers; ciphertext U,v and b copied back)"},
         "gpu_launches": int(launches),
         "roofline": roofline,
+        "dominant_kernel_share_of_step": (gemm_ms / args.steps) / (ms_total / args.steps) if gemm_cnt else None,
         "cpu_baseline": cpu,
         "modular_GOPs": (w.ops_keygen() + w.ops_encaps() + w.ops_decaps()) * world / (ms_step * 1e-3) / 1e9,
         "kernels": per_kernel,
+        "kernels_note": f"event pair around every launch, separate pass of the same {args.steps} steps "
+                        f"({ms_prof_step:.4f} ms per step with the events in the stream)",
         "phases": side,
         "peaks": {"hbm_gbs": peaks["hbm_gbs"], "int8_tops_sustained_est": int8_peak_sus,
                   "int8_tops_burst_est": int8_peak_burst, "source": peaks["source"]},

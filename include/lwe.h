@@ -139,6 +139,21 @@ int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
 int lwe_decaps(lwe_ctx *ctx, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
                uint8_t *d_mubits_out /*[batch][k/8]*/, uint32_t batch, void *stream);
 
+/* ---- N3 (S8(f)): Decaps with the FO re-encryption check -----------------------------
+ * Alg. 5 of the paper without its hashes: (1) m' = Decrypt(sk, c) exactly as
+ * lwe_decaps, written to d_mubits_out; (2) c' = Encrypt(pk, m') with the re-derived coins d_Rbits
+ * (the caller derives them as it did for Encaps -- in the paper through hashes that are outside this
+ * library; in bench.py from (seed, LWE_TAG_R, inst)); (4) d_ok[t] = 1 iff c' == c, i.e. U' == U and
+ * v' == v, else 0 (the caller then selects K or the implicit-rejection key, Alg. 5 l.5-7).
+ * The verdict is formed on the device: c' is never materialised (U' is compared with d_U tile by tile
+ * in the epilogue of the tensor-core GEMM, v' lives in the workspace) and nothing returns to the host
+ * before it (the paper's decaps crosses the bus here).  The work done does not depend on
+ * whether the ciphertext is valid.  d_A must be stored (NULL: LWE_ERR_NULLPTR).  d_ok: batch bytes. */
+int lwe_decaps_fo(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_b /*[batch][m]*/,
+                  const uint16_t *d_U /*[batch][n][k]*/, const uint16_t *d_v /*[batch][k]*/,
+                  const uint16_t *d_s /*[batch][n]*/, const uint8_t *d_Rbits /*[batch][m*k/8]*/,
+                  uint8_t *d_mubits_out /*[batch][k/8]*/, uint8_t *d_ok /*[batch]*/, uint32_t batch, void *stream);
+
 /* ---- end-to-end with HOST buffers -----------------------------------------------
  * One full pass keygen -> encaps -> decaps for `batch` instances whose per-instance
  * inputs live in host memory: copies h_s, h_e, h_Rbits, h_mubits to the device,
@@ -157,12 +172,15 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
  *                      2 / 3 give LWE_ERR_UNSUPPORTED at call time if the shape does not fit.
  * LWE_OPT_PROFILE:     1 = bracket every kernel launch with a CUDA event pair on the
  *                      stream it is launched on (at most 8192 launches are kept between
- *                      resets; later ones are simply not timed); 0 = off (default).
+ *                      resets; later ones are simply not timed); 2 + id = only launches of kernel LWE_K_<id>
+ *                      (one pair per launch of that kernel, nothing around the others); 0 = off (default).
  * LWE_OPT_GEMV_VARIANT: keygen GEMV launch shape, 0 = auto; 1/2 = a warp per row with 4/8 loads in
- *                      flight per lane; 3/4 = a CTA per row with 4/2 loads per thread.  Same result.
+ *                      flight per lane; 3/4 = a CTA per row with 4/2 loads per thread.  With A regenerated
+ *                      (d_A == NULL) 1-4 select CTA size / AES blocks in flight instead.  Same result.
  * LWE_OPT_KEYGEN_PATH: stored-A keygen, 0 = auto (GEMV for batch 1, tensor-core skinny GEMM that reads A
  *                      once for batch >= 2), 1 = force one GEMV per instance, 2 = force the tcgen05 GEMM
- *                      (LWE_ERR_UNSUPPORTED if n > 32768 or 4*batch > 256).
+ *                      (LWE_ERR_UNSUPPORTED if n > 32768 or the batch needs more than 256 operand columns:
+ *                      2 per instance when q divides 2^16, else 3 for n <= 16384, else 4).
  * LWE_OPT_TUNE:        launch-shape knob of the tensor-core kernels for measurements (tile order, L2
  *                      eviction policy of the operand streams, ring depth); 0 = default.  Same result
  *                      for every value.
@@ -177,7 +195,8 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value);
 enum {
     LWE_K_RNG_FILL = 0, LWE_K_SAMPLE_UNIFORM = 1, LWE_K_SAMPLE_CBD = 2, LWE_K_SAMPLE_BITS = 3,
     LWE_K_KEYGEN_STORED = 4, LWE_K_KEYGEN_REGEN = 5, LWE_K_EXPAND_R_V = 6, LWE_K_ENCAPS_TC = 7,
-    LWE_K_ENCAPS_SIMT = 8, LWE_K_DECAPS = 9, LWE_K_KEYGEN_PREP = 10, LWE_K_KEYGEN_TC = 11, LWE_K_COUNT = 12
+    LWE_K_ENCAPS_SIMT = 8, LWE_K_DECAPS = 9, LWE_K_KEYGEN_PREP = 10, LWE_K_KEYGEN_TC = 11, LWE_K_FO_VERDICT = 12,
+    LWE_K_COUNT = 13
 };
 /* Sum of the device durations (milliseconds, CUDA events) and the number of timed launches
  * of kernel `kernel_id` since the last reset.  Waits for the recorded events to complete

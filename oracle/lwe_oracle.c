@@ -420,6 +420,25 @@ void orc_decaps(const uint16_t *U, const uint16_t *v, const uint16_t *s,
     free(bit);
 }
 
+/* O11. Alg. 5 lines 1, 2, 4, in the paper's order: m' <- Decrypt(sk, c); c' <- Encrypt(pk, m') with the
+ * re-derived coins R; verdict c' == c (every element of U and v).  The hashes of lines 3, 5, 7 are outside the
+ * hot path. */
+int orc_decaps_fo(const uint16_t *A, const uint16_t *b, const uint16_t *U, const uint16_t *v,
+                  const uint16_t *s, const uint8_t *Rbits, uint8_t *mubits_out,
+                  uint32_t m, uint32_t n, uint32_t k, uint32_t q)
+{
+    orc_decaps(U, v, s, mubits_out, NULL, n, k, q);                              /* 1: m' */
+    uint16_t *U2 = (uint16_t *)malloc((size_t)n * k * sizeof(uint16_t) + 2);
+    uint16_t *v2 = (uint16_t *)malloc((size_t)k * sizeof(uint16_t) + 2);
+    orc_encaps(A, b, Rbits, mubits_out, U2, v2, m, n, k, q);                     /* 2: c' = (U', v') */
+    int equal = 1;                                                               /* 4: c' == c ? */
+    for (size_t x = 0; x < (size_t)n * k; x++) if (U2[x] != U[x]) equal = 0;
+    for (uint32_t c = 0; c < k; c++) if (v2[c] != v[c]) equal = 0;
+    free(U2);
+    free(v2);
+    return equal;
+}
+
 int orc_num_threads(void)
 {
 #ifdef _OPENMP

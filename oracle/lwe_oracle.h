@@ -114,6 +114,16 @@ void orc_decaps(const uint16_t *U, const uint16_t *v, const uint16_t *s,
  * (= 1 iff q/4 <= d < 3q/4). */
 uint32_t orc_round_bit(uint32_t d, uint32_t q);
 
+/* O11. Decaps with the FO re-encryption check, Alg. 5 lines 1, 2, 4 ("recomputes it
+ * deterministically, and verifies its correctness through re-encryption"): m' = O9(U, v, s) -> mubits_out;
+ * (U', v') = O8(A, b, Rbits, m'); returns 1 iff U' == U and v' == v, else 0.  The hashes of the FO transform
+ * are not part of the hot path; Rbits are the re-derived encryption coins.
+ * Pins: an honest ciphertext is accepted and decrypts to mu; ANY single-element change of (U, v) is rejected
+ * whether or not it changes m' (tests/test_oracle_lwe.py). */
+int orc_decaps_fo(const uint16_t *A, const uint16_t *b, const uint16_t *U, const uint16_t *v,
+                  const uint16_t *s, const uint8_t *Rbits, uint8_t *mubits_out,
+                  uint32_t m, uint32_t n, uint32_t k, uint32_t q);
+
 /* Number of OpenMP threads the loops above will use (1 if built without OpenMP). */
 int orc_num_threads(void);
 

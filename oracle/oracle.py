@@ -17,7 +17,7 @@ __all__ = [
     "TAG_A", "TAG_S", "TAG_E", "TAG_R", "TAG_MU",
     "aes128_encrypt_block", "ctr_bytes", "seed_key", "object_iv",
     "sample_uniform", "sample_uniform_strided", "sample_cbd", "sample_bits",
-    "keygen", "encaps", "encaps_rows", "encaps_v", "decaps", "num_threads",
+    "keygen", "encaps", "encaps_rows", "encaps_v", "decaps", "decaps_fo", "num_threads",
     "cbd_from_word", "round_bit",
 ]
 
@@ -43,6 +43,8 @@ def _L():
         lib.orc_encaps_rows.argtypes = [u16p, u8p, u32p, u32, u16p, u32, u32, u32, u32]
         lib.orc_encaps_v.argtypes = [u16p, u8p, u8p, u16p, u32, u32, u32]
         lib.orc_decaps.argtypes = [u16p, u16p, u16p, u8p, u16p, u32, u32, u32]
+        lib.orc_decaps_fo.argtypes = [u16p, u16p, u16p, u16p, u16p, u8p, u8p, u32, u32, u32, u32]
+        lib.orc_decaps_fo.restype = C.c_int
         lib.orc_num_threads.restype = C.c_int
         lib.orc_cbd_from_word.argtypes = [u32, u32, u32]
         lib.orc_cbd_from_word.restype = C.c_uint16
@@ -169,6 +171,19 @@ def decaps(U, v, s, q: int, return_d: bool = False):
     _L().orc_decaps(_p(U, C.c_uint16), _p(v, C.c_uint16), _p(s, C.c_uint16), _p(out, C.c_uint8),
                     _p(d, C.c_uint16), n, k, q)
     return (out, d) if return_d else out
+
+
+def decaps_fo(A, b, U, v, s, Rbits, q: int):
+    """O11: (m' packed bits, verdict c' == c) of Alg. 5 lines 1, 2, 4"""
+    A, b, U, v, s = _u16(A), _u16(b), _u16(U), _u16(v), _u16(s)
+    m, n = A.shape
+    n2, k = U.shape
+    assert n2 == n and b.shape == (m,) and v.shape == (k,) and s.shape == (n,)
+    Rbits = _u8(Rbits, m * k // 8)
+    out = np.zeros(k // 8, np.uint8)
+    ok = _L().orc_decaps_fo(_p(A, C.c_uint16), _p(b, C.c_uint16), _p(U, C.c_uint16), _p(v, C.c_uint16),
+                            _p(s, C.c_uint16), _p(Rbits, C.c_uint8), _p(out, C.c_uint8), m, n, k, q)
+    return out, int(ok)
 
 
 def cbd_from_word(w: int, q: int, eta: int) -> int:

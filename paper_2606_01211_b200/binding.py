@@ -25,12 +25,12 @@ OPT_KEYGEN_PATH = 4
 OPT_TUNE = 5
 OPT_PANEL_ROWS = 6
 KERNELS = ["rng_fill", "sample_uniform", "sample_cbd", "sample_bits", "keygen_stored", "keygen_regen",
-           "expand_R_v", "encaps_tc", "encaps_simt", "decaps", "keygen_prep", "keygen_tc"]
+           "expand_R_v", "encaps_tc", "encaps_simt", "decaps", "keygen_prep", "keygen_tc", "fo_verdict"]
 
 EXPORTS = [
     "lwe_create", "lwe_destroy", "lwe_strerror", "lwe_last_cuda_error", "lwe_launch_count",
     "lwe_rng_fill", "lwe_sample_uniform", "lwe_sample_cbd", "lwe_sample_bits",
-    "lwe_keygen", "lwe_encaps", "lwe_decaps", "lwe_kem_host", "lwe_set_option",
+    "lwe_keygen", "lwe_encaps", "lwe_decaps", "lwe_decaps_fo", "lwe_kem_host", "lwe_set_option",
     "lwe_profile_read", "lwe_profile_reset",
 ]
 
@@ -75,6 +75,7 @@ def load_library() -> C.CDLL:
     lib.lwe_keygen.argtypes = [vp, vp, u64, vp, vp, vp, u32, vp]
     lib.lwe_encaps.argtypes = [vp, vp, u64, vp, vp, vp, vp, vp, u32, vp]
     lib.lwe_decaps.argtypes = [vp, vp, vp, vp, vp, u32, vp]
+    lib.lwe_decaps_fo.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
     lib.lwe_kem_host.argtypes = [vp, vp, u64, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
     _lib = lib
     return lib
@@ -182,6 +183,11 @@ class Context:
     def decaps(self, d_U, d_v, d_s, d_mubits_out, batch: int = 1, stream=None):
         self._check(self._lib.lwe_decaps(self._h, _ptr(d_U), _ptr(d_v), _ptr(d_s), _ptr(d_mubits_out), batch,
                                          _stream(stream)), "lwe_decaps")
+
+    def decaps_fo(self, d_A, d_b, d_U, d_v, d_s, d_Rbits, d_mubits_out, d_ok, batch: int = 1, stream=None):
+        self._check(self._lib.lwe_decaps_fo(self._h, _ptr(d_A), _ptr(d_b), _ptr(d_U), _ptr(d_v), _ptr(d_s),
+                                            _ptr(d_Rbits), _ptr(d_mubits_out), _ptr(d_ok), batch, _stream(stream)),
+                    "lwe_decaps_fo")
 
     def kem_host(self, d_A, seed_A: int, h_s, h_e, h_Rbits, h_mubits, h_b, h_U, h_v, h_mubits_out, batch: int = 1,
                  stream=None):

@@ -40,6 +40,7 @@ void free_all(Ctx *c)
 {
     cudaFree(c->d_Sx);
     cudaFree(c->d_Apanel);
+    cudaFree(c->d_foflags); cudaFree(c->d_vprime);
     cudaFree(c->d_te0); cudaFree(c->d_Rexp); cudaFree(c->d_vacc); cudaFree(c->d_dacc); cudaFree(c->d_counters);
     cudaFree(c->d_hs); cudaFree(c->d_he); cudaFree(c->d_hb); cudaFree(c->d_hU); cudaFree(c->d_hv);
     cudaFree(c->d_hR); cudaFree(c->d_hmu); cudaFree(c->d_hmuout);
@@ -125,7 +126,7 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
     auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
     ok(dev_alloc(&c->d_te0, 256));
     ok(dev_alloc(&c->d_Rexp, m * k * B));
-    if (p->n <= 32768 && 4 * B <= 256) ok(dev_alloc(&c->d_Sx, keygen_tc_workspace_bytes(*p)));
+    if (keygen_tc_workspace_bytes(*p)) ok(dev_alloc(&c->d_Sx, keygen_tc_workspace_bytes(*p)));
     {
         // row panel of a regenerated A: <= 64 MiB, a multiple of 128 rows (one K block of the GEMM), >= 128
         size_t rows = ((size_t)64 << 20) / (2 * n) / 128 * 128;
@@ -134,6 +135,8 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
         c->panel_rows = c->panel_rows_alloc = (uint32_t)rows;
         ok(dev_alloc(&c->d_Apanel, rows * n));
     }
+    ok(dev_alloc(&c->d_foflags, B));
+    ok(dev_alloc(&c->d_vprime, B * k));
     ok(dev_alloc(&c->d_vacc, k * B));
     ok(dev_alloc(&c->d_dacc, k * B));
     ok(dev_alloc(&c->d_counters, 8 + 2 * B));
@@ -216,7 +219,7 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
     }
     if (option == LWE_OPT_PROFILE) {
         Ctx *c = &ctx->c;
-        if (value != 0 && value != 1) return LWE_ERR_PARAM;
+        if (value < 0 || value > 1 + LWE_K_COUNT) return LWE_ERR_PARAM;
         if (value && !c->ev) {
             DeviceGuard guard(c->device);
             c->ev = new (std::nothrow) cudaEvent_t[2 * kMaxProfEvents]();
@@ -337,23 +340,17 @@ int lwe_keygen(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_
     return LWE_OK;
 }
 
-int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_t *d_b, const uint8_t *d_Rbits,
-               const uint8_t *d_mubits, uint16_t *d_U, uint16_t *d_v, uint32_t batch, void *stream)
+// expand R (+ v) and run U = A^T R.  compare = false: write U (accumulating over the panels of a regenerated A);
+// compare = true (stored A only): write nothing, compare with d_U and OR mismatches into c->d_foflags.
+static int encaps_core(Ctx *c, const uint16_t *d_A, uint64_t seed_A, const uint16_t *d_b, const uint8_t *d_Rbits,
+                       const uint8_t *d_mubits, uint16_t *d_U, uint16_t *d_v, uint32_t batch, bool compare, cudaStream_t st)
 {
-    CHECK_CTX(ctx);
-    Ctx *c = &ctx->c;
-    if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
-    REQUIRE_PTR(d_b); REQUIRE_PTR(d_Rbits); REQUIRE_PTR(d_mubits); REQUIRE_PTR(d_U); REQUIRE_PTR(d_v);
-    REQUIRE_ALIGNED(d_A); REQUIRE_ALIGNED(d_b); REQUIRE_ALIGNED(d_Rbits); REQUIRE_ALIGNED(d_mubits);
-    REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v);
     bool tc = encaps_tc_supported(c, batch);
     if (c->encaps_path == 1) tc = false;
     if (c->encaps_path >= 2 && !tc) return LWE_ERR_UNSUPPORTED;
     // CTA pairs (cta_group::2) by default; path 2 keeps the single-CTA kernel selectable
     const bool pair = tc && c->encaps_path != 2 && encaps_tc2_supported(c, batch);
     if (c->encaps_path == 3 && !pair) return LWE_ERR_UNSUPPORTED;
-    DeviceGuard guard(c->device);
-    cudaStream_t st = (cudaStream_t)stream;
     LAUNCH(c, launch_expand_R_and_v(c, d_b, d_Rbits, d_mubits, d_v, batch, tc, st));
     // Stored A: one pass over all m rows.  d_A == NULL: A is regenerated from seed_A one row panel at a
     // time into the context's panel buffer (rows of A are contiguous ranges of the counter-indexed
@@ -368,11 +365,50 @@ int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_
                                             LWE_TAG_A, 0, 1, st));
             panel = c->d_Apanel;
         }
-        const bool acc = row0 != 0;
-        if (pair) LAUNCH(c, launch_encaps_tc2(c, panel, d_U, batch, row0, rows, acc, st));
-        else if (tc) LAUNCH(c, launch_encaps_tc(c, panel, d_U, batch, row0, rows, acc, st));
-        else LAUNCH(c, launch_encaps_simt(c, panel, d_Rbits, d_U, batch, row0, rows, acc, st));
+        const int mode = compare ? 2 : (row0 != 0 ? 1 : 0);
+        if (pair) LAUNCH(c, launch_encaps_tc2(c, panel, d_U, batch, row0, rows, mode, c->d_foflags, st));
+        else if (tc) LAUNCH(c, launch_encaps_tc(c, panel, d_U, batch, row0, rows, mode, c->d_foflags, st));
+        else LAUNCH(c, launch_encaps_simt(c, panel, d_Rbits, d_U, batch, row0, rows, mode, c->d_foflags, st));
     }
+    return LWE_OK;
+}
+
+int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_t *d_b, const uint8_t *d_Rbits,
+               const uint8_t *d_mubits, uint16_t *d_U, uint16_t *d_v, uint32_t batch, void *stream)
+{
+    CHECK_CTX(ctx);
+    Ctx *c = &ctx->c;
+    if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
+    REQUIRE_PTR(d_b); REQUIRE_PTR(d_Rbits); REQUIRE_PTR(d_mubits); REQUIRE_PTR(d_U); REQUIRE_PTR(d_v);
+    REQUIRE_ALIGNED(d_A); REQUIRE_ALIGNED(d_b); REQUIRE_ALIGNED(d_Rbits); REQUIRE_ALIGNED(d_mubits);
+    REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v);
+    DeviceGuard guard(c->device);
+    return encaps_core(c, d_A, seed_A, d_b, d_Rbits, d_mubits, d_U, d_v, batch, false, (cudaStream_t)stream);
+}
+
+int lwe_decaps_fo(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_b, const uint16_t *d_U, const uint16_t *d_v,
+                  const uint16_t *d_s, const uint8_t *d_Rbits, uint8_t *d_mubits_out, uint8_t *d_ok, uint32_t batch,
+                  void *stream)
+{
+    CHECK_CTX(ctx);
+    Ctx *c = &ctx->c;
+    if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
+    REQUIRE_PTR(d_A); REQUIRE_PTR(d_b); REQUIRE_PTR(d_U); REQUIRE_PTR(d_v); REQUIRE_PTR(d_s); REQUIRE_PTR(d_Rbits);
+    REQUIRE_PTR(d_mubits_out); REQUIRE_PTR(d_ok);
+    REQUIRE_ALIGNED(d_A); REQUIRE_ALIGNED(d_b); REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v); REQUIRE_ALIGNED(d_s);
+    REQUIRE_ALIGNED(d_Rbits); REQUIRE_ALIGNED(d_mubits_out); REQUIRE_ALIGNED(d_ok);
+    if (c->encaps_path >= 2 && !encaps_tc_supported(c, batch)) return LWE_ERR_UNSUPPORTED;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    // Alg. 5: 1. m' <- Decrypt(sk, c)
+    LAUNCH(c, launch_decaps(c, d_U, d_v, d_s, d_mubits_out, batch, st));
+    // 2. c' <- Encrypt(pk, m') with the re-derived coins R; c' = (U', v') is never stored: v' goes to the
+    //    workspace, U' is compared with U tile by tile in the GEMM epilogue
+    LWE_CUDA_TRY(c, cudaMemsetAsync(c->d_foflags, 0, batch * sizeof(uint32_t), st));
+    int rc = encaps_core(c, d_A, 0, d_b, d_Rbits, d_mubits_out, const_cast<uint16_t *>(d_U), c->d_vprime, batch, true, st);
+    if (rc != LWE_OK) return rc;
+    // 4. verdict c' == c per instance, on the device
+    LAUNCH(c, launch_fo_verdict(c, d_v, c->d_vprime, c->d_foflags, d_ok, batch, st));
     return LWE_OK;
 }
 

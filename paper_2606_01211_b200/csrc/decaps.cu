@@ -118,13 +118,44 @@ cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, cons
 {
     const uint32_t n = c->p.n, k = c->p.k;
     const uint32_t rows_per_iter = kDecThreads / (k / 8);
-    uint32_t splits = (uint32_t)((8 * c->sm_count + batch - 1) / batch);
+    // exactly one wave of resident CTAs (a second, partial wave was the tail: 1184 CTAs on 740 slots ran at
+    // 0.54 of HBM): as many row splits per instance as fit the SMs at the kernel's occupancy
+    static int per_sm = 0;
+    if (!per_sm) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, decaps_kernel, kDecThreads, 0) != cudaSuccess || per_sm < 1)
+            per_sm = 1;
+    }
+    uint32_t splits = (uint32_t)(per_sm * c->sm_count) / batch;
     uint32_t max_splits = (n + 4 * rows_per_iter - 1) / (4 * rows_per_iter);       // >= 4 row groups per CTA
     if (splits > max_splits) splits = max_splits;
     if (splits < 1) splits = 1;
     dim3 grid(splits, batch);
     ProfScope prof(c, LWE_K_DECAPS, st);
     decaps_kernel<<<grid, kDecThreads, 0, st>>>(d_U, d_v, d_s, d_out, c->d_dacc, c->d_counters + 8, n, k, c->mq);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+// FO verdict (Alg.5 l.4): ok[t] = 1 iff the re-encrypted ciphertext equals the received one, i.e. no
+// U tile reported a mismatch (flags[t] == 0, set by the compare epilogue of the encaps GEMM) and v' == v.
+// One warp per instance; the whole v row is always read (no early exit).
+__global__ void __launch_bounds__(32)
+fo_verdict_kernel(const uint16_t *__restrict__ v, const uint16_t *__restrict__ vprime, const uint32_t *__restrict__ flags,
+                  uint8_t *__restrict__ ok, uint32_t k)
+{
+    const uint32_t t = blockIdx.x;
+    uint32_t diff = 0;
+    for (uint32_t c = threadIdx.x; c < k; c += 32) diff |= (uint32_t)(v[(size_t)t * k + c] ^ vprime[(size_t)t * k + c]);
+    diff |= flags[t];
+    const uint32_t any = __ballot_sync(0xffffffffu, diff != 0);
+    if (threadIdx.x == 0) ok[t] = any ? 0 : 1;
+}
+
+cudaError_t launch_fo_verdict(Ctx *c, const uint16_t *d_v, const uint16_t *d_vprime, const uint32_t *d_flags,
+                              uint8_t *d_ok, uint32_t batch, cudaStream_t st)
+{
+    ProfScope prof(c, LWE_K_FO_VERDICT, st);
+    fo_verdict_kernel<<<batch, 32, 0, st>>>(d_v, d_vprime, d_flags, d_ok, c->p.k);
     c->launches++;
     return cudaGetLastError();
 }

@@ -165,12 +165,21 @@ cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_
     const uint32_t wpr = k / 32;
     if (k % 32 == 0 && (wpr & (wpr - 1)) == 0 && wpr <= 64) {
         const uint32_t rows_per_iter = kAuxThreads / wpr;
-        uint32_t splits = (uint32_t)((4 * c->sm_count + batch - 1) / batch);
+        const size_t smem = (size_t)k * sizeof(uint32_t);
+        // exactly one wave of resident CTAs (608 CTAs on 296 slots left a third, nearly empty wave)
+        static int per_sm[2] = {0, 0};
+        int &occ = per_sm[write_Rexp ? 1 : 0];
+        if (!occ) {
+            cudaError_t qe = write_Rexp
+                ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, expand_R_and_v_w32_kernel<true>, kAuxThreads, smem)
+                : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, expand_R_and_v_w32_kernel<false>, kAuxThreads, smem);
+            if (qe != cudaSuccess || occ < 1) occ = 1;
+        }
+        uint32_t splits = (uint32_t)(occ * c->sm_count) / batch;
         uint32_t max_splits = (m + 4 * rows_per_iter - 1) / (4 * rows_per_iter);   // >= 4 rows per thread
         if (splits > max_splits) splits = max_splits;
         if (splits < 1) splits = 1;
         dim3 grid(splits, batch);
-        const size_t smem = (size_t)k * sizeof(uint32_t);
         if (write_Rexp)
             expand_R_and_v_w32_kernel<true><<<grid, kAuxThreads, smem, st>>>(
                 d_b, d_Rbits, d_mubits, c->d_Rexp, d_v, c->d_vacc, c->d_counters + 8 + c->p.max_batch, m, k, batch * k, c->mq);
@@ -200,7 +209,8 @@ cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_
 // accumulate: add the residues already in U (row panels of a regenerated A, see tc_common.cuh).
 __global__ void __launch_bounds__(256)
 encaps_simt_kernel(const uint16_t *__restrict__ A, const uint8_t *__restrict__ Rbits, uint16_t *__restrict__ U,
-                   uint32_t m, uint32_t n, uint32_t k, uint32_t row0, uint32_t rows, bool accumulate, ModQ mq)
+                   uint32_t m, uint32_t n, uint32_t k, uint32_t row0, uint32_t rows, int mode, uint32_t *__restrict__ flags,
+                   ModQ mq)
 {
     __shared__ uint32_t sAcc[8][32][8];
     const uint32_t t = blockIdx.z, cb = blockIdx.y, kb = k / 8;
@@ -229,7 +239,14 @@ encaps_simt_kernel(const uint16_t *__restrict__ A, const uint8_t *__restrict__ R
             o[x] = mod_u64(sum, mq);
         }
         uint4 *dst = reinterpret_cast<uint4 *>(U + ((size_t)t * n + j) * k + 8 * cb);
-        if (accumulate) {
+        if (mode == 2) {                                     // FO re-encryption check: compare, write nothing
+            const uint4 p = *dst;
+            const uint32_t diff = (p.x ^ (o[0] | (o[1] << 16))) | (p.y ^ (o[2] | (o[3] << 16))) |
+                                  (p.z ^ (o[4] | (o[5] << 16))) | (p.w ^ (o[6] | (o[7] << 16)));
+            atomicOr(flags + t, diff ? 1u : 0u);
+            return;
+        }
+        if (mode == 1) {
             const uint4 p = *dst;
             const uint32_t old[4] = {p.x, p.y, p.z, p.w};
 #pragma unroll
@@ -243,12 +260,12 @@ encaps_simt_kernel(const uint16_t *__restrict__ A, const uint8_t *__restrict__ R
 }
 
 cudaError_t launch_encaps_simt(Ctx *c, const uint16_t *d_A, const uint8_t *d_Rbits, uint16_t *d_U,
-                               uint32_t batch, uint32_t row0, uint32_t rows, bool accumulate, cudaStream_t st)
+                               uint32_t batch, uint32_t row0, uint32_t rows, int mode, uint32_t *d_flags, cudaStream_t st)
 {
     const uint32_t m = c->p.m, n = c->p.n, k = c->p.k;
     dim3 grid((n + 31) / 32, k / 8, batch), block(32, 8);
     ProfScope prof(c, LWE_K_ENCAPS_SIMT, st);
-    encaps_simt_kernel<<<grid, block, 0, st>>>(d_A, d_Rbits, d_U, m, n, k, row0, rows, accumulate, c->mq);
+    encaps_simt_kernel<<<grid, block, 0, st>>>(d_A, d_Rbits, d_U, m, n, k, row0, rows, mode, d_flags, c->mq);
     c->launches++;
     return cudaGetLastError();
 }

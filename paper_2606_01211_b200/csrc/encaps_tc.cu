@@ -58,10 +58,11 @@ struct TileSched {
     }
 };
 
-template <bool kAccum>
+template <int kMode>
 __global__ void __launch_bounds__(kThreads, 1)
 encaps_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
-                 uint16_t *__restrict__ U, uint32_t m, uint32_t n, uint32_t k, uint32_t ncols_total, ModQ mq)
+                 uint16_t *__restrict__ U, uint32_t *__restrict__ flags, uint32_t m, uint32_t n, uint32_t k,
+                 uint32_t ncols_total, ModQ mq)
 {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
@@ -167,6 +168,7 @@ encaps_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
             const uint32_t j = brow >> 1;                             // column of A / row of U
             const bool odd = lane & 1;
             const uint32_t taddr = tmem_base + ((quarter * 32) << 16) + acc * kTileN;
+            MismatchAcc mism;
 #pragma unroll 1
             for (uint32_t cb = 0; cb < kTileN; cb += 32) {
                 uint32_t r[32];
@@ -183,9 +185,11 @@ encaps_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
                 const uint32_t col = nt * kTileN + cb + (odd ? 16u : 0u);   // first of my 16 columns
                 if (j < n && col < ncols_total) {
                     const uint32_t inst = col / k, c = col - inst * k;
-                    store_u16x16<kAccum>(reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c), o, mq);
+                    const bool bad = store_u16x16<kMode>(reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c), o, mq);
+                    if (kMode == kEpiCompare) mism.note(flags, inst, bad);
                 }
             }
+            if (kMode == kEpiCompare) mism.flush_warp(flags);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(tempty_bar(acc));
@@ -207,7 +211,7 @@ bool encaps_tc_supported(const Ctx *c, uint32_t batch)
 }
 
 cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0, uint32_t rows,
-                             bool accumulate, cudaStream_t st)
+                             int mode, uint32_t *d_flags, cudaStream_t st)
 {
     const lwe_params &p = c->p;
     const uint32_t ncols = batch * p.k;
@@ -215,13 +219,14 @@ cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_
     // d_A holds rows [row0, row0 + rows) of A (the whole matrix when row0 = 0, rows = m)
     if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, rows, kTileK)) return cudaErrorInvalidValue;
     if (!make_map_u8(c, &mapR, c->d_Rexp + (size_t)row0 * ncols, ncols, rows, kTileK)) return cudaErrorInvalidValue;
-    auto kern = accumulate ? encaps_tc_kernel<true> : encaps_tc_kernel<false>;
+    auto kern = mode == kEpiAccum ? encaps_tc_kernel<kEpiAccum>
+              : mode == kEpiCompare ? encaps_tc_kernel<kEpiCompare> : encaps_tc_kernel<kEpiStore>;
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
     if (err != cudaSuccess) return err;
     const uint32_t tiles = ((2 * p.n + kTileM - 1) / kTileM) * ((ncols + kTileN - 1) / kTileN);
     uint32_t grid = tiles < (uint32_t)c->sm_count ? tiles : (uint32_t)c->sm_count;
     ProfScope prof(c, LWE_K_ENCAPS_TC, st);
-    kern<<<grid, kThreads, kSmemBytes, st>>>(mapA, mapR, d_U, rows, p.n, p.k, ncols, c->mq);
+    kern<<<grid, kThreads, kSmemBytes, st>>>(mapA, mapR, d_U, d_flags, rows, p.n, p.k, ncols, c->mq);
     c->launches++;
     return cudaGetLastError();
 }

@@ -77,11 +77,11 @@ struct PairCfg {
     static constexpr uint32_t kSmemBytes = kStages * kBytesStage + 1024 /*align*/ + 256 /*barriers*/;
 };
 
-template <uint32_t kStages, uint32_t kTileK, bool kAccum>
+template <uint32_t kStages, uint32_t kTileK, int kMode>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
-                  uint16_t *__restrict__ U, uint32_t m, uint32_t n, uint32_t k, uint32_t ncols_total, ModQ mq,
-                  uint32_t group_w, uint32_t polA_kind, uint32_t polR_kind)
+                  uint16_t *__restrict__ U, uint32_t *__restrict__ flags, uint32_t m, uint32_t n, uint32_t k,
+                  uint32_t ncols_total, ModQ mq, uint32_t group_w, uint32_t polA_kind, uint32_t polR_kind)
 {
     using Cfg = PairCfg<kStages, kTileK>;
     constexpr uint32_t kBytesA = Cfg::kBytesA, kBytesStage = Cfg::kBytesStage;
@@ -200,6 +200,7 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
             const uint32_t j = brow >> 1;
             const bool odd = lane & 1;
             const uint32_t taddr = tmem_base + ((quarter * 32) << 16) + acc * kTileN;
+            MismatchAcc mism;
 #pragma unroll 1
             for (uint32_t cb = 0; cb < kTileN; cb += 32) {
                 uint32_t r[32];
@@ -216,9 +217,11 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 const uint32_t col = nt * kTileN + cb + (odd ? 16u : 0u);
                 if (j < n && col < ncols_total) {
                     const uint32_t inst = col / k, c = col - inst * k;
-                    store_u16x16<kAccum>(reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c), o, mq);
+                    const bool bad = store_u16x16<kMode>(reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c), o, mq);
+                    if (kMode == kEpiCompare) mism.note(flags, inst, bad);
                 }
             }
+            if (kMode == kEpiCompare) mism.flush_warp(flags);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(acc ? lead_tempty1 : lead_tempty0);
@@ -238,9 +241,9 @@ bool encaps_tc2_supported(const Ctx *c, uint32_t batch)
     return encaps_tc_supported(c, batch) && c->sm_count >= 2;
 }
 
-template <uint32_t kStages, uint32_t kTileK, bool kAccum>
-static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0, uint32_t rows,
-                               cudaStream_t st)
+template <uint32_t kStages, uint32_t kTileK, int kMode>
+static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t *d_flags, uint32_t batch, uint32_t row0,
+                               uint32_t rows, cudaStream_t st)
 {
     using Cfg = PairCfg<kStages, kTileK>;
     const lwe_params &p = c->p;
@@ -249,7 +252,7 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint3
     // d_A holds rows [row0, row0 + rows) of A; the matching rows of the expanded R follow from row0
     if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, rows, kTileK)) return cudaErrorInvalidValue;
     if (!make_map_u8(c, &mapR, c->d_Rexp + (size_t)row0 * ncols, ncols, rows, kTileK)) return cudaErrorInvalidValue;
-    auto kern = encaps_tc2_kernel<kStages, kTileK, kAccum>;
+    auto kern = encaps_tc2_kernel<kStages, kTileK, kMode>;
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes);
     if (err != cudaSuccess) return err;
     const uint32_t tiles = ((2 * p.n + kPairM - 1) / kPairM) * ((ncols + kTileN - 1) / kTileN);
@@ -260,21 +263,22 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint3
     const uint32_t tune = (uint32_t)c->tune;
     const uint32_t gw = (tune & 15u) ? (1u << ((tune & 15u) - 1)) : 8u;
     ProfScope prof(c, LWE_K_ENCAPS_TC, st);
-    kern<<<2 * pairs, kThreads, Cfg::kSmemBytes, st>>>(mapA, mapR, d_U, rows, p.n, p.k, ncols, c->mq, gw,
+    kern<<<2 * pairs, kThreads, Cfg::kSmemBytes, st>>>(mapA, mapR, d_U, d_flags, rows, p.n, p.k, ncols, c->mq, gw,
                                                        (tune >> 4) & 3u, (tune >> 6) & 3u);
     c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0, uint32_t rows,
-                              bool accumulate, cudaStream_t st)
+                              int mode, uint32_t *d_flags, cudaStream_t st)
 {
-    if (accumulate) return launch_pair<6, 128, true>(c, d_A, d_U, batch, row0, rows, st);
+    if (mode == kEpiAccum) return launch_pair<6, 128, kEpiAccum>(c, d_A, d_U, nullptr, batch, row0, rows, st);
+    if (mode == kEpiCompare) return launch_pair<6, 128, kEpiCompare>(c, d_A, d_U, d_flags, batch, row0, rows, st);
     switch ((c->tune >> 8) & 3) {
-    case 1: return launch_pair<7, 128, false>(c, d_A, d_U, batch, row0, rows, st);
-    case 2: return launch_pair<12, 64, false>(c, d_A, d_U, batch, row0, rows, st);
-    case 3: return launch_pair<3, 256, false>(c, d_A, d_U, batch, row0, rows, st);
-    default: return launch_pair<6, 128, false>(c, d_A, d_U, batch, row0, rows, st);
+    case 1: return launch_pair<5, 128, kEpiStore>(c, d_A, d_U, nullptr, batch, row0, rows, st);
+    case 2: return launch_pair<4, 128, kEpiStore>(c, d_A, d_U, nullptr, batch, row0, rows, st);
+    case 3: return launch_pair<3, 256, kEpiStore>(c, d_A, d_U, nullptr, batch, row0, rows, st);
+    default: return launch_pair<6, 128, kEpiStore>(c, d_A, d_U, nullptr, batch, row0, rows, st);
     }
 }
 

@@ -20,6 +20,7 @@
 namespace lwe {
 
 constexpr int kGemvThreads = 256;
+constexpr int kRedBytes = 256;           // per-warp u64 slots of the team reduction (<= 32 warps)
 constexpr int kFlushEvery = 32;          // uint4 loads between flushes: 32*4 = 128 dp2a per accumulator
 
 __device__ __forceinline__ uint4 ldg_stream(const uint4 *p)
@@ -49,42 +50,46 @@ __device__ __forceinline__ void pack_s_to_smem(uint32_t *sS, const uint16_t *__r
     __syncthreads();
 }
 
-template <int TPR>   // threads per row team: 32 (a warp) or kGemvThreads (the CTA)
+// barrier over one row team: the whole CTA, or TPR threads on a named barrier of their own
+template <int TPR, int NT>
+__device__ __forceinline__ void team_sync(uint32_t team)
+{
+    if (TPR == NT) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(TPR) : "memory");
+}
+
+template <int TPR, int NT>   // threads per row team: 32 (a warp) or a multiple of 32 dividing the CTA size NT
 __device__ __forceinline__ uint64_t team_reduce(uint64_t v, uint64_t *sRed)
 {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     if (TPR == 32) return v;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    __syncthreads();                                    // previous row's readers are done
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31, team = threadIdx.x / TPR;
+    team_sync<TPR, NT>(team);                           // previous row's readers are done
     if (lane == 0) sRed[warp] = v;
-    __syncthreads();
+    team_sync<TPR, NT>(team);
     uint64_t t = 0;
 #pragma unroll
-    for (int w = 0; w < kGemvThreads / 32; w++) t += sRed[w];
+    for (int w = 0; w < TPR / 32; w++) t += sRed[team * (TPR / 32) + w];
     return t;
 }
 
 // kRegen = false: A streamed from HBM.  kRegen = true: A never read, every 16-byte
 // chunk (8 elements) is one AES-CTR block of object (seed_A, LWE_TAG_A, inst 0)
 // (+ rejection attempts), S8(c) O4 -- the paper's on-demand A.
-template <int TPR, bool kRegen, int UNR>
-__global__ void __launch_bounds__(kGemvThreads)
+template <int TPR, bool kRegen, int UNR, int NT>
+__global__ void __launch_bounds__(NT)
 keygen_gemv_kernel(const uint16_t *__restrict__ A, AesKey key, const uint32_t *__restrict__ te0,
                    const uint16_t *__restrict__ s, const uint16_t *__restrict__ e, uint16_t *__restrict__ b,
                    uint32_t m, uint32_t n, uint32_t batch, ModQ mq)
 {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     uint32_t *sS = reinterpret_cast<uint32_t *>(smem_raw);                // n/2 words
-    uint64_t *sRed = reinterpret_cast<uint64_t *>(smem_raw + 2 * (size_t)n);  // 8 u64
-    const uint32_t *sTl = nullptr;
-    if (kRegen) {
-        uint32_t *sT = reinterpret_cast<uint32_t *>(smem_raw + 2 * (size_t)n + 64);
-        aes_table_to_smem(sT, te0);
-        sTl = sT + (threadIdx.x & 31);
-    }
+    uint64_t *sRed = reinterpret_cast<uint64_t *>(smem_raw + 2 * (size_t)n);  // one u64 per warp
+    AesTab tab = {};
+    if (kRegen) tab = aes_table_to_smem(smem_raw + 2 * (size_t)n + kRedBytes, te0);
 
-    constexpr int kTeams = kGemvThreads / TPR;
+    constexpr int kTeams = NT / TPR;
     const uint32_t team = threadIdx.x / TPR, tl = threadIdx.x % TPR;
     const uint32_t chunks = n / 8;                       // 16-byte chunks per row
     const uint32_t row0 = blockIdx.x * kTeams + team;
@@ -106,7 +111,7 @@ keygen_gemv_kernel(const uint16_t *__restrict__ A, AesKey key, const uint32_t *_
                 for (int u = 0; u < UNR; u++) {
                     uint32_t c = c0 + u * TPR;
                     if (c < chunks) {
-                        if (kRegen) a[u] = uniform_block(key, sTl, mq, LWE_TAG_A, 0, (uint64_t)i * chunks + c);
+                        if (kRegen) a[u] = uniform_block(key, tab, mq, LWE_TAG_A, 0, (uint64_t)i * chunks + c);
                         else a[u] = ldg_stream(Arow + c);
                     } else {
                         a[u] = make_uint4(0, 0, 0, 0);
@@ -126,7 +131,7 @@ keygen_gemv_kernel(const uint16_t *__restrict__ A, AesKey key, const uint32_t *_
             uint64_t total;
             if (mq.pow2) total = (uint64_t)(lo + (hi << 8));              // exact mod 2^32, q | 2^32
             else total = (sum_lo + lo) + ((sum_hi + hi) << 8);
-            total = team_reduce<TPR>(total, sRed);
+            total = team_reduce<TPR, NT>(total, sRed);
             if (tl == 0) {
                 uint32_t ei = e[(size_t)t * m + i];
                 uint32_t r = mq.pow2 ? (((uint32_t)total + ei) & mq.mask) : mod_u64(total + ei, mq);
@@ -136,13 +141,13 @@ keygen_gemv_kernel(const uint16_t *__restrict__ A, AesKey key, const uint32_t *_
     }
 }
 
-template <int TPR, bool kRegen, int UNR>
+template <int TPR, bool kRegen, int UNR, int NT = kGemvThreads>
 static cudaError_t launch_gemv(Ctx *c, const uint16_t *d_A, const AesKey &key, const uint16_t *d_s,
                                const uint16_t *d_e, uint16_t *d_b, uint32_t batch, cudaStream_t st)
 {
     const uint32_t n = c->p.n, m = c->p.m;
-    size_t smem = 2 * (size_t)n + 64 + (kRegen ? kAesTableBytes : 0);
-    auto kern = keygen_gemv_kernel<TPR, kRegen, UNR>;
+    size_t smem = 2 * (size_t)n + kRedBytes + (kRegen ? kAesTableBytes : 0);
+    auto kern = keygen_gemv_kernel<TPR, kRegen, UNR, NT>;
     // attribute + occupancy are queried once per (instantiation, smem size): host calls, not per launch
     static size_t cached_smem = 0;
     static int cached_per_sm = 0;
@@ -150,18 +155,18 @@ static cudaError_t launch_gemv(Ctx *c, const uint16_t *d_A, const AesKey &key, c
         cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (err != cudaSuccess) return err;
         int q = 0;
-        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&q, kern, kGemvThreads, smem);
+        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&q, kern, NT, smem);
         if (err != cudaSuccess) return err;
         cached_per_sm = q < 1 ? 1 : q;
         cached_smem = smem;
     }
     const int per_sm = cached_per_sm;
-    constexpr int kTeams = kGemvThreads / TPR;
+    constexpr int kTeams = NT / TPR;
     uint32_t grid = (uint32_t)(c->sm_count * per_sm);
     uint32_t need = (m + kTeams - 1) / kTeams;
     if (grid > need) grid = need;
     ProfScope prof(c, kRegen ? LWE_K_KEYGEN_REGEN : LWE_K_KEYGEN_STORED, st);
-    kern<<<grid, kGemvThreads, smem, st>>>(d_A, key, c->d_te0, d_s, d_e, d_b, m, n, batch, c->mq);
+    kern<<<grid, NT, smem, st>>>(d_A, key, c->d_te0, d_s, d_e, d_b, m, n, batch, c->mq);
     c->launches++;
     return cudaGetLastError();
 }
@@ -183,8 +188,19 @@ cudaError_t launch_keygen_stored(Ctx *c, const uint16_t *d_A, const uint16_t *d_
 cudaError_t launch_keygen_regen(Ctx *c, const AesKey &key, const uint16_t *d_s, const uint16_t *d_e,
                                 uint16_t *d_b, uint32_t batch, cudaStream_t st)
 {
-    if (c->p.n >= 4096) return launch_gemv<kGemvThreads, true, 4>(c, nullptr, key, d_s, d_e, d_b, batch, st);
-    return launch_gemv<32, true, 4>(c, nullptr, key, d_s, d_e, d_b, batch, st);
+    // one 64 KB AES table and one copy of s per CTA: large CTAs (4 row teams of 256, or 32 warp teams) keep
+    // 32 warps per SM behind a single table
+    switch (c->gemv_variant) {                           // measurement knob (LWE_OPT_GEMV_VARIANT), same result
+    case 1: return launch_gemv<256, true, 2, 1024>(c, nullptr, key, d_s, d_e, d_b, batch, st);
+    case 2: return launch_gemv<256, true, 1, 768>(c, nullptr, key, d_s, d_e, d_b, batch, st);
+    case 3: return launch_gemv<256, true, 1, 1024>(c, nullptr, key, d_s, d_e, d_b, batch, st);
+    case 4: return launch_gemv<32, true, 2, 1024>(c, nullptr, key, d_s, d_e, d_b, batch, st);
+    default: break;
+    }
+    // measured on B200 (C4, GB/s of A regenerated): 768 threads x 2 blocks in flight 698, 1024 x 2 663,
+    // 4 in flight spills at <= 85 registers and halves the rate
+    if (c->p.n >= 4096) return launch_gemv<256, true, 2, 768>(c, nullptr, key, d_s, d_e, d_b, batch, st);
+    return launch_gemv<32, true, 2, 1024>(c, nullptr, key, d_s, d_e, d_b, batch, st);
 }
 
 }  // namespace lwe

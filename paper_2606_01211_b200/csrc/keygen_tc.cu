@@ -9,16 +9,21 @@
 // Formulation (u8 x u8 -> s32, kind::i8).  A (m x n uint16, row-major) is read in place as the
 // uint8 matrix A8 (m x 2n): k' = 2j is the low byte of A[i][j], k' = 2j+1 the high byte.  Here the
 // contraction index k' is the FAST axis of A8: a K-major operand, the classic TMA/UMMA layout.
-// Each instance t contributes four K-major u8 rows to the B operand Sx (built by keygen_prep_kernel):
-//     col 4t+0: Sx[2j] = lo(s_j), Sx[2j+1] = 0         -> D0 = sum lo(A) lo(s)
-//     col 4t+1: Sx[2j] = hi(s_j), Sx[2j+1] = 0         -> D1 = sum lo(A) hi(s)
-//     col 4t+2: Sx[2j] = 0,       Sx[2j+1] = lo(s_j)   -> D2 = sum hi(A) lo(s)
-//     col 4t+3: Sx[2j] = 0,       Sx[2j+1] = hi(s_j)   -> D3 = sum hi(A) hi(s)
-// and  b[t][i] = (D0 + 2^8 (D1 + D2) + 2^16 D3 + e[t][i]) mod q,  combined in 64 bits.
-// Bounds: every D <= 255^2 n < 2^31 for n <= 33025 (the path is taken for n <= 32768).
+// Each instance t contributes CPI K-major u8 rows to the B operand Sx (built by keygen_prep_kernel):
+//     col 0: Sx[2j] = lo(s_j), Sx[2j+1] = 0         -> D0  = sum lo(A) lo(s)
+//     col 1: Sx[2j] = hi(s_j), Sx[2j+1] = lo(s_j)   -> D12 = sum lo(A) hi(s) + hi(A) lo(s)   (both 2^8 terms at once)
+//     col 2: Sx[2j] = 0,       Sx[2j+1] = hi(s_j)   -> D3  = sum hi(A) hi(s)
+// and  b[t][i] = (D0 + 2^8 D12 + 2^16 D3 + e[t][i]) mod q,  combined in 64 bits.
+//   CPI = 2 when q divides 2^16: the 2^16 D3 term vanishes mod q and col 2 is not needed; the s32 accumulators
+//           may then wrap mod 2^32 harmlessly (q | 2^32).
+//   CPI = 3 otherwise while D12 <= 2 * 255^2 * n < 2^31, i.e. n <= 16384;
+//   CPI = 4 for larger n: the two 2^8 terms in separate columns (hi, 0) and (0, lo), every D <= 255^2 n < 2^31 for
+//           n <= 33025 (the path is taken for n <= 32768).
+// The S operand is re-streamed from L2 by every strip, so its width is what loads the L2->SM path beside the
+// single HBM pass over A: 4 columns per instance made that path carry 2x the A stream (0.68 of HBM); 2 make it 1.5x.
 //
 // Shape.  One CTA owns a 128-row strip of A over the whole contraction (no split-K, no atomics):
-// tile 128 x N x 128 bytes of k' per stage, N = 4*batch rounded up to 16 (<= 256), TMA-fed
+// tile 128 x N x 128 bytes of k' per stage, N = CPI*batch rounded up (<= 256), TMA-fed
 // multi-stage ring sized to fill shared memory (192 KB in flight per SM hides HBM latency), two
 // TMEM accumulators so the epilogue of strip t overlaps the main loop of strip t+1.
 //   warp 0: TMA producer   warp 1: TMEM alloc + MMA issuer   warps 2-5: epilogue (one lane quarter each)
@@ -39,21 +44,39 @@ constexpr uint32_t kSmemBudget = 200 * 1024;
 
 __global__ void __launch_bounds__(256)
 keygen_prep_kernel(const uint16_t *__restrict__ s, uint16_t *__restrict__ Sx, uint32_t n, uint32_t batch,
-                   uint32_t ncols)
+                   uint32_t cpi)
 {
     // Sx viewed as uint16[ncols][n]: word j of a row = bytes (2j, 2j+1)
     const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t col = blockIdx.y;
     if (j >= n) return;
-    const uint32_t t = col >> 2, v = col & 3;
+    const uint32_t t = col / cpi, v = col - t * cpi;
     uint32_t w = 0;
     if (t < batch) {
         const uint32_t sj = s[(size_t)t * n + j];
-        w = (v == 0) ? (sj & 0xffu) : (v == 1) ? (sj >> 8) : (v == 2) ? ((sj & 0xffu) << 8) : (sj & 0xff00u);
+        const uint32_t lo = sj & 0xffu, hi = sj >> 8;
+        if (cpi == 4) w = (v == 0) ? lo : (v == 1) ? hi : (v == 2) ? (lo << 8) : (hi << 8);
+        else w = (v == 0) ? lo : (v == 1) ? (hi | (lo << 8)) : (hi << 8);
     }
     Sx[(size_t)col * n + j] = (uint16_t)w;
 }
 
+// 8 * CPI accumulator columns (= 8 instances) of this warp's 32 TMEM lanes
+template <uint32_t CPI>
+__device__ __forceinline__ void tmem_ld_8inst(uint32_t taddr, uint32_t (&r)[8 * CPI])
+{
+#pragma unroll
+    for (uint32_t g = 0; g < CPI; g++)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                     : "=r"(r[8 * g]), "=r"(r[8 * g + 1]), "=r"(r[8 * g + 2]), "=r"(r[8 * g + 3]), "=r"(r[8 * g + 4]),
+                       "=r"(r[8 * g + 5]), "=r"(r[8 * g + 6]), "=r"(r[8 * g + 7])
+                     : "r"(taddr + 8 * g));
+}
+
+// SLABS: 128-byte K slabs per pipeline stage.  A TMA box is at most 128 bytes wide under SWIZZLE_128B, i.e. 128
+// separate 128-byte pieces of 128 different rows of A; loading SLABS adjacent boxes back to back makes every
+// row piece SLABS*128 contiguous bytes for the memory system.
+template <uint32_t CPI, uint32_t SLABS>
 __global__ void __launch_bounds__(kThreads, 1)
 keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapS,
                  const uint16_t *__restrict__ e, uint16_t *__restrict__ b, uint32_t m, uint32_t n, uint32_t batch,
@@ -62,7 +85,8 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t base = (raw + 1023u) & ~1023u;
-    const uint32_t bytes_stage = kBytesA + N * kTileK;
+    const uint32_t bytes_slab = kBytesA + N * kTileK;
+    const uint32_t bytes_stage = SLABS * bytes_slab;
     const uint32_t bars = base + stages * bytes_stage;
     auto full_bar = [&](uint32_t s) { return bars + 8 * s; };
     auto empty_bar = [&](uint32_t s) { return bars + 8 * (kMaxStages + s); };
@@ -73,7 +97,7 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
 
     const uint32_t warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;   // warp-uniform
     const uint32_t strips = (m + kTileM - 1) / kTileM;
-    const uint32_t k_blocks = (2 * n + kTileK - 1) / kTileK;
+    const uint32_t k_blocks = (2 * n + SLABS * kTileK - 1) / (SLABS * kTileK);      // stages per strip
     const uint32_t acc_cols = (N <= 32) ? 32 : (N <= 64) ? 64 : (N <= 128) ? 128 : 256;   // per accumulator
     const uint32_t tmem_cols = 2 * acc_cols;
 
@@ -104,11 +128,16 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
             for (uint32_t kb = 0; kb < k_blocks; kb++) {
                 mbar_wait(empty_bar(stage), phase ^ 1);
                 const uint32_t sa = base + stage * bytes_stage;
-                const int32_t k0 = (int32_t)(kb * kTileK);
+                const int32_t k0 = (int32_t)(kb * SLABS * kTileK);
                 if (elect_one()) {
-                    mbar_expect_tx(full_bar(stage), bytes_stage);
-                    tma_load_2d(sa, &mapA, full_bar(stage), k0, row0);          // 128 rows x 128 bytes of k'
-                    tma_load_2d(sa + kBytesA, &mapS, full_bar(stage), k0, 0);   // N rows x 128 bytes of k'
+                    mbar_expect_tx(full_bar(stage), bytes_stage);                // out-of-range slabs arrive as zeros
+#pragma unroll
+                    for (uint32_t h = 0; h < SLABS; h++)                         // 128 rows x 128 bytes of k' each
+                        tma_load_2d(sa + h * kBytesA, &mapA, full_bar(stage), k0 + (int32_t)(h * kTileK), row0);
+#pragma unroll
+                    for (uint32_t h = 0; h < SLABS; h++)                         // N rows x 128 bytes of k' each
+                        tma_load_2d(sa + SLABS * kBytesA + h * N * kTileK, &mapS, full_bar(stage),
+                                    k0 + (int32_t)(h * kTileK), 0);
                 }
                 __syncwarp();
                 if (++stage == stages) { stage = 0; phase ^= 1; }
@@ -128,13 +157,16 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
                 const uint32_t sa = base + stage * bytes_stage;
                 if (elect_one()) {
                     // a K step is 32 bytes along the 128-byte swizzled row: advance the start address
-                    uint64_t adesc = make_desc_k_sw128(sa, 1024);
-                    uint64_t bdesc = make_desc_k_sw128(sa + kBytesA, 1024);
 #pragma unroll
-                    for (uint32_t ks = 0; ks < kTileK / kUmmaK; ks++) {
-                        umma_i8(d_tmem, adesc, bdesc, idesc, (kb | ks) ? 1u : 0u);
-                        adesc += kUmmaK >> 4;
-                        bdesc += kUmmaK >> 4;
+                    for (uint32_t h = 0; h < SLABS; h++) {
+                        uint64_t adesc = make_desc_k_sw128(sa + h * kBytesA, 1024);
+                        uint64_t bdesc = make_desc_k_sw128(sa + SLABS * kBytesA + h * N * kTileK, 1024);
+#pragma unroll
+                        for (uint32_t ks = 0; ks < kTileK / kUmmaK; ks++) {
+                            umma_i8(d_tmem, adesc, bdesc, idesc, (kb | h | ks) ? 1u : 0u);
+                            adesc += kUmmaK >> 4;
+                            bdesc += kUmmaK >> 4;
+                        }
                     }
                     umma_commit(empty_bar(stage));
                     if (kb == k_blocks - 1) umma_commit(tfull_bar(acc));
@@ -144,7 +176,7 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
             }
         }
     } else {
-        // epilogue: lane = row of the strip; 32 accumulator columns = 8 instances per tcgen05.ld
+        // epilogue: lane = row of the strip; 8 instances (8 * CPI accumulator columns) per step
         const uint32_t quarter = warp & 3;
         uint32_t it = 0;
         for (uint32_t t = blockIdx.x; t < strips; t += gridDim.x, it++) {
@@ -154,18 +186,26 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
             const uint32_t i = t * kTileM + quarter * 32 + lane;
             const uint32_t taddr = tmem_base + ((quarter * 32) << 16) + acc * acc_cols;
 #pragma unroll 1
-            for (uint32_t cb = 0; cb < 4 * batch; cb += 32) {
-                uint32_t r[32];
-                tmem_ld_32x32b_x32(taddr + cb, r);
+            for (uint32_t i0 = 0; i0 < batch; i0 += 8) {
+                uint32_t r[8 * CPI];
+                tmem_ld_8inst<CPI>(taddr + i0 * CPI, r);
                 tmem_ld_wait();
                 if (i < m) {
 #pragma unroll
                     for (uint32_t x = 0; x < 8; x++) {
-                        const uint32_t inst = (cb >> 2) + x;
+                        const uint32_t inst = i0 + x;
                         if (inst < batch) {
-                            uint64_t tot = (uint64_t)r[4 * x] + (((uint64_t)r[4 * x + 1] + r[4 * x + 2]) << 8) +
-                                           ((uint64_t)r[4 * x + 3] << 16) + e[(size_t)inst * m + i];
-                            uint32_t o = mq.pow2 ? ((uint32_t)tot & mq.mask) : mod_u64(tot, mq);
+                            const uint32_t ei = e[(size_t)inst * m + i];
+                            uint32_t o;
+                            if (CPI == 2) {
+                                o = (r[2 * x] + (r[2 * x + 1] << 8) + ei) & mq.mask;     // q | 2^16: wrap-around is exact
+                            } else {
+                                uint64_t tot = (CPI == 3)
+                                    ? (uint64_t)r[3 * x] + ((uint64_t)r[3 * x + 1] << 8) + ((uint64_t)r[3 * x + 2] << 16)
+                                    : (uint64_t)r[4 * x] + (((uint64_t)r[4 * x + 1] + r[4 * x + 2]) << 8) +
+                                          ((uint64_t)r[4 * x + 3] << 16);
+                                o = mod_u64(tot + ei, mq);
+                            }
                             b[(size_t)inst * m + i] = (uint16_t)o;
                         }
                     }
@@ -182,31 +222,41 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     if (warp == 1) tmem_dealloc(tmem_base, tmem_cols);
 }
 
-uint32_t padded_cols(uint32_t batch) { return (4 * batch + 15u) & ~15u; }
+// columns of the B operand per instance (see the header comment)
+uint32_t cols_per_inst(const lwe_params &p)
+{
+    const bool q_divides_2_16 = (p.q & (p.q - 1)) == 0;               // q <= 65536 always
+    return q_divides_2_16 ? 2u : (p.n <= 16384 ? 3u : 4u);
+}
+// 8 instances per epilogue step and 16-column MMA granularity: whole groups of 8 instances
+uint32_t padded_cols(uint32_t batch, uint32_t cpi) { return (((batch + 7u) & ~7u) * cpi + 15u) & ~15u; }
 
 }  // namespace
 
 size_t keygen_tc_workspace_bytes(const lwe_params &p)
 {
-    return (size_t)padded_cols(p.max_batch) * 2 * p.n;
+    const uint32_t N = padded_cols(p.max_batch, cols_per_inst(p));
+    return (p.n <= 32768 && N <= 256) ? (size_t)N * 2 * p.n : 0;       // 0: the tensor-core keygen is not available
 }
 
 bool keygen_tc_supported(const Ctx *c, uint32_t batch)
 {
     const lwe_params &p = c->p;
-    return c->encode_tiled != nullptr && c->d_Sx != nullptr && p.n <= 32768 && padded_cols(batch) <= 256 &&
-           padded_cols(p.max_batch) <= 256;
+    const uint32_t cpi = cols_per_inst(p);
+    return c->encode_tiled != nullptr && c->d_Sx != nullptr && p.n <= 32768 && padded_cols(batch, cpi) <= 256 &&
+           padded_cols(p.max_batch, cpi) <= 256;
 }
 
 cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, const uint16_t *d_e, uint16_t *d_b,
                              uint32_t batch, cudaStream_t st)
 {
     const lwe_params &p = c->p;
-    const uint32_t N = padded_cols(batch);
+    const uint32_t cpi = cols_per_inst(p);
+    const uint32_t N = padded_cols(batch, cpi);
     {
         ProfScope prof(c, LWE_K_KEYGEN_PREP, st);
         dim3 grid((p.n + 255) / 256, N);
-        keygen_prep_kernel<<<grid, 256, 0, st>>>(d_s, reinterpret_cast<uint16_t *>(c->d_Sx), p.n, batch, N);
+        keygen_prep_kernel<<<grid, 256, 0, st>>>(d_s, reinterpret_cast<uint16_t *>(c->d_Sx), p.n, batch, cpi);
         c->launches++;
         cudaError_t err = cudaGetLastError();
         if (err != cudaSuccess) return err;
@@ -214,21 +264,35 @@ cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, c
     CUtensorMap mapA, mapS;
     if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, p.m, kTileM)) return cudaErrorInvalidValue;
     if (!make_map_u8(c, &mapS, c->d_Sx, 2ull * p.n, N, N)) return cudaErrorInvalidValue;
-    const uint32_t bytes_stage = kBytesA + N * kTileK;
+    // slabs per stage: as wide as leaves >= 3 stages in flight (LWE_OPT_TUNE bits 10-11 force 1 / 2 / 4)
+    const uint32_t bytes_slab = kBytesA + N * kTileK;
+    uint32_t slabs = (3 * 4 * bytes_slab <= kSmemBudget) ? 4 : (3 * 2 * bytes_slab <= kSmemBudget) ? 2 : 1;
+    const uint32_t force = ((uint32_t)c->tune >> 10) & 3u;
+    if (force) slabs = force == 3 ? 4 : force;
+    if (kSmemBudget / (slabs * bytes_slab) < 2) slabs = 1;
+    const uint32_t bytes_stage = slabs * bytes_slab;
     uint32_t stages = kSmemBudget / bytes_stage;
     if (stages > kMaxStages) stages = kMaxStages;
     const uint32_t smem = stages * bytes_stage + 1024 + 256;
-    static int configured = 0;
-    if (!configured) {
-        cudaError_t err = cudaFuncSetAttribute(keygen_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    typedef void (*Kern)(const CUtensorMap, const CUtensorMap, const uint16_t *, uint16_t *, uint32_t, uint32_t, uint32_t,
+                         uint32_t, uint32_t, ModQ);
+    static const Kern table[3][3] = {
+        {keygen_tc_kernel<2, 1>, keygen_tc_kernel<2, 2>, keygen_tc_kernel<2, 4>},
+        {keygen_tc_kernel<3, 1>, keygen_tc_kernel<3, 2>, keygen_tc_kernel<3, 4>},
+        {keygen_tc_kernel<4, 1>, keygen_tc_kernel<4, 2>, keygen_tc_kernel<4, 4>}};
+    const uint32_t si = slabs == 4 ? 2 : slabs - 1;
+    Kern kern = table[cpi - 2][si];
+    static int configured[3][3] = {};
+    if (!configured[cpi - 2][si]) {
+        cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                (int)(kSmemBudget + 1024 + 256));
         if (err != cudaSuccess) return err;
-        configured = 1;
+        configured[cpi - 2][si] = 1;
     }
     const uint32_t strips = (p.m + kTileM - 1) / kTileM;
     const uint32_t grid = strips < (uint32_t)c->sm_count ? strips : (uint32_t)c->sm_count;
     ProfScope prof(c, LWE_K_KEYGEN_TC, st);
-    keygen_tc_kernel<<<grid, kThreads, smem, st>>>(mapA, mapS, d_e, d_b, p.m, p.n, batch, N, stages, c->mq);
+    kern<<<grid, kThreads, smem, st>>>(mapA, mapS, d_e, d_b, p.m, p.n, batch, N, stages, c->mq);
     c->launches++;
     return cudaGetLastError();
 }

@@ -83,6 +83,8 @@ struct Ctx {
     unsigned long long *d_vacc;       // [max_batch*k] u64 partial sums of b^T R
     unsigned long long *d_dacc;       // [max_batch*k] u64 partial sums of U^T s
     unsigned int *d_counters;         // [8 + max_batch] self-resetting "last block" tickets
+    uint32_t *d_foflags;              // [max_batch] mismatch flags of the FO re-encryption check
+    uint16_t *d_vprime;               // [max_batch][k] re-encrypted v'
     // staging for lwe_kem_host
     uint16_t *d_hs, *d_he, *d_hb, *d_hU, *d_hv;
     uint8_t *d_hR, *d_hmu, *d_hmuout;
@@ -111,6 +113,7 @@ struct ProfScope {
     ProfScope(Ctx *c_, int kernel_id, cudaStream_t st_) : c(c_), st(st_), slot(-1)
     {
         if (!c->profile || !c->ev || c->n_ev >= kMaxProfEvents) return;
+        if (c->profile >= 2 && c->profile - 2 != kernel_id) return;      // only one kernel is being timed
         slot = c->n_ev++;
         c->ev_kernel[slot] = (uint8_t)kernel_id;
         cudaEventRecord(c->ev[2 * slot], st);
@@ -159,16 +162,19 @@ cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_
                                   const uint8_t *d_mubits, uint16_t *d_v, uint32_t batch,
                                   bool write_Rexp, cudaStream_t st);
 // The three U = A^T R kernels take a ROW PANEL of A: d_A holds rows [row0, row0 + rows) of the m-row matrix
-// (row0 = 0, rows = m for a stored A); accumulate = add the residues already in d_U (panels after the first
-// when A is regenerated panel by panel).
+// (row0 = 0, rows = m for a stored A).  mode (EpiMode in tc_common.cuh): 0 = store U; 1 = add the residues
+// already in d_U (panels after the first when A is regenerated panel by panel); 2 = write nothing, compare with
+// d_U and OR a mismatch into d_flags[instance] (FO re-encryption check).
 cudaError_t launch_encaps_simt(Ctx *c, const uint16_t *d_A, const uint8_t *d_Rbits, uint16_t *d_U,
-                               uint32_t batch, uint32_t row0, uint32_t rows, bool accumulate, cudaStream_t st);
+                               uint32_t batch, uint32_t row0, uint32_t rows, int mode, uint32_t *d_flags, cudaStream_t st);
 bool encaps_tc_supported(const Ctx *c, uint32_t batch);
 cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0,
-                             uint32_t rows, bool accumulate, cudaStream_t st);
+                             uint32_t rows, int mode, uint32_t *d_flags, cudaStream_t st);
 bool encaps_tc2_supported(const Ctx *c, uint32_t batch);
 cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0,
-                              uint32_t rows, bool accumulate, cudaStream_t st);
+                              uint32_t rows, int mode, uint32_t *d_flags, cudaStream_t st);
+cudaError_t launch_fo_verdict(Ctx *c, const uint16_t *d_v, const uint16_t *d_vprime, const uint32_t *d_flags,
+                              uint8_t *d_ok, uint32_t batch, cudaStream_t st);
 cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
                           uint8_t *d_out, uint32_t batch, cudaStream_t st);
 

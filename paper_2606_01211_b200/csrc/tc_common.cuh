@@ -196,15 +196,28 @@ __host__ __device__ constexpr uint32_t instr_desc_u8(uint32_t M, uint32_t N, boo
            ((M >> 4) << 24);
 }
 
-// Epilogue store of 16 consecutive columns of one row of U (two 16-byte stores).  kAccum: add the residues
-// already stored there (mod q) -- used when the contraction over the rows of A is split into panels
-// (A regenerated panel by panel, encaps with d_A == NULL): a sum of residues mod q is the residue of the sum.
-template <bool kAccum>
-__device__ __forceinline__ void store_u16x16(uint4 *dst, uint32_t (&o)[16], const ModQ &mq)
+// What the U = A^T R kernels do with a finished 16-column piece of a row of U.
+//   kEpiStore:   write it.
+//   kEpiAccum:   add the residues already stored there (mod q) -- the contraction over the rows of A split into
+//                panels (A regenerated panel by panel, encaps with d_A == NULL): a sum of residues mod q is the
+//                residue of the sum.
+//   kEpiCompare: write nothing; compare with what is stored there (the received ciphertext) and report a
+//                mismatch -- the re-encryption check c' = c of the FO transform (Alg.5 l.2-4) without
+//                ever materialising c'.
+enum EpiMode { kEpiStore = 0, kEpiAccum = 1, kEpiCompare = 2 };
+
+template <int kMode>
+__device__ __forceinline__ bool store_u16x16(uint4 *dst, uint32_t (&o)[16], const ModQ &mq)
 {
-    if (kAccum) {
+    if (kMode != kEpiStore) {
         const uint4 p0 = dst[0], p1 = dst[1];
         const uint32_t old[8] = {p0.x, p0.y, p0.z, p0.w, p1.x, p1.y, p1.z, p1.w};
+        if (kMode == kEpiCompare) {
+            uint32_t diff = 0;
+#pragma unroll
+            for (int x = 0; x < 8; x++) diff |= old[x] ^ (o[2 * x] | (o[2 * x + 1] << 16));
+            return diff != 0;
+        }
 #pragma unroll
         for (int x = 0; x < 16; x++) {
             uint32_t val = o[x] + ((x & 1) ? (old[x >> 1] >> 16) : (old[x >> 1] & 0xffffu));   // < 2q
@@ -213,7 +226,36 @@ __device__ __forceinline__ void store_u16x16(uint4 *dst, uint32_t (&o)[16], cons
     }
     dst[0] = make_uint4(o[0] | (o[1] << 16), o[2] | (o[3] << 16), o[4] | (o[5] << 16), o[6] | (o[7] << 16));
     dst[1] = make_uint4(o[8] | (o[9] << 16), o[10] | (o[11] << 16), o[12] | (o[13] << 16), o[14] | (o[15] << 16));
+    return false;
 }
+
+// kEpiCompare bookkeeping of one epilogue lane: mismatches are OR-ed per instance and flushed with ONE
+// reduction per (lane, instance) -- issued whether or not anything differed, so the work done does not depend
+// on the validity of the ciphertext ("constant-time decapsulation path").
+struct MismatchAcc {
+    uint32_t inst = 0xffffffffu, bad = 0;
+    __device__ __forceinline__ void note(uint32_t *flags, uint32_t i, bool b)
+    {
+        if (i != inst) { flush(flags); inst = i; }
+        bad |= b ? 1u : 0u;
+    }
+    __device__ __forceinline__ void flush(uint32_t *flags)
+    {
+        if (inst != 0xffffffffu) atomicOr(flags + inst, bad);
+        bad = 0;
+        inst = 0xffffffffu;
+    }
+    // end of a tile, whole warp converged: lanes holding the same instance share one reduction
+    __device__ __forceinline__ void flush_warp(uint32_t *flags)
+    {
+        const uint32_t grp = __match_any_sync(0xffffffffu, inst);
+        const uint32_t badmask = __ballot_sync(0xffffffffu, bad != 0);
+        if (inst != 0xffffffffu && (threadIdx.x & 31) == (uint32_t)(__ffs(grp) - 1))
+            atomicOr(flags + inst, (badmask & grp) ? 1u : 0u);
+        bad = 0;
+        inst = 0xffffffffu;
+    }
+};
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,

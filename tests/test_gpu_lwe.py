@@ -45,6 +45,7 @@ def test_keygen_stored_matches_oracle(H, m, n, q, batch):
 
 KEYGEN_TC_SHAPES = [  # (m, n, q, batch): forced tcgen05 skinny GEMM (reads A once for the whole batch)
     (512, 256, 65536, 1), (512, 256, 65536, 4), (264, 4096, 65521, 5), (136, 4104, 65521, 2), (1000, 40, 65521, 3),
+    (256, 20000, 65521, 9), (256, 512, 32768, 40), (136, 264, 65536, 128),
     (8, 8, 17, 1), (2048, 1024, 65536, 32), (640, 520, 3329, 33), (384, 1024, 65521, 64), (16384, 8192, 65536, 32),
 ]
 
@@ -70,9 +71,11 @@ def test_keygen_tensor_core_batched_matches_oracle_and_gemv(H, m, n, q, batch):
 
 
 def test_keygen_tensor_core_extreme_values(H):
-    # every byte product and all four plane accumulators at their maxima (n = 32768 is the path's limit)
-    for q in (65536, 65521):
-        m, n, batch = 128, 32768, 2
+    # every byte product and every plane accumulator at its maximum: q = 65536 runs 2 operand columns per
+    # instance and lets the s32 accumulators wrap (exact mod 2^16) at n = 32768, the path's limit; q = 65521 runs
+    # 3 columns up to n = 16384 (the merged 2^8 accumulator just below 2^31) and 4 columns above
+    for q, n in ((65536, 32768), (65521, 32768), (65521, 16384), (65536, 16384)):
+        m, batch = 128, 2
         A = np.full((m, n), 0xFFFF if q == 65536 else q - 1, np.uint16)
         s = np.full((batch, n), 0xFFFF if q == 65536 else q - 1, np.uint16)
         e = np.full((batch, m), q - 1, np.uint16)
@@ -337,3 +340,47 @@ def test_kem_host_pipeline_matches_oracle(H, n, m, k, q, batch, regen):
         assert np.array_equal(gb[t], b), ("b", t)
         assert np.array_equal(gU[t], U) and np.array_equal(gv[t], v), ("U/v", t)
         assert np.array_equal(gout[t], O.decaps(U, v, s[t], q)), ("mu'", t)
+
+
+# ---------------------------------------------------------------- N3: decaps with the FO re-encryption check
+
+@pytest.mark.parametrize("path", **ENCAPS_PATHS)
+@pytest.mark.parametrize("n,m,k,q,batch", [(256, 512, 256, 65536, 1), (192, 392, 256, 65521, 6), (64, 136, 128, 65536, 5),
+                                            (1280, 384, 256, 65521, 3)])
+def test_decaps_fo_matches_oracle_honest_and_tampered(H, path, n, m, k, q, batch):
+    """lwe_decaps_fo against the oracle's Alg. 5 (O11) instance by instance: honest ciphertexts, a tampered element of
+    U in the first / last / a middle tile, a tampered v (small: m' unchanged; large: a bit of m' flips), wrong coins.
+    U is compared inside the GEMM epilogue and is never written (checked)."""
+    import torch
+    A = W.random_u16((m, n), q, 61)
+    s = W.random_u16((batch, n), q, 62)
+    e = W.random_u16((batch, m), 5, 63)
+    Rbits = W.random_bytes(batch * m * k // 8, 64).reshape(batch, -1)
+    mubits = W.random_bytes(batch * k // 8, 65).reshape(batch, -1)
+    b = np.stack([O.keygen(A, s[t], e[t], q) for t in range(batch)])
+    U = np.empty((batch, n, k), np.uint16); v = np.empty((batch, k), np.uint16)
+    for t in range(batch):
+        U[t], v[t] = O.encaps(A, b[t], Rbits[t], mubits[t], k, q)
+    R_in = Rbits.copy()
+    # instance t gets tamper number t (0 = honest)
+    tampers = ["honest", "U_first", "U_last", "v_small", "v_big", "coins"]
+    for t in range(batch):
+        kind = tampers[t % len(tampers)]
+        if kind == "U_first": U[t, 0, 0] = (int(U[t, 0, 0]) + 1) % q
+        if kind == "U_last": U[t, n - 1, k - 1] = (int(U[t, n - 1, k - 1]) + q - 1) % q
+        if kind == "v_small": v[t, 3] = (int(v[t, 3]) + 1) % q
+        if kind == "v_big": v[t, k - 1] = (int(v[t, k - 1]) + q // 2 + 3) % q
+        if kind == "coins": R_in[t, 9] ^= 0x40
+    with B().Context(n, m, k, q, 4, batch) as c:
+        c.set_option(B().OPT_ENCAPS_PATH, path)
+        dU = H.dev(U)
+        out, ok = H.dev_empty_u8(batch, k // 8), H.dev_empty_u8(batch)
+        ok.fill_(7)
+        c.decaps_fo(H.dev(A), H.dev(b), dU, H.dev(v), H.dev(s), H.dev(R_in), out, ok, batch)
+        g_out, g_ok = H.host_u8(out), H.host_u8(ok)
+        assert np.array_equal(H.host_u16(dU), U), "the received ciphertext must not be modified"
+    for t in range(batch):
+        o_out, o_ok = O.decaps_fo(A, b[t], U[t], v[t], s[t], R_in[t], q)
+        assert int(g_ok[t]) == o_ok, (t, tampers[t % len(tampers)])
+        assert np.array_equal(g_out[t], o_out), t
+        assert o_ok == (1 if tampers[t % len(tampers)] == "honest" else 0)

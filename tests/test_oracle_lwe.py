@@ -208,3 +208,58 @@ def test_wrong_secret_does_not_decapsulate():
     s_bad = W.random_u16(s.shape, w.q, 99)
     wrong = unpack_bits(O.decaps(U, v, s_bad, w.q), w.k) != unpack_bits(mubits, w.k)
     assert 64 < wrong.sum() < 192                                       # ~half the bits flip
+
+
+# ---------------------------------------------------------------- O11: FO re-encryption check (Alg. 5)
+
+def fo_case(w, n, m, inst=0):
+    A, s, e, Rbits, mubits = kem_from_seed(w, n, m, inst=inst)
+    b = O.keygen(A, s, e, w.q)
+    U, v = O.encaps(A, b, Rbits, mubits, w.k, w.q)
+    return A, s, b, Rbits, mubits, U, v
+
+
+@pytest.mark.parametrize("w,n,m", [(W.C1, 64, 128), (W.C3, 96, 192)])
+def test_o11_honest_ciphertext_is_accepted_and_decrypts(w, n, m):
+    A, s, b, Rbits, mubits, U, v = fo_case(w, n, m)
+    out, ok = O.decaps_fo(A, b, U, v, s, Rbits, w.q)
+    assert ok == 1 and np.array_equal(out, mubits)
+
+
+@pytest.mark.parametrize("w,n,m", [(W.C1, 64, 128), (W.C3, 96, 192)])
+def test_o11_any_change_of_the_ciphertext_is_rejected(w, n, m):
+    """Alg. 5 l.4: c' = c fails for a tampered c -- both for a change too small to alter m' (the re-encryption
+    of the SAME message differs from the tampered c in that element) and for one that flips a bit of m'."""
+    A, s, b, Rbits, mubits, U, v = fo_case(w, n, m)
+    q, k = w.q, w.k
+    # +1 on one element of v: d moves by 1, far from the threshold -> m' unchanged, verdict 0
+    v1 = v.copy(); v1[7] = (int(v1[7]) + 1) % q
+    out, ok = O.decaps_fo(A, b, U, v1, s, Rbits, q)
+    assert ok == 0 and np.array_equal(out, mubits)
+    # +floor(q/2)+3 on one element of v: that bit of m' flips, and v' = b^T R + m'*floor(q/2) is 3 (or 2, odd q) away
+    v2 = v.copy(); v2[200] = (int(v2[200]) + q // 2 + 3) % q
+    out, ok = O.decaps_fo(A, b, U, v2, s, Rbits, q)
+    flipped = unpack_bits(out, k) != unpack_bits(mubits, k)
+    assert ok == 0 and flipped.sum() == 1 and flipped[200]
+    # one element of U (first, last, middle), +1: rejected
+    for (j, c) in ((0, 0), (n - 1, k - 1), (n // 2, 17)):
+        U1 = U.copy(); U1[j, c] = (int(U1[j, c]) + 1) % q
+        _, ok = O.decaps_fo(A, b, U1, v, s, Rbits, q)
+        assert ok == 0, (j, c)
+    # wrong coins: the re-encryption does not reproduce c
+    R_bad = Rbits.copy(); R_bad[5] ^= 0x10
+    out, ok = O.decaps_fo(A, b, U, v, s, R_bad, q)
+    assert ok == 0 and np.array_equal(out, mubits)
+
+
+def test_o11_coins_are_an_input_exact_half_shift_is_a_valid_ciphertext():
+    """The reading taken (S19): the coins R are an INPUT of the check (the paper derives them
+    through hashes that are outside the hot path).  Then, for q = 2^16, v + q/2 in one position is exactly the
+    encryption of the message with that bit flipped under the same coins, so the check accepts it and m' differs
+    in that bit -- binding the coins to m is the hash layer's job.  Pins the verdict to 'c' == c', nothing more."""
+    w = W.C1
+    A, s, b, Rbits, mubits, U, v = fo_case(w, 64, 128)
+    v2 = v.copy(); v2[31] = (int(v2[31]) + w.q // 2) % w.q
+    out, ok = O.decaps_fo(A, b, U, v2, s, Rbits, w.q)
+    flipped = unpack_bits(out, w.k) != unpack_bits(mubits, w.k)
+    assert ok == 1 and flipped.sum() == 1 and flipped[31]
