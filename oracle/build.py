@@ -39,7 +39,7 @@ def build(force: bool = False) -> Path:
     for cc in _compilers():
         for omp in (["-fopenmp"], []):
             cmd = [cc, "-O2", "-std=c11", "-Wall", "-Wextra", "-fPIC", *omp,
-                   "-shared", "-o", str(LIB), str(SRC[0])]
+                   "-shared", "-o", str(LIB), str(SRC[0]), "-lm"]
             r = subprocess.run(cmd, capture_output=True, text=True)
             if r.returncode == 0:
                 return LIB

@@ -10,6 +10,7 @@
 #include "lwe_oracle.h"
 
 #include <stdlib.h>
+#include <math.h>
 #include <string.h>
 #ifdef _OPENMP
 #include <omp.h>
@@ -437,6 +438,102 @@ int orc_decaps_fo(const uint16_t *A, const uint16_t *b, const uint16_t *U, const
     free(U2);
     free(v2);
     return equal;
+}
+
+/* ================================================================== N2: the paper's own PKE variant
+ * (Table 1 header P:L92: Gaussian sigma for e, r, e1; centred uniform for e2;
+ * binomial eta = 3 for s; square A).  Readings S20-S22 of DESIGN.md section 3. */
+
+/* O12. 16-bit CDT of the rounded Gaussian z = round(sigma * N(0,1)), support [-12, 12]:
+ * C[j] = floor(65536 * Phi((j - 12 + 1/2) / sigma) + 1/2), j = 0..23, Phi the standard normal CDF. */
+void orc_gauss_cdt(double sigma, uint32_t cdt[ORC_GAUSS_CDT_LEN])
+{
+    for (int j = 0; j < ORC_GAUSS_CDT_LEN; j++) {
+        double x = ((double)j - (double)ORC_GAUSS_TAU + 0.5) / sigma;
+        double Phi = 0.5 * erfc(-x / sqrt(2.0));
+        cdt[j] = (uint32_t)floor(65536.0 * Phi + 0.5);
+    }
+}
+
+/* z = -tau + #{ j : w >= C[j] } for a 16-bit stream word w */
+int orc_gauss_from_word(uint32_t w, const uint32_t cdt[ORC_GAUSS_CDT_LEN])
+{
+    int z = -ORC_GAUSS_TAU;
+    for (int j = 0; j < ORC_GAUSS_CDT_LEN; j++)
+        if (w >= cdt[j]) z++;
+    return z;
+}
+
+/* element t: w = LE16(bytes [2t, 2t+1] of KS(key(seed), iv(tag, 0, inst))); z as above.
+ * out_s8 (if not NULL) receives z; out_u16 (if not NULL) receives z mod q in [0, q). */
+void orc_sample_gauss(int8_t *out_s8, uint16_t *out_u16, uint64_t first, uint64_t count,
+                      uint64_t seed, uint32_t tag, uint32_t inst, double sigma, uint32_t q)
+{
+    uint8_t key[16], rk[176];
+    uint32_t cdt[ORC_GAUSS_CDT_LEN];
+    sbox_init();
+    orc_seed_key(seed, key);
+    aes128_expand_key(key, rk);
+    orc_gauss_cdt(sigma, cdt);
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (uint64_t x = 0; x < count; x++) {
+        int z = orc_gauss_from_word(stream_word16(rk, tag, 0, inst, first + x), cdt);
+        if (out_s8) out_s8[x] = (int8_t)z;
+        if (out_u16) out_u16[x] = (uint16_t)((((int64_t)z % (int64_t)q) + (int64_t)q) % (int64_t)q);
+    }
+}
+
+/* O13. Centred uniform on [-bound, bound]: rejection exactly as O4 with modulus q' = 2*bound + 1
+ * (attempt streams), value (c mod q') - bound. */
+void orc_sample_cuniform(int8_t *out, uint64_t first, uint64_t count,
+                         uint64_t seed, uint32_t tag, uint32_t inst, uint32_t bound)
+{
+    uint8_t key[16], rk[176];
+    sbox_init();
+    orc_seed_key(seed, key);
+    aes128_expand_key(key, rk);
+    const uint32_t qq = 2 * bound + 1, T = qq * (65536u / qq);
+    for (uint64_t x = 0; x < count; x++) {
+        uint32_t c = stream_word16(rk, tag, 0, inst, first + x);
+        for (uint32_t attempt = 1; c >= T; attempt++)
+            c = stream_word16(rk, tag, attempt, inst, first + x);
+        out[x] = (int8_t)((int)(c % qq) - (int)bound);
+    }
+}
+
+static uint64_t mod_signed(int64_t x, uint32_t q)
+{
+    int64_t r = x % (int64_t)q;
+    return (uint64_t)(r < 0 ? r + (int64_t)q : r);
+}
+
+/* O14. Encrypt of the paper's PKE for all k bits at once:
+ * U[j*k+c] = (sum_i A[i*n+j]*R[i*k+c] + E1[j*k+c]) mod q
+ * v[c]     = (sum_i t[i]*R[i*k+c] + e2[c] + mu_c*floor(q/2)) mod q        (R, E1, e2 small signed integers) */
+void orc_encaps_pv(const uint16_t *A, const uint16_t *t, const int8_t *R, const int8_t *E1, const int8_t *e2,
+                   const uint8_t *mubits, uint16_t *U, uint16_t *v,
+                   uint32_t m, uint32_t n, uint32_t k, uint32_t q)
+{
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (uint32_t j = 0; j < n; j++)
+        for (uint32_t c = 0; c < k; c++) {
+            uint64_t acc = 0;
+            for (uint32_t i = 0; i < m; i++)
+                acc = (acc + (uint64_t)A[(size_t)i * n + j] * mod_signed(R[(size_t)i * k + c], q)) % q;
+            U[(size_t)j * k + c] = (uint16_t)((acc + mod_signed(E1[(size_t)j * k + c], q)) % q);
+        }
+    for (uint32_t c = 0; c < k; c++) {
+        uint64_t acc = 0;
+        for (uint32_t i = 0; i < m; i++)
+            acc = (acc + (uint64_t)t[i] * mod_signed(R[(size_t)i * k + c], q)) % q;
+        acc = (acc + mod_signed(e2[c], q)) % q;
+        acc = (acc + (uint64_t)get_bit(mubits, c) * (q / 2)) % q;
+        v[c] = (uint16_t)acc;
+    }
 }
 
 int orc_num_threads(void)

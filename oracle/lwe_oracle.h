@@ -124,6 +124,44 @@ int orc_decaps_fo(const uint16_t *A, const uint16_t *b, const uint16_t *U, const
                   const uint16_t *s, const uint8_t *Rbits, uint8_t *mubits_out,
                   uint32_t m, uint32_t n, uint32_t k, uint32_t q);
 
+/* ---- N2: the paper's own PKE variant.  P:L64 (KeyGen / Encrypt / Decrypt; Fig. 1 is an image whose
+ * text is lost), P:L70 (secret ~ binomial eta = 3), Table 1 header P:L92 (Gaussian sigma for e, r, e1;
+ * centred uniform k for e2).  Readings S20-S22 of DESIGN.md section 3:
+ *   KeyGen  t = A s + e,  A in Z_q^{n x n}, s ~ CBD(3)^n (O5), e ~ D_sigma^n (O12)            -> O7 with m = n
+ *   Encrypt (all k bits): R in Z^{n x k}, E1 in Z^{n x k} ~ D_sigma (O12), e2 in Z^k ~ U[-kappa, kappa] (O13)
+ *           U = A^T R + E1,  v = t^T R + e2 + mu floor(q/2)                                  -> O14
+ *   Decrypt = O9.
+ * Object tags of the new streams. */
+enum { ORC_TAG_RG = 6, ORC_TAG_E1 = 7, ORC_TAG_E2 = 8 };
+#define ORC_GAUSS_TAU 12
+#define ORC_GAUSS_CDT_LEN (2 * ORC_GAUSS_TAU)
+
+/* O12. Rounded Gaussian z = round(sigma * N(0,1)) through a 16-bit cumulative table:
+ * C[j] = floor(65536 * Phi((j - 12 + 1/2) / sigma) + 1/2), j = 0..23 (Phi = standard normal CDF, in double);
+ * for the 16-bit stream word w of element t (as in O5): z = -12 + #{ j : w >= C[j] }.
+ * So P(z) = (C[z+12] - C[z+11]) / 65536 with C[-1] = 0, C[24] = 65536: the rounded-Gaussian pmf
+ * Phi((z+1/2)/sigma) - Phi((z-1/2)/sigma) to within 2^-16 per value.  The paper does not describe its sampler.
+ * Pins: the table against an independent normal CDF and against numerical integration of the density; the
+ * exhaustive histogram over all 65536 words; symmetry; mean 0 and variance sigma^2 + 1/12. */
+void orc_gauss_cdt(double sigma, uint32_t cdt[ORC_GAUSS_CDT_LEN]);
+int orc_gauss_from_word(uint32_t w, const uint32_t cdt[ORC_GAUSS_CDT_LEN]);
+void orc_sample_gauss(int8_t *out_s8, uint16_t *out_u16, uint64_t first, uint64_t count,
+                      uint64_t seed, uint32_t tag, uint32_t inst, double sigma, uint32_t q);
+
+/* O13. Centred uniform on [-bound, bound] (Table 1 "centered uniform k (e2)"): O4's rejection rule with modulus
+ * q' = 2*bound + 1 over the attempt streams, value (c mod q') - bound. */
+void orc_sample_cuniform(int8_t *out, uint64_t first, uint64_t count,
+                         uint64_t seed, uint32_t tag, uint32_t inst, uint32_t bound);
+
+/* O14. Encrypt of the paper's PKE, all k bits at once:
+ * U[j*k+c] = (sum_{i<m} A[i*n+j]*R[i*k+c] + E1[j*k+c]) mod q ;
+ * v[c]     = (sum_{i<m} t[i]*R[i*k+c] + e2[c] + mu_c*floor(q/2)) mod q ;   R, E1, e2 signed (int8).
+ * Pins: python big-integer brute force; reduces to O8 for R in {0,1}, E1 = 0, e2 = 0; the noise identity
+ * v - U^T s - mu floor(q/2) = e^T R + e2 - s^T E1 (mod q); every bit recovered on Table 1's first parameter set. */
+void orc_encaps_pv(const uint16_t *A, const uint16_t *t, const int8_t *R, const int8_t *E1, const int8_t *e2,
+                   const uint8_t *mubits, uint16_t *U, uint16_t *v,
+                   uint32_t m, uint32_t n, uint32_t k, uint32_t q);
+
 /* Number of OpenMP threads the loops above will use (1 if built without OpenMP). */
 int orc_num_threads(void);
 

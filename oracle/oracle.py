@@ -12,12 +12,15 @@ import numpy as np
 from . import build as _build
 
 TAG_A, TAG_S, TAG_E, TAG_R, TAG_MU = 1, 2, 3, 4, 5
+TAG_RG, TAG_E1, TAG_E2 = 6, 7, 8          # N2: Gaussian r, e1 and centred-uniform e2 of the paper's PKE
+GAUSS_TAU = 12
 
 __all__ = [
-    "TAG_A", "TAG_S", "TAG_E", "TAG_R", "TAG_MU",
+    "TAG_A", "TAG_S", "TAG_E", "TAG_R", "TAG_MU", "TAG_RG", "TAG_E1", "TAG_E2", "GAUSS_TAU",
     "aes128_encrypt_block", "ctr_bytes", "seed_key", "object_iv",
     "sample_uniform", "sample_uniform_strided", "sample_cbd", "sample_bits",
     "keygen", "encaps", "encaps_rows", "encaps_v", "decaps", "decaps_fo", "num_threads",
+    "gauss_cdt", "gauss_from_word", "sample_gauss", "sample_cuniform", "encaps_pv",
     "cbd_from_word", "round_bit",
 ]
 
@@ -45,6 +48,17 @@ def _L():
         lib.orc_decaps.argtypes = [u16p, u16p, u16p, u8p, u16p, u32, u32, u32]
         lib.orc_decaps_fo.argtypes = [u16p, u16p, u16p, u16p, u16p, u8p, u8p, u32, u32, u32, u32]
         lib.orc_decaps_fo.restype = C.c_int
+        s8p, dbl = C.POINTER(C.c_int8), C.c_double
+        lib.orc_gauss_cdt.argtypes = [dbl, u32p]
+        lib.orc_gauss_cdt.restype = None
+        lib.orc_gauss_from_word.argtypes = [u32, u32p]
+        lib.orc_gauss_from_word.restype = C.c_int
+        lib.orc_sample_gauss.argtypes = [s8p, u16p, u64, u64, u64, u32, u32, dbl, u32]
+        lib.orc_sample_gauss.restype = None
+        lib.orc_sample_cuniform.argtypes = [s8p, u64, u64, u64, u32, u32, u32]
+        lib.orc_sample_cuniform.restype = None
+        lib.orc_encaps_pv.argtypes = [u16p, u16p, s8p, s8p, s8p, u8p, u16p, u16p, u32, u32, u32, u32]
+        lib.orc_encaps_pv.restype = None
         lib.orc_num_threads.restype = C.c_int
         lib.orc_cbd_from_word.argtypes = [u32, u32, u32]
         lib.orc_cbd_from_word.restype = C.c_uint16
@@ -184,6 +198,49 @@ def decaps_fo(A, b, U, v, s, Rbits, q: int):
     ok = _L().orc_decaps_fo(_p(A, C.c_uint16), _p(b, C.c_uint16), _p(U, C.c_uint16), _p(v, C.c_uint16),
                             _p(s, C.c_uint16), _p(Rbits, C.c_uint8), _p(out, C.c_uint8), m, n, k, q)
     return out, int(ok)
+
+
+def gauss_cdt(sigma: float) -> np.ndarray:
+    """O12: the 24-entry 16-bit cumulative table of the rounded Gaussian"""
+    cdt = np.zeros(2 * GAUSS_TAU, np.uint32)
+    _L().orc_gauss_cdt(float(sigma), _p(cdt, C.c_uint32))
+    return cdt
+
+
+def gauss_from_word(w: int, cdt) -> int:
+    cdt = np.ascontiguousarray(cdt, dtype=np.uint32)
+    return int(_L().orc_gauss_from_word(int(w), _p(cdt, C.c_uint32)))
+
+
+def sample_gauss(first: int, count: int, seed: int, tag: int, inst: int, sigma: float, q: int | None = None) -> np.ndarray:
+    """O12: int8 samples (q is None) or their residues mod q as uint16"""
+    if q is None:
+        out = np.zeros(count, np.int8)
+        _L().orc_sample_gauss(_p(out, C.c_int8), None, first, count, seed, tag, inst, float(sigma), 2)
+    else:
+        out = np.zeros(count, np.uint16)
+        _L().orc_sample_gauss(None, _p(out, C.c_uint16), first, count, seed, tag, inst, float(sigma), q)
+    return out
+
+
+def sample_cuniform(first: int, count: int, seed: int, tag: int, inst: int, bound: int) -> np.ndarray:
+    out = np.zeros(count, np.int8)
+    _L().orc_sample_cuniform(_p(out, C.c_int8), first, count, seed, tag, inst, bound)
+    return out
+
+
+def encaps_pv(A, t, R, E1, e2, mubits, q: int):
+    """O14: (U, v) of the paper's Encrypt for all k bits; R [m][k], E1 [n][k], e2 [k] int8"""
+    A, t = _u16(A), _u16(t)
+    m, n = A.shape
+    R, E1, e2 = (np.ascontiguousarray(x, dtype=np.int8) for x in (R, E1, e2))
+    k = e2.shape[0]
+    assert R.shape == (m, k) and E1.shape == (n, k) and t.shape == (m,)
+    mubits = _u8(mubits, k // 8)
+    U, v = np.zeros((n, k), np.uint16), np.zeros(k, np.uint16)
+    _L().orc_encaps_pv(_p(A, C.c_uint16), _p(t, C.c_uint16), _p(R, C.c_int8), _p(E1, C.c_int8), _p(e2, C.c_int8),
+                       _p(mubits, C.c_uint8), _p(U, C.c_uint16), _p(v, C.c_uint16), m, n, k, q)
+    return U, v
 
 
 def cbd_from_word(w: int, q: int, eta: int) -> int:
