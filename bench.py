@@ -307,6 +307,39 @@ def time_call(fn, reps: int = 10, warm: int = 3) -> float:
     return ev0.elapsed_time(ev1) / reps
 
 
+def paper_variant_phase(B, device: int) -> dict:
+    """N2: the paper's own PKE on Table 1's n = 4096 row (q = 12289, sigma = 1.7, e2 in [-3, 3], CBD-3
+    secret, square A), 32 instances sharing A: sampling, KeyGen, Encrypt (tcgen05, signed int8 R), Decrypt."""
+    n, q, sigma, bound = W.PAPER_TABLE1[3]
+    k, Bt, seed = 256, 32, 6
+    dev = torch.device("cuda", device)
+    i16, u8, s8 = (dict(dtype=d, device=dev) for d in (torch.int16, torch.uint8, torch.int8))
+    with B.Context(n, n, k, q, 3, Bt, device) as c:
+        A = torch.empty(n, n, **i16)
+        c.sample_uniform(A, 0, n * n, seed, W.TAG_A)
+        s, e, t = torch.empty(Bt, n, **i16), torch.empty(Bt, n, **i16), torch.empty(Bt, n, **i16)
+        R, E1, e2 = torch.empty(Bt, n, k, **s8), torch.empty(Bt, n, k, **s8), torch.empty(Bt, k, **s8)
+        mu, out = torch.empty(Bt, k // 8, **u8), torch.empty(Bt, k // 8, **u8)
+        U, v = torch.empty(Bt, n, k, **i16), torch.empty(Bt, k, **i16)
+
+        def sample():
+            c.sample_cbd(s, 0, n, seed, W.TAG_S, 0, Bt)
+            c.sample_gauss_u16(e, 0, n, seed, W.TAG_E, 0, Bt, sigma)
+            c.sample_gauss_s8(R, 0, n * k, seed, W.TAG_RG, 0, Bt, sigma)
+            c.sample_gauss_s8(E1, 0, n * k, seed, W.TAG_E1, 0, Bt, sigma)
+            c.sample_cuniform_s8(e2, 0, k, seed, W.TAG_E2, 0, Bt, bound)
+            c.sample_bits(mu, 0, k, seed, W.TAG_MU, 0, Bt)
+
+        t_s = time_call(sample)
+        t_k = time_call(lambda: c.keygen(A, 0, s, e, t, Bt))
+        t_e = time_call(lambda: c.encaps_pv(A, t, R, E1, e2, mu, U, v, Bt))
+        t_d = time_call(lambda: c.decaps(U, v, s, out, Bt))
+        ok = bool(torch.equal(out, mu))
+    return {"config": f"n={n} q={q} sigma={sigma} e2<= {bound} eta=3, 32 instances", "sample_ms": t_s, "keygen_ms": t_k,
+            "encaps_ms": t_e, "decaps_ms": t_d, "kem_per_s": Bt * 1e3 / (t_s + t_k + t_e + t_d),
+            "encaps_int8_TOPs": 4.0 * n * n * k * Bt / (t_e * 1e-3) / 1e12, "all_bits_recovered": ok}
+
+
 def traffic_from_profiles(kernel: str):
     """DRAM bytes per launch of `kernel` from the committed ncu summary (profiles/traffic.json:
     {"<kernel>": {"dram_bytes_per_launch": ..., "source": ...}}), else None."""
@@ -422,6 +455,7 @@ def run_ours(args):
     t3 = time_call(lambda: ctx.decaps_fo(job.A, job.b, job.U, job.v, job.s, job.Rbits, job.out, okflags, Bt))
     side["decaps_fo_B32"] = {"ms": t3, "per_s": Bt * 1e3 / t3, "all_accepted": bool(okflags.all().item()),
                              "kem_per_s_encaps_plus_fo_decaps_B32": Bt * 1e3 / (t + t3)}
+    side["paper_variant_n4096_B32"] = paper_variant_phase(job.B, local)
     buf = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
     t = time_call(lambda: ctx.rng_fill(buf, buf.numel(), bytes(16), bytes(16), 0), reps=5)
     side["rng_fill_1GiB"] = {"ms": t, "GBps": buf.numel() / (t * 1e-3) / 1e9}

@@ -47,7 +47,8 @@ typedef enum {
 } lwe_status;
 
 /* Object tags of the seeded streams (S8(c) O3). */
-enum { LWE_TAG_A = 1, LWE_TAG_S = 2, LWE_TAG_E = 3, LWE_TAG_R = 4, LWE_TAG_MU = 5 };
+enum { LWE_TAG_A = 1, LWE_TAG_S = 2, LWE_TAG_E = 3, LWE_TAG_R = 4, LWE_TAG_MU = 5,
+       LWE_TAG_RG = 6, LWE_TAG_E1 = 7, LWE_TAG_E2 = 8 /* N2: Gaussian r, e1; centred-uniform e2 */ };
 
 /* Problem shape.  n, m multiples of 8 (one AES block = 8 elements); k multiple of 8;
  * q in (1, 65536]; eta in [1, 8]; max_batch >= 1 = the largest `batch` any call
@@ -154,6 +155,39 @@ int lwe_decaps_fo(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_b /*[batc
                   const uint16_t *d_s /*[batch][n]*/, const uint8_t *d_Rbits /*[batch][m*k/8]*/,
                   uint8_t *d_mubits_out /*[batch][k/8]*/, uint8_t *d_ok /*[batch]*/, uint32_t batch, void *stream);
 
+/* ---- N2 (S8(f)): the paper's own PKE variant ------------------------------------------
+ * P:L64 (KeyGen / Encrypt / Decrypt; Fig. 1 is an image whose text is lost), P:L70 (secret: binomial
+ * eta = 3), Table 1 header P:L92 (Gaussian sigma for e, r, e1; centred uniform k for e2).  Readings
+ * S20-S22 of DESIGN.md section 3.  With a context whose m = n (square A) and eta = 3:
+ *   KeyGen : s = lwe_sample_cbd (tag S), e = lwe_sample_gauss_u16 (tag E), t = lwe_keygen(A, s, e)
+ *   Encrypt: R = lwe_sample_gauss_s8 (tag RG, m*k per instance), E1 = lwe_sample_gauss_s8 (tag E1, n*k),
+ *            e2 = lwe_sample_cuniform_s8 (tag E2, k), then lwe_encaps_pv
+ *   Decrypt: lwe_decaps.
+ * Moduli of Table 1 that fit uint16 (3329, 12289) are supported; 65537 needs a 17-bit residue type and is not.
+ *
+ * gauss: element e -> 16-bit stream word w as for cbd; z = -12 + #{ j : w >= C[j] } with the cumulative table
+ *   C[j] = floor(65536 * Phi((j - 12 + 1/2) / sigma) + 1/2), j = 0..23, Phi(x) = erfc(-x / sqrt 2) / 2 evaluated in
+ *   double on the host: the rounded Gaussian round(sigma N(0,1)) to 2^-16 per value.  0.5 <= sigma <= 8.
+ *   _s8 stores z as int8, _u16 stores z mod q.  `first` multiple of 8.
+ * cuniform: centred uniform on [-bound, bound], 1 <= bound <= 127: the rejection rule of uniform with modulus
+ *   2*bound + 1 over the attempt streams, value (c mod (2 bound + 1)) - bound.  Any `first`. */
+int lwe_sample_gauss_s8(lwe_ctx *ctx, int8_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
+                        uint32_t inst0, uint32_t n_inst, double sigma, void *stream);
+int lwe_sample_gauss_u16(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
+                         uint32_t inst0, uint32_t n_inst, double sigma, void *stream);
+int lwe_sample_cuniform_s8(lwe_ctx *ctx, int8_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
+                           uint32_t inst0, uint32_t n_inst, uint32_t bound, void *stream);
+/* d_U[t][j][c] = ( sum_{i<m} A[i][j] * R_t[i][c] + E1_t[j][c] ) mod q
+ * d_v[t][c]    = ( sum_{i<m} d_t[t][i] * R_t[i][c] + e2_t[c] + mu_t[c]*floor(q/2) ) mod q
+ * with R_t = d_R[t] (int8 [m][k]), E1_t = d_E1[t] (int8 [n][k]), e2_t = d_e2[t] (int8 [k]).  Same tcgen05 kind::i8
+ * GEMM as lwe_encaps with the B operand read as SIGNED int8 (no bit expansion: R is copied once into the operand
+ * layout), signed byte-plane accumulators and E1 added in the recombine epilogue; |R| <= 127, m <= 65536.
+ * d_A must be stored.  Shapes the tensor path does not take run on CUDA cores with identical results. */
+int lwe_encaps_pv(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_t /*[batch][m]*/,
+                  const int8_t *d_R /*[batch][m][k]*/, const int8_t *d_E1 /*[batch][n][k]*/,
+                  const int8_t *d_e2 /*[batch][k]*/, const uint8_t *d_mubits /*[batch][k/8]*/,
+                  uint16_t *d_U /*[batch][n][k]*/, uint16_t *d_v /*[batch][k]*/, uint32_t batch, void *stream);
+
 /* ---- end-to-end with HOST buffers -----------------------------------------------
  * One full pass keygen -> encaps -> decaps for `batch` instances whose per-instance
  * inputs live in host memory: copies h_s, h_e, h_Rbits, h_mubits to the device,
@@ -196,7 +230,7 @@ enum {
     LWE_K_RNG_FILL = 0, LWE_K_SAMPLE_UNIFORM = 1, LWE_K_SAMPLE_CBD = 2, LWE_K_SAMPLE_BITS = 3,
     LWE_K_KEYGEN_STORED = 4, LWE_K_KEYGEN_REGEN = 5, LWE_K_EXPAND_R_V = 6, LWE_K_ENCAPS_TC = 7,
     LWE_K_ENCAPS_SIMT = 8, LWE_K_DECAPS = 9, LWE_K_KEYGEN_PREP = 10, LWE_K_KEYGEN_TC = 11, LWE_K_FO_VERDICT = 12,
-    LWE_K_COUNT = 13
+    LWE_K_SAMPLE_GAUSS = 13, LWE_K_SAMPLE_CUNIFORM = 14, LWE_K_PREP_R_PV = 15, LWE_K_COUNT = 16
 };
 /* Sum of the device durations (milliseconds, CUDA events) and the number of timed launches
  * of kernel `kernel_id` since the last reset.  Waits for the recorded events to complete

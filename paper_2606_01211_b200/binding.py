@@ -18,6 +18,7 @@ LWE_OK = 0
 ERRORS = {-1: "LWE_ERR_PARAM", -2: "LWE_ERR_ALIGN", -3: "LWE_ERR_NULLPTR", -4: "LWE_ERR_CUDA",
           -5: "LWE_ERR_UNSUPPORTED"}
 TAG_A, TAG_S, TAG_E, TAG_R, TAG_MU = 1, 2, 3, 4, 5
+TAG_RG, TAG_E1, TAG_E2 = 6, 7, 8
 OPT_ENCAPS_PATH = 1
 OPT_PROFILE = 2
 OPT_GEMV_VARIANT = 3
@@ -25,12 +26,14 @@ OPT_KEYGEN_PATH = 4
 OPT_TUNE = 5
 OPT_PANEL_ROWS = 6
 KERNELS = ["rng_fill", "sample_uniform", "sample_cbd", "sample_bits", "keygen_stored", "keygen_regen",
-           "expand_R_v", "encaps_tc", "encaps_simt", "decaps", "keygen_prep", "keygen_tc", "fo_verdict"]
+           "expand_R_v", "encaps_tc", "encaps_simt", "decaps", "keygen_prep", "keygen_tc", "fo_verdict",
+           "sample_gauss", "sample_cuniform", "prep_R_pv"]
 
 EXPORTS = [
     "lwe_create", "lwe_destroy", "lwe_strerror", "lwe_last_cuda_error", "lwe_launch_count",
     "lwe_rng_fill", "lwe_sample_uniform", "lwe_sample_cbd", "lwe_sample_bits",
-    "lwe_keygen", "lwe_encaps", "lwe_decaps", "lwe_decaps_fo", "lwe_kem_host", "lwe_set_option",
+    "lwe_keygen", "lwe_encaps", "lwe_decaps", "lwe_decaps_fo", "lwe_kem_host",
+    "lwe_sample_gauss_s8", "lwe_sample_gauss_u16", "lwe_sample_cuniform_s8", "lwe_encaps_pv", "lwe_set_option",
     "lwe_profile_read", "lwe_profile_reset",
 ]
 
@@ -76,6 +79,10 @@ def load_library() -> C.CDLL:
     lib.lwe_encaps.argtypes = [vp, vp, u64, vp, vp, vp, vp, vp, u32, vp]
     lib.lwe_decaps.argtypes = [vp, vp, vp, vp, vp, u32, vp]
     lib.lwe_decaps_fo.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
+    for f in (lib.lwe_sample_gauss_s8, lib.lwe_sample_gauss_u16):
+        f.argtypes = [vp, vp, u64, u64, u64, u32, u32, u32, C.c_double, vp]
+    lib.lwe_sample_cuniform_s8.argtypes = [vp, vp, u64, u64, u64, u32, u32, u32, u32, vp]
+    lib.lwe_encaps_pv.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
     lib.lwe_kem_host.argtypes = [vp, vp, u64, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
     _lib = lib
     return lib
@@ -188,6 +195,27 @@ class Context:
         self._check(self._lib.lwe_decaps_fo(self._h, _ptr(d_A), _ptr(d_b), _ptr(d_U), _ptr(d_v), _ptr(d_s),
                                             _ptr(d_Rbits), _ptr(d_mubits_out), _ptr(d_ok), batch, _stream(stream)),
                     "lwe_decaps_fo")
+
+    # -- N2: the paper's own PKE variant
+    def sample_gauss_s8(self, d_out, first: int, count: int, seed: int, tag: int, inst0: int, n_inst: int, sigma: float,
+                        stream=None):
+        self._check(self._lib.lwe_sample_gauss_s8(self._h, _ptr(d_out), first, count, seed, tag, inst0, n_inst,
+                                                  float(sigma), _stream(stream)), "lwe_sample_gauss_s8")
+
+    def sample_gauss_u16(self, d_out, first: int, count: int, seed: int, tag: int, inst0: int, n_inst: int, sigma: float,
+                         stream=None):
+        self._check(self._lib.lwe_sample_gauss_u16(self._h, _ptr(d_out), first, count, seed, tag, inst0, n_inst,
+                                                   float(sigma), _stream(stream)), "lwe_sample_gauss_u16")
+
+    def sample_cuniform_s8(self, d_out, first: int, count: int, seed: int, tag: int, inst0: int, n_inst: int, bound: int,
+                           stream=None):
+        self._check(self._lib.lwe_sample_cuniform_s8(self._h, _ptr(d_out), first, count, seed, tag, inst0, n_inst,
+                                                     bound, _stream(stream)), "lwe_sample_cuniform_s8")
+
+    def encaps_pv(self, d_A, d_t, d_R, d_E1, d_e2, d_mubits, d_U, d_v, batch: int = 1, stream=None):
+        self._check(self._lib.lwe_encaps_pv(self._h, _ptr(d_A), _ptr(d_t), _ptr(d_R), _ptr(d_E1), _ptr(d_e2),
+                                            _ptr(d_mubits), _ptr(d_U), _ptr(d_v), batch, _stream(stream)),
+                    "lwe_encaps_pv")
 
     def kem_host(self, d_A, seed_A: int, h_s, h_e, h_Rbits, h_mubits, h_b, h_U, h_v, h_mubits_out, batch: int = 1,
                  stream=None):

@@ -425,6 +425,75 @@ int lwe_decaps(lwe_ctx *ctx, const uint16_t *d_U, const uint16_t *d_v, const uin
     return LWE_OK;
 }
 
+static int gauss_args(lwe_ctx *ctx, const void *d_out, uint64_t first, uint64_t count, uint32_t tag, uint32_t inst0,
+                      uint32_t n_inst, double sigma)
+{
+    int rc = sampler_args(ctx, d_out, first, count, tag, inst0, n_inst);
+    if (rc != LWE_OK) return rc;
+    if (!(sigma >= 0.5 && sigma <= 8.0)) return LWE_ERR_PARAM;
+    return LWE_OK;
+}
+
+int lwe_sample_gauss_s8(lwe_ctx *ctx, int8_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
+                        uint32_t inst0, uint32_t n_inst, double sigma, void *stream)
+{
+    int rc = gauss_args(ctx, d_out, first, count, tag, inst0, n_inst, sigma);
+    if (rc != LWE_OK || count == 0 || n_inst == 0) return rc;
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_sample_gauss(c, d_out, false, first, count, seed_key_host(seed), tag, inst0, n_inst, sigma,
+                                  (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+int lwe_sample_gauss_u16(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
+                         uint32_t inst0, uint32_t n_inst, double sigma, void *stream)
+{
+    int rc = gauss_args(ctx, d_out, first, count, tag, inst0, n_inst, sigma);
+    if (rc != LWE_OK || count == 0 || n_inst == 0) return rc;
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_sample_gauss(c, d_out, true, first, count, seed_key_host(seed), tag, inst0, n_inst, sigma,
+                                  (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+int lwe_sample_cuniform_s8(lwe_ctx *ctx, int8_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
+                           uint32_t inst0, uint32_t n_inst, uint32_t bound, void *stream)
+{
+    CHECK_CTX(ctx);
+    if (tag == 0 || tag > 255 || bound < 1 || bound > 127) return LWE_ERR_PARAM;
+    if ((uint64_t)inst0 + n_inst > (1ull << 32)) return LWE_ERR_PARAM;
+    if (count == 0 || n_inst == 0) return LWE_OK;
+    REQUIRE_PTR(d_out); REQUIRE_ALIGNED(d_out);
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_sample_cuniform(c, d_out, first, count, seed_key_host(seed), tag, inst0, n_inst, bound,
+                                     (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+int lwe_encaps_pv(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_t, const int8_t *d_R, const int8_t *d_E1,
+                  const int8_t *d_e2, const uint8_t *d_mubits, uint16_t *d_U, uint16_t *d_v, uint32_t batch, void *stream)
+{
+    CHECK_CTX(ctx);
+    Ctx *c = &ctx->c;
+    if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
+    REQUIRE_PTR(d_A); REQUIRE_PTR(d_t); REQUIRE_PTR(d_R); REQUIRE_PTR(d_E1); REQUIRE_PTR(d_e2); REQUIRE_PTR(d_mubits);
+    REQUIRE_PTR(d_U); REQUIRE_PTR(d_v);
+    REQUIRE_ALIGNED(d_A); REQUIRE_ALIGNED(d_t); REQUIRE_ALIGNED(d_R); REQUIRE_ALIGNED(d_E1); REQUIRE_ALIGNED(d_e2);
+    REQUIRE_ALIGNED(d_mubits); REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v);
+    // tensor path: the CTA-pair GEMM; |lo/hi plane accumulator| <= 255 * 127 * m < 2^31 for m <= 65536
+    bool tc = encaps_tc2_supported(c, batch) && c->encaps_path != 1;
+    if (c->encaps_path >= 2 && !tc) return LWE_ERR_UNSUPPORTED;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    LAUNCH(c, launch_prep_R_pv_and_v(c, d_t, d_R, d_e2, d_mubits, d_v, batch, tc, st));
+    if (tc) LAUNCH(c, launch_encaps_tc2_pv(c, d_A, d_E1, d_U, batch, st));
+    else LAUNCH(c, launch_encaps_pv_simt(c, d_A, d_R, d_E1, d_U, batch, st));
+    return LWE_OK;
+}
+
 int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_t *h_s, const uint16_t *h_e,
                  const uint8_t *h_Rbits, const uint8_t *h_mubits, uint16_t *h_b, uint16_t *h_U, uint16_t *h_v,
                  uint8_t *h_mubits_out, uint32_t batch, void *stream)

@@ -270,4 +270,141 @@ cudaError_t launch_encaps_simt(Ctx *c, const uint16_t *d_A, const uint8_t *d_Rbi
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------ N2: the paper's own Encrypt (Gaussian r)
+// prep_R_pv_and_v: one pass over the int8 matrix R of every instance that (i) copies it into the GEMM's operand
+// buffer laid out [i][t*k + c] (one 256-column tile = one instance, as for the binary R) and (ii) accumulates
+// v_c = sum_i t_i R_ic + e2_c + mu_c floor(q/2) mod q (O14; Table 1 header P:L92).
+// grid (row_splits, batch); thread = (row slot, 4 columns = one 32-bit word of int8).
+__global__ void __launch_bounds__(kAuxThreads)
+prep_R_pv_and_v_kernel(const uint16_t *__restrict__ tvec, const int8_t *__restrict__ R, const int8_t *__restrict__ e2,
+                       const uint8_t *__restrict__ mubits, uint8_t *__restrict__ Rexp, uint16_t *__restrict__ v,
+                       unsigned long long *__restrict__ acc, unsigned int *__restrict__ tickets,
+                       uint32_t m, uint32_t k, uint32_t ld_exp, bool write_Rexp, ModQ mq)
+{
+    __shared__ uint32_t sLast;
+    __shared__ unsigned long long sCol[4 * kAuxThreads];
+    const uint32_t t = blockIdx.y;
+    const uint32_t wpr = k / 4;                          // words per row (k % 8 == 0)
+    const uint32_t rows_per_iter = kAuxThreads / wpr ? kAuxThreads / wpr : 1;
+    const uint32_t words_per_thread = (wpr + kAuxThreads - 1) / kAuxThreads;       // > 1 only for k > 1024
+    const uint32_t rslot = threadIdx.x / wpr;
+    const bool active = rslot < rows_per_iter;
+    const int8_t *Rt = R + (size_t)t * m * k;
+    const uint16_t *tt = tvec + (size_t)t * m;
+    for (uint32_t wq = 0; wq < words_per_thread; wq++) {
+        const uint32_t w = (threadIdx.x % wpr) + wq * kAuxThreads;
+        long long a[4] = {0, 0, 0, 0};                   // |t_i r| < 2^16 * 2^7, summed over <= 2^20 rows
+        if (active && w < wpr) {
+            for (uint32_t i = blockIdx.x * rows_per_iter + rslot; i < m; i += gridDim.x * rows_per_iter) {
+                const uint32_t r = __ldg(reinterpret_cast<const uint32_t *>(Rt + (size_t)i * k) + w);
+                const int ti = (int)__ldg(tt + i);
+                if (write_Rexp) *reinterpret_cast<uint32_t *>(Rexp + (size_t)i * ld_exp + (size_t)t * k + 4 * w) = r;
+#pragma unroll
+                for (int x = 0; x < 4; x++) a[x] += (long long)(ti * (int)(int8_t)(r >> (8 * x)));
+            }
+        }
+        // block-level sum over the row slots, then one atomic per column per CTA (two's complement: u64 adds)
+#pragma unroll
+        for (int x = 0; x < 4; x++) sCol[x * kAuxThreads + threadIdx.x] = (active && w < wpr) ? (unsigned long long)a[x] : 0ull;
+        __syncthreads();
+        if (threadIdx.x < wpr && w < wpr) {
+#pragma unroll
+            for (int x = 0; x < 4; x++) {
+                unsigned long long sum = 0;
+                for (uint32_t rs = 0; rs < rows_per_iter; rs++) sum += sCol[x * kAuxThreads + rs * wpr + threadIdx.x];
+                if (sum) atomicAdd(acc + (size_t)t * k + 4 * w + x, sum);
+            }
+        }
+        __syncthreads();
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) sLast = (atomicAdd(tickets + t, 1u) == gridDim.x - 1) ? 1u : 0u;
+    __syncthreads();
+    if (!sLast) return;
+    __threadfence();
+    for (uint32_t c = threadIdx.x; c < k; c += kAuxThreads) {
+        const long long sum = (long long)__ldcg(acc + (size_t)t * k + c);
+        acc[(size_t)t * k + c] = 0;
+        const uint32_t mu = (mubits[(size_t)t * (k / 8) + c / 8] >> (c % 8)) & 1u;
+        long long tot = sum + (long long)e2[(size_t)t * k + c] + (long long)mu * mq.half;
+        long long r = tot % (long long)mq.q;
+        if (r < 0) r += mq.q;
+        v[(size_t)t * k + c] = (uint16_t)r;
+    }
+    if (threadIdx.x == 0) tickets[t] = 0;
+}
+
+cudaError_t launch_prep_R_pv_and_v(Ctx *c, const uint16_t *d_t, const int8_t *d_R, const int8_t *d_e2,
+                                   const uint8_t *d_mubits, uint16_t *d_v, uint32_t batch, bool write_Rexp, cudaStream_t st)
+{
+    const uint32_t m = c->p.m, k = c->p.k;
+    const uint32_t wpr = k / 4;
+    const uint32_t rows_per_iter = kAuxThreads / wpr ? kAuxThreads / wpr : 1;
+    uint32_t splits = (uint32_t)(4 * c->sm_count) / batch;
+    uint32_t max_splits = (m + 4 * rows_per_iter - 1) / (4 * rows_per_iter);
+    if (splits > max_splits) splits = max_splits;
+    if (splits < 1) splits = 1;
+    dim3 grid(splits, batch);
+    ProfScope prof(c, LWE_K_PREP_R_PV, st);
+    prep_R_pv_and_v_kernel<<<grid, kAuxThreads, 0, st>>>(d_t, d_R, d_e2, d_mubits, c->d_Rexp, d_v, c->d_vacc,
+                                                         c->d_counters + 8 + c->p.max_batch, m, k, batch * k, write_Rexp,
+                                                         c->mq);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+// CUDA-core U = A^T R + E1 for the int8 R (shapes the tensor path does not take, and its cross-check).
+// grid (ceil(n/32), k/8, batch), block 32 x 8 as encaps_simt_kernel.
+__global__ void __launch_bounds__(256)
+encaps_pv_simt_kernel(const uint16_t *__restrict__ A, const int8_t *__restrict__ R, const int8_t *__restrict__ E1,
+                      uint16_t *__restrict__ U, uint32_t m, uint32_t n, uint32_t k, ModQ mq)
+{
+    __shared__ long long sAcc[8][32][8];
+    const uint32_t t = blockIdx.z, cb = blockIdx.y;
+    const uint32_t j = blockIdx.x * 32 + threadIdx.x;
+    const int8_t *Rt = R + (size_t)t * m * k;
+    long long a[8];
+#pragma unroll
+    for (int x = 0; x < 8; x++) a[x] = 0;
+    if (j < n) {
+        for (uint32_t i = threadIdx.y; i < m; i += 8) {
+            const int aij = (int)__ldg(A + (size_t)i * n + j);
+            const uint2 r = __ldg(reinterpret_cast<const uint2 *>(Rt + (size_t)i * k + 8 * cb));
+#pragma unroll
+            for (int x = 0; x < 4; x++) {
+                a[x] += (long long)(aij * (int)(int8_t)(r.x >> (8 * x)));
+                a[4 + x] += (long long)(aij * (int)(int8_t)(r.y >> (8 * x)));
+            }
+        }
+    }
+#pragma unroll
+    for (int x = 0; x < 8; x++) sAcc[threadIdx.y][threadIdx.x][x] = a[x];
+    __syncthreads();
+    if (threadIdx.y == 0 && j < n) {
+        const uint2 e1 = *reinterpret_cast<const uint2 *>(E1 + ((size_t)t * n + j) * k + 8 * cb);
+        uint32_t o[8];
+#pragma unroll
+        for (int x = 0; x < 8; x++) {
+            long long sum = (long long)(int8_t)((x < 4 ? e1.x : e1.y) >> (8 * (x & 3)));
+            for (int y = 0; y < 8; y++) sum += sAcc[y][threadIdx.x][x];
+            long long r = sum % (long long)mq.q;
+            o[x] = (uint32_t)(r < 0 ? r + mq.q : r);
+        }
+        *reinterpret_cast<uint4 *>(U + ((size_t)t * n + j) * k + 8 * cb) =
+            make_uint4(o[0] | (o[1] << 16), o[2] | (o[3] << 16), o[4] | (o[5] << 16), o[6] | (o[7] << 16));
+    }
+}
+
+cudaError_t launch_encaps_pv_simt(Ctx *c, const uint16_t *d_A, const int8_t *d_R, const int8_t *d_E1, uint16_t *d_U,
+                                  uint32_t batch, cudaStream_t st)
+{
+    const uint32_t m = c->p.m, n = c->p.n, k = c->p.k;
+    dim3 grid((n + 31) / 32, k / 8, batch), block(32, 8);
+    ProfScope prof(c, LWE_K_ENCAPS_SIMT, st);
+    encaps_pv_simt_kernel<<<grid, block, 0, st>>>(d_A, d_R, d_E1, d_U, m, n, k, c->mq);
+    c->launches++;
+    return cudaGetLastError();
+}
+
 }  // namespace lwe

@@ -36,6 +36,7 @@ constexpr uint32_t kThreads = 192;
 constexpr uint32_t kTmemCols = 512;
 
 constexpr uint32_t kInstrDesc = instr_desc_u8(kPairM, kTileN, true, true);
+constexpr uint32_t kInstrDescSignedB = instr_desc_u8(kPairM, kTileN, true, true, true);     // N2: R holds int8
 
 struct PairSched {
     uint32_t m_tiles, n_tiles, total, g;
@@ -80,7 +81,8 @@ struct PairCfg {
 template <uint32_t kStages, uint32_t kTileK, int kMode>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
-                  uint16_t *__restrict__ U, uint32_t *__restrict__ flags, uint32_t m, uint32_t n, uint32_t k,
+                  uint16_t *__restrict__ U, uint32_t *__restrict__ flags, const int8_t *__restrict__ E1, uint32_t m,
+                  uint32_t n, uint32_t k,
                   uint32_t ncols_total, ModQ mq, uint32_t group_w, uint32_t polA_kind, uint32_t polR_kind)
 {
     using Cfg = PairCfg<kStages, kTileK>;
@@ -173,7 +175,8 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                         uint64_t bdesc = make_desc_mn_sw128(sa + kBytesA, 0, 1024);
 #pragma unroll
                         for (uint32_t ks = 0; ks < kTileK / kUmmaK; ks++) {
-                            umma_i8_pair(d_tmem, adesc, bdesc, kInstrDesc, (kb | ks) ? 1u : 0u);
+                            umma_i8_pair(d_tmem, adesc, bdesc, kMode == kEpiStorePv ? kInstrDescSignedB : kInstrDesc,
+                                         (kb | ks) ? 1u : 0u);
                             adesc += (kUmmaK * 128) >> 4;
                             bdesc += (kUmmaK * 128) >> 4;
                         }
@@ -207,16 +210,30 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 tmem_ld_32x32b_x32(taddr + cb, r);
                 tmem_ld_wait();
                 uint32_t o[16];
+                const uint32_t col = nt * kTileN + cb + (odd ? 16u : 0u);
+                const bool in_range = j < n && col < ncols_total;
+                const uint32_t inst = col / k, c = col - inst * k;
+                uint32_t e1w[4] = {0, 0, 0, 0};                      // 16 int8 of E1[inst][j][c..c+15] (N2 only)
+                if (kMode == kEpiStorePv && in_range) {
+                    const uint4 t4 = *reinterpret_cast<const uint4 *>(E1 + ((size_t)inst * n + j) * k + c);
+                    e1w[0] = t4.x; e1w[1] = t4.y; e1w[2] = t4.z; e1w[3] = t4.w;
+                }
 #pragma unroll
                 for (int x = 0; x < 16; x++) {
                     uint32_t send = odd ? r[x] : r[16 + x];
                     uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 1);
-                    uint32_t val = odd ? (recv + (r[16 + x] << 8)) : (r[x] + (recv << 8));
-                    o[x] = mq.pow2 ? (val & mq.mask) : mod_u32(val, mq);
+                    if (kMode == kEpiStorePv) {
+                        // signed planes: lo = sum lo(A) r, hi = sum hi(A) r; U = lo + 256 hi + e1 mod q
+                        const int32_t lo = (int32_t)(odd ? recv : r[x]), hi = (int32_t)(odd ? r[16 + x] : recv);
+                        const int32_t e1 = (int32_t)(int8_t)(e1w[x >> 2] >> (8 * (x & 3)));
+                        if (mq.pow2) o[x] = ((uint32_t)lo + ((uint32_t)hi << 8) + (uint32_t)e1) & mq.mask;
+                        else o[x] = mod_u32(mod_s32(lo, mq) + 256u * mod_s32(hi, mq) + mod_s32(e1, mq), mq);
+                    } else {
+                        uint32_t val = odd ? (recv + (r[16 + x] << 8)) : (r[x] + (recv << 8));
+                        o[x] = mq.pow2 ? (val & mq.mask) : mod_u32(val, mq);
+                    }
                 }
-                const uint32_t col = nt * kTileN + cb + (odd ? 16u : 0u);
-                if (j < n && col < ncols_total) {
-                    const uint32_t inst = col / k, c = col - inst * k;
+                if (in_range) {
                     const bool bad = store_u16x16<kMode>(reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c), o, mq);
                     if (kMode == kEpiCompare) mism.note(flags, inst, bad);
                 }
@@ -242,8 +259,8 @@ bool encaps_tc2_supported(const Ctx *c, uint32_t batch)
 }
 
 template <uint32_t kStages, uint32_t kTileK, int kMode>
-static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t *d_flags, uint32_t batch, uint32_t row0,
-                               uint32_t rows, cudaStream_t st)
+static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t *d_flags, const int8_t *d_E1,
+                               uint32_t batch, uint32_t row0, uint32_t rows, cudaStream_t st)
 {
     using Cfg = PairCfg<kStages, kTileK>;
     const lwe_params &p = c->p;
@@ -263,7 +280,7 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint3
     const uint32_t tune = (uint32_t)c->tune;
     const uint32_t gw = (tune & 15u) ? (1u << ((tune & 15u) - 1)) : 8u;
     ProfScope prof(c, LWE_K_ENCAPS_TC, st);
-    kern<<<2 * pairs, kThreads, Cfg::kSmemBytes, st>>>(mapA, mapR, d_U, d_flags, rows, p.n, p.k, ncols, c->mq, gw,
+    kern<<<2 * pairs, kThreads, Cfg::kSmemBytes, st>>>(mapA, mapR, d_U, d_flags, d_E1, rows, p.n, p.k, ncols, c->mq, gw,
                                                        (tune >> 4) & 3u, (tune >> 6) & 3u);
     c->launches++;
     return cudaGetLastError();
@@ -272,14 +289,21 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint3
 cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0, uint32_t rows,
                               int mode, uint32_t *d_flags, cudaStream_t st)
 {
-    if (mode == kEpiAccum) return launch_pair<6, 128, kEpiAccum>(c, d_A, d_U, nullptr, batch, row0, rows, st);
-    if (mode == kEpiCompare) return launch_pair<6, 128, kEpiCompare>(c, d_A, d_U, d_flags, batch, row0, rows, st);
+    if (mode == kEpiAccum) return launch_pair<6, 128, kEpiAccum>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
+    if (mode == kEpiCompare) return launch_pair<6, 128, kEpiCompare>(c, d_A, d_U, d_flags, nullptr, batch, row0, rows, st);
     switch ((c->tune >> 8) & 3) {
-    case 1: return launch_pair<5, 128, kEpiStore>(c, d_A, d_U, nullptr, batch, row0, rows, st);
-    case 2: return launch_pair<4, 128, kEpiStore>(c, d_A, d_U, nullptr, batch, row0, rows, st);
-    case 3: return launch_pair<3, 256, kEpiStore>(c, d_A, d_U, nullptr, batch, row0, rows, st);
-    default: return launch_pair<6, 128, kEpiStore>(c, d_A, d_U, nullptr, batch, row0, rows, st);
+    case 1: return launch_pair<5, 128, kEpiStore>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
+    case 2: return launch_pair<4, 128, kEpiStore>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
+    case 3: return launch_pair<3, 256, kEpiStore>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
+    default: return launch_pair<6, 128, kEpiStore>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
     }
+}
+
+// N2: U = A^T R + E1 mod q with the int8 operand R already laid out in the context's operand buffer
+cudaError_t launch_encaps_tc2_pv(Ctx *c, const uint16_t *d_A, const int8_t *d_E1, uint16_t *d_U, uint32_t batch,
+                                 cudaStream_t st)
+{
+    return launch_pair<6, 128, kEpiStorePv>(c, d_A, d_U, nullptr, d_E1, batch, 0, c->p.m, st);
 }
 
 }  // namespace lwe

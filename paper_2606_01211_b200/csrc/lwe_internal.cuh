@@ -173,6 +173,17 @@ cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_
 bool encaps_tc2_supported(const Ctx *c, uint32_t batch);
 cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0,
                               uint32_t rows, int mode, uint32_t *d_flags, cudaStream_t st);
+// N2 (the paper's own PKE variant)
+cudaError_t launch_sample_gauss(Ctx *c, void *d_out, bool as_u16, uint64_t first, uint64_t count, const AesKey &key,
+                                uint32_t tag, uint32_t inst0, uint32_t n_inst, double sigma, cudaStream_t st);
+cudaError_t launch_sample_cuniform(Ctx *c, int8_t *d_out, uint64_t first, uint64_t count, const AesKey &key, uint32_t tag,
+                                   uint32_t inst0, uint32_t n_inst, uint32_t bound, cudaStream_t st);
+cudaError_t launch_prep_R_pv_and_v(Ctx *c, const uint16_t *d_t, const int8_t *d_R, const int8_t *d_e2,
+                                   const uint8_t *d_mubits, uint16_t *d_v, uint32_t batch, bool write_Rexp, cudaStream_t st);
+cudaError_t launch_encaps_tc2_pv(Ctx *c, const uint16_t *d_A, const int8_t *d_E1, uint16_t *d_U, uint32_t batch,
+                                 cudaStream_t st);
+cudaError_t launch_encaps_pv_simt(Ctx *c, const uint16_t *d_A, const int8_t *d_R, const int8_t *d_E1, uint16_t *d_U,
+                                  uint32_t batch, cudaStream_t st);
 cudaError_t launch_fo_verdict(Ctx *c, const uint16_t *d_v, const uint16_t *d_vprime, const uint32_t *d_flags,
                               uint8_t *d_ok, uint32_t batch, cudaStream_t st);
 cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,

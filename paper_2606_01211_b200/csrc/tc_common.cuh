@@ -190,10 +190,11 @@ __device__ __forceinline__ uint64_t make_desc_k_sw128(uint32_t saddr, uint32_t s
 
 // Instruction descriptor for kind::i8: D = s32 (c_format 2 at [4,6)), A = B = u8 (format 0 at [7,10),
 // [10,13)), A / B major-ness at bits 15 / 16 (1 = MN-major), N>>3 at [17,23), M>>4 at [24,29).
-__host__ __device__ constexpr uint32_t instr_desc_u8(uint32_t M, uint32_t N, bool a_mn_major, bool b_mn_major)
+__host__ __device__ constexpr uint32_t instr_desc_u8(uint32_t M, uint32_t N, bool a_mn_major, bool b_mn_major,
+                                                     bool b_signed = false)
 {
-    return (2u << 4) | ((a_mn_major ? 1u : 0u) << 15) | ((b_mn_major ? 1u : 0u) << 16) | ((N >> 3) << 17) |
-           ((M >> 4) << 24);
+    return (2u << 4) | ((b_signed ? 1u : 0u) << 10) | ((a_mn_major ? 1u : 0u) << 15) | ((b_mn_major ? 1u : 0u) << 16) |
+           ((N >> 3) << 17) | ((M >> 4) << 24);
 }
 
 // What the U = A^T R kernels do with a finished 16-column piece of a row of U.
@@ -204,12 +205,22 @@ __host__ __device__ constexpr uint32_t instr_desc_u8(uint32_t M, uint32_t N, boo
 //   kEpiCompare: write nothing; compare with what is stored there (the received ciphertext) and report a
 //                mismatch -- the re-encryption check c' = c of the FO transform (Alg.5 l.2-4) without
 //                ever materialising c'.
-enum EpiMode { kEpiStore = 0, kEpiAccum = 1, kEpiCompare = 2 };
+//   kEpiStorePv: the paper's own Encrypt (N2): the B operand is signed (Gaussian r), the accumulators are signed,
+//                and E1[j][c] is added before the reduction: U = A^T R + E1 mod q.
+enum EpiMode { kEpiStore = 0, kEpiAccum = 1, kEpiCompare = 2, kEpiStorePv = 3 };
+
+// signed 32-bit value -> canonical residue in [0, q)
+__device__ __forceinline__ uint32_t mod_s32(int32_t x, const ModQ &mq)
+{
+    if (x >= 0) return mod_u32((uint32_t)x, mq);
+    const uint32_t r = mod_u32((uint32_t)(-(int64_t)x), mq);
+    return r ? mq.q - r : 0u;
+}
 
 template <int kMode>
 __device__ __forceinline__ bool store_u16x16(uint4 *dst, uint32_t (&o)[16], const ModQ &mq)
 {
-    if (kMode != kEpiStore) {
+    if (kMode == kEpiAccum || kMode == kEpiCompare) {
         const uint4 p0 = dst[0], p1 = dst[1];
         const uint32_t old[8] = {p0.x, p0.y, p0.z, p0.w, p1.x, p1.y, p1.z, p1.w};
         if (kMode == kEpiCompare) {

@@ -53,6 +53,10 @@ CONFIGS = {w.name: w for w in (C1, C2, C3, C4, C5)}
 
 # object tags of the seeded streams -- labels, not arithmetic
 TAG_A, TAG_S, TAG_E, TAG_R, TAG_MU = 1, 2, 3, 4, 5
+TAG_RG, TAG_E1, TAG_E2 = 6, 7, 8                      # N2: Gaussian r, e1 and centred-uniform e2 (paper's own PKE)
+
+# Table 1 of the paper, the rows whose modulus fits uint16: (n, q, sigma, k of e2); eta = 3 for s
+PAPER_TABLE1 = [(512, 3329, 2.3, 3), (1024, 12289, 2.3, 3), (2048, 12289, 2.3, 3), (4096, 12289, 1.7, 3)]
 
 
 def shard_instances(batch: int, rank: int, world_size: int) -> range:
