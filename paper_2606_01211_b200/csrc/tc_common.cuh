@@ -209,14 +209,6 @@ __host__ __device__ constexpr uint32_t instr_desc_u8(uint32_t M, uint32_t N, boo
 //                and E1[j][c] is added before the reduction: U = A^T R + E1 mod q.
 enum EpiMode { kEpiStore = 0, kEpiAccum = 1, kEpiCompare = 2, kEpiStorePv = 3 };
 
-// signed 32-bit value -> canonical residue in [0, q)
-__device__ __forceinline__ uint32_t mod_s32(int32_t x, const ModQ &mq)
-{
-    if (x >= 0) return mod_u32((uint32_t)x, mq);
-    const uint32_t r = mod_u32((uint32_t)(-(int64_t)x), mq);
-    return r ? mq.q - r : 0u;
-}
-
 template <int kMode>
 __device__ __forceinline__ bool store_u16x16(uint4 *dst, uint32_t (&o)[16], const ModQ &mq)
 {
