@@ -220,9 +220,13 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
  *                      for every value.
  * LWE_OPT_PANEL_ROWS:  rows of A regenerated per panel by lwe_encaps(d_A == NULL): a multiple of 8 in
  *                      [8, default]; 0 = default (<= 64 MiB of A per panel, a multiple of 128 rows).  Same
- *                      result for every value (tests use it to cross many panels at small sizes). */
+ *                      result for every value (tests use it to cross many panels at small sizes).
+ * LWE_OPT_REGEN_PATH:  lwe_encaps(d_A == NULL), 0 = auto (one instance with k <= 256: A tiles generated straight into
+ *                      the GEMM's shared-memory operand, A never touches HBM -- S8(f) N4; otherwise row panels),
+ *                      1 = always row panels, 2 = force the fused kernel (LWE_ERR_UNSUPPORTED if batch > 1 or
+ *                      k > 256 or the tensor path does not take the shape).  Same result for every value. */
 enum { LWE_OPT_ENCAPS_PATH = 1, LWE_OPT_PROFILE = 2, LWE_OPT_GEMV_VARIANT = 3, LWE_OPT_KEYGEN_PATH = 4, LWE_OPT_TUNE = 5,
-       LWE_OPT_PANEL_ROWS = 6 };
+       LWE_OPT_PANEL_ROWS = 6, LWE_OPT_REGEN_PATH = 7 };
 int lwe_set_option(lwe_ctx *ctx, int option, int64_t value);
 
 /* Kernel ids for lwe_profile_read (one per __global__ function of the library). */
@@ -230,7 +234,7 @@ enum {
     LWE_K_RNG_FILL = 0, LWE_K_SAMPLE_UNIFORM = 1, LWE_K_SAMPLE_CBD = 2, LWE_K_SAMPLE_BITS = 3,
     LWE_K_KEYGEN_STORED = 4, LWE_K_KEYGEN_REGEN = 5, LWE_K_EXPAND_R_V = 6, LWE_K_ENCAPS_TC = 7,
     LWE_K_ENCAPS_SIMT = 8, LWE_K_DECAPS = 9, LWE_K_KEYGEN_PREP = 10, LWE_K_KEYGEN_TC = 11, LWE_K_FO_VERDICT = 12,
-    LWE_K_SAMPLE_GAUSS = 13, LWE_K_SAMPLE_CUNIFORM = 14, LWE_K_PREP_R_PV = 15, LWE_K_COUNT = 16
+    LWE_K_SAMPLE_GAUSS = 13, LWE_K_SAMPLE_CUNIFORM = 14, LWE_K_PREP_R_PV = 15, LWE_K_ENCAPS_REGEN_TC = 16, LWE_K_COUNT = 17
 };
 /* Sum of the device durations (milliseconds, CUDA events) and the number of timed launches
  * of kernel `kernel_id` since the last reset.  Waits for the recorded events to complete

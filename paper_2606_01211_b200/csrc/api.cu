@@ -40,7 +40,7 @@ void free_all(Ctx *c)
 {
     cudaFree(c->d_Sx);
     cudaFree(c->d_Apanel);
-    cudaFree(c->d_foflags); cudaFree(c->d_vprime);
+    cudaFree(c->d_foflags); cudaFree(c->d_vprime); cudaFree(c->d_tile_locks);
     cudaFree(c->d_te0); cudaFree(c->d_Rexp); cudaFree(c->d_vacc); cudaFree(c->d_dacc); cudaFree(c->d_counters);
     cudaFree(c->d_hs); cudaFree(c->d_he); cudaFree(c->d_hb); cudaFree(c->d_hU); cudaFree(c->d_hv);
     cudaFree(c->d_hR); cudaFree(c->d_hmu); cudaFree(c->d_hmuout);
@@ -137,6 +137,7 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
     }
     ok(dev_alloc(&c->d_foflags, B));
     ok(dev_alloc(&c->d_vprime, B * k));
+    ok(dev_alloc(&c->d_tile_locks, encaps_regen_lock_words(*p)));
     ok(dev_alloc(&c->d_vacc, k * B));
     ok(dev_alloc(&c->d_dacc, k * B));
     ok(dev_alloc(&c->d_counters, 8 + 2 * B));
@@ -158,6 +159,7 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
         ok(cudaMemset(c->d_vacc, 0, k * B * sizeof(unsigned long long)));
         ok(cudaMemset(c->d_dacc, 0, k * B * sizeof(unsigned long long)));
         ok(cudaMemset(c->d_counters, 0, (8 + 2 * B) * sizeof(unsigned int)));
+        ok(cudaMemset(c->d_tile_locks, 0, encaps_regen_lock_words(*p) * sizeof(uint32_t)));
     }
     if (e != cudaSuccess) {
         free_all(c);
@@ -215,6 +217,11 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
         if (value == 0) { c->panel_rows = c->panel_rows_alloc; return LWE_OK; }
         if (value < 8 || value % 8 || value > (int64_t)c->panel_rows_alloc) return LWE_ERR_PARAM;
         c->panel_rows = (uint32_t)value;
+        return LWE_OK;
+    }
+    if (option == LWE_OPT_REGEN_PATH) {
+        if (value < 0 || value > 2) return LWE_ERR_PARAM;
+        ctx->c.regen_path = (int)value;
         return LWE_OK;
     }
     if (option == LWE_OPT_PROFILE) {
@@ -351,7 +358,15 @@ static int encaps_core(Ctx *c, const uint16_t *d_A, uint64_t seed_A, const uint1
     // CTA pairs (cta_group::2) by default; path 2 keeps the single-CTA kernel selectable
     const bool pair = tc && c->encaps_path != 2 && encaps_tc2_supported(c, batch);
     if (c->encaps_path == 3 && !pair) return LWE_ERR_UNSUPPORTED;
+    // one instance, A regenerated: generate the A tiles straight into the GEMM's shared-memory operand (N4)
+    const bool fused = !d_A && !compare && tc && c->encaps_path != 1 && c->regen_path != 1 &&
+                       encaps_regen_tc_supported(c, batch);
+    if (!d_A && c->regen_path == 2 && !fused) return LWE_ERR_UNSUPPORTED;
     LAUNCH(c, launch_expand_R_and_v(c, d_b, d_Rbits, d_mubits, d_v, batch, tc, st));
+    if (fused) {
+        LAUNCH(c, launch_encaps_regen_tc(c, seed_key_host(seed_A), d_U, st));
+        return LWE_OK;
+    }
     // Stored A: one pass over all m rows.  d_A == NULL: A is regenerated from seed_A one row panel at a
     // time into the context's panel buffer (rows of A are contiguous ranges of the counter-indexed
     // stream) and the contraction is accumulated over the panels; A is never held in full.

@@ -70,6 +70,7 @@ struct Ctx {
     int gemv_variant;                 // LWE_OPT_GEMV_VARIANT
     int keygen_path;                  // LWE_OPT_KEYGEN_PATH
     int tune;                         // LWE_OPT_TUNE: launch-shape experiments, no semantic effect
+    int regen_path;                   // LWE_OPT_REGEN_PATH
 
     // device tables
     uint32_t *d_te0;                  // 256-entry AES T-table (word = 2S | S<<8 | S<<16 | 3S<<24)
@@ -85,6 +86,7 @@ struct Ctx {
     unsigned int *d_counters;         // [8 + max_batch] self-resetting "last block" tickets
     uint32_t *d_foflags;              // [max_batch] mismatch flags of the FO re-encryption check
     uint16_t *d_vprime;               // [max_batch][k] re-encrypted v'
+    uint32_t *d_tile_locks;           // [2 * n/64] per-tile lock + arrival count of the fused regenerated-A encaps
     // staging for lwe_kem_host
     uint16_t *d_hs, *d_he, *d_hb, *d_hU, *d_hv;
     uint8_t *d_hR, *d_hmu, *d_hmuout;
@@ -171,6 +173,10 @@ bool encaps_tc_supported(const Ctx *c, uint32_t batch);
 cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0,
                              uint32_t rows, int mode, uint32_t *d_flags, cudaStream_t st);
 bool encaps_tc2_supported(const Ctx *c, uint32_t batch);
+// N4: A regenerated inside the GEMM's producer (one instance), encaps_regen_tc.cu
+uint32_t encaps_regen_lock_words(const lwe_params &p);
+bool encaps_regen_tc_supported(const Ctx *c, uint32_t batch);
+cudaError_t launch_encaps_regen_tc(Ctx *c, const AesKey &key, uint16_t *d_U, cudaStream_t st);
 cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0,
                               uint32_t rows, int mode, uint32_t *d_flags, cudaStream_t st);
 // N2 (the paper's own PKE variant)

@@ -226,6 +226,56 @@ def test_encaps_regenerated_A_equals_stored_and_oracle(H, path, m, n, k, q, batc
         assert np.array_equal(Ug[t], Uo), ("U", t)
 
 
+@pytest.mark.parametrize("m,n,k,q,seed,tune", [
+    (512, 256, 256, 65536, 1, 0),           # C1: 4 tiles, one K range each
+    (2048, 1024, 256, 65536, 2, 0),         # C2: 16 tiles x several K ranges combined under the tile locks
+    (1160, 456, 256, 65521, 3, 0),          # prime q (rejection inside the generator), n % 64 != 0, ragged K tail
+    (1160, 456, 256, 65521, 3, 1 << 12),    # 16 generator warps, K block 128, 3-stage ring
+    (200, 72, 128, 40000, 9, 2 << 12),      # k < 256 (second R box out of range), 2-stage ring
+    (4104, 8, 16, 12289, 5, 0),             # one tile, mostly empty; many K ranges
+    (12288, 9472, 256, 65536, 4, 0),        # 148 tiles = exactly one wave of CTAs; two K ranges per tile
+])
+def test_encaps_fused_regenerated_A_matches_oracle(H, m, n, k, q, seed, tune):
+    """S8(f) N4: lwe_encaps(d_A = NULL) for one instance generates the A tiles inside the GEMM's producer (A never in
+    HBM).  Equals the oracle, whose A is its own draw from the same seed, bit for bit; run twice on one context (the
+    per-tile locks and counters reset themselves) and against the row-panel path."""
+    b = W.random_u16((1, m), q, 22)
+    Rbits = W.random_bytes(m * k // 8, 23).reshape(1, -1)
+    mubits = W.random_bytes(k // 8, 24).reshape(1, -1)
+    with B().Context(n, m, k, q, 4, 1) as c:
+        c.set_option(B().OPT_REGEN_PATH, 2)
+        c.set_option(B().OPT_TUNE, tune)
+        U, v = H.dev_empty_u16(1, n, k), H.dev_empty_u16(1, k)
+        got = []
+        for _ in range(2):
+            U.fill_(-1)
+            c.profile_reset()
+            c.set_option(B().OPT_PROFILE, 1)
+            c.encaps(None, seed, H.dev(b), H.dev(Rbits), H.dev(mubits), U, v, 1)
+            got.append((H.host_u16(U).copy(), H.host_u16(v).copy()))
+            assert c.profile_read()["encaps_regen_tc"][1] == 1, "the fused kernel did not run"
+        c.set_option(B().OPT_PROFILE, 0)
+        c.set_option(B().OPT_REGEN_PATH, 1)
+        U.fill_(-1)
+        c.encaps(None, seed, H.dev(b), H.dev(Rbits), H.dev(mubits), U, v, 1)
+        Up = H.host_u16(U).copy()
+    if m * n <= 1 << 22:
+        A = O.sample_uniform(0, m * n, seed, O.TAG_A, 0, q).reshape(m, n)
+        Uo, vo = O.encaps(A, b[0], Rbits[0], mubits[0], k, q)
+    else:                                                       # sampled rows of U (columns of A by counter index)
+        rows = np.unique(np.concatenate([np.arange(0, 70), np.arange(n - 70, n), np.arange(63, n, 997)])).astype(np.uint32)
+        cols = np.stack([O.sample_uniform_strided(int(j), n, m, seed, O.TAG_A, 0, q) for j in rows], axis=1)
+        Usub, vo = O.encaps(cols, b[0], Rbits[0], mubits[0], k, q)
+        Uo = None
+    for Ug, vg in got:
+        assert np.array_equal(vg[0], vo)
+        if Uo is not None:
+            assert np.array_equal(Ug[0], Uo)
+        else:
+            assert np.array_equal(Ug[0][rows], Usub)
+    assert np.array_equal(got[0][0], Up), "fused vs row-panel path"
+
+
 # ---------------------------------------------------------------- decaps
 
 @pytest.mark.parametrize("n,k,q,batch", [(256, 256, 65536, 1), (1000, 256, 65521, 3), (64, 8, 17, 2),
