@@ -440,6 +440,17 @@ def run_ours(args):
     t = time_call(lambda: ctx.encaps(job.A, 0, b1, job.Rbits[:1], job.mubits[:1], job.U[:1], job.v[:1], 1))
     side["encaps_B1"] = {"ms": t, "per_s": 1e3 / t, "int8_TOPs": 4.0 * m * n * k / (t * 1e-3) / 1e12,
                          "A_GBps": 2.0 * m * n / (t * 1e-3) / 1e9}
+    # N4: encaps with A regenerated -- one instance: AES generator fused into the GEMM's producer (A never in HBM);
+    # 32 instances: row panels regenerated into HBM, GEMM accumulated over the panels
+    U_ref = job.U[:1].clone()
+    t = time_call(lambda: ctx.encaps(None, w.seed, b1, job.Rbits[:1], job.mubits[:1], job.U[:1], job.v[:1], 1), reps=5)
+    side["encaps_regen_fused_B1"] = {"ms": t, "per_s": 1e3 / t, "aes_GBps": 2.0 * m * n / (t * 1e-3) / 1e9,
+                                     "equals_stored": bool(torch.equal(job.U[:1], U_ref))}
+    ctx.set_option(job.B.OPT_REGEN_PATH, 1)
+    t = time_call(lambda: ctx.encaps(None, w.seed, b1, job.Rbits[:1], job.mubits[:1], job.U[:1], job.v[:1], 1), reps=5)
+    ctx.set_option(job.B.OPT_REGEN_PATH, 0)
+    side["encaps_regen_panels_B1"] = {"ms": t, "per_s": 1e3 / t, "aes_GBps": 2.0 * m * n / (t * 1e-3) / 1e9}
+    del U_ref
     t = time_call(lambda: ctx.decaps(job.U[:1], job.v[:1], s1, job.out[:1], 1))
     side["decaps_B1"] = {"ms": t, "per_s": 1e3 / t}
     t = time_call(lambda: ctx.keygen(job.A, 0, job.s, job.e, job.b, Bt))
@@ -450,6 +461,8 @@ def run_ours(args):
     side["decaps_B32"] = {"ms": t2, "per_s": Bt * 1e3 / t2, "GOPs": w.ops_decaps() / (t2 * 1e-3) / 1e9,
                           "GBps": 2.0 * n * k * Bt / (t2 * 1e-3) / 1e9}
     side["kem_per_s_encaps_plus_decaps_only_B32"] = Bt * 1e3 / (t + t2)
+    tr = time_call(lambda: ctx.encaps(None, w.seed, job.b, job.Rbits, job.mubits, job.U, job.v, Bt), reps=5)
+    side["encaps_regen_panels_B32"] = {"ms": tr, "per_s": Bt * 1e3 / tr}
     # N3: decaps with the FO re-encryption check (decrypt + re-encrypt + compare on the device, Alg. 5 without hashes)
     okflags = torch.empty(Bt, dtype=torch.uint8, device="cuda")
     t3 = time_call(lambda: ctx.decaps_fo(job.A, job.b, job.U, job.v, job.s, job.Rbits, job.out, okflags, Bt))

@@ -221,12 +221,15 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A,
  * LWE_OPT_PANEL_ROWS:  rows of A regenerated per panel by lwe_encaps(d_A == NULL): a multiple of 8 in
  *                      [8, default]; 0 = default (<= 64 MiB of A per panel, a multiple of 128 rows).  Same
  *                      result for every value (tests use it to cross many panels at small sizes).
+ * LWE_OPT_R_OPERAND:   how the CTA-pair GEMM gets its B operand, 0 = auto (k % 128 == 0: expanded from the packed bits of
+ *                      R inside the kernel, nothing is written to HBM; otherwise from the expanded workspace),
+ *                      1 = always expand R to a u8 matrix in the workspace first.  Same result for every value.
  * LWE_OPT_REGEN_PATH:  lwe_encaps(d_A == NULL), 0 = auto (one instance with k <= 256: A tiles generated straight into
  *                      the GEMM's shared-memory operand, A never touches HBM -- S8(f) N4; otherwise row panels),
  *                      1 = always row panels, 2 = force the fused kernel (LWE_ERR_UNSUPPORTED if batch > 1 or
  *                      k > 256 or the tensor path does not take the shape).  Same result for every value. */
 enum { LWE_OPT_ENCAPS_PATH = 1, LWE_OPT_PROFILE = 2, LWE_OPT_GEMV_VARIANT = 3, LWE_OPT_KEYGEN_PATH = 4, LWE_OPT_TUNE = 5,
-       LWE_OPT_PANEL_ROWS = 6, LWE_OPT_REGEN_PATH = 7 };
+       LWE_OPT_PANEL_ROWS = 6, LWE_OPT_REGEN_PATH = 7, LWE_OPT_R_OPERAND = 8 };
 int lwe_set_option(lwe_ctx *ctx, int option, int64_t value);
 
 /* Kernel ids for lwe_profile_read (one per __global__ function of the library). */

@@ -219,6 +219,11 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
         c->panel_rows = (uint32_t)value;
         return LWE_OK;
     }
+    if (option == LWE_OPT_R_OPERAND) {
+        if (value < 0 || value > 1) return LWE_ERR_PARAM;
+        ctx->c.r_operand = (int)value;
+        return LWE_OK;
+    }
     if (option == LWE_OPT_REGEN_PATH) {
         if (value < 0 || value > 2) return LWE_ERR_PARAM;
         ctx->c.regen_path = (int)value;
@@ -362,7 +367,10 @@ static int encaps_core(Ctx *c, const uint16_t *d_A, uint64_t seed_A, const uint1
     const bool fused = !d_A && !compare && tc && c->encaps_path != 1 && c->regen_path != 1 &&
                        encaps_regen_tc_supported(c, batch);
     if (!d_A && c->regen_path == 2 && !fused) return LWE_ERR_UNSUPPORTED;
-    LAUNCH(c, launch_expand_R_and_v(c, d_b, d_Rbits, d_mubits, d_v, batch, tc, st));
+    // CTA-pair GEMM with k % 128 == 0: the kernel expands its B tiles from the packed bits itself; the pass over R
+    // here then only computes v (no expanded operand is written)
+    const bool bits = pair && c->r_operand != 1 && encaps_tc2_bits_supported(c, batch);
+    LAUNCH(c, launch_expand_R_and_v(c, d_b, d_Rbits, d_mubits, d_v, batch, tc && (fused || !bits), st));   // the fused regenerated-A kernel loads R through TMA
     if (fused) {
         LAUNCH(c, launch_encaps_regen_tc(c, seed_key_host(seed_A), d_U, st));
         return LWE_OK;
@@ -381,7 +389,7 @@ static int encaps_core(Ctx *c, const uint16_t *d_A, uint64_t seed_A, const uint1
             panel = c->d_Apanel;
         }
         const int mode = compare ? 2 : (row0 != 0 ? 1 : 0);
-        if (pair) LAUNCH(c, launch_encaps_tc2(c, panel, d_U, batch, row0, rows, mode, c->d_foflags, st));
+        if (pair) LAUNCH(c, launch_encaps_tc2(c, panel, d_U, batch, row0, rows, mode, c->d_foflags, st, bits ? d_Rbits : nullptr));
         else if (tc) LAUNCH(c, launch_encaps_tc(c, panel, d_U, batch, row0, rows, mode, c->d_foflags, st));
         else LAUNCH(c, launch_encaps_simt(c, panel, d_Rbits, d_U, batch, row0, rows, mode, c->d_foflags, st));
     }

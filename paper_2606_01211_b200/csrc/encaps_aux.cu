@@ -96,14 +96,41 @@ expand_R_and_v_w32_kernel(const uint16_t *__restrict__ b, const uint8_t *__restr
     for (uint32_t c = threadIdx.x; c < k; c += kAuxThreads) sSum[c] = 0;
     __syncthreads();
 
-    uint32_t a[32];                                           // <= 65535 * rows visited (<= 65536) < 2^32
+    // Column sums of b_i R_ic in 16-bit lanes, one byte plane of b at a time: register x holds the partial sums of
+    // columns x and x + 16 of the thread's 32, sum <= 255 * (rows since the last flush) < 2^16 for <= 256 rows.
+    // (r >> x) & 0x00010001 puts the two bits into the two lanes, one IMAD (fma pipe) per byte plane adds the row:
+    // 2 instructions per column, against 3.4 for bit-test + predicated add on the alu pipe alone.
+    uint32_t aL[16], aH[16];
 #pragma unroll
-    for (int x = 0; x < 32; x++) a[x] = 0;
+    for (int x = 0; x < 16; x++) { aL[x] = 0; aH[x] = 0; }
+    // unpack, add up the lanes of the warp that hold the same word column (lane mod wpr) by shuffle, and let one lane
+    // per word column add into the CTA's sums, stored [x][w] so that those lanes hit different banks (32 same-address
+    // shared atomics per thread, 4 lanes deep, had made this flush the longest part of the kernel)
+    auto flush = [&]() {
+        uint32_t vals[32];
+#pragma unroll
+        for (int x = 0; x < 16; x++) {
+            vals[x] = (aL[x] & 0xffffu) + ((aH[x] & 0xffffu) << 8);
+            vals[x + 16] = (aL[x] >> 16) + ((aH[x] >> 16) << 8);
+            aL[x] = 0; aH[x] = 0;
+        }
+        for (uint32_t off = wpr; off < 32; off <<= 1) {
+#pragma unroll
+            for (int x = 0; x < 32; x++) vals[x] += __shfl_xor_sync(0xffffffffu, vals[x], off);
+        }
+        if ((threadIdx.x & 31) < wpr || wpr >= 32) {
+#pragma unroll
+            for (int x = 0; x < 32; x++)
+                if (vals[x]) atomicAdd(&sSum[x * wpr + w], vals[x]);
+        }
+    };
     constexpr int kUnroll = 4;
+    constexpr uint32_t kFlushIters = 256 / kUnroll;           // rows per thread between flushes <= 256
     // a CTA streams one contiguous range of rows
     const uint32_t step = rows_per_iter;
     const uint32_t per_cta = ((m + gridDim.x - 1) / gridDim.x + rows_per_iter - 1) / rows_per_iter * rows_per_iter;
     const uint32_t ibeg = blockIdx.x * per_cta, iend = min(m, ibeg + per_cta);
+    uint32_t iters = 0;
     for (uint32_t i0 = ibeg + rslot; i0 < iend; i0 += kUnroll * step) {
         uint32_t r[kUnroll], bi[kUnroll];
 #pragma unroll
@@ -124,24 +151,22 @@ expand_R_and_v_w32_kernel(const uint16_t *__restrict__ b, const uint8_t *__restr
                 dst[0] = make_uint4(o[0], o[1], o[2], o[3]);
                 dst[1] = make_uint4(o[4], o[5], o[6], o[7]);
             }
+            const uint32_t bl = bi[u] & 0xffu, bh = bi[u] >> 8;
 #pragma unroll
-            for (int x = 0; x < 32; x++)
-                if (r[u] & (1u << x)) a[x] += bi[u];           // bit test into a predicate + predicated add
+            for (int x = 0; x < 16; x++) {
+                const uint32_t two = (r[u] >> x) & 0x00010001u;     // columns x (low lane) and x + 16 (high lane)
+                aL[x] += two * bl;
+                aH[x] += two * bh;
+            }
         }
+        if (++iters == kFlushIters) { flush(); iters = 0; }
     }
-    // lanes of a warp that hold the same word column (lane mod wpr) first meet by shuffle
-    for (uint32_t off = wpr; off < 32; off <<= 1) {
-#pragma unroll
-        for (int x = 0; x < 32; x++) a[x] += __shfl_xor_sync(0xffffffffu, a[x], off);
-    }
-    if ((threadIdx.x & 31) < wpr || wpr >= 32) {
-#pragma unroll
-        for (int x = 0; x < 32; x++)
-            if (a[x]) atomicAdd(&sSum[32 * w + x], a[x]);
-    }
+    flush();
     __syncthreads();
-    for (uint32_t c = threadIdx.x; c < k; c += kAuxThreads)
-        if (sSum[c]) atomicAdd(acc + (size_t)t * k + c, (unsigned long long)sSum[c]);
+    for (uint32_t c = threadIdx.x; c < k; c += kAuxThreads) {
+        const uint32_t sum = sSum[(c & 31u) * wpr + (c >> 5)];
+        if (sum) atomicAdd(acc + (size_t)t * k + c, (unsigned long long)sum);
+    }
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) sLast = (atomicAdd(tickets + t, 1u) == gridDim.x - 1) ? 1u : 0u;

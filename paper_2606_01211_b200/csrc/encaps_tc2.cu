@@ -33,6 +33,11 @@ constexpr uint32_t kPairM = 2 * kCtaM;           // per pair
 constexpr uint32_t kTileN = 256;
 constexpr uint32_t kHalfN = kTileN / 2;          // columns of R staged by each CTA
 constexpr uint32_t kThreads = 192;
+constexpr uint32_t kExpGroups = 2;                  // expander groups per CTA (kBitsB): group j takes K blocks j, j+2, ..
+constexpr uint32_t kExpWarps = 4 * kExpGroups;      // 4 warps = 128 threads = one K row each
+constexpr uint32_t kThreadsBits = kThreads + 32 * kExpWarps;
+constexpr uint32_t kBitStages = 12;                 // ring of packed-bit tiles, deeper than the operand ring
+constexpr uint32_t kBitTileBytes = 128 * 16;        // 128 K rows x 128 columns of bits
 constexpr uint32_t kTmemCols = 512;
 
 constexpr uint32_t kInstrDesc = instr_desc_u8(kPairM, kTileN, true, true);
@@ -76,22 +81,35 @@ struct PairCfg {
     static constexpr uint32_t kBytesB = kHalfN * kTileK;
     static constexpr uint32_t kBytesStage = kBytesA + kBytesB;
     static constexpr uint32_t kSmemBytes = kStages * kBytesStage + 1024 /*align*/ + 256 /*barriers*/;
+    // kBitsB: + a ring of packed-bit tiles (128 K rows x 16 bytes each) and its barriers
+    static constexpr uint32_t kSmemBytesBits = kSmemBytes + kBitStages * kBitTileBytes + 256;
 };
 
-template <uint32_t kStages, uint32_t kTileK, int kMode>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+// kBitsB: the B operand is never expanded in HBM.  Eight extra warps per CTA (two groups taking alternate K blocks)
+// read the packed bits of R (16 bytes = the 128 columns of one K row of this CTA's half tile per thread), spread them to {0,1} bytes and store
+// them into the stage's B buffer in the swizzled layout TMA would have produced; the stage's full barrier then
+// counts the arrivals of one group of each CTA (8 warps) beside the A bytes.  Needs k % 128 == 0 (a half tile lies inside
+// one instance) and kTileK == 128 (one row per expander thread).  Against the expanded operand this removes the
+// 128 MiB expanded-R write per batch and every DRAM / L2 re-read of it by the GEMM (16x fewer operand bytes).
+template <uint32_t kStages, uint32_t kTileK, int kMode, bool kBitsB>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kBitsB ? kThreadsBits : kThreads, 1)
 encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
                   uint16_t *__restrict__ U, uint32_t *__restrict__ flags, const int8_t *__restrict__ E1, uint32_t m,
                   uint32_t n, uint32_t k,
                   uint32_t ncols_total, ModQ mq, uint32_t group_w, uint32_t polA_kind, uint32_t polR_kind,
-                  uint32_t pv_bias, uint32_t pv_e1bias)
+                  uint32_t pv_bias, uint32_t pv_e1bias, const __grid_constant__ CUtensorMap mapBits, uint32_t bits_row0,
+                  uint32_t bits_rows_per_inst)
 {
+    static_assert(!kBitsB || kTileK == 128, "one K row per expander thread");
     using Cfg = PairCfg<kStages, kTileK>;
     constexpr uint32_t kBytesA = Cfg::kBytesA, kBytesStage = Cfg::kBytesStage;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t base = (raw + 1023u) & ~1023u;
-    const uint32_t bars = base + kStages * kBytesStage;
+    const uint32_t bits_ring = base + kStages * kBytesStage;                        // kBitsB only
+    const uint32_t bars = bits_ring + (kBitsB ? kBitStages * kBitTileBytes : 0u);
+    auto bfull_bar = [&](uint32_t s) { return bars + 256 + 8 * s; };                // kBitsB only
+    auto bempty_bar = [&](uint32_t s) { return bars + 256 + 8 * (kBitStages + s); };
     auto full_bar = [&](uint32_t s) { return bars + 8 * s; };
     auto empty_bar = [&](uint32_t s) { return bars + 8 * (kStages + s); };
     auto tfull_bar = [&](uint32_t a) { return bars + 8 * (2 * kStages + a); };
@@ -114,12 +132,19 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
         asm volatile("prefetch.tensormap [%0];" ::"l"(&mapA) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&mapR) : "memory");
         for (uint32_t s = 0; s < kStages; s++) {
-            mbar_init(full_bar(s), 1);                            // the leader's expect_tx arrival
+            mbar_init(full_bar(s), kBitsB ? 1 + 2 * 4 : 1);       // the leader's expect_tx arrival (+ one expander group per CTA)
             mbar_init(empty_bar(s), 1);                           // one multicast commit
         }
         for (uint32_t a = 0; a < 2; a++) {
             mbar_init(tfull_bar(a), 1);
             mbar_init(tempty_bar(a), 8);                          // 4 epilogue warps of each CTA
+        }
+        if (kBitsB) {
+            asm volatile("prefetch.tensormap [%0];" ::"l"(&mapBits) : "memory");
+            for (uint32_t s = 0; s < kBitStages; s++) {
+                mbar_init(bfull_bar(s), 1);
+                mbar_init(bempty_bar(s), 4);                      // one arrival per warp of the consuming group
+            }
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -149,9 +174,9 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 const uint32_t lead_full = map_to_cta(full_bar(stage), 0);
                 const int32_t row = (int32_t)(kb * kTileK);
                 if (elect_one()) {
-                    if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * kBytesStage);   // both CTAs' bytes
+                    if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * (kBitsB ? kBytesA : kBytesStage));   // both CTAs' bytes
                     tma_load_2d_pair_hint(sa, &mapA, lead_full, a_col, row, polA);
-                    tma_load_2d_pair_hint(sa + kBytesA, &mapR, lead_full, r_col, row, polR);
+                    if (!kBitsB) tma_load_2d_pair_hint(sa + kBytesA, &mapR, lead_full, r_col, row, polR);
                 }
                 __syncwarp();
                 if (++stage == kStages) { stage = 0; phase ^= 1; }
@@ -189,7 +214,67 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 }
             }
         }
-    } else {
+    } else if (kBitsB && warp >= 6) {
+        // ===================== B-operand expanders (warps 6..13, both CTAs) =====================
+        // The packed bits of this CTA's half tile (128 K rows x 16 bytes) arrive through their own, deeper TMA ring
+        // (issued kBitStages - 1 K blocks ahead by warp 6), so that only the expansion itself -- not a global-memory
+        // latency -- sits between "stage freed" and "stage full", in parallel with the A tile's TMA.
+        // Two groups of 4 warps take alternate K blocks: a group has two stage periods for its load-expand-store-
+        // fence-arrive chain (one was not enough: the chain, ~600 cycles, exceeds the 512-cycle MMA time of a stage).
+        const uint32_t group = (warp - 6) >> 2;
+        const uint32_t r = ((warp - 6) & 3) * 32 + lane;            // K row of the stage owned by this thread
+        const uint32_t my_tiles = (sched.total > pair) ? (sched.total - pair + n_pairs - 1) / n_pairs : 0u;
+        const uint32_t total_kb = my_tiles * k_blocks;              // K blocks this CTA streams
+        // load cursor (runs ahead) -- only used by warp 6
+        uint32_t lt = pair, lkb = 0, lg = 0, lrow = 0, lcol = 0;
+        auto set_load_tile = [&]() {
+            uint32_t mt, nt;
+            sched.coords(lt, mt, nt);
+            const uint32_t col0 = nt * kTileN + rank * kHalfN;
+            const uint32_t inst = col0 / k;
+            lrow = inst * bits_rows_per_inst + bits_row0;           // instances past the batch: out of range -> zeros
+            lcol = (col0 - inst * k) / 8;
+        };
+        auto issue_load = [&]() {                                   // K block lg of the stream -> ring slot lg % kBitStages
+            const uint32_t bs = lg % kBitStages, bphase = (lg / kBitStages) & 1;
+            mbar_wait(bempty_bar(bs), bphase ^ 1);
+            if (elect_one()) {
+                mbar_expect_tx(bfull_bar(bs), kBitTileBytes);
+                tma_load_2d(bits_ring + bs * kBitTileBytes, &mapBits, bfull_bar(bs), (int32_t)lcol,
+                            (int32_t)(lrow + lkb * kTileK));
+            }
+            __syncwarp();
+            lg++;
+            if (++lkb == k_blocks) { lkb = 0; lt += n_pairs; if (lg < total_kb) set_load_tile(); }
+        };
+        if (warp == 6 && total_kb) set_load_tile();
+        for (uint32_t g = group; g < total_kb; g += kExpGroups) {
+            if (warp == 6)
+                while (lg < total_kb && lg < g + kBitStages - 1) issue_load();
+            const uint32_t bs = g % kBitStages, bphase = (g / kBitStages) & 1;
+            const uint32_t stage = g % kStages, phase = (g / kStages) & 1;
+            mbar_wait(bfull_bar(bs), bphase);
+            uint32_t w[4];
+            asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                         : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(bits_ring + bs * kBitTileBytes + r * 16));
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bempty_bar(bs));
+            mbar_wait(empty_bar(stage), phase ^ 1);                 // the MMAs that read this B buffer have retired
+            const uint32_t srow = base + stage * kBytesStage + kBytesA + r * 128;
+#pragma unroll
+            for (uint32_t c = 0; c < 8; c++) {                      // 16-byte chunk c = columns 16c .. 16c+15
+                const uint32_t bits = w[c >> 1] >> (16 * (c & 1));
+                uint32_t o[4];
+#pragma unroll
+                for (int h = 0; h < 4; h++) o[h] = (((bits >> (4 * h)) & 0xfu) * 0x00204081u) & 0x01010101u;
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
+                             ::"r"(srow + ((c ^ (r & 7)) << 4)), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]) : "memory");
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");        // generic stores -> the MMA's proxy
+            __syncwarp();
+            if (lane == 0) mbar_arrive_remote(map_to_cta(full_bar(stage), 0));
+        }
+    } else if (warp < 6) {
         // ===================== epilogue (warps 2..5, both CTAs) =====================
         const uint32_t quarter = warp & 3;
         const uint32_t lead_tempty0 = map_to_cta(tempty_bar(0), 0), lead_tempty1 = map_to_cta(tempty_bar(1), 0);
@@ -263,9 +348,10 @@ bool encaps_tc2_supported(const Ctx *c, uint32_t batch)
     return encaps_tc_supported(c, batch) && c->sm_count >= 2;
 }
 
-template <uint32_t kStages, uint32_t kTileK, int kMode>
+template <uint32_t kStages, uint32_t kTileK, int kMode, bool kBitsB = false>
 static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t *d_flags, const int8_t *d_E1,
-                               uint32_t batch, uint32_t row0, uint32_t rows, cudaStream_t st)
+                               uint32_t batch, uint32_t row0, uint32_t rows, cudaStream_t st,
+                               const uint8_t *d_Rbits = nullptr)
 {
     using Cfg = PairCfg<kStages, kTileK>;
     const lwe_params &p = c->p;
@@ -274,8 +360,9 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint3
     // d_A holds rows [row0, row0 + rows) of A; the matching rows of the expanded R follow from row0
     if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, rows, kTileK)) return cudaErrorInvalidValue;
     if (!make_map_u8(c, &mapR, c->d_Rexp + (size_t)row0 * ncols, ncols, rows, kTileK)) return cudaErrorInvalidValue;
-    auto kern = encaps_tc2_kernel<kStages, kTileK, kMode>;
-    cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes);
+    auto kern = encaps_tc2_kernel<kStages, kTileK, kMode, kBitsB>;
+    const uint32_t smem_bytes = kBitsB ? Cfg::kSmemBytesBits : Cfg::kSmemBytes;
+    cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (err != cudaSuccess) return err;
     const uint32_t tiles = ((2 * p.n + kPairM - 1) / kPairM) * ((ncols + kTileN - 1) / kTileN);
     uint32_t pairs = (uint32_t)c->sm_count / 2;
@@ -283,21 +370,41 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint3
     // LWE_OPT_TUNE (experiments only): bits 0-3 log2 of the n-tile group width (0 = default 8),
     // bits 4-5 / 6-7 L2 policy of the A / R streams, bits 8-9 ring variant
     const uint32_t tune = (uint32_t)c->tune;
-    const uint32_t gw = (tune & 15u) ? (1u << ((tune & 15u) - 1)) : 8u;
+    // default tile order: with the expanded operand, groups of 8 n-tiles keep the group's R panels in L2 while A is
+    // re-streamed once per group; with the bit operand R is 16x smaller and stays in L2 by itself, so all n-tiles of
+    // an A strip run together and A crosses HBM once (ncu at C4: 1.14 GB -> 0.30 GB read per launch)
+    const uint32_t n_tiles_all = (ncols + kTileN - 1) / kTileN;
+    const uint32_t gw = (tune & 15u) ? (1u << ((tune & 15u) - 1)) : (kBitsB ? n_tiles_all : 8u);
     ProfScope prof(c, LWE_K_ENCAPS_TC, st);
     // signed byte-plane sums of the N2 variant: |plane| <= 255 * 128 * rows <= 65280 * 65536, and twice that plus q
     // stays below 2^32
     const uint64_t plane_max = 255ull * 128ull * rows, q = p.q;
     const uint32_t pv_bias = (uint32_t)((plane_max + q - 1) / q * q), pv_e1bias = (uint32_t)((128 + q - 1) / q * q);
-    kern<<<2 * pairs, kThreads, Cfg::kSmemBytes, st>>>(mapA, mapR, d_U, d_flags, d_E1, rows, p.n, p.k, ncols, c->mq, gw,
-                                                       (tune >> 4) & 3u, (tune >> 6) & 3u, pv_bias, pv_e1bias);
+    // packed bits of R as a byte matrix [batch * m][k / 8]; a bit tile = 128 rows x 16 bytes.  Rows of the panel
+    // past `rows` meet zero-filled rows of A, rows past the last instance are zero-filled by TMA.
+    CUtensorMap mapBits = mapR;
+    if (kBitsB && !make_map_plain_u8(c, &mapBits, d_Rbits, p.k / 8, (uint64_t)batch * p.m, 16, kTileK))
+        return cudaErrorInvalidValue;
+    kern<<<2 * pairs, kBitsB ? kThreadsBits : kThreads, smem_bytes, st>>>(
+        mapA, mapR, d_U, d_flags, d_E1, rows, p.n, p.k, ncols, c->mq, gw, (tune >> 4) & 3u, (tune >> 6) & 3u, pv_bias,
+        pv_e1bias, mapBits, row0, p.m);
     c->launches++;
     return cudaGetLastError();
 }
 
-cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0, uint32_t rows,
-                              int mode, uint32_t *d_flags, cudaStream_t st)
+bool encaps_tc2_bits_supported(const Ctx *c, uint32_t batch)
 {
+    return encaps_tc2_supported(c, batch) && c->p.k % 128 == 0;
+}
+
+cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0, uint32_t rows,
+                              int mode, uint32_t *d_flags, cudaStream_t st, const uint8_t *d_Rbits)
+{
+    if (d_Rbits) {              // B operand expanded from the packed bits inside the kernel
+        if (mode == kEpiAccum) return launch_pair<6, 128, kEpiAccum, true>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st, d_Rbits);
+        if (mode == kEpiCompare) return launch_pair<6, 128, kEpiCompare, true>(c, d_A, d_U, d_flags, nullptr, batch, row0, rows, st, d_Rbits);
+        return launch_pair<6, 128, kEpiStore, true>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st, d_Rbits);
+    }
     if (mode == kEpiAccum) return launch_pair<6, 128, kEpiAccum>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
     if (mode == kEpiCompare) return launch_pair<6, 128, kEpiCompare>(c, d_A, d_U, d_flags, nullptr, batch, row0, rows, st);
     switch ((c->tune >> 8) & 3) {

@@ -71,6 +71,7 @@ struct Ctx {
     int keygen_path;                  // LWE_OPT_KEYGEN_PATH
     int tune;                         // LWE_OPT_TUNE: launch-shape experiments, no semantic effect
     int regen_path;                   // LWE_OPT_REGEN_PATH
+    int r_operand;                    // LWE_OPT_R_OPERAND
 
     // device tables
     uint32_t *d_te0;                  // 256-entry AES T-table (word = 2S | S<<8 | S<<16 | 3S<<24)
@@ -177,8 +178,12 @@ bool encaps_tc2_supported(const Ctx *c, uint32_t batch);
 uint32_t encaps_regen_lock_words(const lwe_params &p);
 bool encaps_regen_tc_supported(const Ctx *c, uint32_t batch);
 cudaError_t launch_encaps_regen_tc(Ctx *c, const AesKey &key, uint16_t *d_U, cudaStream_t st);
+// d_Rbits != NULL: the B operand is expanded from the packed bits inside the kernel (needs
+// encaps_tc2_bits_supported); NULL: it is read from the expanded workspace c->d_Rexp
+bool encaps_tc2_bits_supported(const Ctx *c, uint32_t batch);
 cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0,
-                              uint32_t rows, int mode, uint32_t *d_flags, cudaStream_t st);
+                              uint32_t rows, int mode, uint32_t *d_flags, cudaStream_t st,
+                              const uint8_t *d_Rbits = nullptr);
 // N2 (the paper's own PKE variant)
 cudaError_t launch_sample_gauss(Ctx *c, void *d_out, bool as_u16, uint64_t first, uint64_t count, const AesKey &key,
                                 uint32_t tag, uint32_t inst0, uint32_t n_inst, double sigma, cudaStream_t st);

@@ -125,6 +125,13 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar)
 {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
+// the same with the default (CTA-scope release) semantics: for per-stage producer signals, where the data being
+// published is shared memory already fenced into the async proxy.  The cluster-scope release above blocks the
+// thread for ~1.5k cycles (measured: one per K block made the expander warps, not the tensor pipe, the limit).
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_bar)
+{
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
 // TMA load whose completion bytes are credited to a barrier of the pair's leader CTA
 __device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap *map, uint32_t cluster_bar, int32_t c0,
                                                  int32_t c1)
@@ -276,6 +283,22 @@ inline bool make_map_u8(const Ctx *c, CUtensorMap *map, const void *ptr, uint64_
     CUresult r = ((EncodeTiledFn)c->encode_tiled)(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(ptr), dims,
                                                   strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+// u8 matrix [rows][width] row-major, box {box_w bytes, box_rows}, no swizzle, out-of-bounds -> 0
+inline bool make_map_plain_u8(const Ctx *c, CUtensorMap *map, const void *ptr, uint64_t width, uint64_t rows,
+                              uint32_t box_w, uint32_t box_rows)
+{
+    if (!c->encode_tiled) return false;
+    cuuint64_t dims[2] = {width, rows};
+    cuuint64_t strides[1] = {width};
+    cuuint32_t box[2] = {box_w, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = ((EncodeTiledFn)c->encode_tiled)(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(ptr), dims,
+                                                  strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                  CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                                                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
 }

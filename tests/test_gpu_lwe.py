@@ -136,14 +136,21 @@ ENCAPS_SHAPES = [  # (m, n, k, q, batch)
 
 def run_encaps(H, path, m, n, k, q, batch, A, b, Rbits, mubits):
     with B().Context(n, m, k, q, 4, batch) as c:
-        c.set_option(B().OPT_ENCAPS_PATH, path)
+        set_encaps_path(c, path)
         U, v = H.dev_empty_u16(batch, n, k), H.dev_empty_u16(batch, k)
         U.fill_(-1)
         c.encaps(H.dev(A), 0, H.dev(b), H.dev(Rbits), H.dev(mubits), U, v, batch)
         return H.host_u16(U), H.host_u16(v)
 
 
-ENCAPS_PATHS = dict(argvalues=[3, 2, 1], ids=["tcgen05_pair", "tcgen05", "simt"])
+# 3 = CTA-pair tcgen05 GEMM (B operand expanded from R's packed bits inside the kernel where k % 128 == 0),
+# 13 = the same kernel reading the u8 operand expanded into the workspace, 2 = single-CTA tcgen05, 1 = CUDA cores
+ENCAPS_PATHS = dict(argvalues=[3, 13, 2, 1], ids=["tcgen05_pair", "tcgen05_pair_expandedR", "tcgen05", "simt"])
+
+
+def set_encaps_path(c, path):
+    c.set_option(B().OPT_ENCAPS_PATH, path % 10)
+    c.set_option(B().OPT_R_OPERAND, path // 10)
 
 
 @pytest.mark.parametrize("path", **ENCAPS_PATHS)
@@ -212,7 +219,8 @@ def test_encaps_regenerated_A_equals_stored_and_oracle(H, path, m, n, k, q, batc
     Rbits = W.random_bytes(batch * m * k // 8, 23).reshape(batch, -1)
     mubits = W.random_bytes(batch * k // 8, 24).reshape(batch, -1)
     with B().Context(n, m, k, q, 4, batch) as c:
-        c.set_option(B().OPT_ENCAPS_PATH, path)
+        set_encaps_path(c, path)
+        c.set_option(B().OPT_REGEN_PATH, 1)                    # row panels (the fused kernel has its own test)
         c.set_option(B().OPT_PANEL_ROWS, panel)
         U, v = H.dev_empty_u16(batch, n, k), H.dev_empty_u16(batch, k)
         U.fill_(-1)
@@ -422,7 +430,7 @@ def test_decaps_fo_matches_oracle_honest_and_tampered(H, path, n, m, k, q, batch
         if kind == "v_big": v[t, k - 1] = (int(v[t, k - 1]) + q // 2 + 3) % q
         if kind == "coins": R_in[t, 9] ^= 0x40
     with B().Context(n, m, k, q, 4, batch) as c:
-        c.set_option(B().OPT_ENCAPS_PATH, path)
+        set_encaps_path(c, path)
         dU = H.dev(U)
         out, ok = H.dev_empty_u8(batch, k // 8), H.dev_empty_u8(batch)
         ok.fill_(7)
