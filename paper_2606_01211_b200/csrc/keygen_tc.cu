@@ -80,13 +80,16 @@ template <uint32_t CPI, uint32_t SLABS>
 __global__ void __launch_bounds__(kThreads, 1)
 keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapS,
                  const uint16_t *__restrict__ e, uint16_t *__restrict__ b, uint32_t m, uint32_t n, uint32_t batch,
-                 uint32_t N, uint32_t stages, ModQ mq)
+                 uint32_t N, uint32_t stages, ModQ mq, uint32_t rps)
 {
+    // rps = rows of A per strip (<= 128, a multiple of 8; the TMA box of A has rps rows).  The MMA is always
+    // M = 128: rows rps..127 of the accumulator come from stale shared memory and are never read back.
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t base = (raw + 1023u) & ~1023u;
     const uint32_t bytes_slab = kBytesA + N * kTileK;
     const uint32_t bytes_stage = SLABS * bytes_slab;
+    const uint32_t tx_stage = SLABS * (rps * kTileK + N * kTileK);          // bytes TMA delivers per stage
     const uint32_t bars = base + stages * bytes_stage;
     auto full_bar = [&](uint32_t s) { return bars + 8 * s; };
     auto empty_bar = [&](uint32_t s) { return bars + 8 * (kMaxStages + s); };
@@ -96,7 +99,7 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
 
     const uint32_t warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;   // warp-uniform
-    const uint32_t strips = (m + kTileM - 1) / kTileM;
+    const uint32_t strips = (m + rps - 1) / rps;
     const uint32_t k_blocks = (2 * n + SLABS * kTileK - 1) / (SLABS * kTileK);      // stages per strip
     const uint32_t acc_cols = (N <= 32) ? 32 : (N <= 64) ? 64 : (N <= 128) ? 128 : 256;   // per accumulator
     const uint32_t tmem_cols = 2 * acc_cols;
@@ -124,13 +127,13 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     if (warp == 0) {
         uint32_t stage = 0, phase = 0;
         for (uint32_t t = blockIdx.x; t < strips; t += gridDim.x) {
-            const int32_t row0 = (int32_t)(t * kTileM);
+            const int32_t row0 = (int32_t)(t * rps);
             for (uint32_t kb = 0; kb < k_blocks; kb++) {
                 mbar_wait(empty_bar(stage), phase ^ 1);
                 const uint32_t sa = base + stage * bytes_stage;
                 const int32_t k0 = (int32_t)(kb * SLABS * kTileK);
                 if (elect_one()) {
-                    mbar_expect_tx(full_bar(stage), bytes_stage);                // out-of-range slabs arrive as zeros
+                    mbar_expect_tx(full_bar(stage), tx_stage);                   // out-of-range slabs arrive as zeros
 #pragma unroll
                     for (uint32_t h = 0; h < SLABS; h++)                         // 128 rows x 128 bytes of k' each
                         tma_load_2d(sa + h * kBytesA, &mapA, full_bar(stage), k0 + (int32_t)(h * kTileK), row0);
@@ -181,21 +184,29 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
         uint32_t it = 0;
         for (uint32_t t = blockIdx.x; t < strips; t += gridDim.x, it++) {
             const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
+            const uint32_t rin = quarter * 32 + lane;                    // row inside the strip
+            const uint32_t i = t * rps + rin;
+            const bool row_ok = rin < rps && i < m;
+            // e of the first 32 instances is fetched while the main loop of this strip still runs: with one strip
+            // per CTA nothing else hides the epilogue, and 4 rounds of dependent global loads were ~4 us of 56
+            uint32_t epre[32];
+#pragma unroll
+            for (uint32_t x = 0; x < 32; x++) epre[x] = (row_ok && x < batch) ? (uint32_t)__ldg(e + (size_t)x * m + i) : 0u;
             mbar_wait(tfull_bar(acc), acc_phase);
             tc_fence_after();
-            const uint32_t i = t * kTileM + quarter * 32 + lane;
             const uint32_t taddr = tmem_base + ((quarter * 32) << 16) + acc * acc_cols;
-#pragma unroll 1
-            for (uint32_t i0 = 0; i0 < batch; i0 += 8) {
+#pragma unroll
+            for (uint32_t i0 = 0; i0 < 128; i0 += 8) {
+                if (i0 >= batch) break;
                 uint32_t r[8 * CPI];
                 tmem_ld_8inst<CPI>(taddr + i0 * CPI, r);
                 tmem_ld_wait();
-                if (i < m) {
+                if (row_ok) {
 #pragma unroll
                     for (uint32_t x = 0; x < 8; x++) {
                         const uint32_t inst = i0 + x;
                         if (inst < batch) {
-                            const uint32_t ei = e[(size_t)inst * m + i];
+                            const uint32_t ei = (i0 < 32) ? epre[(i0 + x) & 31] : (uint32_t)e[(size_t)inst * m + i];
                             uint32_t o;
                             if (CPI == 2) {
                                 o = (r[2 * x] + (r[2 * x + 1] << 8) + ei) & mq.mask;     // q | 2^16: wrap-around is exact
@@ -262,7 +273,14 @@ cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, c
         if (err != cudaSuccess) return err;
     }
     CUtensorMap mapA, mapS;
-    if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, p.m, kTileM)) return cudaErrorInvalidValue;
+    // rows per strip: as many strips as fill whole waves of SMs (C4: 16384 rows -> 147 strips of 112 rows instead of
+    // 128 strips of 128 on 148 SMs; each SM keeps its whole shared memory in flight, so more SMs = more bandwidth)
+    const uint32_t waves = (p.m + kTileM * (uint32_t)c->sm_count - 1) / (kTileM * (uint32_t)c->sm_count);
+    uint32_t rps = ((p.m + waves * (uint32_t)c->sm_count - 1) / (waves * (uint32_t)c->sm_count) + 7u) & ~7u;
+    if (rps > kTileM) rps = kTileM;
+    if (rps < 8) rps = 8;
+    if (((uint32_t)c->tune >> 14) & 1u) rps = kTileM;                    // LWE_OPT_TUNE bit 14: 128-row strips
+    if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, p.m, rps)) return cudaErrorInvalidValue;
     if (!make_map_u8(c, &mapS, c->d_Sx, 2ull * p.n, N, N)) return cudaErrorInvalidValue;
     // slabs per stage: as wide as leaves >= 3 stages in flight (LWE_OPT_TUNE bits 10-11 force 1 / 2 / 4)
     const uint32_t bytes_slab = kBytesA + N * kTileK;
@@ -275,7 +293,7 @@ cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, c
     if (stages > kMaxStages) stages = kMaxStages;
     const uint32_t smem = stages * bytes_stage + 1024 + 256;
     typedef void (*Kern)(const CUtensorMap, const CUtensorMap, const uint16_t *, uint16_t *, uint32_t, uint32_t, uint32_t,
-                         uint32_t, uint32_t, ModQ);
+                         uint32_t, uint32_t, ModQ, uint32_t);
     static const Kern table[3][3] = {
         {keygen_tc_kernel<2, 1>, keygen_tc_kernel<2, 2>, keygen_tc_kernel<2, 4>},
         {keygen_tc_kernel<3, 1>, keygen_tc_kernel<3, 2>, keygen_tc_kernel<3, 4>},
@@ -289,10 +307,10 @@ cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, c
         if (err != cudaSuccess) return err;
         configured[cpi - 2][si] = 1;
     }
-    const uint32_t strips = (p.m + kTileM - 1) / kTileM;
+    const uint32_t strips = (p.m + rps - 1) / rps;
     const uint32_t grid = strips < (uint32_t)c->sm_count ? strips : (uint32_t)c->sm_count;
     ProfScope prof(c, LWE_K_KEYGEN_TC, st);
-    kern<<<grid, kThreads, smem, st>>>(mapA, mapS, d_e, d_b, p.m, p.n, batch, N, stages, c->mq);
+    kern<<<grid, kThreads, smem, st>>>(mapA, mapS, d_e, d_b, p.m, p.n, batch, N, stages, c->mq, rps);
     c->launches++;
     return cudaGetLastError();
 }
