@@ -246,10 +246,7 @@ class Job:
     def step(self):
         c, w = self.ctx, self.w
         n, m, k, Bt, seed, i0 = w.n, w.m, w.k, w.batch, w.seed, self.inst0()
-        c.sample_uniform(self.s, 0, n, seed, W.TAG_S, i0, Bt)
-        c.sample_cbd(self.e, 0, m, seed, W.TAG_E, i0, Bt)
-        c.sample_bits(self.Rbits, 0, m * k, seed, W.TAG_R, i0, Bt)
-        c.sample_bits(self.mubits, 0, k, seed, W.TAG_MU, i0, Bt)
+        c.sample_kem(self.s, self.e, self.Rbits, self.mubits, seed, i0, Bt)      # s, e, R, mu in one launch
         c.keygen(self.A, 0, self.s, self.e, self.b, Bt)
         c.encaps(self.A, 0, self.b, self.Rbits, self.mubits, self.U, self.v, Bt)
         c.decaps(self.U, self.v, self.s, self.out, Bt)
@@ -355,10 +352,7 @@ def single_kem_phase(B, device: int) -> dict:
             c.sample_uniform(A, 0, m * n, w.seed, W.TAG_A)
 
             def sample():
-                c.sample_uniform(s, 0, n, w.seed, W.TAG_S)
-                c.sample_cbd(e, 0, m, w.seed, W.TAG_E)
-                c.sample_bits(Rb, 0, m * k, w.seed, W.TAG_R)
-                c.sample_bits(mu, 0, k, w.seed, W.TAG_MU)
+                c.sample_kem(s, e, Rb, mu, w.seed, 0, 1)
 
             t_s = time_call(sample, reps=20)
             t_k = time_call(lambda: c.keygen(A, 0, s, e, b, 1), reps=20)
@@ -366,7 +360,7 @@ def single_kem_phase(B, device: int) -> dict:
             t_d = time_call(lambda: c.decaps(U, v, s, o, 1), reps=20)
             t_r = time_call(lambda: c.encaps(None, w.seed, b, Rb, mu, U, v, 1), reps=10)
             ok = bool(torch.equal(o, mu))
-            # the whole single KEM (8 launches) replayed as ONE CUDA graph: every call only enqueues on the caller's
+            # the whole single KEM (5 launches) replayed as ONE CUDA graph: every call only enqueues on the caller's
             # stream, so the sequence is capturable; this removes the per-call host cost the figures above include
             t_g = None
             try:

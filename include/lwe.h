@@ -104,6 +104,15 @@ int lwe_sample_cbd(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count
 int lwe_sample_bits(lwe_ctx *ctx, uint8_t *d_out, uint64_t first_bit, uint64_t nbits,
                     uint64_t seed, uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream);
 
+/* The four per-instance objects of n_inst KEM instances in ONE launch: exactly what
+ *   lwe_sample_uniform(d_s, 0, n, seed, LWE_TAG_S, inst0, n_inst) + lwe_sample_cbd(d_e, 0, m, seed, LWE_TAG_E, ..)
+ *   + lwe_sample_bits(d_Rbits, 0, m*k, seed, LWE_TAG_R, ..) + lwe_sample_bits(d_mubits, 0, k, seed, LWE_TAG_MU, ..)
+ * write (n, m, k, q, eta of the context).  d_s [n_inst][n], d_e [n_inst][m], d_Rbits [n_inst][m*k/8],
+ * d_mubits [n_inst][k/8].  No new semantics: it saves three kernel launches per batch ("only a seed crosses the
+ * bus"). */
+int lwe_sample_kem(lwe_ctx *ctx, uint16_t *d_s, uint16_t *d_e, uint8_t *d_Rbits, uint8_t *d_mubits, uint64_t seed,
+                   uint32_t inst0, uint32_t n_inst, void *stream);
+
 /* ---- a3 / a3': KeyGen ------------------------------------------------------------
  * d_b[t][i] = ( sum_{j<n} A[i][j] * d_s[t][j] + d_e[t][i] ) mod q,  0 <= t < batch.
  * P:L60 eq.(1).  d_A: m x n row-major, streamed from HBM: once per call for
@@ -237,7 +246,7 @@ enum {
     LWE_K_RNG_FILL = 0, LWE_K_SAMPLE_UNIFORM = 1, LWE_K_SAMPLE_CBD = 2, LWE_K_SAMPLE_BITS = 3,
     LWE_K_KEYGEN_STORED = 4, LWE_K_KEYGEN_REGEN = 5, LWE_K_EXPAND_R_V = 6, LWE_K_ENCAPS_TC = 7,
     LWE_K_ENCAPS_SIMT = 8, LWE_K_DECAPS = 9, LWE_K_KEYGEN_PREP = 10, LWE_K_KEYGEN_TC = 11, LWE_K_FO_VERDICT = 12,
-    LWE_K_SAMPLE_GAUSS = 13, LWE_K_SAMPLE_CUNIFORM = 14, LWE_K_PREP_R_PV = 15, LWE_K_ENCAPS_REGEN_TC = 16, LWE_K_COUNT = 17
+    LWE_K_SAMPLE_GAUSS = 13, LWE_K_SAMPLE_CUNIFORM = 14, LWE_K_PREP_R_PV = 15, LWE_K_ENCAPS_REGEN_TC = 16, LWE_K_SAMPLE_KEM = 17, LWE_K_COUNT = 18
 };
 /* Sum of the device durations (milliseconds, CUDA events) and the number of timed launches
  * of kernel `kernel_id` since the last reset.  Waits for the recorded events to complete

@@ -29,11 +29,11 @@ OPT_REGEN_PATH = 7
 OPT_R_OPERAND = 8
 KERNELS = ["rng_fill", "sample_uniform", "sample_cbd", "sample_bits", "keygen_stored", "keygen_regen",
            "expand_R_v", "encaps_tc", "encaps_simt", "decaps", "keygen_prep", "keygen_tc", "fo_verdict",
-           "sample_gauss", "sample_cuniform", "prep_R_pv", "encaps_regen_tc"]
+           "sample_gauss", "sample_cuniform", "prep_R_pv", "encaps_regen_tc", "sample_kem"]
 
 EXPORTS = [
     "lwe_create", "lwe_destroy", "lwe_strerror", "lwe_last_cuda_error", "lwe_launch_count",
-    "lwe_rng_fill", "lwe_sample_uniform", "lwe_sample_cbd", "lwe_sample_bits",
+    "lwe_rng_fill", "lwe_sample_uniform", "lwe_sample_cbd", "lwe_sample_bits", "lwe_sample_kem",
     "lwe_keygen", "lwe_encaps", "lwe_decaps", "lwe_decaps_fo", "lwe_kem_host",
     "lwe_sample_gauss_s8", "lwe_sample_gauss_u16", "lwe_sample_cuniform_s8", "lwe_encaps_pv", "lwe_set_option",
     "lwe_profile_read", "lwe_profile_reset",
@@ -77,6 +77,7 @@ def load_library() -> C.CDLL:
     lib.lwe_rng_fill.argtypes = [vp, vp, sz, C.c_char_p, C.c_char_p, u64, vp]
     for f in (lib.lwe_sample_uniform, lib.lwe_sample_cbd, lib.lwe_sample_bits):
         f.argtypes = [vp, vp, u64, u64, u64, u32, u32, u32, vp]
+    lib.lwe_sample_kem.argtypes = [vp, vp, vp, vp, vp, u64, u32, u32, vp]
     lib.lwe_keygen.argtypes = [vp, vp, u64, vp, vp, vp, u32, vp]
     lib.lwe_encaps.argtypes = [vp, vp, u64, vp, vp, vp, vp, vp, u32, vp]
     lib.lwe_decaps.argtypes = [vp, vp, vp, vp, vp, u32, vp]
@@ -179,6 +180,10 @@ class Context:
                     stream=None):
         self._check(self._lib.lwe_sample_bits(self._h, _ptr(d_out), first_bit, nbits, seed, tag, inst0, n_inst,
                                               _stream(stream)), "lwe_sample_bits")
+
+    def sample_kem(self, d_s, d_e, d_Rbits, d_mubits, seed: int, inst0: int = 0, n_inst: int = 1, stream=None):
+        self._check(self._lib.lwe_sample_kem(self._h, _ptr(d_s), _ptr(d_e), _ptr(d_Rbits), _ptr(d_mubits), seed, inst0,
+                                             n_inst, _stream(stream)), "lwe_sample_kem")
 
     # -- a3..a6
     def keygen(self, d_A, seed_A: int, d_s, d_e, d_b, batch: int = 1, stream=None):

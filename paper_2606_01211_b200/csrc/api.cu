@@ -335,6 +335,20 @@ int lwe_sample_bits(lwe_ctx *ctx, uint8_t *d_out, uint64_t first_bit, uint64_t n
     return LWE_OK;
 }
 
+int lwe_sample_kem(lwe_ctx *ctx, uint16_t *d_s, uint16_t *d_e, uint8_t *d_Rbits, uint8_t *d_mubits, uint64_t seed,
+                   uint32_t inst0, uint32_t n_inst, void *stream)
+{
+    CHECK_CTX(ctx);
+    if ((uint64_t)inst0 + n_inst > (1ull << 32)) return LWE_ERR_PARAM;
+    if (n_inst == 0) return LWE_OK;
+    REQUIRE_PTR(d_s); REQUIRE_PTR(d_e); REQUIRE_PTR(d_Rbits); REQUIRE_PTR(d_mubits);
+    REQUIRE_ALIGNED(d_s); REQUIRE_ALIGNED(d_e); REQUIRE_ALIGNED(d_Rbits); REQUIRE_ALIGNED(d_mubits);
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_sample_kem(c, d_s, d_e, d_Rbits, d_mubits, seed_key_host(seed), inst0, n_inst, (cudaStream_t)stream));
+    return LWE_OK;
+}
+
 int lwe_keygen(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_t *d_s, const uint16_t *d_e,
                uint16_t *d_b, uint32_t batch, void *stream)
 {

@@ -153,6 +153,8 @@ cudaError_t launch_sample_cbd(Ctx *c, uint16_t *d_out, uint64_t first, uint64_t 
 cudaError_t launch_sample_bits(Ctx *c, uint8_t *d_out, uint64_t first_bit, uint64_t nbits,
                                const AesKey &key, uint32_t tag, uint32_t inst0, uint32_t n_inst,
                                cudaStream_t st);
+cudaError_t launch_sample_kem(Ctx *c, uint16_t *d_s, uint16_t *d_e, uint8_t *d_Rbits, uint8_t *d_mubits, const AesKey &key,
+                              uint32_t inst0, uint32_t n_inst, cudaStream_t st);
 cudaError_t launch_keygen_stored(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, const uint16_t *d_e,
                                  uint16_t *d_b, uint32_t batch, cudaStream_t st);
 size_t keygen_tc_workspace_bytes(const lwe_params &p);

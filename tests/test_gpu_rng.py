@@ -110,3 +110,28 @@ def test_argument_errors_do_not_launch(H, ctx):
         B.Context(256, 512, 256, 70000, 4)                      # q > 65536
     with pytest.raises(B.LweError):
         B.Context(250, 512, 256, 65536, 4)                      # n % 8 != 0
+
+
+@pytest.mark.parametrize("n,m,k,q,eta,inst0,n_inst", [
+    (256, 512, 256, 65536, 4, 0, 1),          # C1
+    (72, 200, 128, 65521, 8, 7, 3),           # prime q (rejection), k/8 = 16 bytes of mu
+    (8, 8, 8, 17, 1, 1 << 20, 5),             # 1-byte mu rows, 8-byte R rows (unaligned row stores)
+    (1024, 2048, 256, 65536, 4, 31, 4),       # C2 x 4 instances
+    (64, 136, 40, 3329, 3, 2, 2),             # k not a multiple of 16: ragged last chunk of every object
+])
+def test_sample_kem_equals_the_four_samplers_and_the_oracle(H, n, m, k, q, eta, inst0, n_inst):
+    """lwe_sample_kem draws s, e, R, mu of n_inst instances in one launch: the same bytes as the four single-object
+    samplers, i.e. as the oracle's O4 / O5 / O6 on tags S, E, R, MU."""
+    seed = 99
+    with H.B.Context(n, m, k, q, eta, n_inst) as c:
+        s, e = H.dev_empty_u16(n_inst, n), H.dev_empty_u16(n_inst, m)
+        R, mu = H.dev_empty_u8(n_inst, m * k // 8), H.dev_empty_u8(n_inst, k // 8)
+        for t in (s, e, R, mu):
+            t.fill_(0x5A)
+        c.sample_kem(s, e, R, mu, seed, inst0, n_inst)
+        gs, ge, gR, gmu = H.host_u16(s), H.host_u16(e), H.host_u8(R), H.host_u8(mu)
+    for t in range(n_inst):
+        assert np.array_equal(gs[t], O.sample_uniform(0, n, seed, O.TAG_S, inst0 + t, q)), ("s", t)
+        assert np.array_equal(ge[t], O.sample_cbd(0, m, seed, O.TAG_E, inst0 + t, q, eta)), ("e", t)
+        assert np.array_equal(gR[t], O.sample_bits(0, m * k, seed, O.TAG_R, inst0 + t)), ("R", t)
+        assert np.array_equal(gmu[t], O.sample_bits(0, k, seed, O.TAG_MU, inst0 + t)), ("mu", t)
