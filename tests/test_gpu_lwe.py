@@ -131,6 +131,10 @@ ENCAPS_SHAPES = [  # (m, n, k, q, batch)
     (2048, 1024, 256, 65536, 1),      # C2
     (1160, 456, 256, 65521, 5),       # 10 K blocks (> ring depth) with a tail, 4 pair tiles (last ragged), 5 N tiles
     (384, 1280, 256, 65536, 2),       # 10 pair tiles x 2: more tiles than a wave of small grids, both accumulators reused
+    (264, 136, 512, 65521, 2),        # k = 512: two N tiles per instance
+    (136, 72, 384, 65536, 3),         # k = 384: N tiles straddle instances (half tiles do not); 12 words of bits per row
+    (520, 64, 64, 3329, 5),           # k = 64: no bit operand (k % 128 != 0), 320 columns
+    (128, 8, 2048, 65536, 1),         # the largest k the ABI takes; a single, mostly empty M tile
 ]
 
 
@@ -287,7 +291,8 @@ def test_encaps_fused_regenerated_A_matches_oracle(H, m, n, k, q, seed, tune):
 # ---------------------------------------------------------------- decaps
 
 @pytest.mark.parametrize("n,k,q,batch", [(256, 256, 65536, 1), (1000, 256, 65521, 3), (64, 8, 17, 2),
-                                          (4096, 128, 65521, 2), (8192, 256, 65536, 4)])
+                                          (4096, 128, 65521, 2), (8192, 256, 65536, 4), (136, 512, 65521, 2),
+                                          (72, 384, 65536, 3), (8, 2048, 65536, 1)])
 def test_decaps_matches_oracle(H, n, k, q, batch):
     U = W.random_u16((batch, n, k), q, 41)
     v = W.random_u16((batch, k), q, 42)
