@@ -472,6 +472,24 @@ def run_ours(args):
                     "frac_of_burst_peak": achieved / int8_peak_burst, "frac_of_nominal_4500": achieved / 4500.0,
                     "algorithmic_int8_ops_per_launch": int8_ops}
 
+    # context for the tensor roofline: the vendor library's own int8 GEMM on this box, same protocol as
+    # MEASURED_PEAKS.json's bf16 figure (8192^3, best of 10, CUDA events).  Not the denominator of `frac`.
+    int8_lib = None
+    try:
+        a8 = torch.randint(-128, 127, (8192, 8192), dtype=torch.int8, device="cuda")
+        b8 = torch.randint(-128, 127, (8192, 8192), dtype=torch.int8, device="cuda")
+        torch._int_mm(a8, b8)
+        best = 1e9
+        for _ in range(10):
+            best = min(best, time_call(lambda: torch._int_mm(a8, b8), reps=1, warm=0))
+        int8_lib = 2.0 * 8192 ** 3 / (best * 1e-3) / 1e12
+        del a8, b8
+    except Exception:                                             # noqa: BLE001 -- optional context only
+        int8_lib = None
+    if roofline is not None:
+        roofline["library_int8_gemm_TOPs_8192cubed_burst"] = int8_lib
+        roofline["frac_of_library_int8_gemm"] = achieved / int8_lib if int8_lib else None
+
     # ---- side measurements (outside the timed step): single-instance calls and the a3' variant
     side = {}
     s1, e1, b1 = job.s[:1], job.e[:1], job.b[:1]
