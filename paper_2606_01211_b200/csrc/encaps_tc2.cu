@@ -17,6 +17,8 @@
 //   warp 0 : TMA producer (both CTAs; completion bytes of both land on the LEADER's full barrier)
 //   warp 1 : TMEM alloc (both CTAs) + MMA issuer (leader CTA only, one lane)
 //   warps 2-5 : epilogue on the CTA's own TMEM lanes, as in encaps_tc.cu
+//   warps 6-13 (kBitsB, the default for k % 128 == 0): expanders -- the B tile is not loaded but built in shared
+//               memory from R's packed bits (see the comment above the kernel); TMA then carries only A
 // Barriers: full[s] lives on the leader (1 arrival + 64 KB of transaction bytes); empty[s] and
 // tmem_full[a] exist in both CTAs and are signalled by multicast tcgen05.commit; tmem_empty[a]
 // lives on the leader and collects the 8 epilogue warps of the pair.
