@@ -363,6 +363,57 @@ def test_full_path_small_matches_oracle_everywhere(H, w, n, m, batch):
         assert np.array_equal(g["out"][t], oi.mubits)                # every bit recovered
 
 
+def test_two_contexts_of_different_shape_interleaved_on_two_streams(H):
+    """Two contexts (different n, m, q, eta) driven alternately on two streams, several rounds: the per-kernel launch
+    state the library caches (shared-memory attributes, occupancy, grids) must not leak between shapes, and the two
+    streams' work may overlap on the device.  Every object of every round equals the oracle."""
+    import torch
+    cfgs = [(W.C1, 256, 512, 2), (W.C3, 512, 1024, 3)]
+    st = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ctxs, As, outs = [], [], [[], []]
+    for w, n, m, batch in cfgs:
+        c = H.make_ctx(w, n=n, m=m, max_batch=batch)
+        dA = H.dev_empty_u16(m, n)
+        c.sample_uniform(dA, 0, m * n, w.seed, W.TAG_A)
+        ctxs.append(c); As.append(dA)
+    torch.cuda.synchronize()
+    try:
+        for rnd in range(3):
+            for x, (w, n, m, batch) in enumerate(cfgs):
+                c, k = ctxs[x], w.k
+                with torch.cuda.stream(st[x]):
+                    s, e, b = H.dev_empty_u16(batch, n), H.dev_empty_u16(batch, m), H.dev_empty_u16(batch, m)
+                    b2 = H.dev_empty_u16(1, m)
+                    Rb, mu = H.dev_empty_u8(batch, m * k // 8), H.dev_empty_u8(batch, k // 8)
+                    U, v, o = H.dev_empty_u16(batch, n, k), H.dev_empty_u16(batch, k), H.dev_empty_u8(batch, k // 8)
+                    c.sample_kem(s, e, Rb, mu, w.seed, 10 * rnd, batch)
+                    c.keygen(As[x], 0, s, e, b, batch)
+                    c.keygen(None, w.seed, s[:1], e[:1], b2, 1)             # A regenerated inside the GEMV
+                    c.encaps(As[x], 0, b, Rb, mu, U, v, batch)
+                    c.decaps(U, v, s, o, batch)
+                    outs[x].append((rnd, s, e, b, b2, Rb, mu, U, v, o))
+        torch.cuda.synchronize()
+        for x, (w, n, m, batch) in enumerate(cfgs):
+            A = H.host_u16(As[x])
+            for rnd, s, e, b, b2, Rb, mu, U, v, o in outs[x]:
+                gs, ge, gb, gb2 = H.host_u16(s), H.host_u16(e), H.host_u16(b), H.host_u16(b2)
+                gR, gmu, gU, gv, go = H.host_u8(Rb), H.host_u8(mu), H.host_u16(U), H.host_u16(v), H.host_u8(o)
+                for t in range(batch):
+                    oi = H.OracleInstance(w, 10 * rnd + t, n, m, with_A=False)
+                    assert np.array_equal(gs[t], oi.s) and np.array_equal(ge[t], oi.e)
+                    assert np.array_equal(gR[t], oi.Rbits) and np.array_equal(gmu[t], oi.mubits)
+                    ob = O.keygen(A, oi.s, oi.e, w.q)
+                    assert np.array_equal(gb[t], ob)
+                    if t == 0:
+                        assert np.array_equal(gb2[0], ob)
+                    oU, ov = O.encaps(A, ob, oi.Rbits, oi.mubits, w.k, w.q)
+                    assert np.array_equal(gU[t], oU) and np.array_equal(gv[t], ov)
+                    assert np.array_equal(go[t], oi.mubits)
+    finally:
+        for c in ctxs:
+            c.close()
+
+
 # ---------------------------------------------------------------- end to end with host buffers
 
 @pytest.mark.parametrize("n,m,k,q,batch,regen", [
