@@ -122,9 +122,10 @@ class Context:
 
     # -- plumbing
     def close(self):
-        if getattr(self, "_h", None) and self._h.value:
-            self._lib.lwe_destroy(self._h)
-            self._h = C.c_void_p()
+        h = getattr(self, "_h", None)
+        if h is not None and h.value:
+            self._h = None                      # first: at interpreter shutdown module globals may already be gone
+            self._lib.lwe_destroy(h)
 
     __del__ = close
 
