@@ -26,10 +26,7 @@ def device_kem(H, c, w, inst0, batch, dA, regen_too=False):
     s, e, b = H.dev_empty_u16(batch, n), H.dev_empty_u16(batch, m), H.dev_empty_u16(batch, m)
     Rbits, mubits = H.dev_empty_u8(batch, m * k // 8), H.dev_empty_u8(batch, k // 8)
     U, v, out = H.dev_empty_u16(batch, n, k), H.dev_empty_u16(batch, k), H.dev_empty_u8(batch, k // 8)
-    c.sample_uniform(s, 0, n, w.seed, W.TAG_S, inst0, batch)
-    c.sample_cbd(e, 0, m, w.seed, W.TAG_E, inst0, batch)
-    c.sample_bits(Rbits, 0, m * k, w.seed, W.TAG_R, inst0, batch)
-    c.sample_bits(mubits, 0, k, w.seed, W.TAG_MU, inst0, batch)
+    c.sample_kem(s, e, Rbits, mubits, w.seed, inst0, batch)          # the launch configuration bench.py times
     c.keygen(dA, 0, s, e, b, batch)
     g = dict(s=s, e=e, b=b, Rbits=Rbits, mubits=mubits, U=U, v=v, out=out)
     if regen_too:
