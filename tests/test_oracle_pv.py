@@ -146,3 +146,36 @@ def test_o14_noise_identity_and_every_bit_recovered(n, q, sigma, bound):
     assert np.array_equal((d.astype(np.int64) - mu * (q // 2)) % q, noise % q)
     assert np.abs(noise).max() < q // 4
     assert np.array_equal(out, mubits)
+
+
+# ---------------------------------------------------------------- the paper's Table 1 as a fixture
+def _table1_rows():
+    from pathlib import Path
+    rows = []
+    for line in (Path(__file__).parent / "golden" / "paper_table1_params.txt").read_text().splitlines():
+        if line.strip() and not line.startswith("#"):
+            n, q, sigma, kappa, eta, hard = line.split()
+            rows.append((int(n), int(q), float(sigma), int(kappa), int(eta), int(hard)))
+    return rows
+
+
+def test_table1_rows_used_by_n2_are_the_papers():
+    """workloads.PAPER_TABLE1 (what the N2 tests and bench.py run) is exactly the uint16-modulus part of the paper's
+    Table 1, with the binomial eta = 3 secret of P:L70."""
+    rows = _table1_rows()
+    assert len(rows) == 9 and all(r[4] == 3 for r in rows)
+    fit = [(n, q, s, kap) for n, q, s, kap, _, _ in rows if q <= 65536]
+    assert fit == list(W.PAPER_TABLE1)
+    assert all(q == 65537 for _, q, _, _, _, _ in rows[4:])
+
+
+@pytest.mark.parametrize("row", range(4))
+def test_table1_rows_decrypt_with_margin(row):
+    """For every Table 1 row the library runs, the decryption noise e^T r + e2 - s^T e1 of the paper's PKE stays far
+    inside the decoding threshold q/4 ("reliable decapsulation"): standard deviation from the closed-form
+    variances of O5 (eta/2), O12 (sigma^2 + 1/12) and O13 (kappa(kappa+1)/3), margin in standard deviations."""
+    n, q, sigma, kappa = W.PAPER_TABLE1[row]
+    var_g = sigma * sigma + 1.0 / 12.0
+    var = n * var_g * var_g + n * 1.5 * var_g + kappa * (kappa + 1) / 3.0        # e^T r  +  s^T e1  +  e2
+    margin = (q / 4.0) / np.sqrt(var)
+    assert margin > 4.0, (n, q, margin)
