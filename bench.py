@@ -386,6 +386,39 @@ def single_kem_phase(B, device: int) -> dict:
     return out
 
 
+def large_kem_phase(B, device: int, hbm_gbs: float) -> dict:
+    """C5 (n = 32768, m = 65536, A = 4 GiB; BJ configs[4]): one instance, A stored and A regenerated from its seed
+    (keygen: AES inside the GEMV; encaps: AES generator fused into the GEMM producer).  Milliseconds per call."""
+    w = W.C5
+    n, m, k = w.n, w.m, w.k
+    free, _ = torch.cuda.mem_get_info(device)
+    if free < 10 * (1 << 30):
+        return {"skipped": "less than 10 GiB of free device memory"}
+    dev = torch.device("cuda", device)
+    i16, u8 = dict(dtype=torch.int16, device=dev), dict(dtype=torch.uint8, device=dev)
+    with B.Context(n, m, k, w.q, w.eta, 1, device) as c:
+        A = torch.empty(m, n, **i16)
+        t_A = time_call(lambda: c.sample_uniform(A, 0, m * n, w.seed, W.TAG_A), reps=2, warm=1)
+        s, e, b, b2 = (torch.empty(1, n, **i16), torch.empty(1, m, **i16), torch.empty(1, m, **i16), torch.empty(1, m, **i16))
+        Rb, mu, o = torch.empty(1, m * k // 8, **u8), torch.empty(1, k // 8, **u8), torch.empty(1, k // 8, **u8)
+        U, v, U2 = torch.empty(1, n, k, **i16), torch.empty(1, k, **i16), torch.empty(1, n, k, **i16)
+        c.sample_kem(s, e, Rb, mu, w.seed, 0, 1)
+        t_k = time_call(lambda: c.keygen(A, 0, s, e, b, 1), reps=5, warm=2)
+        t_kr = time_call(lambda: c.keygen(None, w.seed, s, e, b2, 1), reps=3, warm=1)
+        t_e = time_call(lambda: c.encaps(A, 0, b, Rb, mu, U, v, 1), reps=5, warm=2)
+        t_er = time_call(lambda: c.encaps(None, w.seed, b, Rb, mu, U2, v, 1), reps=3, warm=1)
+        t_d = time_call(lambda: c.decaps(U, v, s, o, 1), reps=5, warm=2)
+        ok = bool(torch.equal(o, mu)) and bool(torch.equal(b, b2)) and bool(torch.equal(U, U2))
+        del A
+    a_bytes = 2.0 * m * n
+    return {"generate_A_ms": t_A, "generate_A_aes_GBps": a_bytes / (t_A * 1e-3) / 1e9,
+            "keygen_stored_ms": t_k, "keygen_stored_frac_hbm": a_bytes / (t_k * 1e-3) / 1e9 / hbm_gbs,
+            "keygen_regen_ms": t_kr, "keygen_regen_aes_GBps": a_bytes / (t_kr * 1e-3) / 1e9,
+            "encaps_stored_ms": t_e, "encaps_stored_A_GBps": a_bytes / (t_e * 1e-3) / 1e9,
+            "encaps_regen_fused_ms": t_er, "encaps_regen_aes_GBps": a_bytes / (t_er * 1e-3) / 1e9,
+            "decaps_ms": t_d, "stored_equals_regenerated_and_all_bits_recovered": ok}
+
+
 def traffic_from_profiles(kernel: str):
     """DRAM bytes per launch of `kernel` from the committed ncu summary (profiles/traffic.json:
     {"<kernel>": {"dram_bytes_per_launch": ..., "source": ...}}), else None."""
@@ -535,6 +568,7 @@ def run_ours(args):
                              "kem_per_s_encaps_plus_fo_decaps_B32": Bt * 1e3 / (t + t3)}
     side["paper_variant_n4096_B32"] = paper_variant_phase(job.B, local)
     side["single_kem_B1"] = single_kem_phase(job.B, local)
+    side["large_kem_C5_B1"] = large_kem_phase(job.B, local, peaks["hbm_gbs"])
     buf = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
     t = time_call(lambda: ctx.rng_fill(buf, buf.numel(), bytes(16), bytes(16), 0), reps=5)
     side["rng_fill_1GiB"] = {"ms": t, "GBps": buf.numel() / (t * 1e-3) / 1e9}
