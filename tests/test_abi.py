@@ -70,3 +70,14 @@ def test_product_does_not_import_the_oracle():
             text = p.read_text()
             assert not re.search(r"^\s*(from|import)\s+paper_2606_01211_b200\b", text, flags=re.M), p
             assert "#include \"../paper" not in text and "lwe_internal" not in text and "lwe.h" not in text, p
+
+
+def test_kernel_id_table_of_the_binding_matches_the_header():
+    """binding.KERNELS[i] names kernel LWE_K_<NAME> = i of include/lwe.h (lwe_profile_read ids)"""
+    import re
+    from paper_2606_01211_b200 import binding as B
+    header = (ROOT / "include" / "lwe.h").read_text()
+    ids = {name: int(i) for name, i in re.findall(r"LWE_K_([A-Z0-9_]+) = (\d+)", header)}
+    assert ids.pop("COUNT") == len(B.KERNELS) == len(ids)
+    for name, i in ids.items():
+        assert B.KERNELS[i].upper() == name, (i, name, B.KERNELS[i])
