@@ -27,6 +27,7 @@ ModQ make_modq(uint32_t q)
     mq.half = q / 2;
     mq.pow2 = is_pow2(q) ? 1u : 0u;
     mq.mask = q - 1;
+    mq.two32 = (uint32_t)((1ull << 32) % q);
     return mq;
 }
 
