@@ -21,9 +21,7 @@ TAG_A, TAG_S, TAG_E, TAG_R, TAG_MU = 1, 2, 3, 4, 5
 TAG_RG, TAG_E1, TAG_E2 = 6, 7, 8
 OPT_ENCAPS_PATH = 1
 OPT_PROFILE = 2
-OPT_GEMV_VARIANT = 3
 OPT_KEYGEN_PATH = 4
-OPT_TUNE = 5
 OPT_PANEL_ROWS = 6
 OPT_REGEN_PATH = 7
 OPT_R_OPERAND = 8

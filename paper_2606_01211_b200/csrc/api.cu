@@ -12,6 +12,47 @@ struct lwe_ctx {
     Ctx c;
 };
 
+namespace lwe {
+
+cudaError_t kernel_prepare(Ctx *c, const void *fn, size_t smem, int threads, int *occ)
+{
+    KernelCfg *k = nullptr;
+    for (int i = 0; i < c->n_kcfg; i++)
+        if (c->kcfg[i].fn == fn) { k = &c->kcfg[i]; break; }
+    if (!k) {
+        // first launch of this function by this context: opt in on the context's device
+        cudaFuncAttributes fa;
+        cudaError_t err = cudaFuncGetAttributes(&fa, fn);
+        if (err != cudaSuccess) return err;
+        const int limit = c->smem_optin - (int)fa.sharedSizeBytes;
+        if (limit > 48 * 1024) {
+            err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, limit);
+            if (err != cudaSuccess) return err;
+        }
+        if ((int)smem > limit && (int)smem > 48 * 1024) return cudaErrorInvalidValue;
+        if (c->n_kcfg >= kMaxKernelCfg) return occ ? cudaErrorInvalidValue : cudaSuccess;   // table full: still configured
+        k = &c->kcfg[c->n_kcfg++];
+        k->fn = fn;
+        k->occ_threads = 0;
+        k->occ_smem = 0;
+        k->occ = 0;
+    }
+    if (occ) {
+        if (!k->occ || k->occ_threads != threads || k->occ_smem != smem) {
+            int q = 0;
+            cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&q, fn, threads, smem);
+            if (err != cudaSuccess) return err;
+            k->occ = q < 1 ? 1 : q;
+            k->occ_threads = threads;
+            k->occ_smem = smem;
+        }
+        *occ = k->occ;
+    }
+    return cudaSuccess;
+}
+
+}  // namespace lwe
+
 namespace {
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -121,6 +162,7 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
     c->mq = make_modq(p->q);
     c->device = device;
     c->sm_count = prop.multiProcessorCount;
+    c->smem_optin = (int)prop.sharedMemPerBlockOptin;
 
     const size_t B = p->max_batch, n = p->n, m = p->m, k = p->k;
     cudaError_t e = cudaSuccess;
@@ -201,16 +243,6 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
     if (option == LWE_OPT_KEYGEN_PATH) {
         if (value < 0 || value > 2) return LWE_ERR_PARAM;
         ctx->c.keygen_path = (int)value;
-        return LWE_OK;
-    }
-    if (option == LWE_OPT_GEMV_VARIANT) {
-        if (value < 0 || value > 4) return LWE_ERR_PARAM;
-        ctx->c.gemv_variant = (int)value;
-        return LWE_OK;
-    }
-    if (option == LWE_OPT_TUNE) {
-        if (value < 0 || value > 0xffff) return LWE_ERR_PARAM;
-        ctx->c.tune = (int)value;
         return LWE_OK;
     }
     if (option == LWE_OPT_PANEL_ROWS) {
@@ -390,14 +422,15 @@ static int encaps_core(Ctx *c, const uint16_t *d_A, uint64_t seed_A, const uint1
         LAUNCH(c, launch_encaps_regen_tc(c, seed_key_host(seed_A), d_U, st));
         return LWE_OK;
     }
-    // Stored A: one pass over all m rows.  d_A == NULL: A is regenerated from seed_A one row panel at a
+    // Stored A: one pass over all m rows (m > 65536: passes of 65536 rows, the most a 32-bit byte-plane sum holds,
+    // accumulated mod q).  d_A == NULL: A is regenerated from seed_A one row panel at a
     // time into the context's panel buffer (rows of A are contiguous ranges of the counter-indexed
     // stream) and the contraction is accumulated over the panels; A is never held in full.
-    const uint32_t m = c->p.m, step = d_A ? m : c->panel_rows;
+    const uint32_t m = c->p.m, step = d_A ? (m < 65536u ? m : 65536u) : c->panel_rows;
     const AesKey keyA = d_A ? AesKey() : seed_key_host(seed_A);
     for (uint32_t row0 = 0; row0 < m; row0 += step) {
         const uint32_t rows = (m - row0 < step) ? (m - row0) : step;
-        const uint16_t *panel = d_A;
+        const uint16_t *panel = d_A ? d_A + (size_t)row0 * c->p.n : nullptr;
         if (!d_A) {
             LAUNCH(c, launch_sample_uniform(c, c->d_Apanel, (uint64_t)row0 * c->p.n, (uint64_t)rows * c->p.n, keyA,
                                             LWE_TAG_A, 0, 1, st));
@@ -436,6 +469,7 @@ int lwe_decaps_fo(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_b, const 
     REQUIRE_ALIGNED(d_A); REQUIRE_ALIGNED(d_b); REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v); REQUIRE_ALIGNED(d_s);
     REQUIRE_ALIGNED(d_Rbits); REQUIRE_ALIGNED(d_mubits_out); REQUIRE_ALIGNED(d_ok);
     if (c->encaps_path >= 2 && !encaps_tc_supported(c, batch)) return LWE_ERR_UNSUPPORTED;
+    if (c->p.m > 65536u) return LWE_ERR_UNSUPPORTED;     // the compare epilogue needs the whole sum in one pass
     DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
     // Alg. 5: 1. m' <- Decrypt(sk, c)
@@ -468,7 +502,7 @@ static int gauss_args(lwe_ctx *ctx, const void *d_out, uint64_t first, uint64_t 
 {
     int rc = sampler_args(ctx, d_out, first, count, tag, inst0, n_inst);
     if (rc != LWE_OK) return rc;
-    if (!(sigma >= 0.5 && sigma <= 8.0)) return LWE_ERR_PARAM;
+    if (!(sigma >= 0.5 && sigma <= 2.8)) return LWE_ERR_PARAM;   // the 24-entry table spans [-12, 12]: see lwe.h
     return LWE_OK;
 }
 
@@ -522,7 +556,7 @@ int lwe_encaps_pv(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_t, const 
     REQUIRE_ALIGNED(d_A); REQUIRE_ALIGNED(d_t); REQUIRE_ALIGNED(d_R); REQUIRE_ALIGNED(d_E1); REQUIRE_ALIGNED(d_e2);
     REQUIRE_ALIGNED(d_mubits); REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v);
     // tensor path: the CTA-pair GEMM; |lo/hi plane accumulator| <= 255 * 127 * m < 2^31 for m <= 65536
-    bool tc = encaps_tc2_supported(c, batch) && c->encaps_path != 1;
+    bool tc = encaps_tc2_supported(c, batch) && c->encaps_path != 1 && c->p.m <= 65536u;
     if (c->encaps_path >= 2 && !tc) return LWE_ERR_UNSUPPORTED;
     DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
@@ -542,6 +576,8 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint1
     REQUIRE_PTR(h_s); REQUIRE_PTR(h_e); REQUIRE_PTR(h_Rbits); REQUIRE_PTR(h_mubits);
     REQUIRE_PTR(h_b); REQUIRE_PTR(h_v); REQUIRE_PTR(h_mubits_out);
     REQUIRE_ALIGNED(d_A);
+    REQUIRE_ALIGNED(h_s); REQUIRE_ALIGNED(h_e); REQUIRE_ALIGNED(h_Rbits); REQUIRE_ALIGNED(h_mubits);
+    REQUIRE_ALIGNED(h_b); REQUIRE_ALIGNED(h_U); REQUIRE_ALIGNED(h_v); REQUIRE_ALIGNED(h_mubits_out);
     const size_t n = c->p.n, m = c->p.m, k = c->p.k;
     cudaStream_t st = (cudaStream_t)stream;
     DeviceGuard guard(c->device);

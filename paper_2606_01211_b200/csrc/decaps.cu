@@ -120,11 +120,9 @@ cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, cons
     const uint32_t rows_per_iter = kDecThreads / (k / 8);
     // exactly one wave of resident CTAs (a second, partial wave was the tail: 1184 CTAs on 740 slots ran at
     // 0.54 of HBM): as many row splits per instance as fit the SMs at the kernel's occupancy
-    static int per_sm = 0;
-    if (!per_sm) {
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, decaps_kernel, kDecThreads, 0) != cudaSuccess || per_sm < 1)
-            per_sm = 1;
-    }
+    int per_sm = 1;
+    cudaError_t perr = kernel_prepare(c, decaps_kernel, 0, kDecThreads, &per_sm);
+    if (perr != cudaSuccess) return perr;
     uint32_t splits = (uint32_t)(per_sm * c->sm_count) / batch;
     uint32_t max_splits = (n + 4 * rows_per_iter - 1) / (4 * rows_per_iter);       // >= 4 row groups per CTA
     if (splits > max_splits) splits = max_splits;

@@ -192,18 +192,15 @@ cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_
         const uint32_t rows_per_iter = kAuxThreads / wpr;
         const size_t smem = (size_t)k * sizeof(uint32_t);
         // exactly one wave of resident CTAs (608 CTAs on 296 slots left a third, nearly empty wave)
-        static int per_sm[2] = {0, 0};
-        int &occ = per_sm[write_Rexp ? 1 : 0];
-        if (!occ) {
-            cudaError_t qe = write_Rexp
-                ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, expand_R_and_v_w32_kernel<true>, kAuxThreads, smem)
-                : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, expand_R_and_v_w32_kernel<false>, kAuxThreads, smem);
-            if (qe != cudaSuccess || occ < 1) occ = 1;
-        }
+        int occ = 1;
+        cudaError_t perr = write_Rexp ? kernel_prepare(c, expand_R_and_v_w32_kernel<true>, smem, kAuxThreads, &occ)
+                                      : kernel_prepare(c, expand_R_and_v_w32_kernel<false>, smem, kAuxThreads, &occ);
+        if (perr != cudaSuccess) return perr;
         uint32_t splits = (uint32_t)(occ * c->sm_count) / batch;
         uint32_t max_splits = (m + 4 * rows_per_iter - 1) / (4 * rows_per_iter);   // >= 4 rows per thread
         if (splits > max_splits) splits = max_splits;
-        if (splits < 1) splits = 1;
+        const uint32_t min_splits = (m + 65535u) / 65536u;       // a CTA's 32-bit column sums hold <= 65536 rows
+        if (splits < min_splits) splits = min_splits;
         dim3 grid(splits, batch);
         if (write_Rexp)
             expand_R_and_v_w32_kernel<true><<<grid, kAuxThreads, smem, st>>>(
@@ -218,7 +215,8 @@ cudaError_t launch_expand_R_and_v(Ctx *c, const uint16_t *d_b, const uint8_t *d_
     uint32_t splits = (uint32_t)((4 * c->sm_count + batch - 1) / batch);
     uint32_t max_splits = (m + 4 * rows_per_iter - 1) / (4 * rows_per_iter);   // >= 4 row groups per CTA
     if (splits > max_splits) splits = max_splits;
-    if (splits < 1) splits = 1;
+    const uint32_t min_splits = (m + 65535u) / 65536u;           // a thread's 32-bit column sums hold <= 65536 rows
+    if (splits < min_splits) splits = min_splits;
     dim3 grid(splits, batch);
     expand_R_and_v_kernel<<<grid, kAuxThreads, 0, st>>>(d_b, d_Rbits, d_mubits, c->d_Rexp, d_v, c->d_vacc,
                                                         c->d_counters + 8 + c->p.max_batch, m, k,

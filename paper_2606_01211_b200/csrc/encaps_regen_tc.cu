@@ -288,12 +288,8 @@ cudaError_t launch_cfg(Ctx *c, const AesKey &key, uint16_t *d_U, cudaStream_t st
     CUtensorMap mapR;
     if (!make_map_u8(c, &mapR, c->d_Rexp, p.k, p.m, Cfg::kTileK)) return cudaErrorInvalidValue;
     auto kern = encaps_regen_tc_kernel<G, kStages>;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes);
-        if (err != cudaSuccess) return err;
-        configured = true;
-    }
+    cudaError_t perr = kernel_prepare(c, kern, Cfg::kSmemBytes);
+    if (perr != cudaSuccess) return perr;
     const uint32_t m_tiles = (2 * p.n + kTileM - 1) / kTileM;
     const uint32_t k_blocks = (p.m + Cfg::kTileK - 1) / Cfg::kTileK;
     const uint32_t splits = choose_splits(m_tiles, k_blocks, (uint32_t)c->sm_count);
@@ -313,18 +309,13 @@ uint32_t encaps_regen_lock_words(const lwe_params &p) { return 2 * ((2 * p.n + k
 // one instance (N = k <= 256 columns): every A tile feeds exactly one MMA tile
 bool encaps_regen_tc_supported(const Ctx *c, uint32_t batch)
 {
-    return batch == 1 && c->p.k <= kTileN && c->d_tile_locks != nullptr && encaps_tc_supported(c, batch);
+    return batch == 1 && c->p.k <= kTileN && c->p.m <= 65536u && c->d_tile_locks != nullptr && encaps_tc_supported(c, batch);
 }
 
 cudaError_t launch_encaps_regen_tc(Ctx *c, const AesKey &key, uint16_t *d_U, cudaStream_t st)
 {
-    // LWE_OPT_TUNE bits 12-13 (measurements): generator warps / ring depth
-    switch (((uint32_t)c->tune >> 12) & 3u) {
-    case 1: return launch_cfg<16, 3>(c, key, d_U, st);
-    case 2: return launch_cfg<16, 2>(c, key, d_U, st);
-    case 3: return launch_cfg<24, 2>(c, key, d_U, st);
-    default: return launch_cfg<24, 2>(c, key, d_U, st);
-    }
+    // 24 generator warps (K block 192), 2-stage ring: measured best on B200 (16 warps x 3 stages: -6 %)
+    return launch_cfg<24, 2>(c, key, d_U, st);
 }
 
 }  // namespace lwe

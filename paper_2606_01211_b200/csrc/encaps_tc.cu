@@ -206,8 +206,8 @@ encaps_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
 bool encaps_tc_supported(const Ctx *c, uint32_t batch)
 {
     const lwe_params &p = c->p;
-    return c->encode_tiled != nullptr && p.k % 16 == 0 && p.m <= 65536 && (2ull * p.n) % 16 == 0 &&
-           ((uint64_t)batch * p.k) % 16 == 0;
+    // m is not limited here: the callers pass row panels of at most 65536 rows (a byte-plane sum <= 255 * 65536)
+    return c->encode_tiled != nullptr && p.k % 16 == 0 && (2ull * p.n) % 16 == 0 && ((uint64_t)batch * p.k) % 16 == 0;
 }
 
 cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0, uint32_t rows,
@@ -221,7 +221,7 @@ cudaError_t launch_encaps_tc(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_
     if (!make_map_u8(c, &mapR, c->d_Rexp + (size_t)row0 * ncols, ncols, rows, kTileK)) return cudaErrorInvalidValue;
     auto kern = mode == kEpiAccum ? encaps_tc_kernel<kEpiAccum>
               : mode == kEpiCompare ? encaps_tc_kernel<kEpiCompare> : encaps_tc_kernel<kEpiStore>;
-    cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    cudaError_t err = kernel_prepare(c, kern, kSmemBytes);
     if (err != cudaSuccess) return err;
     const uint32_t tiles = ((2 * p.n + kTileM - 1) / kTileM) * ((ncols + kTileN - 1) / kTileN);
     uint32_t grid = tiles < (uint32_t)c->sm_count ? tiles : (uint32_t)c->sm_count;

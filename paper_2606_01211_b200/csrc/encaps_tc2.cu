@@ -59,24 +59,6 @@ struct PairSched {
     }
 };
 
-// L2 eviction policy for a TMA stream: 0 = normal, 1 = evict_first, 2 = evict_last
-__device__ __forceinline__ uint64_t l2_policy(uint32_t kind)
-{
-    uint64_t pol;
-    if (kind == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    else if (kind == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
-    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
-__device__ __forceinline__ void tma_load_2d_pair_hint(uint32_t dst, const CUtensorMap *map, uint32_t cluster_bar,
-                                                      int32_t c0, int32_t c1, uint64_t pol)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
-        " [%0], [%1, {%3, %4}], [%2], %5;"
-        ::"r"(dst), "l"(map), "r"(cluster_bar), "r"(c0), "r"(c1), "l"(pol) : "memory");
-}
-
 template <uint32_t kStages, uint32_t kTileK>
 struct PairCfg {
     static constexpr uint32_t kBytesA = kCtaM * kTileK;
@@ -98,7 +80,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kBitsB ? kThreadsBit
 encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
                   uint16_t *__restrict__ U, uint32_t *__restrict__ flags, const int8_t *__restrict__ E1, uint32_t m,
                   uint32_t n, uint32_t k,
-                  uint32_t ncols_total, ModQ mq, uint32_t group_w, uint32_t polA_kind, uint32_t polR_kind,
+                  uint32_t ncols_total, ModQ mq, uint32_t group_w,
                   uint32_t pv_bias, uint32_t pv_e1bias, const __grid_constant__ CUtensorMap mapBits, uint32_t bits_row0,
                   uint32_t bits_rows_per_inst)
 {
@@ -164,7 +146,6 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
     if (warp == 0) {
         // ===================== TMA producer (both CTAs) =====================
         uint32_t stage = 0, phase = 0;
-        const uint64_t polA = l2_policy(polA_kind), polR = l2_policy(polR_kind);
         for (uint32_t t = pair; t < sched.total; t += n_pairs) {
             uint32_t mt, nt;
             sched.coords(t, mt, nt);
@@ -177,8 +158,8 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 const int32_t row = (int32_t)(kb * kTileK);
                 if (elect_one()) {
                     if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * (kBitsB ? kBytesA : kBytesStage));   // both CTAs' bytes
-                    tma_load_2d_pair_hint(sa, &mapA, lead_full, a_col, row, polA);
-                    if (!kBitsB) tma_load_2d_pair_hint(sa + kBytesA, &mapR, lead_full, r_col, row, polR);
+                    tma_load_2d_pair(sa, &mapA, lead_full, a_col, row);
+                    if (!kBitsB) tma_load_2d_pair(sa + kBytesA, &mapR, lead_full, r_col, row);
                 }
                 __syncwarp();
                 if (++stage == kStages) { stage = 0; phase ^= 1; }
@@ -364,19 +345,16 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint3
     if (!make_map_u8(c, &mapR, c->d_Rexp + (size_t)row0 * ncols, ncols, rows, kTileK)) return cudaErrorInvalidValue;
     auto kern = encaps_tc2_kernel<kStages, kTileK, kMode, kBitsB>;
     const uint32_t smem_bytes = kBitsB ? Cfg::kSmemBytesBits : Cfg::kSmemBytes;
-    cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    cudaError_t err = kernel_prepare(c, kern, smem_bytes);
     if (err != cudaSuccess) return err;
     const uint32_t tiles = ((2 * p.n + kPairM - 1) / kPairM) * ((ncols + kTileN - 1) / kTileN);
     uint32_t pairs = (uint32_t)c->sm_count / 2;
     if (pairs > tiles) pairs = tiles;
-    // LWE_OPT_TUNE (experiments only): bits 0-3 log2 of the n-tile group width (0 = default 8),
-    // bits 4-5 / 6-7 L2 policy of the A / R streams, bits 8-9 ring variant
-    const uint32_t tune = (uint32_t)c->tune;
-    // default tile order: with the expanded operand, groups of 8 n-tiles keep the group's R panels in L2 while A is
+    // tile order: with the expanded operand, groups of 8 n-tiles keep the group's R panels in L2 while A is
     // re-streamed once per group; with the bit operand R is 16x smaller and stays in L2 by itself, so all n-tiles of
     // an A strip run together and A crosses HBM once (ncu at C4: 1.14 GB -> 0.30 GB read per launch)
     const uint32_t n_tiles_all = (ncols + kTileN - 1) / kTileN;
-    const uint32_t gw = (tune & 15u) ? (1u << ((tune & 15u) - 1)) : (kBitsB ? n_tiles_all : 8u);
+    const uint32_t gw = kBitsB ? n_tiles_all : 8u;
     ProfScope prof(c, LWE_K_ENCAPS_TC, st);
     // signed byte-plane sums of the N2 variant: |plane| <= 255 * 128 * rows <= 65280 * 65536, and twice that plus q
     // stays below 2^32
@@ -388,8 +366,7 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint3
     if (kBitsB && !make_map_plain_u8(c, &mapBits, d_Rbits, p.k / 8, (uint64_t)batch * p.m, 16, kTileK))
         return cudaErrorInvalidValue;
     kern<<<2 * pairs, kBitsB ? kThreadsBits : kThreads, smem_bytes, st>>>(
-        mapA, mapR, d_U, d_flags, d_E1, rows, p.n, p.k, ncols, c->mq, gw, (tune >> 4) & 3u, (tune >> 6) & 3u, pv_bias,
-        pv_e1bias, mapBits, row0, p.m);
+        mapA, mapR, d_U, d_flags, d_E1, rows, p.n, p.k, ncols, c->mq, gw, pv_bias, pv_e1bias, mapBits, row0, p.m);
     c->launches++;
     return cudaGetLastError();
 }
@@ -409,12 +386,7 @@ cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32
     }
     if (mode == kEpiAccum) return launch_pair<6, 128, kEpiAccum>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
     if (mode == kEpiCompare) return launch_pair<6, 128, kEpiCompare>(c, d_A, d_U, d_flags, nullptr, batch, row0, rows, st);
-    switch ((c->tune >> 8) & 3) {
-    case 1: return launch_pair<5, 128, kEpiStore>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
-    case 2: return launch_pair<4, 128, kEpiStore>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
-    case 3: return launch_pair<3, 256, kEpiStore>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
-    default: return launch_pair<6, 128, kEpiStore>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
-    }
+    return launch_pair<6, 128, kEpiStore>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
 }
 
 // N2: U = A^T R + E1 mod q with the int8 operand R already laid out in the context's operand buffer

@@ -148,19 +148,10 @@ static cudaError_t launch_gemv(Ctx *c, const uint16_t *d_A, const AesKey &key, c
     const uint32_t n = c->p.n, m = c->p.m;
     size_t smem = 2 * (size_t)n + kRedBytes + (kRegen ? kAesTableBytes : 0);
     auto kern = keygen_gemv_kernel<TPR, kRegen, UNR, NT>;
-    // attribute + occupancy are queried once per (instantiation, smem size): host calls, not per launch
-    static size_t cached_smem = 0;
-    static int cached_per_sm = 0;
-    if (cached_smem != smem) {
-        cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (err != cudaSuccess) return err;
-        int q = 0;
-        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&q, kern, NT, smem);
-        if (err != cudaSuccess) return err;
-        cached_per_sm = q < 1 ? 1 : q;
-        cached_smem = smem;
-    }
-    const int per_sm = cached_per_sm;
+    // shared-memory opt-in and occupancy: once per (context, instantiation, smem size) -- host calls, not per launch
+    int per_sm = 1;
+    cudaError_t perr = kernel_prepare(c, kern, smem, NT, &per_sm);
+    if (perr != cudaSuccess) return perr;
     constexpr int kTeams = NT / TPR;
     uint32_t grid = (uint32_t)(c->sm_count * per_sm);
     uint32_t need = (m + kTeams - 1) / kTeams;
@@ -175,30 +166,17 @@ cudaError_t launch_keygen_stored(Ctx *c, const uint16_t *d_A, const uint16_t *d_
                                  uint16_t *d_b, uint32_t batch, cudaStream_t st)
 {
     AesKey none = {};
-    int v = c->gemv_variant;
-    if (v == 0) v = (c->p.n >= 2048) ? 2 : 1;          // measured on B200: a warp per row, 8 x 16 B in flight per lane
-    switch (v) {
-    case 1: return launch_gemv<32, false, 4>(c, d_A, none, d_s, d_e, d_b, batch, st);
-    case 2: return launch_gemv<32, false, 8>(c, d_A, none, d_s, d_e, d_b, batch, st);
-    case 4: return launch_gemv<kGemvThreads, false, 2>(c, d_A, none, d_s, d_e, d_b, batch, st);
-    default: return launch_gemv<kGemvThreads, false, 4>(c, d_A, none, d_s, d_e, d_b, batch, st);
-    }
+    // measured on B200: a warp per row; 8 x 16 B in flight per lane once a row is at least 4 KB
+    if (c->p.n >= 2048) return launch_gemv<32, false, 8>(c, d_A, none, d_s, d_e, d_b, batch, st);
+    return launch_gemv<32, false, 4>(c, d_A, none, d_s, d_e, d_b, batch, st);
 }
 
 cudaError_t launch_keygen_regen(Ctx *c, const AesKey &key, const uint16_t *d_s, const uint16_t *d_e,
                                 uint16_t *d_b, uint32_t batch, cudaStream_t st)
 {
-    // one 64 KB AES table and one copy of s per CTA: large CTAs (4 row teams of 256, or 32 warp teams) keep
-    // 32 warps per SM behind a single table
-    switch (c->gemv_variant) {                           // measurement knob (LWE_OPT_GEMV_VARIANT), same result
-    case 1: return launch_gemv<256, true, 2, 1024>(c, nullptr, key, d_s, d_e, d_b, batch, st);
-    case 2: return launch_gemv<256, true, 1, 768>(c, nullptr, key, d_s, d_e, d_b, batch, st);
-    case 3: return launch_gemv<256, true, 1, 1024>(c, nullptr, key, d_s, d_e, d_b, batch, st);
-    case 4: return launch_gemv<32, true, 2, 1024>(c, nullptr, key, d_s, d_e, d_b, batch, st);
-    default: break;
-    }
-    // measured on B200 (C4, GB/s of A regenerated): 768 threads x 2 blocks in flight 698, 1024 x 2 663,
-    // 4 in flight spills at <= 85 registers and halves the rate
+    // one 64 KB AES table and one copy of s per CTA: large CTAs (3 row teams of 256, or 32 warp teams) keep
+    // 24-32 warps per SM behind a single table.  Measured on B200 (C4, GB/s of A regenerated): 768 threads x 2
+    // blocks in flight 698, 1024 x 2 663; 4 in flight spills at <= 85 registers and halves the rate
     if (c->p.n >= 4096) return launch_gemv<256, true, 2, 768>(c, nullptr, key, d_s, d_e, d_b, batch, st);
     return launch_gemv<32, true, 2, 1024>(c, nullptr, key, d_s, d_e, d_b, batch, st);
 }

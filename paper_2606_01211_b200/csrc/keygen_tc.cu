@@ -279,34 +279,23 @@ cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, c
     uint32_t rps = ((p.m + waves * (uint32_t)c->sm_count - 1) / (waves * (uint32_t)c->sm_count) + 7u) & ~7u;
     if (rps > kTileM) rps = kTileM;
     if (rps < 8) rps = 8;
-    if (((uint32_t)c->tune >> 14) & 1u) rps = kTileM;                    // LWE_OPT_TUNE bit 14: 128-row strips
     if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, p.m, rps)) return cudaErrorInvalidValue;
     if (!make_map_u8(c, &mapS, c->d_Sx, 2ull * p.n, N, N)) return cudaErrorInvalidValue;
-    // slabs per stage: as wide as leaves >= 3 stages in flight (LWE_OPT_TUNE bits 10-11 force 1 / 2 / 4)
+    // slabs per stage: as wide as leaves >= 3 stages in flight
     const uint32_t bytes_slab = kBytesA + N * kTileK;
-    uint32_t slabs = (3 * 4 * bytes_slab <= kSmemBudget) ? 4 : (3 * 2 * bytes_slab <= kSmemBudget) ? 2 : 1;
-    const uint32_t force = ((uint32_t)c->tune >> 10) & 3u;
-    if (force) slabs = force == 3 ? 4 : force;
-    if (kSmemBudget / (slabs * bytes_slab) < 2) slabs = 1;
+    const uint32_t slabs = (3 * 2 * bytes_slab <= kSmemBudget) ? 2 : 1;
     const uint32_t bytes_stage = slabs * bytes_slab;
     uint32_t stages = kSmemBudget / bytes_stage;
     if (stages > kMaxStages) stages = kMaxStages;
     const uint32_t smem = stages * bytes_stage + 1024 + 256;
     typedef void (*Kern)(const CUtensorMap, const CUtensorMap, const uint16_t *, uint16_t *, uint32_t, uint32_t, uint32_t,
                          uint32_t, uint32_t, ModQ, uint32_t);
-    static const Kern table[3][3] = {
-        {keygen_tc_kernel<2, 1>, keygen_tc_kernel<2, 2>, keygen_tc_kernel<2, 4>},
-        {keygen_tc_kernel<3, 1>, keygen_tc_kernel<3, 2>, keygen_tc_kernel<3, 4>},
-        {keygen_tc_kernel<4, 1>, keygen_tc_kernel<4, 2>, keygen_tc_kernel<4, 4>}};
-    const uint32_t si = slabs == 4 ? 2 : slabs - 1;
-    Kern kern = table[cpi - 2][si];
-    static int configured[3][3] = {};
-    if (!configured[cpi - 2][si]) {
-        cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                               (int)(kSmemBudget + 1024 + 256));
-        if (err != cudaSuccess) return err;
-        configured[cpi - 2][si] = 1;
-    }
+    static const Kern table[3][2] = {{keygen_tc_kernel<2, 1>, keygen_tc_kernel<2, 2>},
+                                     {keygen_tc_kernel<3, 1>, keygen_tc_kernel<3, 2>},
+                                     {keygen_tc_kernel<4, 1>, keygen_tc_kernel<4, 2>}};
+    Kern kern = table[cpi - 2][slabs - 1];
+    cudaError_t perr = kernel_prepare(c, kern, smem);
+    if (perr != cudaSuccess) return perr;
     const uint32_t strips = (p.m + rps - 1) / rps;
     const uint32_t grid = strips < (uint32_t)c->sm_count ? strips : (uint32_t)c->sm_count;
     ProfScope prof(c, LWE_K_KEYGEN_TC, st);

@@ -63,17 +63,30 @@ __host__ __device__ __forceinline__ uint32_t mod_u64(uint64_t x, const ModQ &mq)
 // ---------------------------------------------------------------------------------
 constexpr int kHostChunks = 8;        // lwe_kem_host splits a batch into at most this many chunks
 
+// Per-context (hence per-device) launch state of one __global__ function: whether the opt-in to more than 48 KB
+// of dynamic shared memory has been made ON THIS CONTEXT'S DEVICE (cudaFuncSetAttribute applies to the current
+// device only) and the last occupancy answer.  Nothing of this kind is process-wide: a process may hold contexts
+// on several GPUs.
+struct KernelCfg {
+    const void *fn;
+    int occ_threads;
+    size_t occ_smem;
+    int occ;                          // resident CTAs per SM for (occ_threads, occ_smem); 0 = not asked yet
+};
+constexpr int kMaxKernelCfg = 96;
+
 struct Ctx {
     lwe_params p;
     ModQ mq;
     int device;
     int sm_count;
+    int smem_optin;                   // cudaDevAttrMaxSharedMemoryPerBlockOptin of the device
+    KernelCfg kcfg[kMaxKernelCfg];
+    int n_kcfg;
     int last_cuda_error;
     uint64_t launches;
     int encaps_path;                  // LWE_OPT_ENCAPS_PATH
-    int gemv_variant;                 // LWE_OPT_GEMV_VARIANT
     int keygen_path;                  // LWE_OPT_KEYGEN_PATH
-    int tune;                         // LWE_OPT_TUNE: launch-shape experiments, no semantic effect
     int regen_path;                   // LWE_OPT_REGEN_PATH
     int r_operand;                    // LWE_OPT_R_OPERAND
 
@@ -139,6 +152,17 @@ struct ProfScope {
             return LWE_ERR_CUDA;                                  \
         }                                                         \
     } while (0)
+
+// Before a launch of `fn` with `smem` bytes of dynamic shared memory: on first use by this context raise the
+// function's dynamic shared-memory limit on the context's device to everything the device offers (a limit, not a
+// reservation: contexts of different shapes sharing the function never lower it for each other).  If `occ` is not
+// NULL it receives the resident CTAs per SM for (threads, smem), queried once per distinct pair (>= 1).
+cudaError_t kernel_prepare(Ctx *c, const void *fn, size_t smem, int threads = 0, int *occ = nullptr);
+template <class K>
+inline cudaError_t kernel_prepare(Ctx *c, K fn, size_t smem, int threads = 0, int *occ = nullptr)
+{
+    return kernel_prepare(c, reinterpret_cast<const void *>(fn), smem, threads, occ);
+}
 
 // host-side key expansion (FIPS-197 5.2) into the kernels' word convention
 void aes128_expand_key_host(const uint8_t key[16], AesKey *out);

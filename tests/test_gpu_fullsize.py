@@ -73,7 +73,9 @@ def test_c3_full_size_everything_against_the_oracle(H):
 
 
 def test_c4_bench_configuration_sampled_rows_and_invariants(H):
-    """C4 exactly as bench.py launches it: 32 instances per call against one stored A (keygen as
+    """C4 exactly as bench.py launches it, compared ELEMENT BY ELEMENT on 3 of the 32 instances (b and v in full, 48
+    sampled rows of U); the other 29 instances rest on the exact noise identity over all columns plus full key
+    recovery (an O(mk) check of the O(mnk) contraction).  32 instances per call against one stored A (keygen as
     the tensor-core skinny GEMM, encaps as the CTA-pair tcgen05 GEMM with N = 8192 columns)."""
     w = W.C4
     n, m, k, q, Bt = w.n, w.m, w.k, w.q, w.batch
@@ -152,3 +154,99 @@ def test_c5_stored_and_regenerated_sampled_rows_columns_and_key_recovery(H):
     # everything else: exact identity over all columns + every bit recovered
     assert noise_identity_holds(w, U, v, s, e, Rbits, mubits)
     assert np.array_equal(out, mubits)
+
+
+def test_c4_kem_host_eight_chunks_of_four_real_size_instances(H):
+    """lwe_kem_host in the shape bench.py's e2e leg times: C4, 32 instances in pinned HOST buffers, 8 chunks of 4
+    instances through the copy-in / compute / copy-out pipeline.  Inputs are numpy-seeded (not the method's draws);
+    b and v of every instance in full, 24 sampled rows of U on 4 instances (one per quarter of the chunks), the noise
+    identity and the recovered bits on all 32."""
+    import torch
+    w = W.C4
+    n, m, k, q, Bt = w.n, w.m, w.k, w.q, w.batch
+    rng = np.random.default_rng(88)
+    s = W.random_u16((Bt, n), q, 801)
+    e_signed = rng.integers(-4, 5, (Bt, m))
+    e = (e_signed % q).astype(np.uint16)
+    Rbits = W.random_bytes(Bt * m * k // 8, 802).reshape(Bt, -1)
+    mubits = W.random_bytes(Bt * k // 8, 803).reshape(Bt, -1)
+
+    def pinned(a):
+        return torch.from_numpy(a.view(np.int16) if a.dtype == np.uint16 else a).pin_memory()
+
+    h_s, h_e, h_R, h_mu = pinned(s), pinned(e), pinned(Rbits), pinned(mubits)
+    h_b = torch.zeros(Bt, m, dtype=torch.int16).pin_memory()
+    h_U = torch.zeros(Bt, n, k, dtype=torch.int16).pin_memory()
+    h_v = torch.zeros(Bt, k, dtype=torch.int16).pin_memory()
+    h_out = torch.zeros(Bt, k // 8, dtype=torch.uint8).pin_memory()
+    with H.make_ctx(w) as c:
+        dA = H.dev_empty_u16(m, n)
+        c.sample_uniform(dA, 0, m * n, w.seed, W.TAG_A)
+        c.kem_host(dA, 0, h_s, h_e, h_R, h_mu, h_b, h_U, h_v, h_out, Bt)
+    A = O.sample_uniform(0, m * n, w.seed, O.TAG_A, 0, q).reshape(m, n)
+    gb, gU, gv, gout = (h_b.numpy().view(np.uint16), h_U.numpy().view(np.uint16), h_v.numpy().view(np.uint16), h_out.numpy())
+    for t in range(Bt):
+        bo = O.keygen(A, s[t], e[t], q)
+        assert np.array_equal(gb[t], bo), ("b", t)
+        assert np.array_equal(gv[t], O.encaps_v(bo, Rbits[t], mubits[t], k, q)), ("v", t)
+        assert noise_identity_holds(w, gU[t], gv[t], s[t], e[t], Rbits[t], mubits[t]), t
+        assert np.array_equal(gout[t], mubits[t]), f"instance {t}: not every bit recovered"
+        if t in (1, 10, 21, 31):
+            rows = np.unique(np.concatenate([[0, 64, n - 1], rng.integers(0, n, 21)])).astype(np.uint32)
+            assert np.array_equal(gU[t][rows], O.encaps_rows(A, Rbits[t], rows, k, q)), ("U", t)
+
+
+def test_paper_variant_n4096_batch32_as_bench_times_it(H):
+    """N2 at the size bench.py's `paper_variant_n4096_B32` phase times (Table 1 row n = 4096, q = 12289, sigma = 1.7,
+    e2 in [-3, 3], eta = 3): every object drawn on the device from the seed as the phase does; t and v in full and
+    40 sampled rows of U element by element on 3 instances, the exact noise identity
+    v - U^T s - mu floor(q/2) = e^T R + e2 - s^T E1 (mod q) and every recovered bit on all 32."""
+    import torch
+    n, q, sigma, bound = W.PAPER_TABLE1[3]
+    k, Bt, seed = 256, 32, 6
+    s8 = dict(dtype=torch.int8, device="cuda")
+    from paper_2606_01211_b200 import binding as Bd
+    with Bd.Context(n, n, k, q, 3, Bt) as c:
+        dA = H.dev_empty_u16(n, n)
+        c.sample_uniform(dA, 0, n * n, seed, W.TAG_A)
+        s, e, t = H.dev_empty_u16(Bt, n), H.dev_empty_u16(Bt, n), H.dev_empty_u16(Bt, n)
+        R, E1, e2 = torch.empty(Bt, n, k, **s8), torch.empty(Bt, n, k, **s8), torch.empty(Bt, k, **s8)
+        mu, out = H.dev_empty_u8(Bt, k // 8), H.dev_empty_u8(Bt, k // 8)
+        U, v = H.dev_empty_u16(Bt, n, k), H.dev_empty_u16(Bt, k)
+        c.sample_cbd(s, 0, n, seed, W.TAG_S, 0, Bt)
+        c.sample_gauss_u16(e, 0, n, seed, W.TAG_E, 0, Bt, sigma)
+        c.sample_gauss_s8(R, 0, n * k, seed, W.TAG_RG, 0, Bt, sigma)
+        c.sample_gauss_s8(E1, 0, n * k, seed, W.TAG_E1, 0, Bt, sigma)
+        c.sample_cuniform_s8(e2, 0, k, seed, W.TAG_E2, 0, Bt, bound)
+        c.sample_bits(mu, 0, k, seed, W.TAG_MU, 0, Bt)
+        c.keygen(dA, 0, s, e, t, Bt)
+        c.encaps_pv(dA, t, R, E1, e2, mu, U, v, Bt)
+        c.decaps(U, v, s, out, Bt)
+        gA, gt, gU, gv, gout = H.host_u16(dA), H.host_u16(t), H.host_u16(U), H.host_u16(v), H.host_u8(out)
+    A = O.sample_uniform(0, n * n, seed, O.TAG_A, 0, q).reshape(n, n)
+    assert np.array_equal(gA, A)
+    rng = np.random.default_rng(4096)
+    centred = lambda x: np.where(x.astype(np.int64) > q // 2, x.astype(np.int64) - q, x.astype(np.int64))  # noqa: E731
+    for b in range(Bt):
+        so = O.sample_cbd(0, n, seed, O.TAG_S, b, q, 3)
+        eo = O.sample_gauss(0, n, seed, O.TAG_E, b, sigma, q)
+        Ro = O.sample_gauss(0, n * k, seed, O.TAG_RG, b, sigma).reshape(n, k)
+        E1o = O.sample_gauss(0, n * k, seed, O.TAG_E1, b, sigma).reshape(n, k)
+        e2o = O.sample_cuniform(0, k, seed, O.TAG_E2, b, bound)
+        muo = O.sample_bits(0, k, seed, O.TAG_MU, b)
+        mub = np.unpackbits(muo, bitorder="little")[:k].astype(np.int64)
+        # exact identity over all columns (python-size integers stay far below 2^63 here)
+        ss, ee = centred(so), centred(eo)
+        Us = (gU[b].astype(np.int64).T @ ss)
+        lhs = (gv[b].astype(np.int64) - Us - mub * (q // 2)) % q
+        rhs = (ee @ Ro.astype(np.int64) + e2o.astype(np.int64) - ss @ E1o.astype(np.int64)) % q
+        assert np.array_equal(lhs, rhs), b
+        assert np.array_equal(gout[b], muo), f"instance {b}: not every bit recovered"
+        if b in (0, 17, Bt - 1):
+            to = O.keygen(A, so, eo, q)
+            assert np.array_equal(gt[b], to), b
+            rows = np.unique(np.concatenate([[0, 63, 64, n - 1], rng.integers(0, n, 36)]))
+            # rows of U = A^T R + E1: the oracle on the sampled columns of A (an n x |rows| matrix)
+            Uo, vo = O.encaps_pv(np.ascontiguousarray(A[:, rows]), to, Ro, E1o[rows], e2o, muo, q)
+            assert np.array_equal(gU[b][rows], Uo), b
+            assert np.array_equal(gv[b], vo), b

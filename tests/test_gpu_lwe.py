@@ -188,6 +188,26 @@ def test_encaps_extreme_accumulators(H, path):
         assert np.all(v == (m * (q - 1) + q // 2) % q)
 
 
+@pytest.mark.parametrize("path", **ENCAPS_PATHS)
+def test_encaps_more_than_65536_rows_worst_case(H, path):
+    """m = 131072 > 65536: the contraction runs in passes of 65536 rows whose residues are added mod q; with
+    A = q-1 and R = all ones every 32-bit partial sum (byte planes, recombined value, the column sums of v) sits at
+    its bound in both passes.  A wrap anywhere changes the result."""
+    for q in (65536, 65521):
+        m, n, k = 131072, 64, 256
+        A = np.full((m, n), q - 1, np.uint16)
+        b = np.full((2, m), q - 1, np.uint16)
+        Rbits = np.full((2, m * k // 8), 0xFF, np.uint8)
+        Rbits[1, : (m // 2) * k // 8 : 2] = 0x55           # second instance: a mixed pattern in the first pass
+        mubits = np.full((2, k // 8), 0xFF, np.uint8)
+        U, v = run_encaps(H, path, m, n, k, q, 2, A, b, Rbits, mubits)
+        assert np.all(U[0] == (m * (q - 1)) % q)
+        assert np.all(v[0] == (m * (q - 1) + q // 2) % q)
+        ones = np.unpackbits(Rbits[1], bitorder="little").reshape(m, k).sum(axis=0).astype(np.int64)
+        assert np.array_equal(U[1], np.broadcast_to((ones * (q - 1)) % q, (n, k)))
+        assert np.array_equal(v[1], (ones * (q - 1) + q // 2) % q)
+
+
 @pytest.mark.parametrize("path", [3, 2], ids=["tcgen05_pair", "tcgen05"])
 def test_encaps_one_hot_R_picks_a_row_of_A(H, path):
     m, n, k, q = 256, 128, 256, 65521
@@ -238,16 +258,15 @@ def test_encaps_regenerated_A_equals_stored_and_oracle(H, path, m, n, k, q, batc
         assert np.array_equal(Ug[t], Uo), ("U", t)
 
 
-@pytest.mark.parametrize("m,n,k,q,seed,tune", [
-    (512, 256, 256, 65536, 1, 0),           # C1: 4 tiles, one K range each
-    (2048, 1024, 256, 65536, 2, 0),         # C2: 16 tiles x several K ranges combined under the tile locks
-    (1160, 456, 256, 65521, 3, 0),          # prime q (rejection inside the generator), n % 64 != 0, ragged K tail
-    (1160, 456, 256, 65521, 3, 1 << 12),    # 16 generator warps, K block 128, 3-stage ring
-    (200, 72, 128, 40000, 9, 2 << 12),      # k < 256 (second R box out of range), 2-stage ring
-    (4104, 8, 16, 12289, 5, 0),             # one tile, mostly empty; many K ranges
-    (12288, 9472, 256, 65536, 4, 0),        # 148 tiles = exactly one wave of CTAs; two K ranges per tile
+@pytest.mark.parametrize("m,n,k,q,seed", [
+    (512, 256, 256, 65536, 1),           # C1: 4 tiles, one K range each
+    (2048, 1024, 256, 65536, 2),         # C2: 16 tiles x several K ranges combined under the tile locks
+    (1160, 456, 256, 65521, 3),          # prime q (rejection inside the generator), n % 64 != 0, ragged K tail
+    (200, 72, 128, 40000, 9),            # k < 256 (second R box out of range)
+    (4104, 8, 16, 12289, 5),             # one tile, mostly empty; many K ranges
+    (12288, 9472, 256, 65536, 4),        # 148 tiles = exactly one wave of CTAs; two K ranges per tile
 ])
-def test_encaps_fused_regenerated_A_matches_oracle(H, m, n, k, q, seed, tune):
+def test_encaps_fused_regenerated_A_matches_oracle(H, m, n, k, q, seed):
     """S8(f) N4: lwe_encaps(d_A = NULL) for one instance generates the A tiles inside the GEMM's producer (A never in
     HBM).  Equals the oracle, whose A is its own draw from the same seed, bit for bit; run twice on one context (the
     per-tile locks and counters reset themselves) and against the row-panel path."""
@@ -256,7 +275,6 @@ def test_encaps_fused_regenerated_A_matches_oracle(H, m, n, k, q, seed, tune):
     mubits = W.random_bytes(k // 8, 24).reshape(1, -1)
     with B().Context(n, m, k, q, 4, 1) as c:
         c.set_option(B().OPT_REGEN_PATH, 2)
-        c.set_option(B().OPT_TUNE, tune)
         U, v = H.dev_empty_u16(1, n, k), H.dev_empty_u16(1, k)
         got = []
         for _ in range(2):
@@ -321,6 +339,45 @@ def test_decaps_rounding_boundaries(H):
             got = H.unpack_bits(H.host_u8(out)[0], k)
         want = np.array([1 if (4 * int(d) >= q and 4 * int(d) < 3 * q) else 0 for d in v[0]])
         assert np.array_equal(got, want)
+
+
+@pytest.mark.parametrize("q", [65521, 40000, 12289, 3329])
+def test_decaps_u64_sum_reduction_at_its_edges(H, q):
+    """The 64-bit column sum sum_j U[j][c] s[j] is reduced mod q without a 64-bit remainder ((hi mod q)(2^32 mod q) +
+    lo, Barrett steps).  Columns are built so that the exact sum S = hi 2^32 + lo hits the edges of every
+    step (hi, lo in {0, 1, q-1, q, q+1, 2q-1, ..., 2^32-1}); each S is used by TWO columns whose v puts d exactly on
+    the two sides of the decision boundary q/4, so an error of even 1 in S mod q flips one of the two bits."""
+    k, nmax = 256, 200000
+    top = (q - 1) * (q - 1)
+    his = [h for h in (0, 1, 2, q - 2, q - 1, q, q + 1, 2 * q - 1, 2 * q, 3 * q - 1, 3 * q + 1)
+           if (h + 1) << 32 <= (nmax - 8) * top]
+    los = [0, 1, q - 1, q, q + 1, (1 << 32) - 1, (1 << 32) - q, (1 << 32) - q - 1, 1 << 31, 123456789]
+    sums = [(h << 32) + lo for h in his for lo in los][: k // 2]
+    n_top = max(S // top for S in sums)
+    n = ((n_top + 2 + 7) // 8) * 8                         # rows [0, n_top): s = q-1; row n_top: s = q-1; row n_top+1: s = 1
+    s = np.zeros((1, n), np.uint16)
+    s[0, : n_top + 1] = q - 1
+    s[0, n_top + 1] = 1
+    U = np.zeros((1, n, k), np.uint16)
+    v = np.zeros((1, k), np.uint16)
+    lo_edge = -(-q // 4)                                   # smallest d with 4d >= q
+    want = np.zeros(k, np.uint8)
+    for x, S in enumerate(sums):
+        a, rem = divmod(S, top)
+        b_, rem2 = divmod(rem, q - 1)
+        for c, d in ((2 * x, lo_edge), (2 * x + 1, lo_edge - 1)):
+            U[0, :a, c] = q - 1
+            U[0, n_top, c] = b_
+            U[0, n_top + 1, c] = rem2
+            v[0, c] = (S + d) % q                          # d = v - S mod q
+            want[c] = 1 if 4 * d >= q and 4 * d < 3 * q else 0
+        assert a * top + b_ * (q - 1) + rem2 == S and b_ < q and rem2 < q
+    with B().Context(n, 8, k, q, 4, 1) as c:
+        out = H.dev_empty_u8(1, k // 8)
+        c.decaps(H.dev(U), H.dev(v), H.dev(s), out, 1)
+        got = H.unpack_bits(H.host_u8(out)[0], k)
+    assert np.array_equal(got[: 2 * len(sums)], want[: 2 * len(sums)])
+    assert np.array_equal(got, H.unpack_bits(O.decaps(U[0], v[0], s[0], q), k))
 
 
 # ---------------------------------------------------------------- whole path from seeds
@@ -414,6 +471,51 @@ def test_two_contexts_of_different_shape_interleaved_on_two_streams(H):
             c.close()
 
 
+def test_contexts_on_two_devices_in_one_process(H):
+    """Launch state (shared-memory opt-ins, occupancy) is per context, i.e. per device: after a full pass on device
+    0 the same calls on a context of device 1 must work and agree with the oracle.  Needs two GPUs."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one GPU")
+    w, n, m, batch = W.C3, 512, 1024, 2
+    res = []
+    for device in (0, 1, 0):
+        with torch.cuda.device(device):
+            c = B().Context(n, m, w.k, w.q, w.eta, batch, device)
+            dA = torch.empty(m, n, dtype=torch.int16, device=f"cuda:{device}")
+            c.sample_uniform(dA, 0, m * n, w.seed, W.TAG_A)
+            dev_tensors = {}
+            k = w.k
+            mk = lambda *shape, dt=torch.int16: torch.empty(*shape, dtype=dt, device=f"cuda:{device}")  # noqa: E731
+            s, e, b, b2 = mk(batch, n), mk(batch, m), mk(batch, m), mk(1, m)
+            Rb, mu, o = mk(batch, m * k // 8, dt=torch.uint8), mk(batch, k // 8, dt=torch.uint8), mk(batch, k // 8, dt=torch.uint8)
+            U, v, U2, v2 = mk(batch, n, k), mk(batch, k), mk(1, n, k), mk(1, k)
+            c.sample_kem(s, e, Rb, mu, w.seed, 0, batch)
+            c.keygen(dA, 0, s, e, b, batch)                       # tensor-core skinny GEMM
+            c.keygen(None, w.seed, s[:1], e[:1], b2, 1)           # AES inside the GEMV (64 KB table: needs the opt-in)
+            c.encaps(dA, 0, b, Rb, mu, U, v, batch)
+            c.encaps(None, w.seed, b[:1], Rb[:1], mu[:1], U2, v2, 1)   # fused regenerated-A GEMM
+            c.decaps(U, v, s, o, batch)
+            torch.cuda.synchronize(device)
+            res.append(dict(A=dA.cpu().numpy().view(np.uint16), b=b.cpu().numpy().view(np.uint16),
+                            b2=b2.cpu().numpy().view(np.uint16), U=U.cpu().numpy().view(np.uint16),
+                            U2=U2.cpu().numpy().view(np.uint16), v=v.cpu().numpy().view(np.uint16), o=o.cpu().numpy(),
+                            mu=mu.cpu().numpy()))
+            c.close()
+            del dev_tensors
+    oA = O.sample_uniform(0, m * n, w.seed, O.TAG_A, 0, w.q).reshape(m, n)
+    for r in res:
+        assert np.array_equal(r["A"], oA)
+        for t in range(batch):
+            oi = H.OracleInstance(w, t, n, m, with_A=False)
+            ob = O.keygen(oA, oi.s, oi.e, w.q)
+            oU, ov = O.encaps(oA, ob, oi.Rbits, oi.mubits, w.k, w.q)
+            assert np.array_equal(r["b"][t], ob) and np.array_equal(r["U"][t], oU) and np.array_equal(r["v"][t], ov)
+            assert np.array_equal(r["o"][t], oi.mubits)
+            if t == 0:
+                assert np.array_equal(r["b2"][0], ob) and np.array_equal(r["U2"][0], oU)
+
+
 # ---------------------------------------------------------------- end to end with host buffers
 
 @pytest.mark.parametrize("n,m,k,q,batch,regen", [
@@ -454,6 +556,27 @@ def test_kem_host_pipeline_matches_oracle(H, n, m, k, q, batch, regen):
         assert np.array_equal(gb[t], b), ("b", t)
         assert np.array_equal(gU[t], U) and np.array_equal(gv[t], v), ("U/v", t)
         assert np.array_equal(gout[t], O.decaps(U, v, s[t], q)), ("mu'", t)
+
+
+def test_kem_host_rejects_misaligned_host_pointers(H):
+    """include/lwe.h: every h_* pointer must be 16-byte aligned -> LWE_ERR_ALIGN before anything is enqueued"""
+    import torch
+    n, m, k, q = 64, 128, 256, 65536
+    with B().Context(n, m, k, q, 4, 1) as c:
+        dA = H.dev_empty_u16(m, n)
+        c.sample_uniform(dA, 0, m * n, 1, W.TAG_A)
+        pin = lambda *shape, dt=torch.int16: torch.zeros(*shape, dtype=dt).pin_memory()  # noqa: E731
+        good = dict(h_s=pin(1, n), h_e=pin(1, m), h_R=pin(1, m * k // 8, dt=torch.uint8), h_mu=pin(1, k // 8, dt=torch.uint8),
+                    h_b=pin(1, m), h_U=pin(1, n, k), h_v=pin(1, k), h_out=pin(1, k // 8, dt=torch.uint8))
+        order = ["h_s", "h_e", "h_R", "h_mu", "h_b", "h_U", "h_v", "h_out"]
+        c.kem_host(dA, 0, *[good[x] for x in order], 1)
+        before = good["h_b"].clone()
+        for bad in order:
+            args = [good[x].data_ptr() + (2 if x == bad else 0) for x in order]
+            with pytest.raises(B().LweError) as ei:
+                c.kem_host(dA, 0, *args, 1)
+            assert ei.value.code == -2, bad
+        assert torch.equal(good["h_b"], before)
 
 
 # ---------------------------------------------------------------- N3: decaps with the FO re-encryption check

@@ -27,6 +27,17 @@ def test_o12_table_is_the_rounded_gaussian_cdf(sigma):
 
 
 @pytest.mark.parametrize("sigma", SIGMAS)
+def test_o12_integer_table_equals_the_60_digit_golden(sigma):
+    """The INTEGER table itself, entry by entry, against tests/golden/gauss_cdt_table1.txt (written by
+    make_gauss_cdt_golden.py with python `decimal` at 60 digits from a series for Phi: no libm, no oracle, no CUDA).
+    The oracle and the CUDA host code both use libm's erfc in double; this pin fixes what they must produce."""
+    from conftest import read_golden
+    gold = [int(x) for x in read_golden("gauss_cdt_table1.txt")[f"sigma_{sigma}"].split()]
+    assert len(gold) == 2 * O.GAUSS_TAU
+    assert O.gauss_cdt(sigma).tolist() == gold
+
+
+@pytest.mark.parametrize("sigma", SIGMAS)
 def test_o12_exhaustive_histogram_symmetry_and_moments(sigma):
     """all 65536 words: the histogram IS the table's differences; it is the rounded-Gaussian pmf to 2^-16 per
     value, symmetric to one count, with mean 0 and variance sigma^2 + 1/12 (Sheppard) to 1e-3."""
