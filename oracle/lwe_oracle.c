@@ -536,6 +536,152 @@ void orc_encaps_pv(const uint16_t *A, const uint16_t *t, const int8_t *R, const 
     }
 }
 
+/* ================================================================== N2 with q > 65536 (Table 1 rows n >= 8192,
+ * P:L98-102): uint32 residues.  Readings S23-S25 of DESIGN.md section 3. */
+
+/* 32-bit little-endian word t of the stream of (seed, tag, attempt, inst): bytes [4t, 4t+3]. */
+static uint32_t stream_word32(const uint8_t rk[176], uint32_t tag, uint32_t attempt, uint32_t inst, uint64_t t)
+{
+    uint8_t iv[16], ks[16];
+    orc_object_iv(tag, attempt, inst, iv);
+    ctr_block(rk, iv, (4 * t) / 16, ks);
+    unsigned off = (unsigned)((4 * t) % 16);
+    return (uint32_t)ks[off] | ((uint32_t)ks[off + 1] << 8) | ((uint32_t)ks[off + 2] << 16) | ((uint32_t)ks[off + 3] << 24);
+}
+
+/* O4w, element by element, straight from the definition. */
+void orc_sample_uniform32_strided(uint32_t *out, uint64_t first, uint64_t stride, uint64_t count,
+                                  uint64_t seed, uint32_t tag, uint32_t inst, uint32_t q)
+{
+    uint8_t key[16], rk[176];
+    sbox_init();
+    orc_seed_key(seed, key);
+    aes128_expand_key(key, rk);
+    const uint64_t T = (uint64_t)q * ((1ull << 32) / q);        /* q * floor(2^32 / q) <= 2^32 */
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (uint64_t r = 0; r < count; r++) {
+        const uint64_t t = first + r * stride;
+        uint64_t c = stream_word32(rk, tag, 0, inst, t);
+        for (uint32_t attempt = 1; c >= T; attempt++)
+            c = stream_word32(rk, tag, attempt, inst, t);
+        out[r] = (uint32_t)(c % q);
+    }
+}
+
+/* O4w on a contiguous range: the same values, walking the stream one 16-byte block (4 words) at a time so that the
+ * attempt-0 block is encrypted once, not once per word (as orc_sample_uniform does; cross-checked against the
+ * element-wise function above in tests/test_oracle_wide.py). */
+void orc_sample_uniform32(uint32_t *out, uint64_t first, uint64_t count,
+                          uint64_t seed, uint32_t tag, uint32_t inst, uint32_t q)
+{
+    uint8_t key[16], rk[176];
+    sbox_init();
+    orc_seed_key(seed, key);
+    aes128_expand_key(key, rk);
+    const uint64_t T = (uint64_t)q * ((1ull << 32) / q);
+    if (count == 0) return;
+    const uint64_t blk_lo = first / 4, blk_hi = (first + count - 1) / 4;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (uint64_t blk = blk_lo; blk <= blk_hi; blk++) {
+        uint8_t iv[16], ks[16];
+        orc_object_iv(tag, 0, inst, iv);
+        ctr_block(rk, iv, blk, ks);
+        for (unsigned w = 0; w < 4; w++) {
+            uint64_t t = 4 * blk + w;
+            if (t < first || t >= first + count) continue;
+            uint64_t c = (uint64_t)ks[4 * w] | ((uint64_t)ks[4 * w + 1] << 8) | ((uint64_t)ks[4 * w + 2] << 16) |
+                         ((uint64_t)ks[4 * w + 3] << 24);
+            for (uint32_t attempt = 1; c >= T; attempt++)
+                c = stream_word32(rk, tag, attempt, inst, t);
+            out[t - first] = (uint32_t)(c % q);
+        }
+    }
+}
+
+/* O5s. */
+void orc_sample_cbd_s8(int8_t *out, uint64_t first, uint64_t count,
+                       uint64_t seed, uint32_t tag, uint32_t inst, uint32_t eta)
+{
+    uint8_t key[16], rk[176];
+    sbox_init();
+    orc_seed_key(seed, key);
+    aes128_expand_key(key, rk);
+    const unsigned M = (1u << eta) - 1u;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (uint64_t x = 0; x < count; x++) {
+        unsigned w = stream_word16(rk, tag, 0, inst, first + x);
+        out[x] = (int8_t)(popcount16(w & M) - popcount16((w >> 8) & M));
+    }
+}
+
+/* O7w. */
+void orc_keygen_w(const uint32_t *A, const int8_t *s, const int8_t *e, uint32_t *t,
+                  uint32_t m, uint32_t n, uint32_t q)
+{
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (uint32_t i = 0; i < m; i++) {
+        uint64_t acc = 0;
+        for (uint32_t j = 0; j < n; j++)
+            acc = (acc + (uint64_t)A[(size_t)i * n + j] * mod_signed(s[j], q)) % q;
+        t[i] = (uint32_t)((acc + mod_signed(e[i], q)) % q);
+    }
+}
+
+/* O14w. */
+void orc_encaps_pv_w(const uint32_t *A, const uint32_t *t, const int8_t *R, const int8_t *E1, const int8_t *e2,
+                     const uint8_t *mubits, uint32_t *U, uint32_t *v,
+                     uint32_t m, uint32_t n, uint32_t k, uint32_t q)
+{
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (uint32_t j = 0; j < n; j++)
+        for (uint32_t c = 0; c < k; c++) {
+            uint64_t acc = 0;
+            for (uint32_t i = 0; i < m; i++)
+                acc = (acc + (uint64_t)A[(size_t)i * n + j] * mod_signed(R[(size_t)i * k + c], q)) % q;
+            U[(size_t)j * k + c] = (uint32_t)((acc + mod_signed(E1[(size_t)j * k + c], q)) % q);
+        }
+    for (uint32_t c = 0; c < k; c++) {
+        uint64_t acc = 0;
+        for (uint32_t i = 0; i < m; i++)
+            acc = (acc + (uint64_t)t[i] * mod_signed(R[(size_t)i * k + c], q)) % q;
+        acc = (acc + mod_signed(e2[c], q)) % q;
+        acc = (acc + (uint64_t)get_bit(mubits, c) * (q / 2)) % q;
+        v[c] = (uint32_t)acc;
+    }
+}
+
+/* O9w. */
+void orc_decaps_w(const uint32_t *U, const uint32_t *v, const int8_t *s,
+                  uint8_t *mubits_out, uint32_t *d_out, uint32_t n, uint32_t k, uint32_t q)
+{
+    uint8_t *bit = (uint8_t *)malloc(k ? k : 1);
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (uint32_t c = 0; c < k; c++) {
+        uint64_t acc = 0;
+        for (uint32_t j = 0; j < n; j++)
+            acc = (acc + (uint64_t)U[(size_t)j * k + c] * mod_signed(s[j], q)) % q;
+        uint64_t d = ((uint64_t)v[c] + (uint64_t)q - acc) % q;       /* in [0,q) */
+        if (d_out) d_out[c] = (uint32_t)d;
+        bit[c] = (uint8_t)orc_round_bit((uint32_t)d, q);
+    }
+    memset(mubits_out, 0, (k + 7) / 8);
+    for (uint32_t c = 0; c < k; c++)
+        mubits_out[c / 8] = (uint8_t)(mubits_out[c / 8] | (bit[c] << (c % 8)));
+    free(bit);
+}
+
 int orc_num_threads(void)
 {
 #ifdef _OPENMP

@@ -22,8 +22,9 @@
  * conventions O3-O6 (seed->key, tags, bit order) are fixed by SURVEY 8(c) /
  * DESIGN.md and implemented twice, independently, here and in CUDA.
  *
- * All vectors hold canonical representatives in [0, q) as uint16_t (S13).
- * q in (1, 65536].  Everything is integer arithmetic.
+ * All vectors hold canonical representatives in [0, q) as uint16_t (S13), q in (1, 65536]
+ * (uint32_t and q < 2^31 in the *_w / *32 functions of the q = 65537 parameter sets, S23).
+ * Everything is integer arithmetic.
  */
 #ifndef LWE_ORACLE_H
 #define LWE_ORACLE_H
@@ -161,6 +162,51 @@ void orc_sample_cuniform(int8_t *out, uint64_t first, uint64_t count,
 void orc_encaps_pv(const uint16_t *A, const uint16_t *t, const int8_t *R, const int8_t *E1, const int8_t *e2,
                    const uint8_t *mubits, uint16_t *U, uint16_t *v,
                    uint32_t m, uint32_t n, uint32_t k, uint32_t q);
+
+/* ---- N2 on the q = 65537 rows of Table 1 (n = 8192 ... 131072): residues need 17 bits.
+ * Readings S23-S25 of DESIGN.md section 3 (the paper says only "32-bit integers", and gives no sampler):
+ *   S23  residues of a modulus q > 65536 are stored as uint32_t in [0, q);
+ *   S24  uniform mod q on 32-bit stream words: O4 with the word size of the storage type (O4w below);
+ *   S25  the small objects cross the boundary as signed int8: s ~ CBD(eta) in [-eta, eta] (O5s), e, R, E1 ~ D_sigma
+ *        in [-12, 12] (O12), e2 in [-kappa, kappa] (O13).
+ * The functions below take any 2 <= q < 2^31, so that for q <= 65536 they can be pinned against the uint16 ones.
+ *
+ * O4w. Uniform mod q by rejection on 32-bit words, element t: for attempt a = 0,1,..:
+ *   c = LE32(bytes [4t, 4t+3] of KS(key(seed), iv(tag, a, inst))); T = q*floor(2^32/q); accept iff c < T; value c mod q.
+ * Pins: the stream re-derived through OpenSSL with an independent walk over the attempt streams (a modulus with
+ * 25 % rejection included); sub-range == slice; strided == gathered; chi-square uniformity at q = 65537. */
+void orc_sample_uniform32(uint32_t *out, uint64_t first, uint64_t count,
+                          uint64_t seed, uint32_t tag, uint32_t inst, uint32_t q);
+void orc_sample_uniform32_strided(uint32_t *out, uint64_t first, uint64_t stride, uint64_t count,
+                                  uint64_t seed, uint32_t tag, uint32_t inst, uint32_t q);
+
+/* O5s. Centred binomial eta as a SIGNED value: x = popcount(w & M) - popcount((w >> 8) & M) of the element's 16-bit
+ * stream word w exactly as O5, stored as int8 (no modulus involved).  Pin: x mod q == O5's residue, range, sign. */
+void orc_sample_cbd_s8(int8_t *out, uint64_t first, uint64_t count,
+                       uint64_t seed, uint32_t tag, uint32_t inst, uint32_t eta);
+
+/* O7w. KeyGen of the paper's PKE with small signed secret and noise (eq.(1)):
+ * t_i = (sum_{j<n} A[i*n+j]*s[j] + e[i]) mod q in [0, q), A uint32 residues, s, e int8.
+ * Pins: python big-integer brute force (q = 65537, 65539, 100003); equals O7 for q <= 65536; A = 65536 everywhere
+ * with q = 65537 gives t_i = e_i - sum_j s_j (2^16 = -1); linearity. */
+void orc_keygen_w(const uint32_t *A, const int8_t *s, const int8_t *e, uint32_t *t,
+                  uint32_t m, uint32_t n, uint32_t q);
+
+/* O14w. Encrypt of the paper's PKE (O14) on uint32 residues:
+ * U[j*k+c] = (sum_{i<m} A[i*n+j]*R[i*k+c] + E1[j*k+c]) mod q ;
+ * v[c]     = (sum_{i<m} t[i]*R[i*k+c] + e2[c] + mu_c*floor(q/2)) mod q.
+ * Pins: big-integer brute force; equals O14 for q <= 65536; the 2^16 = -1 special case; the noise identity
+ * v - U^T s - mu floor(q/2) = e^T R + e2 - s^T E1 (mod q); every bit recovered on Table 1's n = 8192 row. */
+void orc_encaps_pv_w(const uint32_t *A, const uint32_t *t, const int8_t *R, const int8_t *E1, const int8_t *e2,
+                     const uint8_t *mubits, uint32_t *U, uint32_t *v,
+                     uint32_t m, uint32_t n, uint32_t k, uint32_t q);
+
+/* O9w. Decrypt on uint32 residues with the small signed secret:
+ * d_c = (v[c] - sum_{j<n} U[j*k+c]*s[j]) mod q in [0, q); bit_c = floor((4 d_c + q) / (2q)) mod 2 (S12).
+ * If d_out != NULL it receives d_c.  Pins: big-integer brute force; equals O9 for q <= 65536; exhaustive rounding
+ * over all d for q = 65537. */
+void orc_decaps_w(const uint32_t *U, const uint32_t *v, const int8_t *s,
+                  uint8_t *mubits_out, uint32_t *d_out, uint32_t n, uint32_t k, uint32_t q);
 
 /* Number of OpenMP threads the loops above will use (1 if built without OpenMP). */
 int orc_num_threads(void);

@@ -22,6 +22,7 @@ __all__ = [
     "keygen", "encaps", "encaps_rows", "encaps_v", "decaps", "decaps_fo", "num_threads",
     "gauss_cdt", "gauss_from_word", "sample_gauss", "sample_cuniform", "encaps_pv",
     "cbd_from_word", "round_bit",
+    "sample_uniform32", "sample_uniform32_strided", "sample_cbd_s8", "keygen_w", "encaps_pv_w", "decaps_w",
 ]
 
 _lib = None
@@ -67,6 +68,15 @@ def _L():
         for f in ("orc_aes128_encrypt_block", "orc_ctr_bytes", "orc_seed_key", "orc_object_iv",
                   "orc_sample_uniform", "orc_sample_uniform_strided", "orc_sample_cbd", "orc_sample_bits", "orc_keygen",
                   "orc_encaps", "orc_encaps_rows", "orc_encaps_v", "orc_decaps"):
+            getattr(lib, f).restype = None
+        lib.orc_sample_uniform32.argtypes = [u32p, u64, u64, u64, u32, u32, u32]
+        lib.orc_sample_uniform32_strided.argtypes = [u32p, u64, u64, u64, u64, u32, u32, u32]
+        lib.orc_sample_cbd_s8.argtypes = [s8p, u64, u64, u64, u32, u32, u32]
+        lib.orc_keygen_w.argtypes = [u32p, s8p, s8p, u32p, u32, u32, u32]
+        lib.orc_encaps_pv_w.argtypes = [u32p, u32p, s8p, s8p, s8p, u8p, u32p, u32p, u32, u32, u32, u32]
+        lib.orc_decaps_w.argtypes = [u32p, u32p, s8p, u8p, u32p, u32, u32, u32]
+        for f in ("orc_sample_uniform32", "orc_sample_uniform32_strided", "orc_sample_cbd_s8", "orc_keygen_w",
+                  "orc_encaps_pv_w", "orc_decaps_w"):
             getattr(lib, f).restype = None
         _lib = lib
     return _lib
@@ -241,6 +251,68 @@ def encaps_pv(A, t, R, E1, e2, mubits, q: int):
     _L().orc_encaps_pv(_p(A, C.c_uint16), _p(t, C.c_uint16), _p(R, C.c_int8), _p(E1, C.c_int8), _p(e2, C.c_int8),
                        _p(mubits, C.c_uint8), _p(U, C.c_uint16), _p(v, C.c_uint16), m, n, k, q)
     return U, v
+
+
+# ---- q > 65536 (Table 1 rows n >= 8192): uint32 residues, int8 small objects (readings S23-S25)
+
+def _u32(x):
+    return np.ascontiguousarray(x, dtype=np.uint32)
+
+
+def _s8(x):
+    return np.ascontiguousarray(x, dtype=np.int8)
+
+
+def sample_uniform32(first: int, count: int, seed: int, tag: int, inst: int, q: int) -> np.ndarray:
+    out = np.zeros(count, np.uint32)
+    _L().orc_sample_uniform32(_p(out, C.c_uint32), first, count, seed, tag, inst, q)
+    return out
+
+
+def sample_uniform32_strided(first: int, stride: int, count: int, seed: int, tag: int, inst: int, q: int) -> np.ndarray:
+    out = np.zeros(count, np.uint32)
+    _L().orc_sample_uniform32_strided(_p(out, C.c_uint32), first, stride, count, seed, tag, inst, q)
+    return out
+
+
+def sample_cbd_s8(first: int, count: int, seed: int, tag: int, inst: int, eta: int) -> np.ndarray:
+    out = np.zeros(count, np.int8)
+    _L().orc_sample_cbd_s8(_p(out, C.c_int8), first, count, seed, tag, inst, eta)
+    return out
+
+
+def keygen_w(A, s, e, q: int) -> np.ndarray:
+    """O7w: t = A s + e mod q; A uint32 [m][n], s int8 [n], e int8 [m]"""
+    A, s, e = _u32(A), _s8(s), _s8(e)
+    m, n = A.shape
+    assert s.shape == (n,) and e.shape == (m,)
+    t = np.zeros(m, np.uint32)
+    _L().orc_keygen_w(_p(A, C.c_uint32), _p(s, C.c_int8), _p(e, C.c_int8), _p(t, C.c_uint32), m, n, q)
+    return t
+
+
+def encaps_pv_w(A, t, R, E1, e2, mubits, q: int):
+    """O14w: (U, v) uint32; A uint32 [m][n], t uint32 [m], R [m][k], E1 [n][k], e2 [k] int8"""
+    A, t = _u32(A), _u32(t)
+    m, n = A.shape
+    R, E1, e2 = _s8(R), _s8(E1), _s8(e2)
+    k = e2.shape[0]
+    assert R.shape == (m, k) and E1.shape == (n, k) and t.shape == (m,)
+    mubits = _u8(mubits, k // 8)
+    U, v = np.zeros((n, k), np.uint32), np.zeros(k, np.uint32)
+    _L().orc_encaps_pv_w(_p(A, C.c_uint32), _p(t, C.c_uint32), _p(R, C.c_int8), _p(E1, C.c_int8), _p(e2, C.c_int8),
+                         _p(mubits, C.c_uint8), _p(U, C.c_uint32), _p(v, C.c_uint32), m, n, k, q)
+    return U, v
+
+
+def decaps_w(U, v, s, q: int, return_d: bool = False):
+    U, v, s = _u32(U), _u32(v), _s8(s)
+    n, k = U.shape
+    assert v.shape == (k,) and s.shape == (n,)
+    out = np.zeros(k // 8, np.uint8)
+    d = np.zeros(k, np.uint32)
+    _L().orc_decaps_w(_p(U, C.c_uint32), _p(v, C.c_uint32), _p(s, C.c_int8), _p(out, C.c_uint8), _p(d, C.c_uint32), n, k, q)
+    return (out, d) if return_d else out
 
 
 def cbd_from_word(w: int, q: int, eta: int) -> int:
