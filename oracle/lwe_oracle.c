@@ -690,3 +690,14 @@ int orc_num_threads(void)
     return 1;
 #endif
 }
+
+int orc_set_num_threads(int threads)
+{
+    int prev = orc_num_threads();
+#ifdef _OPENMP
+    if (threads >= 1) omp_set_num_threads(threads);
+#else
+    (void)threads;
+#endif
+    return prev;
+}

@@ -208,8 +208,11 @@ void orc_encaps_pv_w(const uint32_t *A, const uint32_t *t, const int8_t *R, cons
 void orc_decaps_w(const uint32_t *U, const uint32_t *v, const int8_t *s,
                   uint8_t *mubits_out, uint32_t *d_out, uint32_t n, uint32_t k, uint32_t q);
 
-/* Number of OpenMP threads the loops above will use (1 if built without OpenMP). */
+/* Number of OpenMP threads the loops above will use (1 if built without OpenMP), and a setter so that the timed
+ * CPU baseline can report a 1-thread and an all-core figure (the paper's OpenMP baseline).  Returns
+ * the previous value; no effect without OpenMP.  Changes no arithmetic. */
 int orc_num_threads(void);
+int orc_set_num_threads(int threads);
 
 #ifdef __cplusplus
 }

@@ -22,7 +22,7 @@ __all__ = [
     "keygen", "encaps", "encaps_rows", "encaps_v", "decaps", "decaps_fo", "num_threads",
     "gauss_cdt", "gauss_from_word", "sample_gauss", "sample_cuniform", "encaps_pv",
     "cbd_from_word", "round_bit",
-    "sample_uniform32", "sample_uniform32_strided", "sample_cbd_s8", "keygen_w", "encaps_pv_w", "decaps_w",
+    "set_num_threads", "sample_uniform32", "sample_uniform32_strided", "sample_cbd_s8", "keygen_w", "encaps_pv_w", "decaps_w",
 ]
 
 _lib = None
@@ -61,6 +61,8 @@ def _L():
         lib.orc_encaps_pv.argtypes = [u16p, u16p, s8p, s8p, s8p, u8p, u16p, u16p, u32, u32, u32, u32]
         lib.orc_encaps_pv.restype = None
         lib.orc_num_threads.restype = C.c_int
+        lib.orc_set_num_threads.argtypes = [C.c_int]
+        lib.orc_set_num_threads.restype = C.c_int
         lib.orc_cbd_from_word.argtypes = [u32, u32, u32]
         lib.orc_cbd_from_word.restype = C.c_uint16
         lib.orc_round_bit.argtypes = [u32, u32]
@@ -325,3 +327,8 @@ def round_bit(d: int, q: int) -> int:
 
 def num_threads() -> int:
     return int(_L().orc_num_threads())
+
+
+def set_num_threads(threads: int) -> int:
+    """OpenMP threads of the loops from now on; returns the previous setting"""
+    return int(_L().orc_set_num_threads(int(threads)))

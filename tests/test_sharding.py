@@ -52,3 +52,27 @@ def test_world_size_2_gloo_reduction_and_disjoint_shards():
     assert res[0][0] == res[1][0] == 11.0                  # max over ranks
     assert res[0][1] == res[1][1] == 32                    # all instances counted once
     assert (res[0][2], res[0][3]) == (0, 15) and (res[1][2], res[1][3]) == (16, 31)
+
+
+def test_bench_spawns_its_own_ranks_for_gpus_2_dry_run():
+    """`python bench.py --gpus 2` started as a PLAIN process (no torchrun, no WORLD_SIZE) must produce the two ranks
+    itself.  --dry-run runs that launch path and the rank plumbing (instance-id assignment, barrier, max / sum
+    reduction, one JSON line from rank 0) on CPU/gloo; it prints no measurement."""
+    import json
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parent.parent
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, str(root / "bench.py"), "--gpus", "2", "--dry-run", "--steps", "3", "--warmup", "1"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout                           # rank 0 alone prints
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["dry_run"] is True and line["value"] is None
+    assert line["ms_per_step"] == 11.0                         # max over ranks of (10 + rank)
+    assert line["units_per_step"] == 64                        # 32 instances per rank, summed
+    ids = line["instance_ids_first_3_steps"]
+    spans = sorted(tuple(x) for rank_ids in ids for x in rank_ids)
+    assert spans == [(32 * i, 32 * i + 31) for i in range(6)]  # disjoint over ranks and steps, nothing skipped
