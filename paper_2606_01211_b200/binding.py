@@ -27,7 +27,7 @@ OPT_REGEN_PATH = 7
 OPT_R_OPERAND = 8
 KERNELS = ["rng_fill", "sample_uniform", "sample_cbd", "sample_bits", "keygen_stored", "keygen_regen",
            "expand_R_v", "encaps_tc", "encaps_simt", "decaps", "keygen_prep", "keygen_tc", "fo_verdict",
-           "sample_gauss", "sample_cuniform", "prep_R_pv", "encaps_regen_tc", "sample_kem"]
+           "sample_gauss", "sample_cuniform", "prep_R_pv", "encaps_regen_tc", "sample_kem", "wide_pack", "wide_keygen"]
 
 EXPORTS = [
     "lwe_create", "lwe_destroy", "lwe_strerror", "lwe_last_cuda_error", "lwe_launch_count",
@@ -35,6 +35,8 @@ EXPORTS = [
     "lwe_keygen", "lwe_encaps", "lwe_decaps", "lwe_decaps_fo", "lwe_kem_host",
     "lwe_sample_gauss_s8", "lwe_sample_gauss_u16", "lwe_sample_cuniform_s8", "lwe_encaps_pv", "lwe_set_option",
     "lwe_profile_read", "lwe_profile_reset",
+    "lwe_sample_uniform_u32", "lwe_sample_cbd_s8", "lwe_wide_load_matrix", "lwe_wide_load_matrix_seeded", "lwe_wide_keygen",
+    "lwe_wide_encaps", "lwe_wide_decaps",
 ]
 
 
@@ -85,6 +87,13 @@ def load_library() -> C.CDLL:
     lib.lwe_sample_cuniform_s8.argtypes = [vp, vp, u64, u64, u64, u32, u32, u32, u32, vp]
     lib.lwe_encaps_pv.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
     lib.lwe_kem_host.argtypes = [vp, vp, u64, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
+    for f in (lib.lwe_sample_uniform_u32, lib.lwe_sample_cbd_s8):
+        f.argtypes = [vp, vp, u64, u64, u64, u32, u32, u32, vp]
+    lib.lwe_wide_load_matrix.argtypes = [vp, vp, vp]
+    lib.lwe_wide_load_matrix_seeded.argtypes = [vp, u64, vp]
+    lib.lwe_wide_keygen.argtypes = [vp, vp, vp, vp, u32, vp]
+    lib.lwe_wide_encaps.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
+    lib.lwe_wide_decaps.argtypes = [vp, vp, vp, vp, vp, u32, vp]
     _lib = lib
     return lib
 
@@ -222,6 +231,35 @@ class Context:
         self._check(self._lib.lwe_encaps_pv(self._h, _ptr(d_A), _ptr(d_t), _ptr(d_R), _ptr(d_E1), _ptr(d_e2),
                                             _ptr(d_mubits), _ptr(d_U), _ptr(d_v), batch, _stream(stream)),
                     "lwe_encaps_pv")
+
+    # -- wide contexts (q > 65536: uint32 residues, int8 small objects)
+    def sample_uniform_u32(self, d_out, first: int, count: int, seed: int, tag: int, inst0: int = 0, n_inst: int = 1,
+                           stream=None):
+        self._check(self._lib.lwe_sample_uniform_u32(self._h, _ptr(d_out), first, count, seed, tag, inst0, n_inst,
+                                                     _stream(stream)), "lwe_sample_uniform_u32")
+
+    def sample_cbd_s8(self, d_out, first: int, count: int, seed: int, tag: int, inst0: int = 0, n_inst: int = 1,
+                      stream=None):
+        self._check(self._lib.lwe_sample_cbd_s8(self._h, _ptr(d_out), first, count, seed, tag, inst0, n_inst,
+                                                _stream(stream)), "lwe_sample_cbd_s8")
+
+    def wide_load_matrix(self, d_A, stream=None):
+        self._check(self._lib.lwe_wide_load_matrix(self._h, _ptr(d_A), _stream(stream)), "lwe_wide_load_matrix")
+
+    def wide_load_matrix_seeded(self, seed_A: int, stream=None):
+        self._check(self._lib.lwe_wide_load_matrix_seeded(self._h, seed_A, _stream(stream)), "lwe_wide_load_matrix_seeded")
+
+    def wide_keygen(self, d_s, d_e, d_t, batch: int = 1, stream=None):
+        self._check(self._lib.lwe_wide_keygen(self._h, _ptr(d_s), _ptr(d_e), _ptr(d_t), batch, _stream(stream)),
+                    "lwe_wide_keygen")
+
+    def wide_encaps(self, d_t, d_R, d_E1, d_e2, d_mubits, d_U, d_v, batch: int = 1, stream=None):
+        self._check(self._lib.lwe_wide_encaps(self._h, _ptr(d_t), _ptr(d_R), _ptr(d_E1), _ptr(d_e2), _ptr(d_mubits),
+                                              _ptr(d_U), _ptr(d_v), batch, _stream(stream)), "lwe_wide_encaps")
+
+    def wide_decaps(self, d_U, d_v, d_s, d_mubits_out, batch: int = 1, stream=None):
+        self._check(self._lib.lwe_wide_decaps(self._h, _ptr(d_U), _ptr(d_v), _ptr(d_s), _ptr(d_mubits_out), batch,
+                                              _stream(stream)), "lwe_wide_decaps")
 
     def kem_host(self, d_A, seed_A: int, h_s, h_e, h_Rbits, h_mubits, h_b, h_U, h_v, h_mubits_out, batch: int = 1,
                  stream=None):

@@ -80,6 +80,9 @@ cudaError_t dev_alloc(T **p, size_t count)
 
 void free_all(Ctx *c)
 {
+    cudaFree(c->d_A16); cudaFree(c->d_exc_col_cnt); cudaFree(c->d_exc_col_rows); cudaFree(c->d_exc_row_cnt);
+    cudaFree(c->d_exc_row_cols); cudaFree(c->d_exc_overflow);
+    if (c->h_exc_overflow) cudaFreeHost(c->h_exc_overflow);
     cudaFree(c->d_Sx);
     cudaFree(c->d_Apanel);
     cudaFree(c->d_foflags); cudaFree(c->d_vprime); cudaFree(c->d_tile_locks);
@@ -115,7 +118,20 @@ struct DeviceGuard {
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
+// exception-list capacity of a wide context: 4x the expected number of elements >= 2^16 per column (row) of a
+// uniform A plus 16, rounded up to a power of two (q = 65537, m = 8192: expected 0.125, capacity 16)
+uint32_t exc_capacity(uint32_t len, uint32_t q)
+{
+    const double mean = (double)len * (double)(q - 65536u) / (double)q;
+    uint32_t want = (uint32_t)(4.0 * mean) + 16u, cap = 16u;
+    while (cap < want) cap <<= 1;
+    return cap;
+}
+
 #define CHECK_CTX(ctx) do { if (!(ctx)) return LWE_ERR_NULLPTR; } while (0)
+// the uint16 entry points do not exist for a modulus that needs 17 bits, and vice versa
+#define REQUIRE_NARROW(ctx) do { if ((ctx)->c.wide) return LWE_ERR_UNSUPPORTED; } while (0)
+#define REQUIRE_WIDE(ctx) do { if (!(ctx)->c.wide) return LWE_ERR_UNSUPPORTED; } while (0)
 #define REQUIRE_PTR(p) do { if (!(p)) return LWE_ERR_NULLPTR; } while (0)
 #define REQUIRE_ALIGNED(p) do { if (!aligned16(p)) return LWE_ERR_ALIGN; } while (0)
 #define LAUNCH(c, expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { (c)->last_cuda_error = (int)_e; return LWE_ERR_CUDA; } } while (0)
@@ -142,8 +158,11 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
     if (!out || !p) return LWE_ERR_NULLPTR;
     *out = nullptr;
     if (p->n == 0 || p->m == 0 || p->k == 0 || p->n % 8 || p->m % 8 || p->k % 8) return LWE_ERR_PARAM;
-    if (p->q < 2 || p->q > 65536 || p->eta < 1 || p->eta > 8 || p->max_batch < 1) return LWE_ERR_PARAM;
+    if (p->q < 2 || p->q > 65536u + 1024u || p->eta < 1 || p->eta > 8 || p->max_batch < 1) return LWE_ERR_PARAM;
     if (p->k > 2048 || p->n > (1u << 20) || p->m > (1u << 20)) return LWE_ERR_PARAM;
+    const bool wide = p->q > 65536u;
+    if (wide && (p->k > 1024 || p->m > 65536u || exc_capacity(p->m, p->q) > 1024u || exc_capacity(p->n, p->q) > 1024u))
+        return LWE_ERR_UNSUPPORTED;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return LWE_ERR_UNSUPPORTED;
@@ -163,6 +182,7 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
     c->device = device;
     c->sm_count = prop.multiProcessorCount;
     c->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    c->wide = wide ? 1u : 0u;
 
     const size_t B = p->max_batch, n = p->n, m = p->m, k = p->k;
     cudaError_t e = cudaSuccess;
@@ -184,9 +204,20 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
     ok(dev_alloc(&c->d_vacc, k * B));
     ok(dev_alloc(&c->d_dacc, k * B));
     ok(dev_alloc(&c->d_counters, 8 + 2 * B));
-    ok(dev_alloc(&c->d_hs, B * n)); ok(dev_alloc(&c->d_he, B * m)); ok(dev_alloc(&c->d_hb, B * m));
-    ok(dev_alloc(&c->d_hU, B * n * k)); ok(dev_alloc(&c->d_hv, B * k));
-    ok(dev_alloc(&c->d_hR, B * m * k / 8)); ok(dev_alloc(&c->d_hmu, B * k / 8)); ok(dev_alloc(&c->d_hmuout, B * k / 8));
+    if (wide) {
+        // the packed public matrix and its exception lists (lwe_wide_load_matrix); no lwe_kem_host staging
+        c->exc_cap_col = exc_capacity(p->m, p->q);
+        c->exc_cap_row = exc_capacity(p->n, p->q);
+        ok(dev_alloc(&c->d_A16, m * n));
+        ok(dev_alloc(&c->d_exc_col_cnt, n)); ok(dev_alloc(&c->d_exc_col_rows, n * c->exc_cap_col));
+        ok(dev_alloc(&c->d_exc_row_cnt, m)); ok(dev_alloc(&c->d_exc_row_cols, m * c->exc_cap_row));
+        ok(dev_alloc(&c->d_exc_overflow, 4));
+        ok(cudaMallocHost(reinterpret_cast<void **>(&c->h_exc_overflow), 16));
+    } else {
+        ok(dev_alloc(&c->d_hs, B * n)); ok(dev_alloc(&c->d_he, B * m)); ok(dev_alloc(&c->d_hb, B * m));
+        ok(dev_alloc(&c->d_hU, B * n * k)); ok(dev_alloc(&c->d_hv, B * k));
+        ok(dev_alloc(&c->d_hR, B * m * k / 8)); ok(dev_alloc(&c->d_hmu, B * k / 8)); ok(dev_alloc(&c->d_hmuout, B * k / 8));
+    }
     ok(cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
     ok(cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
     ok(cudaEventCreateWithFlags(&c->ev_entry, cudaEventDisableTiming));
@@ -339,7 +370,9 @@ int lwe_sample_uniform(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t c
                        uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream)
 {
     int rc = sampler_args(ctx, d_out, first, count, tag, inst0, n_inst);
-    if (rc != LWE_OK || count == 0 || n_inst == 0) return rc;
+    if (rc != LWE_OK) return rc;
+    REQUIRE_NARROW(ctx);
+    if (count == 0 || n_inst == 0) return rc;
     Ctx *c = &ctx->c;
     DeviceGuard guard(c->device);
     LAUNCH(c, launch_sample_uniform(c, d_out, first, count, seed_key_host(seed), tag, inst0, n_inst, (cudaStream_t)stream));
@@ -350,7 +383,9 @@ int lwe_sample_cbd(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count
                    uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream)
 {
     int rc = sampler_args(ctx, d_out, first, count, tag, inst0, n_inst);
-    if (rc != LWE_OK || count == 0 || n_inst == 0) return rc;
+    if (rc != LWE_OK) return rc;
+    REQUIRE_NARROW(ctx);
+    if (count == 0 || n_inst == 0) return rc;
     Ctx *c = &ctx->c;
     DeviceGuard guard(c->device);
     LAUNCH(c, launch_sample_cbd(c, d_out, first, count, seed_key_host(seed), tag, inst0, n_inst, (cudaStream_t)stream));
@@ -372,6 +407,7 @@ int lwe_sample_kem(lwe_ctx *ctx, uint16_t *d_s, uint16_t *d_e, uint8_t *d_Rbits,
                    uint32_t inst0, uint32_t n_inst, void *stream)
 {
     CHECK_CTX(ctx);
+    REQUIRE_NARROW(ctx);
     if ((uint64_t)inst0 + n_inst > (1ull << 32)) return LWE_ERR_PARAM;
     if (n_inst == 0) return LWE_OK;
     REQUIRE_PTR(d_s); REQUIRE_PTR(d_e); REQUIRE_PTR(d_Rbits); REQUIRE_PTR(d_mubits);
@@ -386,6 +422,7 @@ int lwe_keygen(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_
                uint16_t *d_b, uint32_t batch, void *stream)
 {
     CHECK_CTX(ctx);
+    REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
     if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
     REQUIRE_PTR(d_s); REQUIRE_PTR(d_e); REQUIRE_PTR(d_b);
@@ -448,6 +485,7 @@ int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_
                const uint8_t *d_mubits, uint16_t *d_U, uint16_t *d_v, uint32_t batch, void *stream)
 {
     CHECK_CTX(ctx);
+    REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
     if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
     REQUIRE_PTR(d_b); REQUIRE_PTR(d_Rbits); REQUIRE_PTR(d_mubits); REQUIRE_PTR(d_U); REQUIRE_PTR(d_v);
@@ -462,6 +500,7 @@ int lwe_decaps_fo(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_b, const 
                   void *stream)
 {
     CHECK_CTX(ctx);
+    REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
     if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
     REQUIRE_PTR(d_A); REQUIRE_PTR(d_b); REQUIRE_PTR(d_U); REQUIRE_PTR(d_v); REQUIRE_PTR(d_s); REQUIRE_PTR(d_Rbits);
@@ -488,6 +527,7 @@ int lwe_decaps(lwe_ctx *ctx, const uint16_t *d_U, const uint16_t *d_v, const uin
                uint8_t *d_mubits_out, uint32_t batch, void *stream)
 {
     CHECK_CTX(ctx);
+    REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
     if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
     REQUIRE_PTR(d_U); REQUIRE_PTR(d_v); REQUIRE_PTR(d_s); REQUIRE_PTR(d_mubits_out);
@@ -522,7 +562,9 @@ int lwe_sample_gauss_u16(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t
                          uint32_t inst0, uint32_t n_inst, double sigma, void *stream)
 {
     int rc = gauss_args(ctx, d_out, first, count, tag, inst0, n_inst, sigma);
-    if (rc != LWE_OK || count == 0 || n_inst == 0) return rc;
+    if (rc != LWE_OK) return rc;
+    REQUIRE_NARROW(ctx);
+    if (count == 0 || n_inst == 0) return rc;
     Ctx *c = &ctx->c;
     DeviceGuard guard(c->device);
     LAUNCH(c, launch_sample_gauss(c, d_out, true, first, count, seed_key_host(seed), tag, inst0, n_inst, sigma,
@@ -549,6 +591,7 @@ int lwe_encaps_pv(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_t, const 
                   const int8_t *d_e2, const uint8_t *d_mubits, uint16_t *d_U, uint16_t *d_v, uint32_t batch, void *stream)
 {
     CHECK_CTX(ctx);
+    REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
     if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
     REQUIRE_PTR(d_A); REQUIRE_PTR(d_t); REQUIRE_PTR(d_R); REQUIRE_PTR(d_E1); REQUIRE_PTR(d_e2); REQUIRE_PTR(d_mubits);
@@ -560,9 +603,149 @@ int lwe_encaps_pv(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_t, const 
     if (c->encaps_path >= 2 && !tc) return LWE_ERR_UNSUPPORTED;
     DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
-    LAUNCH(c, launch_prep_R_pv_and_v(c, d_t, d_R, d_e2, d_mubits, d_v, batch, tc, st));
-    if (tc) LAUNCH(c, launch_encaps_tc2_pv(c, d_A, d_E1, d_U, batch, st));
+    // k % 128 == 0: the GEMM reads R in place (no operand copy); the pass over R then only computes v
+    const bool inplace = tc && c->r_operand != 1 && encaps_tc2_r_inplace_supported(c, batch);
+    LAUNCH(c, launch_prep_R_pv_and_v(c, d_t, d_R, d_e2, d_mubits, d_v, batch, tc && !inplace, st));
+    if (tc) LAUNCH(c, launch_encaps_tc2_pv(c, d_A, d_E1, d_U, batch, st, inplace ? d_R : nullptr));
     else LAUNCH(c, launch_encaps_pv_simt(c, d_A, d_R, d_E1, d_U, batch, st));
+    return LWE_OK;
+}
+
+// ---------------------------------------------------------------------------------- wide contexts (q > 65536)
+
+int lwe_sample_uniform_u32(lwe_ctx *ctx, uint32_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
+                           uint32_t inst0, uint32_t n_inst, void *stream)
+{
+    CHECK_CTX(ctx);
+    REQUIRE_WIDE(ctx);
+    if (tag == 0 || tag > 255) return LWE_ERR_PARAM;
+    if ((uint64_t)inst0 + n_inst > (1ull << 32)) return LWE_ERR_PARAM;
+    if (first % 4) return LWE_ERR_ALIGN;
+    if (count == 0 || n_inst == 0) return LWE_OK;
+    REQUIRE_PTR(d_out); REQUIRE_ALIGNED(d_out);
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_sample_uniform32(c, d_out, first, count, seed_key_host(seed), tag, inst0, n_inst, (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+int lwe_sample_cbd_s8(lwe_ctx *ctx, int8_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
+                      uint32_t inst0, uint32_t n_inst, void *stream)
+{
+    int rc = sampler_args(ctx, d_out, first, count, tag, inst0, n_inst);
+    if (rc != LWE_OK || count == 0 || n_inst == 0) return rc;
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_sample_cbd_s8(c, d_out, first, count, seed_key_host(seed), tag, inst0, n_inst, (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+// pack rows of A given in panels; checks the exception lists afterwards (host synchronisation)
+static int wide_finish_load(Ctx *c, cudaStream_t st)
+{
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->h_exc_overflow, c->d_exc_overflow, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    LWE_CUDA_TRY(c, cudaStreamSynchronize(st));
+    if (*c->h_exc_overflow) return (*c->h_exc_overflow & 2u) ? LWE_ERR_PARAM : LWE_ERR_UNSUPPORTED;
+    c->A_loaded = 1;
+    return LWE_OK;
+}
+
+static int wide_begin_load(Ctx *c, cudaStream_t st)
+{
+    c->A_loaded = 0;
+    LWE_CUDA_TRY(c, cudaMemsetAsync(c->d_exc_col_cnt, 0, (size_t)c->p.n * sizeof(uint32_t), st));
+    LWE_CUDA_TRY(c, cudaMemsetAsync(c->d_exc_row_cnt, 0, (size_t)c->p.m * sizeof(uint32_t), st));
+    LWE_CUDA_TRY(c, cudaMemsetAsync(c->d_exc_overflow, 0, sizeof(uint32_t), st));
+    return LWE_OK;
+}
+
+int lwe_wide_load_matrix(lwe_ctx *ctx, const uint32_t *d_A, void *stream)
+{
+    CHECK_CTX(ctx);
+    REQUIRE_WIDE(ctx);
+    REQUIRE_PTR(d_A); REQUIRE_ALIGNED(d_A);
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = wide_begin_load(c, st);
+    if (rc != LWE_OK) return rc;
+    LAUNCH(c, launch_wide_pack(c, d_A, 0, c->p.m, st));
+    return wide_finish_load(c, st);
+}
+
+int lwe_wide_load_matrix_seeded(lwe_ctx *ctx, uint64_t seed_A, void *stream)
+{
+    CHECK_CTX(ctx);
+    REQUIRE_WIDE(ctx);
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = wide_begin_load(c, st);
+    if (rc != LWE_OK) return rc;
+    // the uint32 A never exists in full: one row panel at a time through the context's panel buffer
+    const AesKey key = seed_key_host(seed_A);
+    uint32_t *panel = reinterpret_cast<uint32_t *>(c->d_Apanel);
+    uint32_t step = c->panel_rows_alloc / 2;                   // the buffer holds panel_rows_alloc rows of uint16
+    if (step < 1) step = 1;
+    for (uint32_t row0 = 0; row0 < c->p.m; row0 += step) {
+        const uint32_t rows = (c->p.m - row0 < step) ? (c->p.m - row0) : step;
+        LAUNCH(c, launch_sample_uniform32(c, panel, (uint64_t)row0 * c->p.n, (uint64_t)rows * c->p.n, key, LWE_TAG_A, 0, 1, st));
+        LAUNCH(c, launch_wide_pack(c, panel, row0, rows, st));
+    }
+    return wide_finish_load(c, st);
+}
+
+int lwe_wide_keygen(lwe_ctx *ctx, const int8_t *d_s, const int8_t *d_e, uint32_t *d_t, uint32_t batch, void *stream)
+{
+    CHECK_CTX(ctx);
+    REQUIRE_WIDE(ctx);
+    Ctx *c = &ctx->c;
+    if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
+    if (!c->A_loaded) return LWE_ERR_PARAM;
+    REQUIRE_PTR(d_s); REQUIRE_PTR(d_e); REQUIRE_PTR(d_t);
+    REQUIRE_ALIGNED(d_s); REQUIRE_ALIGNED(d_e); REQUIRE_ALIGNED(d_t);
+    const bool tc = c->keygen_path != 1 && wide_keygen_tc_supported(c, batch);
+    if (c->keygen_path == 2 && !tc) return LWE_ERR_UNSUPPORTED;
+    DeviceGuard guard(c->device);
+    if (tc) LAUNCH(c, launch_wide_keygen_tc(c, d_s, d_e, d_t, batch, (cudaStream_t)stream));
+    else LAUNCH(c, launch_wide_keygen_simt(c, d_s, d_e, d_t, batch, (cudaStream_t)stream));
+    return LWE_OK;
+}
+
+int lwe_wide_encaps(lwe_ctx *ctx, const uint32_t *d_t, const int8_t *d_R, const int8_t *d_E1, const int8_t *d_e2,
+                    const uint8_t *d_mubits, uint32_t *d_U, uint32_t *d_v, uint32_t batch, void *stream)
+{
+    CHECK_CTX(ctx);
+    REQUIRE_WIDE(ctx);
+    Ctx *c = &ctx->c;
+    if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
+    if (!c->A_loaded) return LWE_ERR_PARAM;
+    REQUIRE_PTR(d_t); REQUIRE_PTR(d_R); REQUIRE_PTR(d_E1); REQUIRE_PTR(d_e2); REQUIRE_PTR(d_mubits); REQUIRE_PTR(d_U);
+    REQUIRE_PTR(d_v);
+    REQUIRE_ALIGNED(d_t); REQUIRE_ALIGNED(d_R); REQUIRE_ALIGNED(d_E1); REQUIRE_ALIGNED(d_e2); REQUIRE_ALIGNED(d_mubits);
+    REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v);
+    const bool tc = encaps_tc2_supported(c, batch) && c->encaps_path != 1;
+    if (c->encaps_path >= 2 && !tc) return LWE_ERR_UNSUPPORTED;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool inplace = tc && encaps_tc2_r_inplace_supported(c, batch);
+    LAUNCH(c, launch_wide_v(c, d_t, d_R, d_e2, d_mubits, d_v, batch, tc && !inplace, st));
+    if (tc) LAUNCH(c, launch_wide_encaps_tc2(c, d_R, d_E1, d_U, batch, st));
+    else LAUNCH(c, launch_wide_encaps_simt(c, d_R, d_E1, d_U, batch, st));
+    return LWE_OK;
+}
+
+int lwe_wide_decaps(lwe_ctx *ctx, const uint32_t *d_U, const uint32_t *d_v, const int8_t *d_s, uint8_t *d_mubits_out,
+                    uint32_t batch, void *stream)
+{
+    CHECK_CTX(ctx);
+    REQUIRE_WIDE(ctx);
+    Ctx *c = &ctx->c;
+    if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
+    REQUIRE_PTR(d_U); REQUIRE_PTR(d_v); REQUIRE_PTR(d_s); REQUIRE_PTR(d_mubits_out);
+    REQUIRE_ALIGNED(d_U); REQUIRE_ALIGNED(d_v); REQUIRE_ALIGNED(d_s); REQUIRE_ALIGNED(d_mubits_out);
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_wide_decaps(c, d_U, d_v, d_s, d_mubits_out, batch, (cudaStream_t)stream));
     return LWE_OK;
 }
 
@@ -571,6 +754,7 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint1
                  uint8_t *h_mubits_out, uint32_t batch, void *stream)
 {
     CHECK_CTX(ctx);
+    REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
     if (batch == 0 || batch > c->p.max_batch) return LWE_ERR_PARAM;
     REQUIRE_PTR(h_s); REQUIRE_PTR(h_e); REQUIRE_PTR(h_Rbits); REQUIRE_PTR(h_mubits);

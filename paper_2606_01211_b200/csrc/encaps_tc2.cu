@@ -75,15 +75,32 @@ struct PairCfg {
 // counts the arrivals of one group of each CTA (8 warps) beside the A bytes.  Needs k % 128 == 0 (a half tile lies inside
 // one instance) and kTileK == 128 (one row per expander thread).  Against the expanded operand this removes the
 // 128 MiB expanded-R write per batch and every DRAM / L2 re-read of it by the GEMM (16x fewer operand bytes).
+// The signed-R modes (N2) beside the accumulators.  r_inplace: the B operand is read IN PLACE from the caller's int8
+// R [batch][m_full][k] (a half tile lies inside one instance when k % 128 == 0; rows of the next instance that a
+// ragged last K block drags in meet zero-filled rows of A) -- no operand copy is made.  Wide contexts: the
+// exception list of column j (rows i with A[i][j] >= 2^16) and R itself, for the 2^16 R[i][c] terms.
+struct PvArgs {
+    const int8_t *E1;
+    uint32_t bias, e1bias, two_step;      // see launch_pair
+    uint32_t r_inplace, m_full;
+    const int8_t *R;
+    const uint32_t *exc_cnt, *exc_rows;
+    uint32_t exc_cap, delta;              // delta = q - 2^16: 2^16 = -delta (mod q)
+};
+
 template <uint32_t kStages, uint32_t kTileK, int kMode, bool kBitsB>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kBitsB ? kThreadsBits : kThreads, 1)
 encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
-                  uint16_t *__restrict__ U, uint32_t *__restrict__ flags, const int8_t *__restrict__ E1, uint32_t m,
+                  void *__restrict__ U_, uint32_t *__restrict__ flags, uint32_t m,
                   uint32_t n, uint32_t k,
-                  uint32_t ncols_total, ModQ mq, uint32_t group_w,
-                  uint32_t pv_bias, uint32_t pv_e1bias, const __grid_constant__ CUtensorMap mapBits, uint32_t bits_row0,
+                  uint32_t ncols_total, ModQ mq, uint32_t group_w, PvArgs pv,
+                  const __grid_constant__ CUtensorMap mapBits, uint32_t bits_row0,
                   uint32_t bits_rows_per_inst)
 {
+    constexpr bool kPv = (kMode == kEpiStorePv || kMode == kEpiStorePvW);
+    uint16_t *U = static_cast<uint16_t *>(U_);
+    uint32_t *U32 = static_cast<uint32_t *>(U_);
+    const int8_t *E1 = pv.E1;
     static_assert(!kBitsB || kTileK == 128, "one K row per expander thread");
     using Cfg = PairCfg<kStages, kTileK>;
     constexpr uint32_t kBytesA = Cfg::kBytesA, kBytesStage = Cfg::kBytesStage;
@@ -150,7 +167,12 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
             uint32_t mt, nt;
             sched.coords(t, mt, nt);
             const int32_t a_col = (int32_t)(mt * kPairM + rank * kCtaM);
-            const int32_t r_col = (int32_t)(nt * kTileN + rank * kHalfN);
+            int32_t r_col = (int32_t)(nt * kTileN + rank * kHalfN), r_row0 = 0;
+            if (kPv && pv.r_inplace) {                     // this half tile inside R [batch][m_full][k]
+                const uint32_t inst = (uint32_t)r_col / k;
+                r_col -= (int32_t)(inst * k);
+                r_row0 = (int32_t)(inst * pv.m_full);      // past the batch: out of range -> zeros
+            }
             for (uint32_t kb = 0; kb < k_blocks; kb++) {
                 mbar_wait(empty_bar(stage), phase ^ 1);
                 const uint32_t sa = base + stage * kBytesStage;
@@ -159,7 +181,7 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 if (elect_one()) {
                     if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * (kBitsB ? kBytesA : kBytesStage));   // both CTAs' bytes
                     tma_load_2d_pair(sa, &mapA, lead_full, a_col, row);
-                    if (!kBitsB) tma_load_2d_pair(sa + kBytesA, &mapR, lead_full, r_col, row);
+                    if (!kBitsB) tma_load_2d_pair(sa + kBytesA, &mapR, lead_full, r_col, r_row0 + row);
                 }
                 __syncwarp();
                 if (++stage == kStages) { stage = 0; phase ^= 1; }
@@ -184,7 +206,7 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                         uint64_t bdesc = make_desc_mn_sw128(sa + kBytesA, 0, 1024);
 #pragma unroll
                         for (uint32_t ks = 0; ks < kTileK / kUmmaK; ks++) {
-                            umma_i8_pair(d_tmem, adesc, bdesc, kMode == kEpiStorePv ? kInstrDescSignedB : kInstrDesc,
+                            umma_i8_pair(d_tmem, adesc, bdesc, kPv ? kInstrDescSignedB : kInstrDesc,
                                          (kb | ks) ? 1u : 0u);
                             adesc += (kUmmaK * 128) >> 4;
                             bdesc += (kUmmaK * 128) >> 4;
@@ -283,32 +305,56 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 const bool in_range = j < n && col < ncols_total;
                 const uint32_t inst = col / k, c = col - inst * k;
                 uint32_t e1w[4] = {0, 0, 0, 0};                      // 16 int8 of E1[inst][j][c..c+15] (N2 only)
-                if (kMode == kEpiStorePv && in_range) {
+                if (kPv && in_range) {
                     const uint4 t4 = *reinterpret_cast<const uint4 *>(E1 + ((size_t)inst * n + j) * k + c);
                     e1w[0] = t4.x; e1w[1] = t4.y; e1w[2] = t4.z; e1w[3] = t4.w;
+                }
+                // wide: corr[x] = sum over the exceptions i of column j of R[inst][i][c + x]  (rare: ~m/65537 per column)
+                int corr[16];
+                if (kMode == kEpiStorePvW) {
+#pragma unroll
+                    for (int x = 0; x < 16; x++) corr[x] = 0;
+                    const uint32_t cnt = in_range ? min(__ldg(pv.exc_cnt + j), pv.exc_cap) : 0u;
+                    for (uint32_t y = 0; y < cnt; y++) {
+                        const uint32_t i = __ldg(pv.exc_rows + (size_t)j * pv.exc_cap + y);
+                        const uint4 r4 = __ldg(reinterpret_cast<const uint4 *>(pv.R + ((size_t)inst * pv.m_full + i) * k + c));
+                        const uint32_t rw[4] = {r4.x, r4.y, r4.z, r4.w};
+#pragma unroll
+                        for (int x = 0; x < 16; x++) corr[x] += (int)(int8_t)(rw[x >> 2] >> (8 * (x & 3)));
+                    }
                 }
 #pragma unroll
                 for (int x = 0; x < 16; x++) {
                     uint32_t send = odd ? r[x] : r[16 + x];
                     uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 1);
-                    if (kMode == kEpiStorePv) {
-                        // signed planes: lo = sum lo(A) r, hi = sum hi(A) r; U = lo + 256 hi + e1 mod q
+                    if (kPv) {
+                        // signed planes: lo = sum lo(A) r, hi = sum hi(A) r; U = lo + 256 hi + e1 (- delta corr) mod q
                         const int32_t lo = (int32_t)(odd ? recv : r[x]), hi = (int32_t)(odd ? r[16 + x] : recv);
-                        const int32_t e1 = (int32_t)(int8_t)(e1w[x >> 2] >> (8 * (x & 3)));
+                        int32_t e1 = (int32_t)(int8_t)(e1w[x >> 2] >> (8 * (x & 3)));
+                        if (kMode == kEpiStorePvW) e1 -= (int32_t)pv.delta * corr[x];       // 2^16 = -delta (mod q)
                         // general q: straight-line unsigned arithmetic (a branch per sign serialised the 16
-                        // elements: 0.65 ms instead of 0.17 ms at n = 4096).  pv_bias is a multiple of q >= 255 *
-                        // 128 * m, so plane + pv_bias is the same residue in [0, 2^32); pv_e1bias likewise >= 128.
+                        // elements: 0.65 ms instead of 0.17 ms at n = 4096).  pv.bias is a multiple of q >= 255 *
+                        // 128 * rows, so plane + bias is the same residue in [0, 2^32); pv.e1bias likewise covers e1.
                         if (mq.pow2) o[x] = ((uint32_t)lo + ((uint32_t)hi << 8) + (uint32_t)e1) & mq.mask;
-                        else o[x] = mod_u32(mod_u32((uint32_t)lo + pv_bias, mq) + 256u * mod_u32((uint32_t)hi + pv_bias, mq) +
-                                            ((uint32_t)e1 + pv_e1bias), mq);
+                        else if (pv.two_step)           // (lo + bias) + 256 (hi mod q) + e1 stays below 2^32: one reduction less
+                            o[x] = mod_u32(((uint32_t)lo + pv.bias) + 256u * mod_u32((uint32_t)hi + pv.bias, mq) +
+                                           ((uint32_t)e1 + pv.e1bias), mq);
+                        else o[x] = mod_u32(mod_u32((uint32_t)lo + pv.bias, mq) + 256u * mod_u32((uint32_t)hi + pv.bias, mq) +
+                                            ((uint32_t)e1 + pv.e1bias), mq);
                     } else {
                         uint32_t val = odd ? (recv + (r[16 + x] << 8)) : (r[x] + (recv << 8));
                         o[x] = mq.pow2 ? (val & mq.mask) : mod_u32(val, mq);
                     }
                 }
                 if (in_range) {
-                    const bool bad = store_u16x16<kMode>(reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c), o, mq);
-                    if (kMode == kEpiCompare) mism.note(flags, inst, bad);
+                    if (kMode == kEpiStorePvW) {
+                        uint4 *dst = reinterpret_cast<uint4 *>(U32 + ((size_t)inst * n + j) * k + c);
+#pragma unroll
+                        for (int x = 0; x < 4; x++) dst[x] = make_uint4(o[4 * x], o[4 * x + 1], o[4 * x + 2], o[4 * x + 3]);
+                    } else {
+                        const bool bad = store_u16x16<kMode>(reinterpret_cast<uint4 *>(U + ((size_t)inst * n + j) * k + c), o, mq);
+                        if (kMode == kEpiCompare) mism.note(flags, inst, bad);
+                    }
                 }
             }
             if (kMode == kEpiCompare) mism.flush_warp(flags);
@@ -331,10 +377,12 @@ bool encaps_tc2_supported(const Ctx *c, uint32_t batch)
     return encaps_tc_supported(c, batch) && c->sm_count >= 2;
 }
 
+// signed-R modes: d_R = the caller's R [batch][m][k] (the wide epilogue reads its exception rows there); r_inplace:
+// the B operand is read in place from it instead of from the copy in c->d_Rexp
 template <uint32_t kStages, uint32_t kTileK, int kMode, bool kBitsB = false>
-static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t *d_flags, const int8_t *d_E1,
+static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, void *d_U, uint32_t *d_flags, const int8_t *d_E1,
                                uint32_t batch, uint32_t row0, uint32_t rows, cudaStream_t st,
-                               const uint8_t *d_Rbits = nullptr)
+                               const uint8_t *d_Rbits = nullptr, const int8_t *d_R = nullptr, bool r_inplace = false)
 {
     using Cfg = PairCfg<kStages, kTileK>;
     const lwe_params &p = c->p;
@@ -342,7 +390,11 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint3
     CUtensorMap mapA, mapR;
     // d_A holds rows [row0, row0 + rows) of A; the matching rows of the expanded R follow from row0
     if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, rows, kTileK)) return cudaErrorInvalidValue;
-    if (!make_map_u8(c, &mapR, c->d_Rexp + (size_t)row0 * ncols, ncols, rows, kTileK)) return cudaErrorInvalidValue;
+    if (r_inplace) {
+        if (!make_map_u8(c, &mapR, d_R, p.k, (uint64_t)batch * p.m, kTileK)) return cudaErrorInvalidValue;
+    } else if (!make_map_u8(c, &mapR, c->d_Rexp + (size_t)row0 * ncols, ncols, rows, kTileK)) {
+        return cudaErrorInvalidValue;
+    }
     auto kern = encaps_tc2_kernel<kStages, kTileK, kMode, kBitsB>;
     const uint32_t smem_bytes = kBitsB ? Cfg::kSmemBytesBits : Cfg::kSmemBytes;
     cudaError_t err = kernel_prepare(c, kern, smem_bytes);
@@ -356,22 +408,42 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint3
     const uint32_t n_tiles_all = (ncols + kTileN - 1) / kTileN;
     const uint32_t gw = kBitsB ? n_tiles_all : 8u;
     ProfScope prof(c, LWE_K_ENCAPS_TC, st);
-    // signed byte-plane sums of the N2 variant: |plane| <= 255 * 128 * rows <= 65280 * 65536, and twice that plus q
-    // stays below 2^32
+    // signed byte-plane sums of the N2 variant: |plane| <= 255 * 128 * rows; bias = the next multiple of q, so that
+    // plane + bias is the same residue in [0, 2 bias] < 2^32 (rows <= 65536).  e1 (and, wide, e1 - delta * corr with
+    // |corr| <= 128 * capacity) gets its own bias.  two_step: (lo + bias) + 256 (hi mod q) + (e1 + e1bias) < 2^32.
+    PvArgs pv = {};
     const uint64_t plane_max = 255ull * 128ull * rows, q = p.q;
-    const uint32_t pv_bias = (uint32_t)((plane_max + q - 1) / q * q), pv_e1bias = (uint32_t)((128 + q - 1) / q * q);
+    const uint64_t delta = c->wide ? q - 65536u : 0u;
+    const uint64_t e1_max = 128ull + delta * 128ull * c->exc_cap_col;
+    pv.E1 = d_E1;
+    pv.bias = (uint32_t)((plane_max + q - 1) / q * q);
+    pv.e1bias = (uint32_t)((e1_max + q - 1) / q * q);
+    pv.two_step = (2ull * pv.bias + 256ull * q + 2ull * pv.e1bias < (1ull << 32)) ? 1u : 0u;
+    pv.r_inplace = r_inplace ? 1u : 0u;
+    pv.m_full = p.m;
+    pv.R = d_R;
+    pv.exc_cnt = c->d_exc_col_cnt;
+    pv.exc_rows = c->d_exc_col_rows;
+    pv.exc_cap = c->exc_cap_col;
+    pv.delta = (uint32_t)delta;
     // packed bits of R as a byte matrix [batch * m][k / 8]; a bit tile = 128 rows x 16 bytes.  Rows of the panel
     // past `rows` meet zero-filled rows of A, rows past the last instance are zero-filled by TMA.
     CUtensorMap mapBits = mapR;
     if (kBitsB && !make_map_plain_u8(c, &mapBits, d_Rbits, p.k / 8, (uint64_t)batch * p.m, 16, kTileK))
         return cudaErrorInvalidValue;
     kern<<<2 * pairs, kBitsB ? kThreadsBits : kThreads, smem_bytes, st>>>(
-        mapA, mapR, d_U, d_flags, d_E1, rows, p.n, p.k, ncols, c->mq, gw, pv_bias, pv_e1bias, mapBits, row0, p.m);
+        mapA, mapR, d_U, d_flags, rows, p.n, p.k, ncols, c->mq, gw, pv, mapBits, row0, p.m);
     c->launches++;
     return cudaGetLastError();
 }
 
 bool encaps_tc2_bits_supported(const Ctx *c, uint32_t batch)
+{
+    return encaps_tc2_supported(c, batch) && c->p.k % 128 == 0;
+}
+
+// a 128-column half tile must lie inside one instance's k columns
+bool encaps_tc2_r_inplace_supported(const Ctx *c, uint32_t batch)
 {
     return encaps_tc2_supported(c, batch) && c->p.k % 128 == 0;
 }
@@ -389,11 +461,18 @@ cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32
     return launch_pair<6, 128, kEpiStore>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
 }
 
-// N2: U = A^T R + E1 mod q with the int8 operand R already laid out in the context's operand buffer
+// N2: U = A^T R + E1 mod q; the int8 operand R is read in place (d_R) or from the copy in the context's operand buffer
 cudaError_t launch_encaps_tc2_pv(Ctx *c, const uint16_t *d_A, const int8_t *d_E1, uint16_t *d_U, uint32_t batch,
-                                 cudaStream_t st)
+                                 cudaStream_t st, const int8_t *d_R)
 {
-    return launch_pair<6, 128, kEpiStorePv>(c, d_A, d_U, nullptr, d_E1, batch, 0, c->p.m, st);
+    return launch_pair<6, 128, kEpiStorePv>(c, d_A, d_U, nullptr, d_E1, batch, 0, c->p.m, st, nullptr, d_R, d_R != nullptr);
+}
+
+// N2 on a wide context: A = the packed low-16 matrix + exception lists, U uint32
+cudaError_t launch_wide_encaps_tc2(Ctx *c, const int8_t *d_R, const int8_t *d_E1, uint32_t *d_U, uint32_t batch, cudaStream_t st)
+{
+    return launch_pair<6, 128, kEpiStorePvW>(c, c->d_A16, d_U, nullptr, d_E1, batch, 0, c->p.m, st, nullptr, d_R,
+                                             encaps_tc2_r_inplace_supported(c, batch));
 }
 
 }  // namespace lwe

@@ -61,6 +61,31 @@ keygen_prep_kernel(const uint16_t *__restrict__ s, uint16_t *__restrict__ Sx, ui
     Sx[(size_t)col * n + j] = (uint16_t)w;
 }
 
+// Wide path (q > 65536, wide.cu): the secret is a small SIGNED integer (int8), so two operand columns per instance
+// suffice for any q:  col 0: Sx[2j] = s_j, Sx[2j+1] = 0 -> D_lo = sum lo(A16) s;  col 1: Sx[2j] = 0, Sx[2j+1] = s_j ->
+// D_hi = sum hi(A16) s, with the B operand read as signed int8:  t = D_lo + 2^8 D_hi + 2^16 sum_{exceptions} s_j + e.
+__global__ void __launch_bounds__(256)
+keygen_prep_s8_kernel(const int8_t *__restrict__ s, uint16_t *__restrict__ Sx, uint32_t n, uint32_t batch)
+{
+    const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t col = blockIdx.y;
+    if (j >= n) return;
+    const uint32_t t = col >> 1;
+    uint32_t w = 0;
+    if (t < batch) {
+        const uint32_t sj = (uint8_t)s[(size_t)t * n + j];
+        w = (col & 1u) ? (sj << 8) : sj;
+    }
+    Sx[(size_t)col * n + j] = (uint16_t)w;
+}
+
+// what the wide epilogue needs beside the accumulators: the exception lists of the rows and the secrets themselves
+struct KgWide {
+    const uint32_t *row_cnt, *row_cols;
+    uint32_t cap;
+    const int8_t *s;
+};
+
 // 8 * CPI accumulator columns (= 8 instances) of this warp's 32 TMEM lanes
 template <uint32_t CPI>
 __device__ __forceinline__ void tmem_ld_8inst(uint32_t taddr, uint32_t (&r)[8 * CPI])
@@ -76,12 +101,19 @@ __device__ __forceinline__ void tmem_ld_8inst(uint32_t taddr, uint32_t (&r)[8 * 
 // SLABS: 128-byte K slabs per pipeline stage.  A TMA box is at most 128 bytes wide under SWIZZLE_128B, i.e. 128
 // separate 128-byte pieces of 128 different rows of A; loading SLABS adjacent boxes back to back makes every
 // row piece SLABS*128 contiguous bytes for the memory system.
-template <uint32_t CPI, uint32_t SLABS>
+// kWide (CPI = 2): A is the low-16 matrix of a wide context, the B operand holds signed int8 secrets, e is int8, b is
+// uint32, and the epilogue adds the 2^16-weighted exceptions of its row (see keygen_prep_s8_kernel).
+template <uint32_t CPI, uint32_t SLABS, bool kWide = false>
 __global__ void __launch_bounds__(kThreads, 1)
 keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapS,
-                 const uint16_t *__restrict__ e, uint16_t *__restrict__ b, uint32_t m, uint32_t n, uint32_t batch,
-                 uint32_t N, uint32_t stages, ModQ mq, uint32_t rps)
+                 const void *__restrict__ e_, void *__restrict__ b_, uint32_t m, uint32_t n, uint32_t batch,
+                 uint32_t N, uint32_t stages, ModQ mq, uint32_t rps, KgWide wd)
 {
+    static_assert(!kWide || CPI == 2, "the wide path uses two signed operand columns per instance");
+    const uint16_t *e = static_cast<const uint16_t *>(e_);
+    uint16_t *b = static_cast<uint16_t *>(b_);
+    const int8_t *e8 = static_cast<const int8_t *>(e_);
+    uint32_t *b32 = static_cast<uint32_t *>(b_);
     // rps = rows of A per strip (<= 128, a multiple of 8; the TMA box of A has rps rows).  The MMA is always
     // M = 128: rows rps..127 of the accumulator come from stale shared memory and are never read back.
     extern __shared__ uint8_t smem_raw[];
@@ -147,7 +179,7 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
             }
         }
     } else if (warp == 1) {
-        const uint32_t idesc = instr_desc_u8(kTileM, N, false, false);      // both operands K-major
+        const uint32_t idesc = instr_desc_u8(kTileM, N, false, false, kWide);   // both operands K-major; wide: signed S
         uint32_t stage = 0, phase = 0, it = 0;
         for (uint32_t t = blockIdx.x; t < strips; t += gridDim.x, it++) {
             const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
@@ -191,7 +223,10 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
             // per CTA nothing else hides the epilogue, and 4 rounds of dependent global loads were ~4 us of 56
             uint32_t epre[32];
 #pragma unroll
-            for (uint32_t x = 0; x < 32; x++) epre[x] = (row_ok && x < batch) ? (uint32_t)__ldg(e + (size_t)x * m + i) : 0u;
+            for (uint32_t x = 0; x < 32; x++)
+                epre[x] = (row_ok && x < batch) ? (kWide ? (uint32_t)(int)__ldg(e8 + (size_t)x * m + i)
+                                                         : (uint32_t)__ldg(e + (size_t)x * m + i)) : 0u;
+            const uint32_t exc = (kWide && row_ok) ? min(__ldg(wd.row_cnt + i), wd.cap) : 0u;
             mbar_wait(tfull_bar(acc), acc_phase);
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((quarter * 32) << 16) + acc * acc_cols;
@@ -206,6 +241,15 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
                     for (uint32_t x = 0; x < 8; x++) {
                         const uint32_t inst = i0 + x;
                         if (inst < batch) {
+                            if (kWide) {
+                                const int ei = (i0 < 32) ? (int)epre[(i0 + x) & 31] : (int)e8[(size_t)inst * m + i];
+                                long long tot = (long long)(int)r[2 * x] + 256ll * (int)r[2 * x + 1] + ei;
+                                for (uint32_t y = 0; y < exc; y++)         // elements >= 2^16 of this row: rare
+                                    tot += 65536ll * (int)wd.s[(size_t)inst * n + wd.row_cols[(size_t)i * wd.cap + y]];
+                                long long rr = tot % (long long)mq.q;
+                                b32[(size_t)inst * m + i] = (uint32_t)(rr < 0 ? rr + mq.q : rr);
+                                continue;
+                            }
                             const uint32_t ei = (i0 < 32) ? epre[(i0 + x) & 31] : (uint32_t)e[(size_t)inst * m + i];
                             uint32_t o;
                             if (CPI == 2) {
@@ -246,6 +290,10 @@ uint32_t padded_cols(uint32_t batch, uint32_t cpi) { return (((batch + 7u) & ~7u
 
 size_t keygen_tc_workspace_bytes(const lwe_params &p)
 {
+    if (p.q > 65536u) {                                                 // wide context: two signed columns per instance
+        const uint32_t Nw = padded_cols(p.max_batch, 2);
+        return (p.n <= 65536 && Nw <= 256) ? (size_t)Nw * 2 * p.n : 0;
+    }
     const uint32_t N = padded_cols(p.max_batch, cols_per_inst(p));
     return (p.n <= 32768 && N <= 256) ? (size_t)N * 2 * p.n : 0;       // 0: the tensor-core keygen is not available
 }
@@ -288,8 +336,8 @@ cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, c
     uint32_t stages = kSmemBudget / bytes_stage;
     if (stages > kMaxStages) stages = kMaxStages;
     const uint32_t smem = stages * bytes_stage + 1024 + 256;
-    typedef void (*Kern)(const CUtensorMap, const CUtensorMap, const uint16_t *, uint16_t *, uint32_t, uint32_t, uint32_t,
-                         uint32_t, uint32_t, ModQ, uint32_t);
+    typedef void (*Kern)(const CUtensorMap, const CUtensorMap, const void *, void *, uint32_t, uint32_t, uint32_t,
+                         uint32_t, uint32_t, ModQ, uint32_t, KgWide);
     static const Kern table[3][2] = {{keygen_tc_kernel<2, 1>, keygen_tc_kernel<2, 2>},
                                      {keygen_tc_kernel<3, 1>, keygen_tc_kernel<3, 2>},
                                      {keygen_tc_kernel<4, 1>, keygen_tc_kernel<4, 2>}};
@@ -299,7 +347,52 @@ cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, c
     const uint32_t strips = (p.m + rps - 1) / rps;
     const uint32_t grid = strips < (uint32_t)c->sm_count ? strips : (uint32_t)c->sm_count;
     ProfScope prof(c, LWE_K_KEYGEN_TC, st);
-    kern<<<grid, kThreads, smem, st>>>(mapA, mapS, d_e, d_b, p.m, p.n, batch, N, stages, c->mq, rps);
+    kern<<<grid, kThreads, smem, st>>>(mapA, mapS, d_e, d_b, p.m, p.n, batch, N, stages, c->mq, rps, KgWide{});
+    c->launches++;
+    return cudaGetLastError();
+}
+
+// ---- wide path: t = A s + e on uint32 residues, A = the context's packed matrix (wide.cu)
+bool wide_keygen_tc_supported(const Ctx *c, uint32_t batch)
+{
+    // |D| <= 255 * 128 * n < 2^31 for n <= 65536
+    return c->encode_tiled != nullptr && c->d_Sx != nullptr && c->p.n <= 65536 && padded_cols(batch, 2) <= 256 &&
+           padded_cols(c->p.max_batch, 2) <= 256;
+}
+
+cudaError_t launch_wide_keygen_tc(Ctx *c, const int8_t *d_s, const int8_t *d_e, uint32_t *d_t, uint32_t batch, cudaStream_t st)
+{
+    const lwe_params &p = c->p;
+    const uint32_t N = padded_cols(batch, 2);
+    {
+        ProfScope prof(c, LWE_K_KEYGEN_PREP, st);
+        dim3 grid((p.n + 255) / 256, N);
+        keygen_prep_s8_kernel<<<grid, 256, 0, st>>>(d_s, reinterpret_cast<uint16_t *>(c->d_Sx), p.n, batch);
+        c->launches++;
+        cudaError_t err = cudaGetLastError();
+        if (err != cudaSuccess) return err;
+    }
+    CUtensorMap mapA, mapS;
+    const uint32_t waves = (p.m + kTileM * (uint32_t)c->sm_count - 1) / (kTileM * (uint32_t)c->sm_count);
+    uint32_t rps = ((p.m + waves * (uint32_t)c->sm_count - 1) / (waves * (uint32_t)c->sm_count) + 7u) & ~7u;
+    if (rps > kTileM) rps = kTileM;
+    if (rps < 8) rps = 8;
+    if (!make_map_u8(c, &mapA, c->d_A16, 2ull * p.n, p.m, rps)) return cudaErrorInvalidValue;
+    if (!make_map_u8(c, &mapS, c->d_Sx, 2ull * p.n, N, N)) return cudaErrorInvalidValue;
+    const uint32_t bytes_slab = kBytesA + N * kTileK;
+    const uint32_t slabs = (3 * 2 * bytes_slab <= kSmemBudget) ? 2 : 1;
+    const uint32_t bytes_stage = slabs * bytes_slab;
+    uint32_t stages = kSmemBudget / bytes_stage;
+    if (stages > kMaxStages) stages = kMaxStages;
+    const uint32_t smem = stages * bytes_stage + 1024 + 256;
+    auto kern = slabs == 2 ? keygen_tc_kernel<2, 2, true> : keygen_tc_kernel<2, 1, true>;
+    cudaError_t perr = kernel_prepare(c, kern, smem);
+    if (perr != cudaSuccess) return perr;
+    const uint32_t strips = (p.m + rps - 1) / rps;
+    const uint32_t grid = strips < (uint32_t)c->sm_count ? strips : (uint32_t)c->sm_count;
+    ProfScope prof(c, LWE_K_KEYGEN_TC, st);
+    const KgWide wd = {c->d_exc_row_cnt, c->d_exc_row_cols, c->exc_cap_row, d_s};
+    kern<<<grid, kThreads, smem, st>>>(mapA, mapS, d_e, d_t, p.m, p.n, batch, N, stages, c->mq, rps, wd);
     c->launches++;
     return cudaGetLastError();
 }

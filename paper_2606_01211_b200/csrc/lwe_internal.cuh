@@ -105,6 +105,19 @@ struct Ctx {
     uint32_t *d_foflags;              // [max_batch] mismatch flags of the FO re-encryption check
     uint16_t *d_vprime;               // [max_batch][k] re-encrypted v'
     uint32_t *d_tile_locks;           // [2 * n/64] per-tile lock + arrival count of the fused regenerated-A encaps
+    // wide contexts (q > 65536: Table 1's q = 65537 rows): the public matrix held by the context, packed by
+    // lwe_wide_load_matrix -- its low 16 bits as a uint16 matrix the tensor kernels read exactly like a narrow A, and the
+    // few elements >= 2^16 as per-column and per-row exception lists (slot lists of fixed capacity)
+    uint32_t wide;                    // 1 if q > 65536
+    uint32_t A_loaded;                // lwe_wide_load_matrix has completed on this context
+    uint16_t *d_A16;                  // [m][n] low 16 bits of A
+    uint32_t exc_cap_col, exc_cap_row;// slots per column / per row
+    uint32_t *d_exc_col_cnt;          // [n] elements >= 2^16 in column j (may exceed the capacity: overflow)
+    uint32_t *d_exc_col_rows;         // [n][exc_cap_col] their row indices
+    uint32_t *d_exc_row_cnt;          // [m]
+    uint32_t *d_exc_row_cols;         // [m][exc_cap_row] their column indices
+    uint32_t *d_exc_overflow;         // [1] set by the pack kernel when a slot list is full
+    uint32_t *h_exc_overflow;         // pinned host copy read by lwe_wide_load_matrix
     // staging for lwe_kem_host
     uint16_t *d_hs, *d_he, *d_hb, *d_hU, *d_hv;
     uint8_t *d_hR, *d_hmu, *d_hmuout;
@@ -221,10 +234,28 @@ cudaError_t launch_sample_cuniform(Ctx *c, int8_t *d_out, uint64_t first, uint64
                                    uint32_t inst0, uint32_t n_inst, uint32_t bound, cudaStream_t st);
 cudaError_t launch_prep_R_pv_and_v(Ctx *c, const uint16_t *d_t, const int8_t *d_R, const int8_t *d_e2,
                                    const uint8_t *d_mubits, uint16_t *d_v, uint32_t batch, bool write_Rexp, cudaStream_t st);
+// d_R != NULL (needs k % 128 == 0): the B operand is read in place from the caller's int8 R [batch][m][k]; NULL: from
+// the operand copy in c->d_Rexp
+bool encaps_tc2_r_inplace_supported(const Ctx *c, uint32_t batch);
 cudaError_t launch_encaps_tc2_pv(Ctx *c, const uint16_t *d_A, const int8_t *d_E1, uint16_t *d_U, uint32_t batch,
-                                 cudaStream_t st);
+                                 cudaStream_t st, const int8_t *d_R = nullptr);
 cudaError_t launch_encaps_pv_simt(Ctx *c, const uint16_t *d_A, const int8_t *d_R, const int8_t *d_E1, uint16_t *d_U,
                                   uint32_t batch, cudaStream_t st);
+// wide path (q > 65536), wide.cu / rng_kernels.cu / keygen_tc.cu / encaps_tc2.cu
+cudaError_t launch_sample_uniform32(Ctx *c, uint32_t *d_out, uint64_t first, uint64_t count, const AesKey &key, uint32_t tag,
+                                    uint32_t inst0, uint32_t n_inst, cudaStream_t st);
+cudaError_t launch_sample_cbd_s8(Ctx *c, int8_t *d_out, uint64_t first, uint64_t count, const AesKey &key, uint32_t tag,
+                                 uint32_t inst0, uint32_t n_inst, cudaStream_t st);
+cudaError_t launch_wide_pack(Ctx *c, const uint32_t *d_A, uint32_t row0, uint32_t rows, cudaStream_t st);
+cudaError_t launch_wide_keygen_simt(Ctx *c, const int8_t *d_s, const int8_t *d_e, uint32_t *d_t, uint32_t batch, cudaStream_t st);
+bool wide_keygen_tc_supported(const Ctx *c, uint32_t batch);
+cudaError_t launch_wide_keygen_tc(Ctx *c, const int8_t *d_s, const int8_t *d_e, uint32_t *d_t, uint32_t batch, cudaStream_t st);
+cudaError_t launch_wide_v(Ctx *c, const uint32_t *d_t, const int8_t *d_R, const int8_t *d_e2, const uint8_t *d_mubits,
+                          uint32_t *d_v, uint32_t batch, bool write_Rexp, cudaStream_t st);
+cudaError_t launch_wide_encaps_simt(Ctx *c, const int8_t *d_R, const int8_t *d_E1, uint32_t *d_U, uint32_t batch, cudaStream_t st);
+cudaError_t launch_wide_encaps_tc2(Ctx *c, const int8_t *d_R, const int8_t *d_E1, uint32_t *d_U, uint32_t batch, cudaStream_t st);
+cudaError_t launch_wide_decaps(Ctx *c, const uint32_t *d_U, const uint32_t *d_v, const int8_t *d_s, uint8_t *d_out,
+                               uint32_t batch, cudaStream_t st);
 cudaError_t launch_fo_verdict(Ctx *c, const uint16_t *d_v, const uint16_t *d_vprime, const uint32_t *d_flags,
                               uint8_t *d_ok, uint32_t batch, cudaStream_t st);
 cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,

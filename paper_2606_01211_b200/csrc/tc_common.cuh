@@ -214,7 +214,9 @@ __host__ __device__ constexpr uint32_t instr_desc_u8(uint32_t M, uint32_t N, boo
 //                ever materialising c'.
 //   kEpiStorePv: the paper's own Encrypt (N2): the B operand is signed (Gaussian r), the accumulators are signed,
 //                and E1[j][c] is added before the reduction: U = A^T R + E1 mod q.
-enum EpiMode { kEpiStore = 0, kEpiAccum = 1, kEpiCompare = 2, kEpiStorePv = 3 };
+//   kEpiStorePvW: the same on a wide context (q > 65536, wide.cu): A is the low-16 matrix, the elements >= 2^16 of
+//                column j come from its exception list (2^16 R[i][c] each), U is written as uint32.
+enum EpiMode { kEpiStore = 0, kEpiAccum = 1, kEpiCompare = 2, kEpiStorePv = 3, kEpiStorePvW = 4 };
 
 template <int kMode>
 __device__ __forceinline__ bool store_u16x16(uint4 *dst, uint32_t (&o)[16], const ModQ &mq)

@@ -1,0 +1,401 @@
+"""GPU parity of the wide path (S8(f) N2 on Table 1's q = 65537 rows): uint32 residues, int8 small objects,
+the public matrix packed into a low-16 matrix + exception lists (lwe_wide_load_matrix), KeyGen / Encrypt on tcgen05 and on
+CUDA cores, Decrypt -- every output against the oracle's O4w / O5s / O7w / O14w / O9w, bit for bit, through the C ABI.
+Moduli: 65537 (the paper's), 65539 and 66560 (elements >= 2^16 whose low half is not zero, and a list density of
+1.5 %: cases q = 65537 cannot reach)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle as O  # noqa: E402
+from paper_2606_01211_b200 import workloads as W  # noqa: E402
+
+F4 = 65537
+
+
+@pytest.fixture(scope="module")
+def H():
+    import gpu_helpers
+    return gpu_helpers
+
+
+def B():
+    from paper_2606_01211_b200 import binding
+    return binding
+
+
+def T():
+    import torch
+    return torch
+
+
+def dev32(a):
+    return T().from_numpy(np.ascontiguousarray(a, dtype=np.uint32).view(np.int32)).cuda()
+
+
+def dev8(a):
+    return T().from_numpy(np.ascontiguousarray(a, dtype=np.int8)).cuda()
+
+
+def empty32(*shape):
+    return T().empty(*shape, dtype=T().int32, device="cuda")
+
+
+def empty8(*shape):
+    return T().empty(*shape, dtype=T().int8, device="cuda")
+
+
+def host32(t):
+    T().cuda.synchronize()
+    return t.cpu().numpy().view(np.uint32)
+
+
+def host8(t):
+    T().cuda.synchronize()
+    return t.cpu().numpy()
+
+
+def random_A(m, n, q, seed, extra_big=0):
+    rng = np.random.default_rng(seed)
+    A = rng.integers(0, q, (m, n), dtype=np.uint64).astype(np.uint32)
+    if extra_big:                                          # sprinkle elements >= 2^16 (all of them for q = 65537: 65536)
+        idx = rng.integers(0, m * n, extra_big)
+        A.ravel()[idx] = rng.integers(65536, q, extra_big, dtype=np.uint64).astype(np.uint32)
+    return A
+
+
+# ---------------------------------------------------------------- samplers
+
+@pytest.mark.parametrize("q", [F4, 65539, 66560])
+@pytest.mark.parametrize("first,count,n_inst", [(0, 4096, 1), (40, 1000, 3), (4, 13, 2), (0, 1 << 16, 2)])
+def test_uniform_u32_matches_oracle(q, first, count, n_inst):
+    seed, inst0 = 19, 3
+    with B().Context(64, 64, 256, q, 3, 1) as c:
+        out = empty32(n_inst, count)
+        c.sample_uniform_u32(out, first, count, seed, W.TAG_A, inst0, n_inst)
+        g = host32(out)
+    for t in range(n_inst):
+        assert np.array_equal(g[t], O.sample_uniform32(first, count, seed, O.TAG_A, inst0 + t, q)), t
+    assert g.max() < q
+
+
+@pytest.mark.parametrize("eta", [1, 3, 8])
+def test_cbd_s8_matches_oracle(eta):
+    seed, inst0, n_inst, first, count = 7, 2, 3, 16, 3001
+    with B().Context(64, 64, 256, F4, eta, 1) as c:
+        out = empty8(n_inst, count)
+        c.sample_cbd_s8(out, first, count, seed, W.TAG_S, inst0, n_inst)
+        g = host8(out)
+    for t in range(n_inst):
+        assert np.array_equal(g[t], O.sample_cbd_s8(first, count, seed, O.TAG_S, inst0 + t, eta)), t
+
+
+# ---------------------------------------------------------------- KeyGen
+
+WIDE_KEYGEN_SHAPES = [  # (m, n, q, batch, extra elements >= 2^16)
+    (512, 256, F4, 1, 0), (512, 256, F4, 4, 300), (264, 4096, 65539, 5, 200), (136, 4104, 66560, 2, 0),
+    (1000, 40, F4, 3, 50), (8, 8, F4, 1, 3), (2048, 1024, F4, 32, 500), (640, 520, 65539, 33, 100),
+    (384, 1024, 66560, 64, 0), (256, 20000, F4, 9, 400),
+]
+
+
+@pytest.mark.parametrize("path", [2, 1], ids=["tcgen05", "simt"])
+@pytest.mark.parametrize("m,n,q,batch,big", WIDE_KEYGEN_SHAPES)
+def test_wide_keygen_matches_oracle(path, m, n, q, batch, big):
+    rng = np.random.default_rng(m + n)
+    A = random_A(m, n, q, 11, big)
+    s = rng.integers(-3, 4, (batch, n)).astype(np.int8)
+    e = rng.integers(-12, 13, (batch, m)).astype(np.int8)
+    with B().Context(n, m, 256, q, 3, batch) as c:
+        c.wide_load_matrix(dev32(A))
+        c.set_option(B().OPT_KEYGEN_PATH, path)
+        t = empty32(batch, m)
+        t.fill_(-1)
+        c.wide_keygen(dev8(s), dev8(e), t, batch)
+        g = host32(t)
+    check = range(batch) if m * n * batch <= (1 << 24) else (0, batch // 2, batch - 1)
+    for b in check:
+        assert np.array_equal(g[b], O.keygen_w(A, s[b], e[b], q)), (m, n, q, b)
+
+
+def test_wide_keygen_extreme_values():
+    """A = q - 1 in its low half's maximum (65535) and |s| = 127: every byte product and both plane accumulators at
+    their bounds at n = 65536, the path's limit; then the same with the sign flipped"""
+    m, batch = 128, 2
+    for q, n in ((F4, 65536), (66560, 16384)):
+        for sign in (1, -1):
+            A = np.full((m, n), 65535, np.uint32)
+            A[:, :3] = q - 1                                 # three exceptions per row
+            s = np.full((batch, n), 127 * sign, np.int8)
+            e = np.full((batch, m), -128 if sign < 0 else 127, np.int8)
+            with B().Context(n, m, 256, q, 3, batch) as c:
+                c.wide_load_matrix(dev32(A))
+                c.set_option(B().OPT_KEYGEN_PATH, 2)
+                t = empty32(batch, m)
+                c.wide_keygen(dev8(s), dev8(e), t, batch)
+                g = host32(t)
+            want = (((n - 3) * 65535 + 3 * (q - 1)) * 127 * sign + (-128 if sign < 0 else 127)) % q
+            assert np.all(g == want), (q, n, sign)
+
+
+def test_wide_load_refuses_what_it_cannot_hold():
+    """a matrix with more elements >= 2^16 in a column than the slot lists hold -> LWE_ERR_UNSUPPORTED at load time
+    (never a wrong result); an element >= q -> LWE_ERR_PARAM; using the context without a matrix -> LWE_ERR_PARAM"""
+    m = n = 256
+    with B().Context(n, m, 256, F4, 3, 1) as c:
+        t = empty32(1, m)
+        with pytest.raises(B().LweError) as ei:
+            c.wide_keygen(empty8(1, n), empty8(1, m), t, 1)
+        assert ei.value.code == -1
+        A = np.full((m, n), 65536, np.uint32)                # 2^16 = -1 everywhere: 256 exceptions per column
+        with pytest.raises(B().LweError) as ei:
+            c.wide_load_matrix(dev32(A))
+        assert ei.value.code == -5
+        with pytest.raises(B().LweError) as ei:              # ... and the context holds no matrix afterwards
+            c.wide_keygen(empty8(1, n), empty8(1, m), t, 1)
+        assert ei.value.code == -1
+        A = random_A(m, n, F4, 5)
+        A[7, 9] = F4
+        with pytest.raises(B().LweError) as ei:
+            c.wide_load_matrix(dev32(A))
+        assert ei.value.code == -1
+        A[7, 9] = 65536
+        c.wide_load_matrix(dev32(A))                              # fine now
+        s, e = np.ones((1, n), np.int8), np.zeros((1, m), np.int8)
+        c.wide_keygen(dev8(s), dev8(e), t, 1)
+        assert np.array_equal(host32(t)[0], O.keygen_w(A, s[0], e[0], F4))
+    # the narrow entry points do not exist on a wide context, and vice versa
+    with B().Context(64, 64, 256, F4, 3, 1) as c:
+        with pytest.raises(B().LweError) as ei:
+            c.sample_uniform(T().empty(64, dtype=T().int16, device="cuda"), 0, 64, 1, W.TAG_A)
+        assert ei.value.code == -5
+    with B().Context(64, 64, 256, 12289, 3, 1) as c:
+        with pytest.raises(B().LweError) as ei:
+            c.sample_uniform_u32(empty32(64), 0, 64, 1, W.TAG_A)
+        assert ei.value.code == -5
+
+
+# ---------------------------------------------------------------- Encrypt
+
+WIDE_ENCAPS_SHAPES = [  # (n = m, k, q, batch, extra big)
+    (256, 256, F4, 1, 0), (192, 256, F4, 3, 100), (200, 128, 65539, 3, 60), (456, 256, 66560, 5, 0),
+    (1280, 256, F4, 2, 300), (64, 16, F4, 2, 10), (136, 384, F4, 3, 40), (520, 64, 65539, 5, 80), (264, 512, F4, 2, 50),
+]
+
+
+@pytest.mark.parametrize("path", [0, 1], ids=["tcgen05_pair", "simt"])
+@pytest.mark.parametrize("n,k,q,batch,big", WIDE_ENCAPS_SHAPES)
+def test_wide_encaps_matches_oracle(path, n, k, q, batch, big):
+    rng = np.random.default_rng(n + k)
+    m = n
+    A = random_A(m, n, q, 71, big)
+    t = rng.integers(0, q, (batch, m), dtype=np.uint64).astype(np.uint32)
+    R = rng.integers(-12, 13, (batch, m, k)).astype(np.int8)
+    E1 = rng.integers(-12, 13, (batch, n, k)).astype(np.int8)
+    e2 = rng.integers(-3, 4, (batch, k)).astype(np.int8)
+    mubits = W.random_bytes(batch * k // 8, 73).reshape(batch, -1)
+    with B().Context(n, m, k, q, 3, batch) as c:
+        c.wide_load_matrix(dev32(A))
+        c.set_option(B().OPT_ENCAPS_PATH, path)
+        U, v = empty32(batch, n, k), empty32(batch, k)
+        U.fill_(-1)
+        for _ in range(2):                                   # twice: the workspace is left clean
+            c.wide_encaps(dev32(t), dev8(R), dev8(E1), dev8(e2), T().from_numpy(mubits).cuda(), U, v, batch)
+        gU, gv = host32(U), host32(v)
+    for b in range(batch):
+        Uo, vo = O.encaps_pv_w(A, t[b], R[b], E1[b], e2[b], mubits[b], q)
+        assert np.array_equal(gv[b], vo), ("v", b)
+        bad = np.argwhere(gU[b] != Uo)
+        assert bad.size == 0, (f"U mismatch inst {b}: {len(bad)} entries, first {bad[:5].tolist()}")
+
+
+@pytest.mark.parametrize("path", [0, 1], ids=["tcgen05_pair", "simt"])
+def test_wide_encaps_extreme_accumulators(path):
+    """|R| = 127, A's low half = 65535, m = 65536 (the path's limit): both signed byte-plane accumulators at
+    +/- 255*127*65536, every column with exceptions, the two- and three-reduction recombinations at their bounds"""
+    m, n_small, k, batch = 65536, 64, 256, 1
+    for q in (F4, 66560):
+        for sign in (1, -1):
+            A = np.full((m, n_small), 65535, np.uint32)
+            A[:5, :] = q - 1                                 # five exceptions in every column
+            t = np.full((batch, m), q - 1, np.uint32)
+            R = np.full((batch, m, k), 127 * sign, np.int8)
+            E1 = np.full((batch, n_small, k), -128 if sign < 0 else 127, np.int8)
+            e2 = np.full((batch, k), 3 * sign, np.int8)
+            mubits = np.full((batch, k // 8), 0xFF, np.uint8)
+            with B().Context(n_small, m, k, q, 3, batch) as c:
+                c.wide_load_matrix(dev32(A))
+                c.set_option(B().OPT_ENCAPS_PATH, path)
+                U, v = empty32(batch, n_small, k), empty32(batch, k)
+                c.wide_encaps(dev32(t), dev8(R), dev8(E1), dev8(e2), T().from_numpy(mubits).cuda(), U, v, batch)
+                gU, gv = host32(U), host32(v)
+            e1 = -128 if sign < 0 else 127
+            assert np.all(gU == (((m - 5) * 65535 + 5 * (q - 1)) * 127 * sign + e1) % q), (q, sign)
+            assert np.all(gv == (m * (q - 1) * 127 * sign + 3 * sign + q // 2) % q), (q, sign)
+
+
+# ---------------------------------------------------------------- Decrypt
+
+@pytest.mark.parametrize("n,k,q,batch", [(256, 256, F4, 1), (1000, 256, 65539, 3), (64, 8, F4, 2), (4096, 128, 66560, 2),
+                                          (8192, 256, F4, 4), (136, 512, F4, 2), (72, 384, F4, 3), (8, 1024, F4, 1)])
+def test_wide_decaps_matches_oracle(n, k, q, batch):
+    rng = np.random.default_rng(n * k)
+    U = rng.integers(0, q, (batch, n, k), dtype=np.uint64).astype(np.uint32)
+    U[:, 0, :] = q - 1
+    v = rng.integers(0, q, (batch, k), dtype=np.uint64).astype(np.uint32)
+    s = rng.integers(-3, 4, (batch, n)).astype(np.int8)
+    with B().Context(n, 8, k, q, 3, batch) as c:
+        out = T().empty(batch, k // 8, dtype=T().uint8, device="cuda")
+        for _ in range(2):
+            out.fill_(0xEE)
+            c.wide_decaps(dev32(U), dev32(v), dev8(s), out, batch)
+            got = host8(out)
+            for b in range(batch):
+                assert np.array_equal(got[b], O.decaps_w(U[b], v[b], s[b], q)), (n, k, q, b)
+
+
+def test_wide_decaps_extremes_and_rounding_boundaries():
+    """|s| = 127 with U = q - 1 over n = 65536 rows (the 32-bit partial sums between flushes at their bound), and
+    U = 0, v = d swept over the decision boundaries of q = 65537"""
+    q, k = F4, 256
+    n = 65536
+    for sign in (1, -1):
+        U = np.full((1, n, k), q - 1, np.uint32)
+        s = np.full((1, n), 127 * sign, np.int8)
+        v = np.arange(k, dtype=np.uint32)[None, :] * 257 % q
+        with B().Context(n, 8, k, q, 3, 1) as c:
+            out = T().empty(1, k // 8, dtype=T().uint8, device="cuda")
+            c.wide_decaps(dev32(U), dev32(v), dev8(s), out, 1)
+            assert np.array_equal(host8(out)[0], O.decaps_w(U[0], v[0], s[0], q))
+    n = 8
+    edges = [0, 1, q // 4 - 1, q // 4, q // 4 + 1, q // 2, 3 * q // 4 - 1, 3 * q // 4, 3 * q // 4 + 1, q - 1]
+    v = np.array([(edges * 26)[:k]], np.uint32)
+    with B().Context(n, 8, k, q, 3, 1) as c:
+        out = T().empty(1, k // 8, dtype=T().uint8, device="cuda")
+        c.wide_decaps(dev32(np.zeros((1, n, k), np.uint32)), dev32(v), dev8(np.ones((1, n), np.int8)), out, 1)
+        got = np.unpackbits(host8(out)[0], bitorder="little")[:k]
+    want = np.array([1 if (4 * int(d) >= q and 4 * int(d) < 3 * q) else 0 for d in v[0]])
+    assert np.array_equal(got, want)
+
+
+# ---------------------------------------------------------------- whole path from seeds
+
+def device_pke(c, n, k, sigma, kappa, seed, inst0, batch):
+    torch = T()
+    s, e = empty8(batch, n), empty8(batch, n)
+    R, E1, e2 = empty8(batch, n, k), empty8(batch, n, k), empty8(batch, k)
+    mu = torch.empty(batch, k // 8, dtype=torch.uint8, device="cuda")
+    out = torch.empty(batch, k // 8, dtype=torch.uint8, device="cuda")
+    t, U, v = empty32(batch, n), empty32(batch, n, k), empty32(batch, k)
+    c.sample_cbd_s8(s, 0, n, seed, W.TAG_S, inst0, batch)
+    c.sample_gauss_s8(e, 0, n, seed, W.TAG_E, inst0, batch, sigma)
+    c.sample_gauss_s8(R, 0, n * k, seed, W.TAG_RG, inst0, batch, sigma)
+    c.sample_gauss_s8(E1, 0, n * k, seed, W.TAG_E1, inst0, batch, sigma)
+    c.sample_cuniform_s8(e2, 0, k, seed, W.TAG_E2, inst0, batch, kappa)
+    c.sample_bits(mu, 0, k, seed, W.TAG_MU, inst0, batch)
+    c.wide_keygen(s, e, t, batch)
+    c.wide_encaps(t, R, E1, e2, mu, U, v, batch)
+    c.wide_decaps(U, v, s, out, batch)
+    return dict(s=s, e=e, R=R, E1=E1, e2=e2, mu=mu, out=out, t=t, U=U, v=v)
+
+
+def oracle_draw(n, k, sigma, kappa, seed, inst):
+    s = O.sample_cbd_s8(0, n, seed, O.TAG_S, inst, 3)
+    e = O.sample_gauss(0, n, seed, O.TAG_E, inst, sigma)
+    R = O.sample_gauss(0, n * k, seed, O.TAG_RG, inst, sigma).reshape(n, k)
+    E1 = O.sample_gauss(0, n * k, seed, O.TAG_E1, inst, sigma).reshape(n, k)
+    e2 = O.sample_cuniform(0, k, seed, O.TAG_E2, inst, kappa)
+    mu = O.sample_bits(0, k, seed, O.TAG_MU, inst)
+    return s, e, R, E1, e2, mu
+
+
+def noise_identity(U, v, s, e, R, E1, e2, mubits, q):
+    k = v.size
+    mub = np.unpackbits(mubits, bitorder="little")[:k].astype(np.int64)
+    ss = s.astype(np.int64)
+    Us = U.astype(np.int64).T @ ss                             # exact in int64
+    lhs = (v.astype(np.int64) - Us - mub * (q // 2)) % q
+    rhs = (e.astype(np.int64) @ R.astype(np.int64) + e2.astype(np.int64) - ss @ E1.astype(np.int64)) % q
+    return np.array_equal(lhs, rhs)
+
+
+def test_wide_full_path_small_matches_oracle_everywhere():
+    """n = 1024, q = 65537 with Table 1's sigma = 1.2, kappa = 2: every object drawn on the device from the seed, every
+    output against the oracle's own draw, stored and seeded load of A give the same results"""
+    n, q, sigma, kappa, k, seed, inst0, batch = 1024, F4, 1.2, 2, 256, 33, 4, 3
+    with B().Context(n, n, k, q, 3, batch) as c:
+        dA = empty32(n, n)
+        c.sample_uniform_u32(dA, 0, n * n, seed, W.TAG_A)
+        c.wide_load_matrix(dA)
+        g = device_pke(c, n, k, sigma, kappa, seed, inst0, batch)
+        got = {name: (host32(x) if x.dtype == T().int32 else host8(x)) for name, x in g.items()}
+        gA = host32(dA)
+        c.wide_load_matrix_seeded(seed)
+        g2 = device_pke(c, n, k, sigma, kappa, seed, inst0, batch)
+        T().cuda.synchronize()
+        assert T().equal(g["t"], g2["t"]) and T().equal(g["U"], g2["U"]) and T().equal(g["v"], g2["v"])
+    A = O.sample_uniform32(0, n * n, seed, O.TAG_A, 0, q).reshape(n, n)
+    assert np.array_equal(gA, A)
+    for b in range(batch):
+        s, e, R, E1, e2, mu = oracle_draw(n, k, sigma, kappa, seed, inst0 + b)
+        assert np.array_equal(got["s"][b], s) and np.array_equal(got["e"][b], e)
+        assert np.array_equal(got["R"][b], R) and np.array_equal(got["E1"][b], E1) and np.array_equal(got["e2"][b], e2)
+        t = O.keygen_w(A, s, e, q)
+        U, v = O.encaps_pv_w(A, t, R, E1, e2, mu, q)
+        assert np.array_equal(got["t"][b], t)
+        assert np.array_equal(got["U"][b], U) and np.array_equal(got["v"][b], v)
+        assert np.array_equal(got["out"][b], O.decaps_w(U, v, s, q))
+        assert np.array_equal(got["out"][b], mu), "not every bit recovered"
+
+
+@pytest.mark.parametrize("n,batch,seeded", [(8192, 32, False), (16384, 8, True)])
+def test_table1_rows_n8192_n16384_sampled_rows_identity_and_recovery(n, batch, seeded):
+    """Table 1 rows 5-6 (q = 65537, sigma = 1.2, e2 in [-2, 2], eta = 3) at full size in the launch
+    configuration bench.py times (n = 8192: 32 instances sharing A).  n = 8192: the oracle draws all of A, so t and v
+    are compared in full and 40 sampled rows of U x all 256 columns element by element, on two instances.  n = 16384:
+    A is loaded on the device from its seed panel by panel (the uint32 matrix, 1 GiB, never exists) and the oracle
+    recomputes 48 sampled rows of t (rows of A are contiguous stream ranges) and 40 sampled rows of U (columns of A
+    drawn by counter index).  On the first, a middle and the last instance the exact noise identity over all columns
+    ties v to U, s, e, R, E1, e2; every bit of every instance is recovered."""
+    q, sigma, kappa, k, seed, inst0 = F4, 1.2, 2, 256, 8, 16
+    rng = np.random.default_rng(n)
+    trows = np.unique(np.concatenate([[0, 1, n - 1], rng.integers(0, n, 45)]))
+    urows = np.unique(np.concatenate([[0, 1, 63, 64, n - 1], rng.integers(0, n, 35)]))
+    with B().Context(n, n, k, q, 3, batch) as c:
+        if seeded:
+            c.wide_load_matrix_seeded(seed)
+        else:
+            dA = empty32(n, n)
+            c.sample_uniform_u32(dA, 0, n * n, seed, W.TAG_A)
+            c.wide_load_matrix(dA)
+            del dA
+        g = device_pke(c, n, k, sigma, kappa, seed, inst0, batch)
+        T().cuda.synchronize()
+        assert T().equal(g["out"], g["mu"]), "not every bit of every instance recovered"
+        check = sorted({0, batch // 2, batch - 1})
+        got = {name: {b: (host32(x[b]) if x.dtype == T().int32 else host8(x[b])) for b in check} for name, x in g.items()}
+    if n <= 8192:
+        A = O.sample_uniform32(0, n * n, seed, O.TAG_A, 0, q).reshape(n, n)
+        A_rows, A_cols = A[trows], np.ascontiguousarray(A[:, urows])
+    else:
+        A = None
+        A_rows = np.stack([O.sample_uniform32(int(i) * n, n, seed, O.TAG_A, 0, q) for i in trows])
+        A_cols = np.stack([O.sample_uniform32_strided(int(j), n, n, seed, O.TAG_A, 0, q) for j in urows], axis=1)
+    for b in check:
+        s, e, R, E1, e2, mu = oracle_draw(n, k, sigma, kappa, seed, inst0 + b)
+        assert np.array_equal(got["s"][b], s) and np.array_equal(got["e"][b], e) and np.array_equal(got["mu"][b], mu)
+        assert np.array_equal(got["R"][b], R) and np.array_equal(got["E1"][b], E1) and np.array_equal(got["e2"][b], e2)
+        assert noise_identity(got["U"][b], got["v"][b], s, e, R, E1, e2, mu, q), b
+        assert np.array_equal(got["out"][b], mu)
+        if b == check[1]:
+            continue
+        if A is not None:
+            t = O.keygen_w(A, s, e, q)
+            assert np.array_equal(got["t"][b], t), b
+            Uo, vo = O.encaps_pv_w(A_cols, t, R, E1[urows], e2, mu, q)
+            assert np.array_equal(got["v"][b], vo), b
+        else:
+            assert np.array_equal(got["t"][b][trows], O.keygen_w(A_rows, s, e[trows], q)), b
+            Uo, _ = O.encaps_pv_w(A_cols, np.zeros(n, np.uint32), R, E1[urows], e2, mu, q)
+        assert np.array_equal(got["U"][b][urows], Uo), b
