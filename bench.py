@@ -499,12 +499,68 @@ def paper_variant_phase(B, device: int) -> dict:
 
         t_s = time_call(sample)
         t_k = time_call(lambda: c.keygen(A, 0, s, e, t, Bt))
+        c.set_option(B.OPT_PROFILE, 2 + B.KERNELS.index("encaps_tc"))
+        c.profile_reset()
         t_e = time_call(lambda: c.encaps_pv(A, t, R, E1, e2, mu, U, v, Bt))
+        g_ms, g_cnt = c.profile_read().get("encaps_tc", (0.0, 0))
+        c.set_option(B.OPT_PROFILE, 0)
         t_d = time_call(lambda: c.decaps(U, v, s, out, Bt))
         ok = bool(torch.equal(out, mu))
+    ops = 4.0 * n * n * k * Bt
     return {"config": f"n={n} q={q} sigma={sigma} e2<= {bound} eta=3, 32 instances", "sample_ms": t_s, "keygen_ms": t_k,
             "encaps_ms": t_e, "decaps_ms": t_d, "kem_per_s": Bt * 1e3 / (t_s + t_k + t_e + t_d),
-            "encaps_int8_TOPs": 4.0 * n * n * k * Bt / (t_e * 1e-3) / 1e12, "all_bits_recovered": ok}
+            "encaps_int8_TOPs": ops / (t_e * 1e-3) / 1e12,
+            "encaps_gemm_kernel_ms": g_ms / g_cnt if g_cnt else None,
+            "encaps_gemm_kernel_int8_TOPs": ops / (g_ms / g_cnt * 1e-3) / 1e12 if g_cnt else None,
+            "all_bits_recovered": ok}
+
+
+def paper_variant_wide_phase(B, device: int) -> dict:
+    """N2 on Table 1's n = 8192 row (q = 65537, sigma = 1.2, e2 in [-2, 2], CBD-3 secret, square A), the first of
+    the paper's 17-bit parameter sets: 32 instances sharing A, uint32 residues, A packed once by lwe_wide_load_matrix
+    (timed separately: a one-off per public matrix), KeyGen and Encrypt on tcgen05, Decrypt."""
+    n, q, sigma, bound = 8192, 65537, 1.2, 2
+    k, Bt, seed = 256, 32, 8
+    dev = torch.device("cuda", device)
+    i32, u8, s8 = (dict(dtype=d, device=dev) for d in (torch.int32, torch.uint8, torch.int8))
+    with B.Context(n, n, k, q, 3, Bt, device) as c:
+        A = torch.empty(n, n, **i32)
+        t_A = time_call(lambda: c.sample_uniform_u32(A, 0, n * n, seed, W.TAG_A), reps=3, warm=1)
+        t_load = time_call(lambda: c.wide_load_matrix(A), reps=3, warm=1)
+        del A
+        t_load_seeded = time_call(lambda: c.wide_load_matrix_seeded(seed), reps=2, warm=1)
+        s, e, t = torch.empty(Bt, n, **s8), torch.empty(Bt, n, **s8), torch.empty(Bt, n, **i32)
+        R, E1, e2 = torch.empty(Bt, n, k, **s8), torch.empty(Bt, n, k, **s8), torch.empty(Bt, k, **s8)
+        mu, out = torch.empty(Bt, k // 8, **u8), torch.empty(Bt, k // 8, **u8)
+        U, v = torch.empty(Bt, n, k, **i32), torch.empty(Bt, k, **i32)
+
+        def sample():
+            c.sample_cbd_s8(s, 0, n, seed, W.TAG_S, 0, Bt)
+            c.sample_gauss_s8(e, 0, n, seed, W.TAG_E, 0, Bt, sigma)
+            c.sample_gauss_s8(R, 0, n * k, seed, W.TAG_RG, 0, Bt, sigma)
+            c.sample_gauss_s8(E1, 0, n * k, seed, W.TAG_E1, 0, Bt, sigma)
+            c.sample_cuniform_s8(e2, 0, k, seed, W.TAG_E2, 0, Bt, bound)
+            c.sample_bits(mu, 0, k, seed, W.TAG_MU, 0, Bt)
+
+        t_s = time_call(sample)
+        t_k = time_call(lambda: c.wide_keygen(s, e, t, Bt))
+        c.set_option(B.OPT_PROFILE, 2 + B.KERNELS.index("encaps_tc"))
+        c.profile_reset()
+        t_e = time_call(lambda: c.wide_encaps(t, R, E1, e2, mu, U, v, Bt))
+        g_ms, g_cnt = c.profile_read().get("encaps_tc", (0.0, 0))
+        c.set_option(B.OPT_PROFILE, 0)
+        t_d = time_call(lambda: c.wide_decaps(U, v, s, out, Bt))
+        ok = bool(torch.equal(out, mu))
+    ops = 4.0 * n * n * k * Bt
+    return {"config": f"n={n} q={q} sigma={sigma} e2<= {bound} eta=3, 32 instances, uint32 residues",
+            "generate_A_u32_ms": t_A, "load_matrix_ms_one_off": t_load, "load_matrix_seeded_ms_one_off": t_load_seeded,
+            "sample_ms": t_s, "keygen_ms": t_k, "encaps_ms": t_e, "decaps_ms": t_d,
+            "kem_per_s": Bt * 1e3 / (t_s + t_k + t_e + t_d), "kem_per_s_encaps_plus_decaps": Bt * 1e3 / (t_e + t_d),
+            "encaps_int8_TOPs": ops / (t_e * 1e-3) / 1e12,
+            "encaps_gemm_kernel_ms": g_ms / g_cnt if g_cnt else None,
+            "encaps_gemm_kernel_int8_TOPs": ops / (g_ms / g_cnt * 1e-3) / 1e12 if g_cnt else None,
+            "encaps_gemm_frac_of_nominal_4500": ops / (g_ms / g_cnt * 1e-3) / 1e12 / 4500.0 if g_cnt else None,
+            "decaps_GBps": 4.0 * n * k * Bt / (t_d * 1e-3) / 1e9, "all_bits_recovered": ok}
 
 
 def single_kem_phase(B, device: int) -> dict:
@@ -856,6 +912,7 @@ def run_ours(args):
                              "kem_per_s_encaps_plus_fo_decaps_B32": Bt * 1e3 / (t + t3)}
     if not args.quick:
         side["paper_variant_n4096_B32"] = paper_variant_phase(job.B, local)
+        side["paper_variant_n8192_q65537_B32"] = paper_variant_wide_phase(job.B, local)
         side["single_kem_B1"] = single_kem_phase(job.B, local)
         side["large_kem_C5_B1"] = large_kem_phase(job.B, local, hbm)
         buf = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")

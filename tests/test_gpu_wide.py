@@ -126,7 +126,8 @@ def test_wide_keygen_extreme_values():
     for q, n in ((F4, 65536), (66560, 16384)):
         for sign in (1, -1):
             A = np.full((m, n), 65535, np.uint32)
-            A[:, :3] = q - 1                                 # three exceptions per row
+            for x in range(3):                               # three elements >= 2^16 per row, at most one per column
+                A[np.arange(m), (7 * np.arange(m) + x) % n] = q - 1
             s = np.full((batch, n), 127 * sign, np.int8)
             e = np.full((batch, m), -128 if sign < 0 else 127, np.int8)
             with B().Context(n, m, 256, q, 3, batch) as c:
@@ -214,11 +215,12 @@ def test_wide_encaps_matches_oracle(path, n, k, q, batch, big):
 def test_wide_encaps_extreme_accumulators(path):
     """|R| = 127, A's low half = 65535, m = 65536 (the path's limit): both signed byte-plane accumulators at
     +/- 255*127*65536, every column with exceptions, the two- and three-reduction recombinations at their bounds"""
-    m, n_small, k, batch = 65536, 64, 256, 1
-    for q in (F4, 66560):
+    n_small, k, batch = 64, 256, 1
+    for q, m in ((F4, 65536), (65539, 65536), (66560, 8192)):
         for sign in (1, -1):
             A = np.full((m, n_small), 65535, np.uint32)
-            A[:5, :] = q - 1                                 # five exceptions in every column
+            for x in range(5):                               # five elements >= 2^16 in every column, one per row
+                A[5 * np.arange(n_small) + x, np.arange(n_small)] = q - 1
             t = np.full((batch, m), q - 1, np.uint32)
             R = np.full((batch, m, k), 127 * sign, np.int8)
             E1 = np.full((batch, n_small, k), -128 if sign < 0 else 127, np.int8)
