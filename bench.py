@@ -741,6 +741,11 @@ def sustained_block(job: Job, seconds: float, ms_step_burst: float, peaks: dict)
     return out
 
 
+PHASES = {"paper_variant_n4096_B32": paper_variant_phase, "paper_variant_n8192_q65537_B32": paper_variant_wide_phase,
+          "single_kem_B1": single_kem_phase,
+          "large_kem_C5_B1": lambda B, device: large_kem_phase(B, device, measured_peaks()["hbm_gbs"])}
+
+
 def run_dry(args):
     """--dry-run: the rank plumbing of the GPU arm on CPU/gloo, no CUDA, no measurement (tests/test_sharding.py)."""
     rank, world, _ = env_rank()
@@ -981,7 +986,14 @@ def main():
     ap.add_argument("--quick", action="store_true", help="headline step, e2e and the C4 phases only (no sustained loop, "
                     "no C1-C3/C5/N2 phases, CPU baseline on C1 and C4): for ncu passes and smoke runs")
     ap.add_argument("--dry-run", action="store_true", help="rank plumbing on CPU/gloo only; prints no measurement")
+    ap.add_argument("--phase", choices=sorted(PHASES), help="run ONE side phase alone and print its JSON (for ncu captures "
+                    "of the kernels the headline step does not launch); no headline line is printed")
     args = ap.parse_args()
+    if args.phase:
+        from paper_2606_01211_b200 import binding as B
+        torch.cuda.set_device(0)
+        print(json.dumps({"phase": args.phase, "result": PHASES[args.phase](B, 0)}), flush=True)
+        return
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and (args.impl == "ours" or args.dry_run):
         sys.exit(respawn_under_torchrun(args))
     if args.dry_run:

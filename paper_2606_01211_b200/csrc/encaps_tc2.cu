@@ -38,6 +38,11 @@ constexpr uint32_t kThreads = 192;
 constexpr uint32_t kExpGroups = 2;                  // expander groups per CTA (kBitsB): group j takes K blocks j, j+2, ..
 constexpr uint32_t kExpWarps = 4 * kExpGroups;      // 4 warps = 128 threads = one K row each
 constexpr uint32_t kThreadsBits = kThreads + 32 * kExpWarps;
+// the signed-R modes (N2) run EIGHT epilogue warps per CTA, two per TMEM lane quarter, each taking half of the tile's
+// columns: their epilogue (two Barrett reductions, E1, the exception terms, 32-bit stores) costs ~40 instructions
+// per element, and with four warps it -- not the tensor pipe -- set the pace (ncu: epilogue warps busy 81 % of the
+// time, tensor pipe 65 %; profiles/r2_wide_gemm_*)
+constexpr uint32_t kThreadsPv = kThreads + 128;
 constexpr uint32_t kBitStages = 12;                 // ring of packed-bit tiles, deeper than the operand ring
 constexpr uint32_t kBitTileBytes = 128 * 16;        // 128 K rows x 128 columns of bits
 constexpr uint32_t kTmemCols = 512;
@@ -89,7 +94,8 @@ struct PvArgs {
 };
 
 template <uint32_t kStages, uint32_t kTileK, int kMode, bool kBitsB>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kBitsB ? kThreadsBits : kThreads, 1)
+__global__ void __cluster_dims__(2, 1, 1)
+__launch_bounds__(kBitsB ? kThreadsBits : ((kMode == kEpiStorePv || kMode == kEpiStorePvW) ? kThreadsPv : kThreads), 1)
 encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapR,
                   void *__restrict__ U_, uint32_t *__restrict__ flags, uint32_t m,
                   uint32_t n, uint32_t k,
@@ -138,7 +144,7 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
         }
         for (uint32_t a = 0; a < 2; a++) {
             mbar_init(tfull_bar(a), 1);
-            mbar_init(tempty_bar(a), 8);                          // 4 epilogue warps of each CTA
+            mbar_init(tempty_bar(a), kPv ? 16 : 8);               // 4 (signed-R modes: 8) epilogue warps of each CTA
         }
         if (kBitsB) {
             asm volatile("prefetch.tensormap [%0];" ::"l"(&mapBits) : "memory");
@@ -279,24 +285,26 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
             __syncwarp();
             if (lane == 0) mbar_arrive_remote(map_to_cta(full_bar(stage), 0));
         }
-    } else if (warp < 6) {
-        // ===================== epilogue (warps 2..5, both CTAs) =====================
-        const uint32_t quarter = warp & 3;
+    } else if (warp < 6 || (kPv && !kBitsB)) {
+        // ===================== epilogue (warps 2..5, both CTAs; signed-R modes: warps 2..9) =====================
+        const uint32_t quarter = warp & 3;                           // the TMEM lane quarter a warp may read
+        const uint32_t cb_lo = (kPv && warp >= 6) ? kTileN / 2 : 0u; // warps 6..9 take the upper half of the columns
+        const uint32_t cb_hi = (kPv && warp < 6) ? kTileN / 2 : kTileN;
         const uint32_t lead_tempty0 = map_to_cta(tempty_bar(0), 0), lead_tempty1 = map_to_cta(tempty_bar(1), 0);
         uint32_t it = 0;
         for (uint32_t t = pair; t < sched.total; t += n_pairs, it++) {
             uint32_t mt, nt;
             sched.coords(t, mt, nt);
             const uint32_t acc = it & 1, acc_phase = (it >> 1) & 1;
-            mbar_wait(tfull_bar(acc), acc_phase);
-            tc_fence_after();
             const uint32_t brow = mt * kPairM + rank * kCtaM + quarter * 32 + lane;   // byte-row of D
             const uint32_t j = brow >> 1;
             const bool odd = lane & 1;
             const uint32_t taddr = tmem_base + ((quarter * 32) << 16) + acc * kTileN;
             MismatchAcc mism;
-#pragma unroll 1
-            for (uint32_t cb = 0; cb < kTileN; cb += 32) {
+            // wide: number of elements >= 2^16 in column j of A (rare: ~m/65537 per column)
+            const uint32_t exc = (kMode == kEpiStorePvW && j < n) ? min(__ldg(pv.exc_cnt + j), pv.exc_cap) : 0u;
+            // one 32-column piece of the tile: this lane's 16 columns of row j
+            auto do_chunk = [&](uint32_t cb, const uint4 &e1v) {
                 uint32_t r[32];
                 tmem_ld_32x32b_x32(taddr + cb, r);
                 tmem_ld_wait();
@@ -304,17 +312,13 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 const uint32_t col = nt * kTileN + cb + (odd ? 16u : 0u);
                 const bool in_range = j < n && col < ncols_total;
                 const uint32_t inst = col / k, c = col - inst * k;
-                uint32_t e1w[4] = {0, 0, 0, 0};                      // 16 int8 of E1[inst][j][c..c+15] (N2 only)
-                if (kPv && in_range) {
-                    const uint4 t4 = *reinterpret_cast<const uint4 *>(E1 + ((size_t)inst * n + j) * k + c);
-                    e1w[0] = t4.x; e1w[1] = t4.y; e1w[2] = t4.z; e1w[3] = t4.w;
-                }
-                // wide: corr[x] = sum over the exceptions i of column j of R[inst][i][c + x]  (rare: ~m/65537 per column)
+                const uint32_t e1w[4] = {e1v.x, e1v.y, e1v.z, e1v.w};   // 16 int8 of E1[inst][j][c..c+15] (N2 only)
+                // wide: corr[x] = sum over the exceptions i of column j of R[inst][i][c + x]
                 int corr[16];
                 if (kMode == kEpiStorePvW) {
 #pragma unroll
                     for (int x = 0; x < 16; x++) corr[x] = 0;
-                    const uint32_t cnt = in_range ? min(__ldg(pv.exc_cnt + j), pv.exc_cap) : 0u;
+                    const uint32_t cnt = in_range ? exc : 0u;
                     for (uint32_t y = 0; y < cnt; y++) {
                         const uint32_t i = __ldg(pv.exc_rows + (size_t)j * pv.exc_cap + y);
                         const uint4 r4 = __ldg(reinterpret_cast<const uint4 *>(pv.R + ((size_t)inst * pv.m_full + i) * k + c));
@@ -323,25 +327,40 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                         for (int x = 0; x < 16; x++) corr[x] += (int)(int8_t)(rw[x >> 2] >> (8 * (x & 3)));
                     }
                 }
+                if (kPv) {
+                    // signed planes: lo = sum lo(A) r, hi = sum hi(A) r; U = lo + 256 hi + e1 (- delta corr) mod q.
+                    // General q: straight-line unsigned arithmetic (a branch per sign serialised the 16 elements:
+                    // 0.65 ms instead of 0.17 ms at n = 4096).  pv.bias is a multiple of q >= 255 * 128 * rows, so
+                    // plane + bias is the same residue in [0, 2^32); pv.e1bias likewise covers e1.  The kind of
+                    // reduction is decided once per piece, not per element.
+                    uint32_t lo[16], hi[16], e1[16];
 #pragma unroll
-                for (int x = 0; x < 16; x++) {
-                    uint32_t send = odd ? r[x] : r[16 + x];
-                    uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 1);
-                    if (kPv) {
-                        // signed planes: lo = sum lo(A) r, hi = sum hi(A) r; U = lo + 256 hi + e1 (- delta corr) mod q
-                        const int32_t lo = (int32_t)(odd ? recv : r[x]), hi = (int32_t)(odd ? r[16 + x] : recv);
-                        int32_t e1 = (int32_t)(int8_t)(e1w[x >> 2] >> (8 * (x & 3)));
-                        if (kMode == kEpiStorePvW) e1 -= (int32_t)pv.delta * corr[x];       // 2^16 = -delta (mod q)
-                        // general q: straight-line unsigned arithmetic (a branch per sign serialised the 16
-                        // elements: 0.65 ms instead of 0.17 ms at n = 4096).  pv.bias is a multiple of q >= 255 *
-                        // 128 * rows, so plane + bias is the same residue in [0, 2^32); pv.e1bias likewise covers e1.
-                        if (mq.pow2) o[x] = ((uint32_t)lo + ((uint32_t)hi << 8) + (uint32_t)e1) & mq.mask;
-                        else if (pv.two_step)           // (lo + bias) + 256 (hi mod q) + e1 stays below 2^32: one reduction less
-                            o[x] = mod_u32(((uint32_t)lo + pv.bias) + 256u * mod_u32((uint32_t)hi + pv.bias, mq) +
-                                           ((uint32_t)e1 + pv.e1bias), mq);
-                        else o[x] = mod_u32(mod_u32((uint32_t)lo + pv.bias, mq) + 256u * mod_u32((uint32_t)hi + pv.bias, mq) +
-                                            ((uint32_t)e1 + pv.e1bias), mq);
+                    for (int x = 0; x < 16; x++) {
+                        const uint32_t recv = __shfl_xor_sync(0xffffffffu, odd ? r[x] : r[16 + x], 1);
+                        lo[x] = odd ? recv : r[x];
+                        hi[x] = odd ? r[16 + x] : recv;
+                        int32_t ev = (int32_t)(int8_t)(e1w[x >> 2] >> (8 * (x & 3)));
+                        if (kMode == kEpiStorePvW) ev -= (int32_t)pv.delta * corr[x];       // 2^16 = -delta (mod q)
+                        e1[x] = (uint32_t)ev;
+                    }
+                    const uint32_t bias = pv.bias, e1bias = pv.e1bias;
+                    if (mq.pow2) {
+#pragma unroll
+                        for (int x = 0; x < 16; x++) o[x] = (lo[x] + (hi[x] << 8) + e1[x]) & mq.mask;
+                    } else if (pv.two_step) {   // (lo + bias) + 256 (hi mod q) + e1 stays below 2^32: one reduction less
+#pragma unroll
+                        for (int x = 0; x < 16; x++)
+                            o[x] = mod_u32((lo[x] + bias) + 256u * mod_u32(hi[x] + bias, mq) + (e1[x] + e1bias), mq);
                     } else {
+#pragma unroll
+                        for (int x = 0; x < 16; x++)
+                            o[x] = mod_u32(mod_u32(lo[x] + bias, mq) + 256u * mod_u32(hi[x] + bias, mq) + (e1[x] + e1bias), mq);
+                    }
+                } else {
+#pragma unroll
+                    for (int x = 0; x < 16; x++) {
+                        uint32_t send = odd ? r[x] : r[16 + x];
+                        uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 1);
                         uint32_t val = odd ? (recv + (r[16 + x] << 8)) : (r[x] + (recv << 8));
                         o[x] = mq.pow2 ? (val & mq.mask) : mod_u32(val, mq);
                     }
@@ -356,6 +375,33 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                         if (kMode == kEpiCompare) mism.note(flags, inst, bad);
                     }
                 }
+            };
+            if constexpr (kPv) {
+                // E1 of the NEXT piece is fetched before the current one is processed, and the first before the
+                // accumulator is ready: a dependent global load per piece after tfull made the epilogue (not the
+                // tensor pipe) the limit at n = 8192 (0.71 ms instead of ~0.5).  The loop stays rolled: unrolled it
+                // is 160 KB of code and thrashes the instruction cache (1.22 ms).
+                auto e1_load = [&](uint32_t cb) {
+                    const uint32_t col = nt * kTileN + cb + (odd ? 16u : 0u);
+                    const uint32_t inst = col / k, c = col - inst * k;
+                    return (j < n && col < ncols_total)
+                        ? __ldg(reinterpret_cast<const uint4 *>(E1 + ((size_t)inst * n + j) * k + c)) : make_uint4(0, 0, 0, 0);
+                };
+                uint4 e1cur = e1_load(cb_lo);
+                mbar_wait(tfull_bar(acc), acc_phase);
+                tc_fence_after();
+#pragma unroll 1
+                for (uint32_t cb = cb_lo; cb < cb_hi; cb += 32) {
+                    const uint4 e1next = (cb + 32 < cb_hi) ? e1_load(cb + 32) : make_uint4(0, 0, 0, 0);
+                    do_chunk(cb, e1cur);
+                    e1cur = e1next;
+                }
+            } else {
+                mbar_wait(tfull_bar(acc), acc_phase);
+                tc_fence_after();
+                const uint4 zero = make_uint4(0, 0, 0, 0);
+#pragma unroll 1
+                for (uint32_t cb = 0; cb < kTileN; cb += 32) do_chunk(cb, zero);
             }
             if (kMode == kEpiCompare) mism.flush_warp(flags);
             tc_fence_before();
@@ -431,7 +477,8 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, void *d_U, uint32_t 
     CUtensorMap mapBits = mapR;
     if (kBitsB && !make_map_plain_u8(c, &mapBits, d_Rbits, p.k / 8, (uint64_t)batch * p.m, 16, kTileK))
         return cudaErrorInvalidValue;
-    kern<<<2 * pairs, kBitsB ? kThreadsBits : kThreads, smem_bytes, st>>>(
+    constexpr bool kPvMode = (kMode == kEpiStorePv || kMode == kEpiStorePvW);
+    kern<<<2 * pairs, kBitsB ? kThreadsBits : (kPvMode ? kThreadsPv : kThreads), smem_bytes, st>>>(
         mapA, mapR, d_U, d_flags, rows, p.n, p.k, ncols, c->mq, gw, pv, mapBits, row0, p.m);
     c->launches++;
     return cudaGetLastError();
