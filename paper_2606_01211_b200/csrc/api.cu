@@ -288,6 +288,11 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
         ctx->c.r_operand = (int)value;
         return LWE_OK;
     }
+    if (option == LWE_OPT_V_PATH) {
+        if (value < 0 || value > 1) return LWE_ERR_PARAM;
+        ctx->c.v_path = (int)value;
+        return LWE_OK;
+    }
     if (option == LWE_OPT_REGEN_PATH) {
         if (value < 0 || value > 2) return LWE_ERR_PARAM;
         ctx->c.regen_path = (int)value;
@@ -453,8 +458,11 @@ static int encaps_core(Ctx *c, const uint16_t *d_A, uint64_t seed_A, const uint1
     if (!d_A && c->regen_path == 2 && !fused) return LWE_ERR_UNSUPPORTED;
     // CTA-pair GEMM with k % 128 == 0: the kernel expands its B tiles from the packed bits itself; the pass over R
     // here then only computes v (no expanded operand is written)
-    const bool bits = pair && c->r_operand != 1 && encaps_tc2_bits_supported(c, batch);
-    LAUNCH(c, launch_expand_R_and_v(c, d_b, d_Rbits, d_mubits, d_v, batch, tc && (fused || !bits), st));   // the fused regenerated-A kernel loads R through TMA
+    const bool bits = pair && !fused && c->r_operand != 1 && encaps_tc2_bits_supported(c, batch);
+    // ... and v comes from spare warps of that same kernel (LWE_OPT_V_PATH = 1: from the separate pass below)
+    const bool v_fused = bits && c->v_path != 1 && encaps_tc2_v_fused_supported(c, batch);
+    if (!v_fused)       // one pass over R's bits: v, and the expanded operand for the kernels that read one
+        LAUNCH(c, launch_expand_R_and_v(c, d_b, d_Rbits, d_mubits, d_v, batch, tc && (fused || !bits), st));   // the fused regenerated-A kernel loads R through TMA
     if (fused) {
         LAUNCH(c, launch_encaps_regen_tc(c, seed_key_host(seed_A), d_U, st));
         return LWE_OK;
@@ -474,7 +482,11 @@ static int encaps_core(Ctx *c, const uint16_t *d_A, uint64_t seed_A, const uint1
             panel = c->d_Apanel;
         }
         const int mode = compare ? 2 : (row0 != 0 ? 1 : 0);
-        if (pair) LAUNCH(c, launch_encaps_tc2(c, panel, d_U, batch, row0, rows, mode, c->d_foflags, st, bits ? d_Rbits : nullptr));
+        if (pair) {
+            const bool with_v = v_fused && row0 == 0;               // v spans all m rows: once, with the first panel
+            LAUNCH(c, launch_encaps_tc2(c, panel, d_U, batch, row0, rows, mode, c->d_foflags, st, bits ? d_Rbits : nullptr,
+                                        with_v ? d_b : nullptr, d_mubits, d_v));
+        }
         else if (tc) LAUNCH(c, launch_encaps_tc(c, panel, d_U, batch, row0, rows, mode, c->d_foflags, st));
         else LAUNCH(c, launch_encaps_simt(c, panel, d_Rbits, d_U, batch, row0, rows, mode, c->d_foflags, st));
     }

@@ -74,15 +74,20 @@ decaps_kernel(const uint16_t *__restrict__ U, const uint16_t *__restrict__ v, co
         }
         for (; j < jend; j += rows_per_iter, up += ustep) accumulate_row(a, ldg_stream16(up), __ldg(st + j));
     }
-    // sum the row slots of the CTA in shared memory, then one atomic per column per CTA
-    __shared__ unsigned long long sCol[kDecThreads * 8];
-#pragma unroll
-    for (int x = 0; x < 8; x++) sCol[x * kDecThreads + threadIdx.x] = a[x];      // inactive threads hold zeros
+    // sum the row slots of the CTA in shared memory, then one atomic per column per CTA.  Staged [row slot][column]:
+    // a thread stores its 8 columns as 64 contiguous bytes and thread c then reads column c of every slot -- consecutive
+    // 8-byte words across a warp in both phases (the earlier [x][thread] layout read 8 lanes from one bank: 660 k
+    // conflicts per launch at C4, ncu)
+    __shared__ __align__(16) unsigned long long sCol[kDecThreads * 8];
+    {
+        ulonglong2 *dst = reinterpret_cast<ulonglong2 *>(sCol + (size_t)threadIdx.x * 8);   // = [rslot][cg * 8 + x]
+        dst[0] = make_ulonglong2(a[0], a[1]); dst[1] = make_ulonglong2(a[2], a[3]);
+        dst[2] = make_ulonglong2(a[4], a[5]); dst[3] = make_ulonglong2(a[6], a[7]);
+    }
     __syncthreads();
     for (uint32_t c = threadIdx.x; c < k; c += kDecThreads) {
-        const uint32_t ccg = c >> 3, x = c & 7;
         unsigned long long sum = 0;
-        for (uint32_t rs = 0; rs < rows_per_iter; rs++) sum += sCol[x * kDecThreads + rs * tpr + ccg];
+        for (uint32_t rs = 0; rs < rows_per_iter; rs++) sum += sCol[(size_t)rs * k + c];
         if (sum) atomicAdd(acc + (size_t)t * k + c, sum);
     }
     __threadfence();

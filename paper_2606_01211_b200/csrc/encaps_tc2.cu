@@ -37,7 +37,8 @@ constexpr uint32_t kHalfN = kTileN / 2;          // columns of R staged by each 
 constexpr uint32_t kThreads = 192;
 constexpr uint32_t kExpGroups = 2;                  // expander groups per CTA (kBitsB): group j takes K blocks j, j+2, ..
 constexpr uint32_t kExpWarps = 4 * kExpGroups;      // 4 warps = 128 threads = one K row each
-constexpr uint32_t kThreadsBits = kThreads + 32 * kExpWarps;
+constexpr uint32_t kVWarps = 2;                     // kBitsB: warps computing v = b^T R + mu floor(q/2) beside the GEMM
+constexpr uint32_t kThreadsBits = kThreads + 32 * kExpWarps + 32 * kVWarps;
 // the signed-R modes (N2) run EIGHT epilogue warps per CTA, two per TMEM lane quarter, each taking half of the tile's
 // columns: their epilogue (two Barrett reductions, E1, the exception terms, 32-bit stores) costs ~40 instructions
 // per element, and with four warps it -- not the tensor pipe -- set the pace (ncu: epilogue warps busy 81 % of the
@@ -71,7 +72,8 @@ struct PairCfg {
     static constexpr uint32_t kBytesStage = kBytesA + kBytesB;
     static constexpr uint32_t kSmemBytes = kStages * kBytesStage + 1024 /*align*/ + 256 /*barriers*/;
     // kBitsB: + a ring of packed-bit tiles (128 K rows x 16 bytes each) and its barriers
-    static constexpr uint32_t kSmemBytesBits = kSmemBytes + kBitStages * kBitTileBytes + 256;
+    // ... and the v warps' k <= 2048 column sums
+    static constexpr uint32_t kSmemBytesBits = kSmemBytes + kBitStages * kBitTileBytes + 256 + 2048 * 4 + 16;
 };
 
 // kBitsB: the B operand is never expanded in HBM.  Eight extra warps per CTA (two groups taking alternate K blocks)
@@ -80,6 +82,108 @@ struct PairCfg {
 // counts the arrivals of one group of each CTA (8 warps) beside the A bytes.  Needs k % 128 == 0 (a half tile lies inside
 // one instance) and kTileK == 128 (one row per expander thread).  Against the expanded operand this removes the
 // 128 MiB expanded-R write per batch and every DRAM / L2 re-read of it by the GEMM (16x fewer operand bytes).
+// a5 inside the GEMM (kBitsB): v_c = sum_i b_i R_ic + mu_c floor(q/2) mod q (BJ north_star) is one more
+// "row" of the same contraction, but its left operand b differs per instance, so it cannot ride the tensor pipe
+// without computing batch x batch blocks for a diagonal.  Two spare warps per CTA compute it on the CUDA cores while
+// the MMAs run: 2 instructions per bit of R, ~0.8 % of the SM's issue slots over the kernel's life, and the separate
+// 29 us pass over R's bits (0.09 of HBM, 2.4 % of the step) disappears from the stream.
+struct VArgs {
+    const uint16_t *b;                 // [batch][m]; NULL: v is not computed by this launch
+    const uint8_t *Rbits, *mubits;
+    uint16_t *v;
+    unsigned long long *acc;           // [batch][k] u64 partial sums, left zeroed
+    unsigned int *tickets;             // [batch] self-resetting
+    uint32_t m, batch, splits;         // rows per instance, instances, row ranges per instance
+};
+
+// Executed by the kVWarps * 32 threads `vt` = 0..63 of a CTA; the CTAs share the (instance, row range) units.
+// The arithmetic of expand_R_and_v_w32_kernel (encaps_aux.cu): a thread owns one 32-bit word of R bits (32 columns)
+// of a row; its 32 column sums sit in 16-bit lanes of 2 x 16 registers, one byte plane of b at a time.
+__device__ __forceinline__ void v_warps_role(const VArgs &va, uint32_t vt, uint32_t k, const ModQ &mq, uint32_t *sSum,
+                                             volatile uint32_t *sLast)
+{
+    constexpr uint32_t kVT = 32 * kVWarps;
+    auto vbar = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kVT) : "memory"); };
+    const uint32_t wpr = k / 32;                               // words per row: a power of two <= 64
+    const uint32_t w = vt & (wpr - 1);
+    const uint32_t rows_per_iter = kVT / wpr, rslot = vt / wpr;
+    const uint32_t units = va.batch * va.splits;
+    for (uint32_t u = blockIdx.x; u < units; u += gridDim.x) {
+        const uint32_t t = u / va.splits, sidx = u - t * va.splits;
+        const uint32_t per = ((va.m + va.splits - 1) / va.splits + rows_per_iter - 1) / rows_per_iter * rows_per_iter;
+        const uint32_t ibeg = sidx * per, iend = min(va.m, ibeg + per);
+        const uint32_t *Rt = reinterpret_cast<const uint32_t *>(va.Rbits + (size_t)t * va.m * (k / 8));
+        const uint16_t *bt = va.b + (size_t)t * va.m;
+        for (uint32_t c = vt; c < k; c += kVT) sSum[c] = 0;
+        vbar();
+        uint32_t aL[16], aH[16];
+#pragma unroll
+        for (int x = 0; x < 16; x++) { aL[x] = 0; aH[x] = 0; }
+        auto flush = [&]() {
+            uint32_t vals[32];
+#pragma unroll
+            for (int x = 0; x < 16; x++) {
+                vals[x] = (aL[x] & 0xffffu) + ((aH[x] & 0xffffu) << 8);
+                vals[x + 16] = (aL[x] >> 16) + ((aH[x] >> 16) << 8);
+                aL[x] = 0; aH[x] = 0;
+            }
+            for (uint32_t off = wpr; off < 32; off <<= 1) {
+#pragma unroll
+                for (int x = 0; x < 32; x++) vals[x] += __shfl_xor_sync(0xffffffffu, vals[x], off);
+            }
+            if ((vt & 31) < wpr || wpr >= 32) {
+#pragma unroll
+                for (int x = 0; x < 32; x++)
+                    if (vals[x]) atomicAdd(&sSum[x * wpr + w], vals[x]);
+            }
+        };
+        constexpr int kUnroll = 4;
+        constexpr uint32_t kFlushIters = 256 / kUnroll;       // <= 256 rows per thread between flushes (16-bit lanes)
+        uint32_t iters = 0;
+        for (uint32_t i0 = ibeg + rslot; i0 < iend; i0 += kUnroll * rows_per_iter) {
+            uint32_t r[kUnroll], bi[kUnroll];
+#pragma unroll
+            for (int q = 0; q < kUnroll; q++) {
+                const uint32_t i = i0 + q * rows_per_iter;
+                r[q] = (i < iend) ? __ldg(Rt + (size_t)i * wpr + w) : 0u;
+                bi[q] = (i < iend) ? (uint32_t)__ldg(bt + i) : 0u;
+            }
+#pragma unroll
+            for (int q = 0; q < kUnroll; q++) {
+                const uint32_t bl = bi[q] & 0xffu, bh = bi[q] >> 8;
+#pragma unroll
+                for (int x = 0; x < 16; x++) {
+                    const uint32_t two = (r[q] >> x) & 0x00010001u;     // columns x (low lane) and x + 16 (high lane)
+                    aL[x] += two * bl;
+                    aH[x] += two * bh;
+                }
+            }
+            if (++iters == kFlushIters) { flush(); iters = 0; }
+        }
+        flush();
+        vbar();
+        for (uint32_t c = vt; c < k; c += kVT) {
+            const uint32_t sum = sSum[(c & 31u) * wpr + (c >> 5)];
+            if (sum) atomicAdd(va.acc + (size_t)t * k + c, (unsigned long long)sum);
+        }
+        __threadfence();
+        vbar();
+        if (vt == 0) *sLast = (atomicAdd(va.tickets + t, 1u) == va.splits - 1) ? 1u : 0u;
+        vbar();
+        if (*sLast) {                                          // the last range of instance t: reduce mod q, write v
+            __threadfence();
+            for (uint32_t c = vt; c < k; c += kVT) {
+                const unsigned long long sum = __ldcg(va.acc + (size_t)t * k + c);
+                va.acc[(size_t)t * k + c] = 0;
+                const uint32_t mu = (va.mubits[(size_t)t * (k / 8) + c / 8] >> (c % 8)) & 1u;
+                va.v[(size_t)t * k + c] = (uint16_t)mod_u64(sum + (unsigned long long)mu * mq.half, mq);
+            }
+            if (vt == 0) va.tickets[t] = 0;
+        }
+        vbar();
+    }
+}
+
 // The signed-R modes (N2) beside the accumulators.  r_inplace: the B operand is read IN PLACE from the caller's int8
 // R [batch][m_full][k] (a half tile lies inside one instance when k % 128 == 0; rows of the next instance that a
 // ragged last K block drags in meet zero-filled rows of A) -- no operand copy is made.  Wide contexts: the
@@ -101,7 +205,7 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                   uint32_t n, uint32_t k,
                   uint32_t ncols_total, ModQ mq, uint32_t group_w, PvArgs pv,
                   const __grid_constant__ CUtensorMap mapBits, uint32_t bits_row0,
-                  uint32_t bits_rows_per_inst)
+                  uint32_t bits_rows_per_inst, VArgs va)
 {
     constexpr bool kPv = (kMode == kEpiStorePv || kMode == kEpiStorePvW);
     uint16_t *U = static_cast<uint16_t *>(U_);
@@ -224,6 +328,12 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
             }
+        }
+    } else if (kBitsB && warp >= 6 + kExpWarps) {
+        // ===================== v warps (both CTAs): a5 on the CUDA cores beside the MMAs =====================
+        if (va.b != nullptr) {
+            uint32_t *sSum = reinterpret_cast<uint32_t *>(smem_raw + (bars + 512 - raw));
+            v_warps_role(va, threadIdx.x - 32 * (6 + kExpWarps), k, mq, sSum, sSum + 2048);
         }
     } else if (kBitsB && warp >= 6) {
         // ===================== B-operand expanders (warps 6..13, both CTAs) =====================
@@ -428,7 +538,8 @@ bool encaps_tc2_supported(const Ctx *c, uint32_t batch)
 template <uint32_t kStages, uint32_t kTileK, int kMode, bool kBitsB = false>
 static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, void *d_U, uint32_t *d_flags, const int8_t *d_E1,
                                uint32_t batch, uint32_t row0, uint32_t rows, cudaStream_t st,
-                               const uint8_t *d_Rbits = nullptr, const int8_t *d_R = nullptr, bool r_inplace = false)
+                               const uint8_t *d_Rbits = nullptr, const int8_t *d_R = nullptr, bool r_inplace = false,
+                               const VArgs *vargs = nullptr)
 {
     using Cfg = PairCfg<kStages, kTileK>;
     const lwe_params &p = c->p;
@@ -479,7 +590,7 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, void *d_U, uint32_t 
         return cudaErrorInvalidValue;
     constexpr bool kPvMode = (kMode == kEpiStorePv || kMode == kEpiStorePvW);
     kern<<<2 * pairs, kBitsB ? kThreadsBits : (kPvMode ? kThreadsPv : kThreads), smem_bytes, st>>>(
-        mapA, mapR, d_U, d_flags, rows, p.n, p.k, ncols, c->mq, gw, pv, mapBits, row0, p.m);
+        mapA, mapR, d_U, d_flags, rows, p.n, p.k, ncols, c->mq, gw, pv, mapBits, row0, p.m, vargs ? *vargs : VArgs{});
     c->launches++;
     return cudaGetLastError();
 }
@@ -495,13 +606,31 @@ bool encaps_tc2_r_inplace_supported(const Ctx *c, uint32_t batch)
     return encaps_tc2_supported(c, batch) && c->p.k % 128 == 0;
 }
 
+// k = 32 * 2^j <= 2048: the v warps' word-column reduction needs a power-of-two number of words per row
+bool encaps_tc2_v_fused_supported(const Ctx *c, uint32_t batch)
+{
+    const uint32_t wpr = c->p.k / 32;
+    return encaps_tc2_bits_supported(c, batch) && c->p.k % 32 == 0 && (wpr & (wpr - 1)) == 0 && wpr <= 64;
+}
+
 cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0, uint32_t rows,
-                              int mode, uint32_t *d_flags, cudaStream_t st, const uint8_t *d_Rbits)
+                              int mode, uint32_t *d_flags, cudaStream_t st, const uint8_t *d_Rbits,
+                              const uint16_t *d_b, const uint8_t *d_mubits, uint16_t *d_v)
 {
     if (d_Rbits) {              // B operand expanded from the packed bits inside the kernel
-        if (mode == kEpiAccum) return launch_pair<6, 128, kEpiAccum, true>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st, d_Rbits);
-        if (mode == kEpiCompare) return launch_pair<6, 128, kEpiCompare, true>(c, d_A, d_U, d_flags, nullptr, batch, row0, rows, st, d_Rbits);
-        return launch_pair<6, 128, kEpiStore, true>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st, d_Rbits);
+        VArgs va = {};
+        if (d_b) {              // ... and v computed by the kernel's spare warps (all m rows, whatever the panel)
+            const uint32_t grid = 2 * min((uint32_t)c->sm_count / 2,
+                                          ((2 * c->p.n + kPairM - 1) / kPairM) * ((batch * c->p.k + kTileN - 1) / kTileN));
+            uint32_t splits = (grid + batch - 1) / batch;
+            const uint32_t min_splits = (c->p.m + 65535u) / 65536u, max_splits = (c->p.m + 63u) / 64u;
+            if (splits > max_splits) splits = max_splits;
+            if (splits < min_splits) splits = min_splits;
+            va = VArgs{d_b, d_Rbits, d_mubits, d_v, c->d_vacc, c->d_counters + 8 + c->p.max_batch, c->p.m, batch, splits};
+        }
+        if (mode == kEpiAccum) return launch_pair<6, 128, kEpiAccum, true>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st, d_Rbits, nullptr, false, &va);
+        if (mode == kEpiCompare) return launch_pair<6, 128, kEpiCompare, true>(c, d_A, d_U, d_flags, nullptr, batch, row0, rows, st, d_Rbits, nullptr, false, &va);
+        return launch_pair<6, 128, kEpiStore, true>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st, d_Rbits, nullptr, false, &va);
     }
     if (mode == kEpiAccum) return launch_pair<6, 128, kEpiAccum>(c, d_A, d_U, nullptr, nullptr, batch, row0, rows, st);
     if (mode == kEpiCompare) return launch_pair<6, 128, kEpiCompare>(c, d_A, d_U, d_flags, nullptr, batch, row0, rows, st);

@@ -89,6 +89,7 @@ struct Ctx {
     int keygen_path;                  // LWE_OPT_KEYGEN_PATH
     int regen_path;                   // LWE_OPT_REGEN_PATH
     int r_operand;                    // LWE_OPT_R_OPERAND
+    int v_path;                       // LWE_OPT_V_PATH
 
     // device tables
     uint32_t *d_te0;                  // 256-entry AES T-table (word = 2S | S<<8 | S<<16 | 3S<<24)
@@ -222,11 +223,15 @@ uint32_t encaps_regen_lock_words(const lwe_params &p);
 bool encaps_regen_tc_supported(const Ctx *c, uint32_t batch);
 cudaError_t launch_encaps_regen_tc(Ctx *c, const AesKey &key, uint16_t *d_U, cudaStream_t st);
 // d_Rbits != NULL: the B operand is expanded from the packed bits inside the kernel (needs
-// encaps_tc2_bits_supported); NULL: it is read from the expanded workspace c->d_Rexp
+// encaps_tc2_bits_supported); NULL: it is read from the expanded workspace c->d_Rexp.
+// d_b != NULL (with d_Rbits; needs encaps_tc2_v_fused_supported): v = b^T R + mu floor(q/2) of all m rows is computed
+// by spare warps of the same kernel and written to d_v (no separate pass over R's bits)
 bool encaps_tc2_bits_supported(const Ctx *c, uint32_t batch);
+bool encaps_tc2_v_fused_supported(const Ctx *c, uint32_t batch);
 cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32_t batch, uint32_t row0,
                               uint32_t rows, int mode, uint32_t *d_flags, cudaStream_t st,
-                              const uint8_t *d_Rbits = nullptr);
+                              const uint8_t *d_Rbits = nullptr, const uint16_t *d_b = nullptr,
+                              const uint8_t *d_mubits = nullptr, uint16_t *d_v = nullptr);
 // N2 (the paper's own PKE variant)
 cudaError_t launch_sample_gauss(Ctx *c, void *d_out, bool as_u16, uint64_t first, uint64_t count, const AesKey &key,
                                 uint32_t tag, uint32_t inst0, uint32_t n_inst, double sigma, cudaStream_t st);

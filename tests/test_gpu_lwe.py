@@ -147,14 +147,17 @@ def run_encaps(H, path, m, n, k, q, batch, A, b, Rbits, mubits):
         return H.host_u16(U), H.host_u16(v)
 
 
-# 3 = CTA-pair tcgen05 GEMM (B operand expanded from R's packed bits inside the kernel where k % 128 == 0),
-# 13 = the same kernel reading the u8 operand expanded into the workspace, 2 = single-CTA tcgen05, 1 = CUDA cores
-ENCAPS_PATHS = dict(argvalues=[3, 13, 2, 1], ids=["tcgen05_pair", "tcgen05_pair_expandedR", "tcgen05", "simt"])
+# 3 = CTA-pair tcgen05 GEMM (B operand expanded from R's packed bits inside the kernel where k % 128 == 0, v computed by
+# spare warps of the same kernel where k = 32 * 2^j), 103 = the same with v from the separate pass over R,
+# 13 = the pair kernel reading the u8 operand expanded into the workspace, 2 = single-CTA tcgen05, 1 = CUDA cores
+ENCAPS_PATHS = dict(argvalues=[3, 103, 13, 2, 1],
+                    ids=["tcgen05_pair", "tcgen05_pair_separate_v", "tcgen05_pair_expandedR", "tcgen05", "simt"])
 
 
 def set_encaps_path(c, path):
     c.set_option(B().OPT_ENCAPS_PATH, path % 10)
-    c.set_option(B().OPT_R_OPERAND, path // 10)
+    c.set_option(B().OPT_R_OPERAND, (path // 10) % 10)
+    c.set_option(B().OPT_V_PATH, path // 100)
 
 
 @pytest.mark.parametrize("path", **ENCAPS_PATHS)
