@@ -38,13 +38,26 @@ struct AesTab {
     uint32_t o0, o1;       // 4*lane, 128 + 4*lane
 };
 
-// Fills the table (all threads of the CTA), synchronises, and returns the calling lane's view.
+// Fills the table (all NT threads of the CTA), synchronises, and returns the calling lane's view.
+// NT = the CTA size, a compile-time constant: the ~16 loads of a thread are then issued back to back and the fill
+// costs one memory latency.  With a run-time stride the loop stays rolled, every store waits for its own load, and
+// 16 serial L2 latencies made ~7 of the ~10 us a sampler launch takes before its first AES block (measured: a sampler
+// call of 8 elements, 10.2 us).
+template <int NT>
 __device__ __forceinline__ AesTab aes_table_to_smem(void *smem, const uint32_t *__restrict__ te0)
 {
     uint32_t *w = reinterpret_cast<uint32_t *>(smem);
-    for (int idx = threadIdx.x; idx < kAesTableBytes / 4; idx += blockDim.x) {
-        const uint32_t t = __ldg(te0 + (idx >> 6));
-        w[idx] = (idx & 32) ? __byte_perm(t, t, 0x2103) : t;      // second half of the row: rotl8
+    constexpr int kWords = kAesTableBytes / 4, kIters = (kWords + NT - 1) / NT;
+    uint32_t t[kIters];
+#pragma unroll
+    for (int it = 0; it < kIters; it++) {
+        const int idx = threadIdx.x + it * NT;
+        t[it] = (idx < kWords) ? __ldg(te0 + (idx >> 6)) : 0u;
+    }
+#pragma unroll
+    for (int it = 0; it < kIters; it++) {
+        const int idx = threadIdx.x + it * NT;
+        if (idx < kWords) w[idx] = (idx & 32) ? __byte_perm(t[it], t[it], 0x2103) : t[it];   // second half of the row: rotl8
     }
     __syncthreads();
     AesTab tab;

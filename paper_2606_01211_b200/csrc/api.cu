@@ -29,6 +29,11 @@ cudaError_t kernel_prepare(Ctx *c, const void *fn, size_t smem, int threads, int
             err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, limit);
             if (err != cudaSuccess) return err;
         }
+        // kernels that need a large dynamic shared memory are launched with the SM's maximal shared-memory carve-out:
+        // the driver's default sized the generator kernels (2 x 64 KB per SM wanted) for ONE resident CTA (ncu:
+        // launch__occupancy_limit_shared_mem = 1)
+        if (smem > 48 * 1024)
+            cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
         if ((int)smem > limit && (int)smem > 48 * 1024) return cudaErrorInvalidValue;
         if (c->n_kcfg >= kMaxKernelCfg) return occ ? cudaErrorInvalidValue : cudaSuccess;   // table full: still configured
         k = &c->kcfg[c->n_kcfg++];

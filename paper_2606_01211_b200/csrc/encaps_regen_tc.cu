@@ -97,7 +97,7 @@ encaps_regen_tc_kernel(const __grid_constant__ CUtensorMap mapR, AesKey key, con
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) tmem_alloc(tmem_slot, kTmemCols);
-    const AesTab tab = aes_table_to_smem(gbase + tab_off, te0);          // all threads; ends with __syncthreads()
+    const AesTab tab = aes_table_to_smem<Cfg::kThreads>(gbase + tab_off, te0);          // all threads; ends with __syncthreads()
     tc_fence_before();
     __syncthreads();
     tc_fence_after();

@@ -87,7 +87,7 @@ keygen_gemv_kernel(const uint16_t *__restrict__ A, AesKey key, const uint32_t *_
     uint32_t *sS = reinterpret_cast<uint32_t *>(smem_raw);                // n/2 words
     uint64_t *sRed = reinterpret_cast<uint64_t *>(smem_raw + 2 * (size_t)n);  // one u64 per warp
     AesTab tab = {};
-    if (kRegen) tab = aes_table_to_smem(smem_raw + 2 * (size_t)n + kRedBytes, te0);
+    if (kRegen) tab = aes_table_to_smem<NT>(smem_raw + 2 * (size_t)n + kRedBytes, te0);
 
     constexpr int kTeams = NT / TPR;
     const uint32_t team = threadIdx.x / TPR, tl = threadIdx.x % TPR;
