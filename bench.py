@@ -746,6 +746,80 @@ PHASES = {"paper_variant_n4096_B32": paper_variant_phase, "paper_variant_n8192_q
           "large_kem_C5_B1": lambda B, device: large_kem_phase(B, device, measured_peaks()["hbm_gbs"])}
 
 
+def pipelined_phase(job: Job, steps: int) -> dict:
+    """N3's pipeline half ("removing sync points"; Alg. 5): consecutive batches alternate between TWO
+    contexts on TWO streams, so that the short kernels of batch i+1 (sampling, keygen) and the decaps of batch i-1 can
+    run in the gaps of batch i's GEMM (mostly its last, partial wave of tiles).  Same work per batch as the headline
+    step (`step`) and as step + FO decapsulation (`step_fo`: decaps with the re-encryption check instead of the plain
+    decaps, i.e. a second GEMM per batch).  KEM/s over `steps` batches, events on both streams, every batch's
+    recovered bits checked at the end."""
+    B, w = job.B, job.w
+    Bt = w.batch
+    dev = job.A.device
+    jobs = [job, Job.__new__(Job)]
+    j1 = jobs[1]
+    j1.B, j1.w, j1.rank, j1.world, j1.step_no = B, w, job.rank, job.world, 0
+    j1.ctx = B.Context(w.n, w.m, w.k, w.q, w.eta, max_batch=Bt, device=dev.index)
+    j1.A = job.A                                               # the public matrix is shared
+    for name in ("s", "e", "b", "Rbits", "mubits", "U", "v", "out"):
+        setattr(j1, name, torch.empty_like(getattr(job, name)))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    okflags = [torch.empty(Bt, dtype=torch.uint8, device=dev) for _ in range(2)]
+    bad = torch.zeros((), dtype=torch.int64, device=dev)
+
+    def run(fo: bool, n_steps: int):
+        e0 = torch.cuda.Event(enable_timing=True)
+        ends = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        e0.record(streams[0])
+        streams[1].wait_event(e0)
+        for i in range(n_steps):
+            x = i & 1
+            j, st = jobs[x], streams[x]
+            i0 = step_instance_ids(job.step_no + i, job.rank, job.world, Bt)[0]
+            with torch.cuda.stream(st):
+                c = j.ctx
+                c.sample_kem(j.s, j.e, j.Rbits, j.mubits, w.seed, i0, Bt)
+                c.keygen(j.A, 0, j.s, j.e, j.b, Bt)
+                c.encaps(j.A, 0, j.b, j.Rbits, j.mubits, j.U, j.v, Bt)
+                if fo:
+                    c.decaps_fo(j.A, j.b, j.U, j.v, j.s, j.Rbits, j.out, okflags[x], Bt)
+                else:
+                    c.decaps(j.U, j.v, j.s, j.out, Bt)
+                if i >= n_steps - 2:
+                    bad.add_((j.out != j.mubits).sum())
+        for x in range(2):
+            ends[x].record(streams[x])
+        torch.cuda.synchronize()
+        job.step_no += n_steps
+        return max(e0.elapsed_time(ends[0]), e0.elapsed_time(ends[1])) / n_steps
+
+    out = {}
+    try:
+        run(False, 6)
+        ms = run(False, steps)
+        out["step"] = {"ms_per_batch": ms, "kem_per_s": Bt * 1e3 / ms}
+        run(True, 4)
+        ms_fo = run(True, steps)
+        out["step_fo"] = {"ms_per_batch": ms_fo, "kem_per_s": Bt * 1e3 / ms_fo,
+                          "all_accepted": bool(okflags[0].all().item() and okflags[1].all().item())}
+        # the same step + FO decaps on ONE stream, for the comparison
+        def serial_fo():
+            c = job.ctx
+            c.sample_kem(job.s, job.e, job.Rbits, job.mubits, w.seed, job.inst0(), Bt)
+            c.keygen(job.A, 0, job.s, job.e, job.b, Bt)
+            c.encaps(job.A, 0, job.b, job.Rbits, job.mubits, job.U, job.v, Bt)
+            c.decaps_fo(job.A, job.b, job.U, job.v, job.s, job.Rbits, job.out, okflags[0], Bt)
+            job.step_no += 1
+        t = time_call(serial_fo, reps=steps, warm=3)
+        out["step_fo_one_stream"] = {"ms_per_batch": t, "kem_per_s": Bt * 1e3 / t}
+        out["mismatching_bytes"] = int(bad.item())
+        out["recipe"] = "two contexts, two streams, batches alternate; a context is never used from two streams at once"
+    finally:
+        j1.ctx.close()
+    return out
+
+
 def run_dry(args):
     """--dry-run: the rank plumbing of the GPU arm on CPU/gloo, no CUDA, no measurement (tests/test_sharding.py)."""
     rank, world, _ = env_rank()
@@ -915,15 +989,19 @@ def run_ours(args):
     t3 = time_call(lambda: ctx.decaps_fo(job.A, job.b, job.U, job.v, job.s, job.Rbits, job.out, okflags, Bt))
     side["decaps_fo_B32"] = {"ms": t3, "per_s": Bt * 1e3 / t3, "all_accepted": bool(okflags.all().item()),
                              "kem_per_s_encaps_plus_fo_decaps_B32": Bt * 1e3 / (t + t3)}
+    side["pipelined_B32"] = pipelined_phase(job, args.steps)
     if not args.quick:
         side["paper_variant_n4096_B32"] = paper_variant_phase(job.B, local)
         side["paper_variant_n8192_q65537_B32"] = paper_variant_wide_phase(job.B, local)
         side["single_kem_B1"] = single_kem_phase(job.B, local)
         side["large_kem_C5_B1"] = large_kem_phase(job.B, local, hbm)
-        buf = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
-        t = time_call(lambda: ctx.rng_fill(buf, buf.numel(), bytes(16), bytes(16), 0), reps=5)
-        side["rng_fill_1GiB"] = {"ms": t, "GBps": buf.numel() / (t * 1e-3) / 1e9}
-        del buf
+    buf = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
+    t = time_call(lambda: ctx.rng_fill(buf, buf.numel(), bytes(16), bytes(16), 0), reps=5)
+    t16 = time_each(lambda: ctx.rng_fill(buf, 16 << 20, bytes(16), bytes(16), 0), reps=20)["median"]
+    side["rng_fill_1GiB"] = {"ms": t, "GBps": buf.numel() / (t * 1e-3) / 1e9,
+                             "frac_of_alu_pipe_bound_805GBps": buf.numel() / (t * 1e-3) / 1e9 / 805.0,
+                             "fill_16MiB_us": t16 * 1e3, "fill_16MiB_GBps": (16 << 20) / (t16 * 1e-3) / 1e9}
+    del buf
 
     # ---- LAST on the device (everything above is burst-regime; these loops leave the chip power-capped and warm for
     # seconds): the same step for >= 3 s with its clock / power record, then the library's int8 GEMM burst + sustained

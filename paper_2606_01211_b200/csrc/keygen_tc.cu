@@ -84,6 +84,9 @@ struct KgWide {
     const uint32_t *row_cnt, *row_cols;
     uint32_t cap;
     const int8_t *s;
+    // 32-bit reduction of the signed sums: bias / ebias are multiples of q above |D| <= 255 * 128 * n and above
+    // |e - delta * corr| (corr = sum of the secrets at the row's exceptions), delta = q - 2^16 (2^16 = -delta mod q)
+    uint32_t bias, ebias, delta;
 };
 
 // 8 * CPI accumulator columns (= 8 instances) of this warp's 32 TMEM lanes
@@ -242,12 +245,15 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
                         const uint32_t inst = i0 + x;
                         if (inst < batch) {
                             if (kWide) {
-                                const int ei = (i0 < 32) ? (int)epre[(i0 + x) & 31] : (int)e8[(size_t)inst * m + i];
-                                long long tot = (long long)(int)r[2 * x] + 256ll * (int)r[2 * x + 1] + ei;
+                                int ei = (i0 < 32) ? (int)epre[(i0 + x) & 31] : (int)e8[(size_t)inst * m + i];
                                 for (uint32_t y = 0; y < exc; y++)         // elements >= 2^16 of this row: rare
-                                    tot += 65536ll * (int)wd.s[(size_t)inst * n + wd.row_cols[(size_t)i * wd.cap + y]];
-                                long long rr = tot % (long long)mq.q;
-                                b32[(size_t)inst * m + i] = (uint32_t)(rr < 0 ? rr + mq.q : rr);
+                                    ei -= (int)wd.delta * (int)wd.s[(size_t)inst * n + wd.row_cols[(size_t)i * wd.cap + y]];
+                                // three 32-bit Barrett steps on biased (non-negative) values; a 64-bit remainder per
+                                // element (~150 instructions) made this epilogue, not HBM, the kernel's limit
+                                // (ncu: 67 us for 136 MB, DRAM 25 %)
+                                b32[(size_t)inst * m + i] =
+                                    mod_u32(mod_u32(r[2 * x] + wd.bias, mq) + 256u * mod_u32(r[2 * x + 1] + wd.bias, mq) +
+                                            ((uint32_t)ei + wd.ebias), mq);
                                 continue;
                             }
                             const uint32_t ei = (i0 < 32) ? epre[(i0 + x) & 31] : (uint32_t)e[(size_t)inst * m + i];
@@ -391,7 +397,10 @@ cudaError_t launch_wide_keygen_tc(Ctx *c, const int8_t *d_s, const int8_t *d_e, 
     const uint32_t strips = (p.m + rps - 1) / rps;
     const uint32_t grid = strips < (uint32_t)c->sm_count ? strips : (uint32_t)c->sm_count;
     ProfScope prof(c, LWE_K_KEYGEN_TC, st);
-    const KgWide wd = {c->d_exc_row_cnt, c->d_exc_row_cols, c->exc_cap_row, d_s};
+    const uint64_t q = p.q, delta = q - 65536u;
+    const uint64_t plane_max = 255ull * 128ull * p.n, e_max = 128ull + delta * 128ull * c->exc_cap_row;
+    const KgWide wd = {c->d_exc_row_cnt, c->d_exc_row_cols, c->exc_cap_row, d_s,
+                       (uint32_t)((plane_max + q - 1) / q * q), (uint32_t)((e_max + q - 1) / q * q), (uint32_t)delta};
     kern<<<grid, kThreads, smem, st>>>(mapA, mapS, d_e, d_t, p.m, p.n, batch, N, stages, c->mq, rps, wd);
     c->launches++;
     return cudaGetLastError();

@@ -474,6 +474,50 @@ def test_two_contexts_of_different_shape_interleaved_on_two_streams(H):
             c.close()
 
 
+def test_pipelined_batches_on_two_contexts_and_streams_with_fo_decaps(H):
+    """The two-context / two-stream pipeline bench.py reports as `pipelined_B32` (S8(f) N3): five consecutive
+    batches alternate between two contexts on two streams (same shape, shared A), each batch = sample_kem -> keygen ->
+    encaps -> decaps with the FO re-encryption check; kernels of neighbouring batches may overlap on the device.
+    Every object of every batch equals the oracle, every honest ciphertext is accepted."""
+    import torch
+    w, n, m, batch, nb = W.C2, 384, 776, 3, 5
+    k, q = w.k, w.q
+    st = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ctxs = [H.make_ctx(w, n=n, m=m, max_batch=batch) for _ in range(2)]
+    dA = H.dev_empty_u16(m, n)
+    ctxs[0].sample_uniform(dA, 0, m * n, w.seed, W.TAG_A)
+    torch.cuda.synchronize()
+    outs = []
+    try:
+        for i in range(nb):
+            c = ctxs[i & 1]
+            with torch.cuda.stream(st[i & 1]):
+                s, e, b = H.dev_empty_u16(batch, n), H.dev_empty_u16(batch, m), H.dev_empty_u16(batch, m)
+                Rb, mu = H.dev_empty_u8(batch, m * k // 8), H.dev_empty_u8(batch, k // 8)
+                U, v = H.dev_empty_u16(batch, n, k), H.dev_empty_u16(batch, k)
+                o, ok = H.dev_empty_u8(batch, k // 8), H.dev_empty_u8(batch)
+                c.sample_kem(s, e, Rb, mu, w.seed, 100 * i, batch)
+                c.keygen(dA, 0, s, e, b, batch)
+                c.encaps(dA, 0, b, Rb, mu, U, v, batch)
+                c.decaps_fo(dA, b, U, v, s, Rb, o, ok, batch)
+                outs.append((i, s, e, b, Rb, mu, U, v, o, ok))
+        torch.cuda.synchronize()
+        A = H.host_u16(dA)
+        assert np.array_equal(A, O.sample_uniform(0, m * n, w.seed, O.TAG_A, 0, q).reshape(m, n))
+        for i, s, e, b, Rb, mu, U, v, o, ok in outs:
+            gb, gU, gv, go, gok = H.host_u16(b), H.host_u16(U), H.host_u16(v), H.host_u8(o), H.host_u8(ok)
+            for t in range(batch):
+                oi = H.OracleInstance(w, 100 * i + t, n, m, with_A=False)
+                ob = O.keygen(A, oi.s, oi.e, q)
+                oU, ov = O.encaps(A, ob, oi.Rbits, oi.mubits, k, q)
+                assert np.array_equal(gb[t], ob) and np.array_equal(gU[t], oU) and np.array_equal(gv[t], ov), (i, t)
+                o_out, o_ok = O.decaps_fo(A, ob, oU, ov, oi.s, oi.Rbits, q)
+                assert np.array_equal(go[t], o_out) and np.array_equal(go[t], oi.mubits) and int(gok[t]) == o_ok == 1, (i, t)
+    finally:
+        for c in ctxs:
+            c.close()
+
+
 def test_contexts_on_two_devices_in_one_process(H):
     """Launch state (shared-memory opt-ins, occupancy) is per context, i.e. per device: after a full pass on device
     0 the same calls on a context of device 1 must work and agree with the oracle.  Needs two GPUs."""
