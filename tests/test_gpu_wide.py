@@ -351,16 +351,18 @@ def test_wide_full_path_small_matches_oracle_everywhere():
         assert np.array_equal(got["out"][b], mu), "not every bit recovered"
 
 
-@pytest.mark.parametrize("n,batch,seeded", [(8192, 32, False), (16384, 8, True)])
-def test_table1_rows_n8192_n16384_sampled_rows_identity_and_recovery(n, batch, seeded):
-    """Table 1 rows 5-6 (q = 65537, sigma = 1.2, e2 in [-2, 2], eta = 3) at full size in the launch
-    configuration bench.py times (n = 8192: 32 instances sharing A).  n = 8192: the oracle draws all of A, so t and v
+@pytest.mark.parametrize("n,batch,seeded,sigma,kappa", [(8192, 32, False, 1.2, 2), (16384, 8, True, 1.2, 2),
+                                                      (32768, 2, True, 1.0, 2), (65536, 1, True, 1.0, 1)])
+def test_table1_rows_q65537_sampled_rows_identity_and_recovery(n, batch, seeded, sigma, kappa):
+    """Table 1 rows 5-8 (P:L98-101: q = 65537; n = 8192, 16384: sigma = 1.2, e2 in [-2, 2]; n = 32768: sigma = 1.0, [-2, 2];
+    n = 65536: sigma = 1.0, [-1, 1]; eta = 3) at full size; n = 8192 in the launch configuration bench.py times (32 instances
+    sharing A).  n = 8192: the oracle draws all of A, so t and v
     are compared in full and 40 sampled rows of U x all 256 columns element by element, on two instances.  n = 16384:
     A is loaded on the device from its seed panel by panel (the uint32 matrix, 1 GiB, never exists) and the oracle
     recomputes 48 sampled rows of t (rows of A are contiguous stream ranges) and 40 sampled rows of U (columns of A
     drawn by counter index).  On the first, a middle and the last instance the exact noise identity over all columns
     ties v to U, s, e, R, E1, e2; every bit of every instance is recovered."""
-    q, sigma, kappa, k, seed, inst0 = F4, 1.2, 2, 256, 8, 16
+    q, k, seed, inst0 = F4, 256, 8, 16
     rng = np.random.default_rng(n)
     trows = np.unique(np.concatenate([[0, 1, n - 1], rng.integers(0, n, 45)]))
     urows = np.unique(np.concatenate([[0, 1, 63, 64, n - 1], rng.integers(0, n, 35)]))
@@ -375,7 +377,7 @@ def test_table1_rows_n8192_n16384_sampled_rows_identity_and_recovery(n, batch, s
         g = device_pke(c, n, k, sigma, kappa, seed, inst0, batch)
         T().cuda.synchronize()
         assert T().equal(g["out"], g["mu"]), "not every bit of every instance recovered"
-        check = sorted({0, batch // 2, batch - 1})
+        check = sorted({0, batch // 2, batch - 1}) if n <= 16384 else [0]      # the oracle's draws of R, E1 cost O(n k)
         got = {name: {b: (host32(x[b]) if x.dtype == T().int32 else host8(x[b])) for b in check} for name, x in g.items()}
     if n <= 8192:
         A = O.sample_uniform32(0, n * n, seed, O.TAG_A, 0, q).reshape(n, n)
@@ -390,7 +392,7 @@ def test_table1_rows_n8192_n16384_sampled_rows_identity_and_recovery(n, batch, s
         assert np.array_equal(got["R"][b], R) and np.array_equal(got["E1"][b], E1) and np.array_equal(got["e2"][b], e2)
         assert noise_identity(got["U"][b], got["v"][b], s, e, R, E1, e2, mu, q), b
         assert np.array_equal(got["out"][b], mu)
-        if b == check[1]:
+        if len(check) > 1 and b == check[1]:
             continue
         if A is not None:
             t = O.keygen_w(A, s, e, q)
