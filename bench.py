@@ -746,7 +746,7 @@ PHASES = {"paper_variant_n4096_B32": paper_variant_phase, "paper_variant_n8192_q
           "large_kem_C5_B1": lambda B, device: large_kem_phase(B, device, measured_peaks()["hbm_gbs"])}
 
 
-def pipelined_phase(job: Job, steps: int) -> dict:
+def pipelined_phase(job: Job, steps: int, sustained_s: float = 0.0) -> dict:
     """N3's pipeline half ("removing sync points"; Alg. 5): consecutive batches alternate between TWO
     contexts on TWO streams, so that the short kernels of batch i+1 (sampling, keygen) and the decaps of batch i-1 can
     run in the gaps of batch i's GEMM (mostly its last, partial wave of tiles).  Same work per batch as the headline
@@ -813,6 +813,19 @@ def pipelined_phase(job: Job, steps: int) -> dict:
             job.step_no += 1
         t = time_call(serial_fo, reps=steps, warm=3)
         out["step_fo_one_stream"] = {"ms_per_batch": t, "kem_per_s": Bt * 1e3 / t}
+        if sustained_s > 0:
+            # the power-capped regime: the same pipeline for >= sustained_s seconds, in blocks of 200 batches; the settled
+            # figure is the median of the last quarter of the blocks
+            blocks = []
+            with ClockSampler(torch.cuda.current_device(), 0.005) as clk:
+                t_end = time.perf_counter() + sustained_s
+                while time.perf_counter() < t_end or len(blocks) < 4:
+                    blocks.append(run(False, 200))
+            tail = blocks[-max(1, len(blocks) // 4):]
+            ms_set = float(np.median(tail))
+            out["step_sustained"] = {"seconds": float(sum(blocks) * 200 / 1e3), "ms_per_batch_first_200": blocks[0],
+                                     "ms_per_batch_settled": ms_set, "kem_per_s_settled": Bt * 1e3 / ms_set,
+                                     "clocks": clk.summary(detail=True)}
         out["mismatching_bytes"] = int(bad.item())
         out["recipe"] = "two contexts, two streams, batches alternate; a context is never used from two streams at once"
     finally:
@@ -990,6 +1003,7 @@ def run_ours(args):
     side["decaps_fo_B32"] = {"ms": t3, "per_s": Bt * 1e3 / t3, "all_accepted": bool(okflags.all().item()),
                              "kem_per_s_encaps_plus_fo_decaps_B32": Bt * 1e3 / (t + t3)}
     side["pipelined_B32"] = pipelined_phase(job, args.steps)
+    pipelined_job = job
     if not args.quick:
         side["paper_variant_n4096_B32"] = paper_variant_phase(job.B, local)
         side["paper_variant_n8192_q65537_B32"] = paper_variant_wide_phase(job.B, local)
@@ -1008,6 +1022,7 @@ def run_ours(args):
     if not args.quick:
         lib_burst = library_int8_gemm(0.0)
         side_sustained = sustained_block(job, 3.0, ms_total / args.steps, peaks)
+        side_sustained["pipelined_two_streams"] = pipelined_phase(pipelined_job, 10, sustained_s=3.0).get("step_sustained")
         lib = library_int8_gemm(3.0)
         lib["burst_TOPs"] = lib_burst.get("burst_TOPs")           # the burst figure taken BEFORE the long loops
     else:
