@@ -166,7 +166,8 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
     if (p->q < 2 || p->q > 65536u + 1024u || p->eta < 1 || p->eta > 8 || p->max_batch < 1) return LWE_ERR_PARAM;
     if (p->k > 2048 || p->n > (1u << 20) || p->m > (1u << 20)) return LWE_ERR_PARAM;
     const bool wide = p->q > 65536u;
-    if (wide && (p->k > 1024 || p->m > 65536u || exc_capacity(p->m, p->q) > 1024u || exc_capacity(p->n, p->q) > 1024u))
+    if (wide && (p->k > 1024 || p->m > 262144u || p->n > 262144u || exc_capacity(p->m, p->q) > 1024u ||
+                 exc_capacity(p->n, p->q) > 1024u))
         return LWE_ERR_UNSUPPORTED;
 
     int ndev = 0;

@@ -195,6 +195,10 @@ struct PvArgs {
     const int8_t *R;
     const uint32_t *exc_cnt, *exc_rows;
     uint32_t exc_cap, delta;              // delta = q - 2^16: 2^16 = -delta (mod q)
+    // wide contexts with m > 65536: the rows are contracted in passes of <= 65536 (a signed byte-plane sum holds no
+    // more); this launch covers rows [row0, row0 + rows) -- only the exceptions in that range count -- and, from the
+    // second pass on (accum), adds the residues already in U (E1 is added by the first pass only: E1 = NULL later)
+    uint32_t row0, rows, accum;
 };
 
 template <uint32_t kStages, uint32_t kTileK, int kMode, bool kBitsB>
@@ -281,7 +285,7 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
             if (kPv && pv.r_inplace) {                     // this half tile inside R [batch][m_full][k]
                 const uint32_t inst = (uint32_t)r_col / k;
                 r_col -= (int32_t)(inst * k);
-                r_row0 = (int32_t)(inst * pv.m_full);      // past the batch: out of range -> zeros
+                r_row0 = (int32_t)(inst * pv.m_full + pv.row0);   // past the batch: out of range -> zeros
             }
             for (uint32_t kb = 0; kb < k_blocks; kb++) {
                 mbar_wait(empty_bar(stage), phase ^ 1);
@@ -431,6 +435,7 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                     const uint32_t cnt = in_range ? exc : 0u;
                     for (uint32_t y = 0; y < cnt; y++) {
                         const uint32_t i = __ldg(pv.exc_rows + (size_t)j * pv.exc_cap + y);
+                        if (i - pv.row0 >= pv.rows) continue;                       // belongs to another row pass
                         const uint4 r4 = __ldg(reinterpret_cast<const uint4 *>(pv.R + ((size_t)inst * pv.m_full + i) * k + c));
                         const uint32_t rw[4] = {r4.x, r4.y, r4.z, r4.w};
 #pragma unroll
@@ -478,6 +483,18 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 if (in_range) {
                     if (kMode == kEpiStorePvW) {
                         uint4 *dst = reinterpret_cast<uint4 *>(U32 + ((size_t)inst * n + j) * k + c);
+                        if (pv.accum) {                                             // a sum of residues is the residue of the sum
+#pragma unroll
+                            for (int x = 0; x < 4; x++) {
+                                const uint4 old = dst[x];
+                                const uint32_t ov[4] = {old.x, old.y, old.z, old.w};
+#pragma unroll
+                                for (int y = 0; y < 4; y++) {
+                                    const uint32_t val = o[4 * x + y] + ov[y];      // < 2q
+                                    o[4 * x + y] = val >= mq.q ? val - mq.q : val;
+                                }
+                            }
+                        }
 #pragma unroll
                         for (int x = 0; x < 4; x++) dst[x] = make_uint4(o[4 * x], o[4 * x + 1], o[4 * x + 2], o[4 * x + 3]);
                     } else {
@@ -494,7 +511,7 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 auto e1_load = [&](uint32_t cb) {
                     const uint32_t col = nt * kTileN + cb + (odd ? 16u : 0u);
                     const uint32_t inst = col / k, c = col - inst * k;
-                    return (j < n && col < ncols_total)
+                    return (E1 != nullptr && j < n && col < ncols_total)
                         ? __ldg(reinterpret_cast<const uint4 *>(E1 + ((size_t)inst * n + j) * k + c)) : make_uint4(0, 0, 0, 0);
                 };
                 uint4 e1cur = e1_load(cb_lo);
@@ -544,6 +561,7 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, void *d_U, uint32_t 
     using Cfg = PairCfg<kStages, kTileK>;
     const lwe_params &p = c->p;
     const uint32_t ncols = batch * p.k;
+    constexpr bool kPvMode = (kMode == kEpiStorePv || kMode == kEpiStorePvW);
     CUtensorMap mapA, mapR;
     // d_A holds rows [row0, row0 + rows) of A; the matching rows of the expanded R follow from row0
     if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, rows, kTileK)) return cudaErrorInvalidValue;
@@ -583,12 +601,14 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, void *d_U, uint32_t 
     pv.exc_rows = c->d_exc_col_rows;
     pv.exc_cap = c->exc_cap_col;
     pv.delta = (uint32_t)delta;
+    pv.row0 = row0;
+    pv.rows = rows;
+    pv.accum = (kPvMode && row0 != 0) ? 1u : 0u;
     // packed bits of R as a byte matrix [batch * m][k / 8]; a bit tile = 128 rows x 16 bytes.  Rows of the panel
     // past `rows` meet zero-filled rows of A, rows past the last instance are zero-filled by TMA.
     CUtensorMap mapBits = mapR;
     if (kBitsB && !make_map_plain_u8(c, &mapBits, d_Rbits, p.k / 8, (uint64_t)batch * p.m, 16, kTileK))
         return cudaErrorInvalidValue;
-    constexpr bool kPvMode = (kMode == kEpiStorePv || kMode == kEpiStorePvW);
     kern<<<2 * pairs, kBitsB ? kThreadsBits : (kPvMode ? kThreadsPv : kThreads), smem_bytes, st>>>(
         mapA, mapR, d_U, d_flags, rows, p.n, p.k, ncols, c->mq, gw, pv, mapBits, row0, p.m, vargs ? *vargs : VArgs{});
     c->launches++;
@@ -644,11 +664,19 @@ cudaError_t launch_encaps_tc2_pv(Ctx *c, const uint16_t *d_A, const int8_t *d_E1
     return launch_pair<6, 128, kEpiStorePv>(c, d_A, d_U, nullptr, d_E1, batch, 0, c->p.m, st, nullptr, d_R, d_R != nullptr);
 }
 
-// N2 on a wide context: A = the packed low-16 matrix + exception lists, U uint32
+// N2 on a wide context: A = the packed low-16 matrix + exception lists, U uint32.  m > 65536: row passes of 65536
+// (Table 1's n = 131072 row), the first adds E1, the later ones add the residues already in U.
 cudaError_t launch_wide_encaps_tc2(Ctx *c, const int8_t *d_R, const int8_t *d_E1, uint32_t *d_U, uint32_t batch, cudaStream_t st)
 {
-    return launch_pair<6, 128, kEpiStorePvW>(c, c->d_A16, d_U, nullptr, d_E1, batch, 0, c->p.m, st, nullptr, d_R,
-                                             encaps_tc2_r_inplace_supported(c, batch));
+    const uint32_t m = c->p.m, step = m < 65536u ? m : 65536u;
+    for (uint32_t row0 = 0; row0 < m; row0 += step) {
+        const uint32_t rows = (m - row0 < step) ? (m - row0) : step;
+        cudaError_t err = launch_pair<6, 128, kEpiStorePvW>(c, c->d_A16 + (size_t)row0 * c->p.n, d_U, nullptr,
+                                                            row0 == 0 ? d_E1 : nullptr, batch, row0, rows, st, nullptr, d_R,
+                                                            encaps_tc2_r_inplace_supported(c, batch));
+        if (err != cudaSuccess) return err;
+    }
+    return cudaSuccess;
 }
 
 }  // namespace lwe

@@ -59,7 +59,9 @@ wide_pack_kernel(const uint32_t *__restrict__ A, uint16_t *__restrict__ A16, uin
 }
 
 // ------------------------------------------------------------------ KeyGen on CUDA cores (one warp per row)
-// t[b][i] = (sum_j A[i][j] s[b][j] + e[b][i]) mod q,  A[i][j] = A16[i][j] + 2^16 [j in exceptions of row i]
+// t[b][i] = (sum_j A[i][j] s[b][j] + e[b][i]) mod q,  A[i][j] = A16[i][j] + 2^16 [j in exceptions of row i].
+// Any n (the tensor-core kernel holds n <= 65536: Table 1's n = 131072 row runs here); 16-byte loads of A16 (8 elements)
+// against 8 secrets, products accumulated in 32 bits (|a s| < 2^23) and flushed into 64 bits every 128 steps.
 __global__ void __launch_bounds__(kThreads)
 wide_keygen_simt_kernel(const uint16_t *__restrict__ A16, const uint32_t *__restrict__ row_cnt,
                         const uint32_t *__restrict__ row_cols, uint32_t cap_row, const int8_t *__restrict__ s,
@@ -67,11 +69,27 @@ wide_keygen_simt_kernel(const uint16_t *__restrict__ A16, const uint32_t *__rest
                         uint32_t q)
 {
     const uint32_t lane = threadIdx.x & 31, warps = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t chunks = n / 8;
     for (uint32_t i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; i < m; i += warps) {
+        const uint4 *Arow = reinterpret_cast<const uint4 *>(A16 + (size_t)i * n);
         for (uint32_t b = 0; b < batch; b++) {
             const int8_t *sb = s + (size_t)b * n;
+            const uint2 *sb8 = reinterpret_cast<const uint2 *>(sb);
             long long acc = 0;
-            for (uint32_t j = lane; j < n; j += 32) acc += (long long)((int)A16[(size_t)i * n + j] * (int)sb[j]);
+            int part = 0;
+            uint32_t since = 0;
+            for (uint32_t c = lane; c < chunks; c += 32) {
+                const uint4 a = __ldg(Arow + c);
+                const uint2 sv = __ldg(sb8 + c);
+                const uint32_t aw[4] = {a.x, a.y, a.z, a.w}, sw[2] = {sv.x, sv.y};
+#pragma unroll
+                for (int x = 0; x < 8; x++) {
+                    const int av = (int)((aw[x >> 1] >> (16 * (x & 1))) & 0xffffu);
+                    part += av * (int)(int8_t)(sw[x >> 2] >> (8 * (x & 3)));
+                }
+                if (++since == 16) { acc += part; part = 0; since = 0; }    // 128 products of < 2^23 each
+            }
+            acc += part;
             const uint32_t cnt = min(row_cnt[i], cap_row);
             for (uint32_t x = lane; x < cnt; x += 32) acc += 65536ll * (int)sb[row_cols[(size_t)i * cap_row + x]];
 #pragma unroll

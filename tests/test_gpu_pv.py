@@ -112,9 +112,9 @@ def test_encaps_pv_extreme_accumulators(H, path):
             assert np.all(gv == (m * (q - 1) * 127 * sign + 3 * sign + q // 2) % q), (q, sign)
 
 
-@pytest.mark.parametrize("n,q,sigma,bound,batch", [(512, 3329, 2.3, 3, 2), (1024, 12289, 2.3, 3, 1)])
+@pytest.mark.parametrize("n,q,sigma,bound,batch", [(512, 3329, 2.3, 3, 2), (1024, 12289, 2.3, 3, 1), (2048, 12289, 2.3, 3, 1)])
 def test_pv_full_path_from_seeds_matches_oracle_and_recovers_every_bit(H, n, q, sigma, bound, batch):
-    """Table 1 rows 1-2: every object drawn on the device from the seed, KeyGen (t = A s + e) ->
+    """Table 1 rows 1-3 (row 4 at the size bench.py times it: tests/test_gpu_fullsize.py): every object drawn on the device from the seed, KeyGen (t = A s + e) ->
     Encrypt (U = A^T R + E1, v = t^T R + e2 + mu q/2) -> Decrypt, each output against the oracle's own draw."""
     import torch
     seed, k, inst0 = 41, 256, 3

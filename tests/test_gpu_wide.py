@@ -237,6 +237,65 @@ def test_wide_encaps_extreme_accumulators(path):
             assert np.all(gv == (m * (q - 1) * 127 * sign + 3 * sign + q // 2) % q), (q, sign)
 
 
+@pytest.mark.parametrize("path", [0, 1], ids=["tcgen05_pair", "simt"])
+def test_wide_encaps_more_than_65536_rows(path):
+    """m = 131072 (Table 1's last row has m = n = 131072): the tensor path contracts the rows in two passes of 65536; the
+    second adds the residues of the first, E1 enters once, and every element >= 2^16 counts in exactly one pass
+    (exceptions sit on both sides of row 65536).  Random operands against the oracle, then the accumulator bounds."""
+    m, n_small, k, batch, q = 131072, 64, 128, 2, F4
+    rng = np.random.default_rng(131072)
+    A = random_A(m, n_small, q, 5, 300)
+    A[65535, :8] = q - 1
+    A[65536, 8:16] = q - 1
+    t = rng.integers(0, q, (batch, m), dtype=np.uint64).astype(np.uint32)
+    R = rng.integers(-12, 13, (batch, m, k)).astype(np.int8)
+    E1 = rng.integers(-12, 13, (batch, n_small, k)).astype(np.int8)
+    e2 = rng.integers(-2, 3, (batch, k)).astype(np.int8)
+    mubits = W.random_bytes(batch * k // 8, 9).reshape(batch, -1)
+    with B().Context(n_small, m, k, q, 3, batch) as c:
+        c.wide_load_matrix(dev32(A))
+        c.set_option(B().OPT_ENCAPS_PATH, path)
+        U, v = empty32(batch, n_small, k), empty32(batch, k)
+        U.fill_(-1)
+        c.wide_encaps(dev32(t), dev8(R), dev8(E1), dev8(e2), T().from_numpy(mubits).cuda(), U, v, batch)
+        gU, gv = host32(U), host32(v)
+        for b in range(batch):
+            Uo, vo = O.encaps_pv_w(A, t[b], R[b], E1[b], e2[b], mubits[b], q)
+            assert np.array_equal(gv[b], vo), ("v", b)
+            assert np.array_equal(gU[b], Uo), ("U", b)
+        # bounds: |R| = 127, low halves 65535, both passes at +/- 255 * 127 * 65536
+        A2 = np.full((m, n_small), 65535, np.uint32)
+        for x in range(4):
+            A2[30000 * x + 7 * np.arange(n_small), np.arange(n_small)] = q - 1     # rows 0 .. 90441: both passes
+        R2 = np.full((1, m, k), -127, np.int8)
+        E12 = np.full((1, n_small, k), -128, np.int8)
+        c.wide_load_matrix(dev32(A2))
+        c.wide_encaps(dev32(t[:1]), dev8(R2), dev8(E12), dev8(e2[:1]), T().from_numpy(mubits[:1]).cuda(), U[:1], v[:1], 1)
+        assert np.all(host32(U[:1]) == (((m - 4) * 65535 + 4 * (q - 1)) * -127 - 128) % q)
+
+
+def test_wide_keygen_beyond_the_tensor_kernels_n():
+    """n = 131072 > 65536 (Table 1's last row): the skinny tensor-core GEMM's byte-plane sums do not hold it, KeyGen
+    runs on the CUDA cores (forcing the tensor path is refused); |s| = 127 puts the 32-bit partial sums at their bound"""
+    m, n, q, batch = 72, 131072, F4, 2
+    rng = np.random.default_rng(7)
+    A = random_A(m, n, q, 13, 200)
+    s = rng.integers(-3, 4, (batch, n)).astype(np.int8)
+    s[1, :] = 127
+    e = rng.integers(-12, 13, (batch, m)).astype(np.int8)
+    with B().Context(n, m, 256, q, 3, batch) as c:
+        c.wide_load_matrix(dev32(A))
+        t = empty32(batch, m)
+        c.wide_keygen(dev8(s), dev8(e), t, batch)
+        g = host32(t)
+        c.set_option(B().OPT_KEYGEN_PATH, 2)
+        with pytest.raises(B().LweError) as ei:
+            c.wide_keygen(dev8(s), dev8(e), t, batch)
+        assert ei.value.code == -5
+    for b in range(batch):
+        assert np.array_equal(g[b], O.keygen_w(A, s[b], e[b], q)), b
+
+
 # ---------------------------------------------------------------- Decrypt
 
 @pytest.mark.parametrize("n,k,q,batch", [(256, 256, F4, 1), (1000, 256, 65539, 3), (64, 8, F4, 2), (4096, 128, 66560, 2),
@@ -403,3 +462,27 @@ def test_table1_rows_q65537_sampled_rows_identity_and_recovery(n, batch, seeded,
             assert np.array_equal(got["t"][b][trows], O.keygen_w(A_rows, s, e[trows], q)), b
             Uo, _ = O.encaps_pv_w(A_cols, np.zeros(n, np.uint32), R, E1[urows], e2, mu, q)
         assert np.array_equal(got["U"][b][urows], Uo), b
+
+
+def test_table1_last_row_n131072_sampled_rows():
+    """Table 1 row 9 (n = 131072, q = 65537, sigma = 1.0, e2 in [-1, 1], eta = 3), one instance: A loaded from
+    its seed panel by panel (A16 = 32 GiB; the uint32 matrix, 64 GiB, never exists), KeyGen on the CUDA cores, Encrypt in two
+    row passes on tcgen05, Decrypt.  40 sampled rows of t and 24 sampled rows of U against the oracle, every bit recovered."""
+    n, q, sigma, kappa, k, seed, inst = 131072, F4, 1.0, 1, 256, 8, 3
+    rng = np.random.default_rng(n)
+    trows = np.unique(np.concatenate([[0, 65535, 65536, n - 1], rng.integers(0, n, 36)]))
+    urows = np.unique(np.concatenate([[0, 63, n - 1], rng.integers(0, n, 21)]))
+    with B().Context(n, n, k, q, 3, 1) as c:
+        c.wide_load_matrix_seeded(seed)
+        g = device_pke(c, n, k, sigma, kappa, seed, inst, 1)
+        T().cuda.synchronize()
+        assert T().equal(g["out"], g["mu"]), "not every bit recovered"
+        got = {name: (host32(x[0]) if x.dtype == T().int32 else host8(x[0])) for name, x in g.items()}
+    s, e, R, E1, e2, mu = oracle_draw(n, k, sigma, kappa, seed, inst)
+    assert np.array_equal(got["s"], s) and np.array_equal(got["e"], e) and np.array_equal(got["R"], R)
+    A_rows = np.stack([O.sample_uniform32(int(i) * n, n, seed, O.TAG_A, 0, q) for i in trows])
+    assert np.array_equal(got["t"][trows], O.keygen_w(A_rows, s, e[trows], q))
+    A_cols = np.stack([O.sample_uniform32_strided(int(j), n, n, seed, O.TAG_A, 0, q) for j in urows], axis=1)
+    Uo, _ = O.encaps_pv_w(A_cols, np.zeros(n, np.uint32), R, E1[urows], e2, mu, q)
+    assert np.array_equal(got["U"][urows], Uo)
+    assert noise_identity(got["U"], got["v"], s, e, R, E1, e2, mu, q)
