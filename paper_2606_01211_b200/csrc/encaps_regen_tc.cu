@@ -58,7 +58,7 @@ __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: 
 
 template <uint32_t G, uint32_t kStages>
 __global__ void __launch_bounds__(RegenCfg<G, kStages>::kThreads, 1)
-encaps_regen_tc_kernel(const __grid_constant__ CUtensorMap mapR, AesKey key, const uint32_t *__restrict__ te0,
+encaps_regen_tc_kernel(const __grid_constant__ CUtensorMap mapR, const __grid_constant__ AesKey key, const uint32_t *__restrict__ te0,
                        uint16_t *__restrict__ U, uint32_t *__restrict__ locks, uint32_t m, uint32_t n, uint32_t k,
                        uint32_t splits, ModQ mq)
 {

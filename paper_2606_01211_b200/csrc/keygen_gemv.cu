@@ -79,7 +79,7 @@ __device__ __forceinline__ uint64_t team_reduce(uint64_t v, uint64_t *sRed)
 // (+ rejection attempts), S8(c) O4 -- the paper's on-demand A.
 template <int TPR, bool kRegen, int UNR, int NT>
 __global__ void __launch_bounds__(NT)
-keygen_gemv_kernel(const uint16_t *__restrict__ A, AesKey key, const uint32_t *__restrict__ te0,
+keygen_gemv_kernel(const uint16_t *__restrict__ A, const __grid_constant__ AesKey key, const uint32_t *__restrict__ te0,
                    const uint16_t *__restrict__ s, const uint16_t *__restrict__ e, uint16_t *__restrict__ b,
                    uint32_t m, uint32_t n, uint32_t batch, ModQ mq)
 {
