@@ -26,6 +26,7 @@ OPT_PANEL_ROWS = 6
 OPT_REGEN_PATH = 7
 OPT_R_OPERAND = 8
 OPT_V_PATH = 9
+OPT_PDL = 10
 KERNELS = ["rng_fill", "sample_uniform", "sample_cbd", "sample_bits", "keygen_stored", "keygen_regen",
            "expand_R_v", "encaps_tc", "encaps_simt", "decaps", "keygen_prep", "keygen_tc", "fo_verdict",
            "sample_gauss", "sample_cuniform", "prep_R_pv", "encaps_regen_tc", "sample_kem", "wide_pack", "wide_keygen"]

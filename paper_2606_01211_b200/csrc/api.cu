@@ -294,6 +294,11 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
         ctx->c.r_operand = (int)value;
         return LWE_OK;
     }
+    if (option == LWE_OPT_PDL) {
+        if (value < 0 || value > 1) return LWE_ERR_PARAM;
+        ctx->c.no_pdl = value ? 0 : 1;
+        return LWE_OK;
+    }
     if (option == LWE_OPT_V_PATH) {
         if (value < 0 || value > 1) return LWE_ERR_PARAM;
         ctx->c.v_path = (int)value;

@@ -40,6 +40,8 @@ decaps_kernel(const uint16_t *__restrict__ U, const uint16_t *__restrict__ v, co
               uint32_t n, uint32_t k, ModQ mq)
 {
     __shared__ uint32_t sLast;
+    pdl_trigger();
+    pdl_wait();
     const uint32_t t = blockIdx.y;                       // instance
     const uint32_t tpr = k / 8;                          // threads per row
     const uint32_t rows_per_iter = kDecThreads / tpr;    // >= 1 (k <= 2048 checked by the host)
@@ -134,9 +136,7 @@ cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, cons
     if (splits < 1) splits = 1;
     dim3 grid(splits, batch);
     ProfScope prof(c, LWE_K_DECAPS, st);
-    decaps_kernel<<<grid, kDecThreads, 0, st>>>(d_U, d_v, d_s, d_out, c->d_dacc, c->d_counters + 8, n, k, c->mq);
-    c->launches++;
-    return cudaGetLastError();
+    return launch_k(c, decaps_kernel, grid, kDecThreads, 0, st, d_U, d_v, d_s, d_out, c->d_dacc, c->d_counters + 8, n, k, c->mq);
 }
 
 // FO verdict (Alg.5 l.4): ok[t] = 1 iff the re-encrypted ciphertext equals the received one, i.e. no

@@ -263,11 +263,13 @@ encaps_tc2_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    pdl_trigger();
     if (warp == 1) tmem_alloc_pair(tmem_slot, kTmemCols);
     tc_fence_before();
     cluster_sync_all();                                           // barriers of BOTH CTAs are initialised
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    pdl_wait();                          // the prologue above overlapped the previous kernel; its outputs are needed now
 
     // The producer and MMA roles run WARP-CONVERGENT loops and elect one lane only around the
     // instructions that must be issued once: inside a divergent `if (lane == 0)` region the compiler
@@ -609,10 +611,9 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, void *d_U, uint32_t 
     CUtensorMap mapBits = mapR;
     if (kBitsB && !make_map_plain_u8(c, &mapBits, d_Rbits, p.k / 8, (uint64_t)batch * p.m, 16, kTileK))
         return cudaErrorInvalidValue;
-    kern<<<2 * pairs, kBitsB ? kThreadsBits : (kPvMode ? kThreadsPv : kThreads), smem_bytes, st>>>(
-        mapA, mapR, d_U, d_flags, rows, p.n, p.k, ncols, c->mq, gw, pv, mapBits, row0, p.m, vargs ? *vargs : VArgs{});
-    c->launches++;
-    return cudaGetLastError();
+    return launch_k(c, kern, 2 * pairs, kBitsB ? kThreadsBits : (kPvMode ? kThreadsPv : kThreads), smem_bytes, st,
+                    mapA, mapR, d_U, d_flags, rows, p.n, p.k, ncols, c->mq, gw, pv, mapBits, row0, p.m,
+                    vargs ? *vargs : VArgs{});
 }
 
 bool encaps_tc2_bits_supported(const Ctx *c, uint32_t batch)

@@ -87,7 +87,9 @@ keygen_gemv_kernel(const uint16_t *__restrict__ A, const __grid_constant__ AesKe
     uint32_t *sS = reinterpret_cast<uint32_t *>(smem_raw);                // n/2 words
     uint64_t *sRed = reinterpret_cast<uint64_t *>(smem_raw + 2 * (size_t)n);  // one u64 per warp
     AesTab tab = {};
+    pdl_trigger();
     if (kRegen) tab = aes_table_to_smem<NT>(smem_raw + 2 * (size_t)n + kRedBytes, te0);
+    pdl_wait();
 
     constexpr int kTeams = NT / TPR;
     const uint32_t team = threadIdx.x / TPR, tl = threadIdx.x % TPR;
@@ -157,9 +159,7 @@ static cudaError_t launch_gemv(Ctx *c, const uint16_t *d_A, const AesKey &key, c
     uint32_t need = (m + kTeams - 1) / kTeams;
     if (grid > need) grid = need;
     ProfScope prof(c, kRegen ? LWE_K_KEYGEN_REGEN : LWE_K_KEYGEN_STORED, st);
-    kern<<<grid, NT, smem, st>>>(d_A, key, c->d_te0, d_s, d_e, d_b, m, n, batch, c->mq);
-    c->launches++;
-    return cudaGetLastError();
+    return launch_k(c, kern, grid, NT, smem, st, d_A, key, c->d_te0, d_s, d_e, d_b, m, n, batch, c->mq);
 }
 
 cudaError_t launch_keygen_stored(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, const uint16_t *d_e,

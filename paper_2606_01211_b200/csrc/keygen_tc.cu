@@ -47,6 +47,8 @@ keygen_prep_kernel(const uint16_t *__restrict__ s, uint16_t *__restrict__ Sx, ui
                    uint32_t cpi)
 {
     // Sx viewed as uint16[ncols][n]: word j of a row = bytes (2j, 2j+1)
+    pdl_trigger();
+    pdl_wait();
     const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t col = blockIdx.y;
     if (j >= n) return;
@@ -67,6 +69,8 @@ keygen_prep_kernel(const uint16_t *__restrict__ s, uint16_t *__restrict__ Sx, ui
 __global__ void __launch_bounds__(256)
 keygen_prep_s8_kernel(const int8_t *__restrict__ s, uint16_t *__restrict__ Sx, uint32_t n, uint32_t batch)
 {
+    pdl_trigger();
+    pdl_wait();
     const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t col = blockIdx.y;
     if (j >= n) return;
@@ -152,11 +156,13 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    pdl_trigger();
     if (warp == 1) tmem_alloc(tmem_slot, tmem_cols);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    pdl_wait();                          // everything above overlapped the previous kernel; its outputs are needed now
 
     // warp-convergent role loops, one elected lane around the issue (see encaps_tc2.cu)
     if (warp == 0) {
@@ -321,9 +327,8 @@ cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, c
     {
         ProfScope prof(c, LWE_K_KEYGEN_PREP, st);
         dim3 grid((p.n + 255) / 256, N);
-        keygen_prep_kernel<<<grid, 256, 0, st>>>(d_s, reinterpret_cast<uint16_t *>(c->d_Sx), p.n, batch, cpi);
-        c->launches++;
-        cudaError_t err = cudaGetLastError();
+        cudaError_t err = launch_k(c, keygen_prep_kernel, grid, 256, 0, st, d_s, reinterpret_cast<uint16_t *>(c->d_Sx), p.n,
+                                   batch, cpi);
         if (err != cudaSuccess) return err;
     }
     CUtensorMap mapA, mapS;
@@ -353,9 +358,7 @@ cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, c
     const uint32_t strips = (p.m + rps - 1) / rps;
     const uint32_t grid = strips < (uint32_t)c->sm_count ? strips : (uint32_t)c->sm_count;
     ProfScope prof(c, LWE_K_KEYGEN_TC, st);
-    kern<<<grid, kThreads, smem, st>>>(mapA, mapS, d_e, d_b, p.m, p.n, batch, N, stages, c->mq, rps, KgWide{});
-    c->launches++;
-    return cudaGetLastError();
+    return launch_k(c, kern, grid, kThreads, smem, st, mapA, mapS, d_e, d_b, p.m, p.n, batch, N, stages, c->mq, rps, KgWide{});
 }
 
 // ---- wide path: t = A s + e on uint32 residues, A = the context's packed matrix (wide.cu)
@@ -373,9 +376,8 @@ cudaError_t launch_wide_keygen_tc(Ctx *c, const int8_t *d_s, const int8_t *d_e, 
     {
         ProfScope prof(c, LWE_K_KEYGEN_PREP, st);
         dim3 grid((p.n + 255) / 256, N);
-        keygen_prep_s8_kernel<<<grid, 256, 0, st>>>(d_s, reinterpret_cast<uint16_t *>(c->d_Sx), p.n, batch);
-        c->launches++;
-        cudaError_t err = cudaGetLastError();
+        cudaError_t err = launch_k(c, keygen_prep_s8_kernel, grid, 256, 0, st, d_s, reinterpret_cast<uint16_t *>(c->d_Sx),
+                                   p.n, batch);
         if (err != cudaSuccess) return err;
     }
     CUtensorMap mapA, mapS;
@@ -401,9 +403,7 @@ cudaError_t launch_wide_keygen_tc(Ctx *c, const int8_t *d_s, const int8_t *d_e, 
     const uint64_t plane_max = 255ull * 128ull * p.n, e_max = 128ull + delta * 128ull * c->exc_cap_row;
     const KgWide wd = {c->d_exc_row_cnt, c->d_exc_row_cols, c->exc_cap_row, d_s,
                        (uint32_t)((plane_max + q - 1) / q * q), (uint32_t)((e_max + q - 1) / q * q), (uint32_t)delta};
-    kern<<<grid, kThreads, smem, st>>>(mapA, mapS, d_e, d_t, p.m, p.n, batch, N, stages, c->mq, rps, wd);
-    c->launches++;
-    return cudaGetLastError();
+    return launch_k(c, kern, grid, kThreads, smem, st, mapA, mapS, d_e, d_t, p.m, p.n, batch, N, stages, c->mq, rps, wd);
 }
 
 }  // namespace lwe

@@ -90,6 +90,7 @@ struct Ctx {
     int regen_path;                   // LWE_OPT_REGEN_PATH
     int r_operand;                    // LWE_OPT_R_OPERAND
     int v_path;                       // LWE_OPT_V_PATH
+    int no_pdl;                       // LWE_OPT_PDL = 0: programmatic dependent launch off
 
     // device tables
     uint32_t *d_te0;                  // 256-entry AES T-table (word = 2S | S<<8 | S<<16 | 3S<<24)
@@ -176,6 +177,33 @@ template <class K>
 inline cudaError_t kernel_prepare(Ctx *c, K fn, size_t smem, int threads = 0, int *occ = nullptr)
 {
     return kernel_prepare(c, reinterpret_cast<const void *>(fn), smem, threads, occ);
+}
+
+// Programmatic dependent launch (the paper's goal of removing sync points, carried down to kernel boundaries).
+// A kernel launched through launch_k may be scheduled while its predecessor in the stream still runs: everything it
+// does before pdl_wait() -- barrier initialisation, TMEM allocation, tensor-map prefetch, the AES table fill -- overlaps
+// the predecessor's tail and the launch latency; pdl_wait() returns once the predecessor has completed and its memory
+// is visible, and NO access to memory another kernel may write or read for writing may precede it.  pdl_trigger()
+// lets the successor be scheduled as soon as every CTA of this kernel has started.  Without the launch attribute
+// (LWE_OPT_PDL = 0) both are no-ops.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <class... KArgs, class... Args>
+inline cudaError_t launch_k(Ctx *c, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = c->no_pdl ? 0 : 1;
+    c->launches++;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
 // host-side key expansion (FIPS-197 5.2) into the kernels' word convention
