@@ -306,6 +306,8 @@ prep_R_pv_and_v_kernel(const uint16_t *__restrict__ tvec, const int8_t *__restri
 {
     __shared__ uint32_t sLast;
     __shared__ unsigned long long sCol[4 * kAuxThreads];
+    pdl_trigger();
+    pdl_wait();
     const uint32_t t = blockIdx.y;
     const uint32_t wpr = k / 4;                          // words per row (k % 8 == 0)
     const uint32_t rows_per_iter = kAuxThreads / wpr ? kAuxThreads / wpr : 1;
@@ -370,11 +372,8 @@ cudaError_t launch_prep_R_pv_and_v(Ctx *c, const uint16_t *d_t, const int8_t *d_
     if (splits < 1) splits = 1;
     dim3 grid(splits, batch);
     ProfScope prof(c, LWE_K_PREP_R_PV, st);
-    prep_R_pv_and_v_kernel<<<grid, kAuxThreads, 0, st>>>(d_t, d_R, d_e2, d_mubits, c->d_Rexp, d_v, c->d_vacc,
-                                                         c->d_counters + 8 + c->p.max_batch, m, k, batch * k, write_Rexp,
-                                                         c->mq);
-    c->launches++;
-    return cudaGetLastError();
+    return launch_k(c, prep_R_pv_and_v_kernel, grid, kAuxThreads, 0, st, d_t, d_R, d_e2, d_mubits, c->d_Rexp, d_v, c->d_vacc,
+                    c->d_counters + 8 + c->p.max_batch, m, k, batch * k, write_Rexp, c->mq);
 }
 
 // CUDA-core U = A^T R + E1 for the int8 R (shapes the tensor path does not take, and its cross-check).

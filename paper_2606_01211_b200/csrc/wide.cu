@@ -111,6 +111,8 @@ wide_v_kernel(const uint32_t *__restrict__ tvec, const int8_t *__restrict__ R, c
 {
     __shared__ uint32_t sLast;
     __shared__ unsigned long long sCol[4 * kThreads];
+    pdl_trigger();
+    pdl_wait();
     const uint32_t b = blockIdx.y;
     const uint32_t wpr = k / 4;
     const uint32_t rows_per_iter = kThreads / wpr ? kThreads / wpr : 1;
@@ -233,6 +235,8 @@ wide_decaps_kernel(const uint32_t *__restrict__ U, const uint32_t *__restrict__ 
 {
     __shared__ uint32_t sLast;
     __shared__ long long sCol[kThreads * 4];
+    pdl_trigger();
+    pdl_wait();
     const uint32_t b = blockIdx.y;
     const uint32_t tpr = k / 4;                          // threads per row (k <= 1024 on this path)
     const uint32_t rows_per_iter = kThreads / tpr;
@@ -355,10 +359,8 @@ cudaError_t launch_wide_v(Ctx *c, const uint32_t *d_t, const int8_t *d_R, const 
     if (splits < 1) splits = 1;
     dim3 grid(splits, batch);
     ProfScope prof(c, LWE_K_PREP_R_PV, st);
-    wide_v_kernel<<<grid, kThreads, 0, st>>>(d_t, d_R, d_e2, d_mubits, c->d_Rexp, d_v, c->d_vacc,
-                                             c->d_counters + 8 + c->p.max_batch, m, k, batch * k, write_Rexp, c->p.q);
-    c->launches++;
-    return cudaGetLastError();
+    return launch_k(c, wide_v_kernel, grid, kThreads, 0, st, d_t, d_R, d_e2, d_mubits, c->d_Rexp, d_v, c->d_vacc,
+                    c->d_counters + 8 + c->p.max_batch, m, k, batch * k, write_Rexp, c->p.q);
 }
 
 cudaError_t launch_wide_encaps_simt(Ctx *c, const int8_t *d_R, const int8_t *d_E1, uint32_t *d_U, uint32_t batch, cudaStream_t st)
@@ -386,9 +388,8 @@ cudaError_t launch_wide_decaps(Ctx *c, const uint32_t *d_U, const uint32_t *d_v,
     if (splits < 1) splits = 1;
     dim3 grid(splits, batch);
     ProfScope prof(c, LWE_K_DECAPS, st);
-    wide_decaps_kernel<<<grid, kThreads, 0, st>>>(d_U, d_v, d_s, d_out, c->d_dacc, c->d_counters + 8, n, k, c->p.q);
-    c->launches++;
-    return cudaGetLastError();
+    return launch_k(c, wide_decaps_kernel, grid, kThreads, 0, st, d_U, d_v, d_s, d_out, c->d_dacc, c->d_counters + 8, n, k,
+                    c->p.q);
 }
 
 }  // namespace lwe

@@ -423,6 +423,48 @@ def test_full_path_small_matches_oracle_everywhere(H, w, n, m, batch):
         assert np.array_equal(g["out"][t], oi.mubits)                # every bit recovered
 
 
+@pytest.mark.parametrize("pdl", [0, 1], ids=["stream_order", "programmatic_dependent_launch"])
+def test_full_path_back_to_back_batches_with_and_without_pdl(H, pdl):
+    """LWE_OPT_PDL: with programmatic dependent launch a kernel's prologue overlaps its predecessor's tail and it waits on
+    the device before touching data.  Six batches enqueued back to back on one stream REUSING the same buffers (so
+    that every kernel overwrites what its predecessor still reads or wrote: write-after-read and read-after-write
+    across every kernel boundary); the last batch and a checksum of all equal the oracle."""
+    import torch
+    w, n, m, batch = W.C3, 512, 1024, 3
+    k, q = w.k, w.q
+    with H.make_ctx(w, n=n, m=m, max_batch=batch) as c:
+        c.set_option(B().OPT_PDL, pdl)
+        dA = H.dev_empty_u16(m, n)
+        c.sample_uniform(dA, 0, m * n, w.seed, W.TAG_A)
+        s, e, b = H.dev_empty_u16(batch, n), H.dev_empty_u16(batch, m), H.dev_empty_u16(batch, m)
+        Rb, mu = H.dev_empty_u8(batch, m * k // 8), H.dev_empty_u8(batch, k // 8)
+        U, v, o = H.dev_empty_u16(batch, n, k), H.dev_empty_u16(batch, k), H.dev_empty_u8(batch, k // 8)
+        acc_v = torch.zeros(batch, k, dtype=torch.int64, device="cuda")
+        bad = torch.zeros((), dtype=torch.int64, device="cuda")
+        for i in range(6):
+            c.sample_kem(s, e, Rb, mu, w.seed, 10 * i, batch)
+            c.keygen(dA, 0, s, e, b, batch)
+            c.encaps(dA, 0, b, Rb, mu, U, v, batch)
+            c.decaps(U, v, s, o, batch)
+            acc_v += v.to(torch.int64) & 0xFFFF
+            bad += (o != mu).sum()
+        torch.cuda.synchronize()
+        assert int(bad.item()) == 0
+        A, gb, gU, gv = H.host_u16(dA), H.host_u16(b), H.host_u16(U), H.host_u16(v)
+        g_acc = acc_v.cpu().numpy()
+    want_acc = np.zeros((batch, k), np.int64)
+    for i in range(6):
+        for t in range(batch):
+            oi = H.OracleInstance(w, 10 * i + t, n, m, with_A=False)
+            ob = O.keygen(A, oi.s, oi.e, q)
+            ov = O.encaps_v(ob, oi.Rbits, oi.mubits, k, q)
+            want_acc[t] += ov
+            if i == 5:
+                oU, ov2 = O.encaps(A, ob, oi.Rbits, oi.mubits, k, q)
+                assert np.array_equal(gb[t], ob) and np.array_equal(gU[t], oU) and np.array_equal(gv[t], ov2)
+    assert np.array_equal(g_acc, want_acc)
+
+
 def test_two_contexts_of_different_shape_interleaved_on_two_streams(H):
     """Two contexts (different n, m, q, eta) driven alternately on two streams, several rounds: the per-kernel launch
     state the library caches (shared-memory attributes, occupancy, grids) must not leak between shapes, and the two
