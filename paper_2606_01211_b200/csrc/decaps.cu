@@ -54,9 +54,10 @@ decaps_kernel(const uint16_t *__restrict__ U, const uint16_t *__restrict__ v, co
 #pragma unroll
     for (int x = 0; x < 8; x++) a[x] = 0;
     if (active) {
-        // a CTA streams one contiguous range of rows; 4 independent 16-byte loads in flight per thread:
-        // the pass is HBM-bound (2nk bytes of U)
-        constexpr int kUnroll = 4;
+        // a CTA streams one contiguous range of rows; 8 independent 16-byte loads in flight per thread: the pass is
+        // HBM-bound (2nk bytes of U) only with ~100 KB in flight per SM (4 loads per thread left it latency-bound at
+        // 4.2 TB/s: ncu, round 2)
+        constexpr int kUnroll = 8;
         const uint32_t per_cta = ((n + gridDim.x - 1) / gridDim.x + rows_per_iter - 1) / rows_per_iter * rows_per_iter;
         const uint32_t jbeg = blockIdx.x * per_cta, jend = min(n, jbeg + per_cta);
         const size_t row_u4 = k / 8;                      // uint4 per row
