@@ -407,6 +407,11 @@ class Job:
         self.ctx.kem_host(self.A, 0, self.h_s, self.h_e, self.h_R, self.h_mu, self.h_b, self.h_U, self.h_v,
                           self.h_out, self.w.batch)
 
+    def e2e_step_no_U(self):
+        """the same call with h_U = NULL (an optional output of lwe_kem_host): the ciphertext matrix stays on the device"""
+        self.ctx.kem_host(self.A, 0, self.h_s, self.h_e, self.h_R, self.h_mu, self.h_b, None, self.h_v,
+                          self.h_out, self.w.batch)
+
 
 def timed(fn, steps: int, world: int):
     """K calls of fn between barriers/synchronize, CUDA events on the current stream.  Returns (ms total from the
@@ -909,6 +914,10 @@ def run_ours(args):
     ok = ok and bool(torch.equal(job.h_out, job.h_mu))
     ms_e2e, _ = reduce_over_ranks(ms_e2e_total / args.steps, Bt)
     e2e_value = units / (ms_e2e * 1e-3)
+    # context for the number above (which is PCIe-bound on the 128 MiB of U per step): the same call without reading U back
+    ms_e2e_nou_total, _ = timed(job.e2e_step_no_U, args.steps, world)
+    ok = ok and bool(torch.equal(job.h_out, job.h_mu))
+    ms_e2e_nou, _ = reduce_over_ranks(ms_e2e_nou_total / args.steps, Bt)
 
     if rank != 0:
         if world > 1:
@@ -1050,7 +1059,11 @@ def run_ours(args):
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": job.h2d, "d2h_bytes_per_step": job.d2h,
                 "ms_per_step": ms_e2e, "ms_per_step_stats_rank0": stats_ms(per_e2e),
-                "api": "lwe_kem_host (pinned host buffers; ciphertext U,v and b copied back)"},
+                "api": "lwe_kem_host (pinned host buffers; ciphertext U,v and b copied back)",
+                "d2h_GBps": job.d2h / (ms_e2e * 1e-3) / 1e9,
+                "without_reading_U_back": {"value": units / (ms_e2e_nou * 1e-3), "ms_per_step": ms_e2e_nou,
+                                           "d2h_bytes_per_step": job.d2h - job.h_U.numel() * job.h_U.element_size(),
+                                           "note": "h_U = NULL: context only, the headline e2e copies the whole ciphertext"}},
         "gpu_launches": int(launches),
         "roofline": roofline,
         "dominant_kernel_share_of_step": (gemm_ms / args.steps) / (ms_total / args.steps) if gemm_cnt else None,
