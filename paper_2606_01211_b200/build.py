@@ -55,8 +55,6 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False, extra_flags=()) -> Path:
-    """LWE_NVCC_EXTRA (environment, optional): extra nvcc flags, e.g. -DLWE_RNG_THREADS=256 for a sweep."""
-    extra_flags = [*extra_flags, *os.environ.get("LWE_NVCC_EXTRA", "").split()]
     if not force and not needs_build():
         return LIB
     nvcc = _nvcc()

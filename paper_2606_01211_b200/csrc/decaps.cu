@@ -20,25 +20,38 @@ __device__ __forceinline__ uint4 ldg_stream16(const uint4 *p)
     return r;
 }
 
-// acc += x * y with a 32 x 32 -> 64 bit multiply-add (one IMAD.WIDE)
-__device__ __forceinline__ void mad_wide(unsigned long long &acc, uint32_t x, uint32_t y)
-{
-    asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc) : "r"(x), "r"(y));
-}
+// Column accumulators of one thread (8 adjacent columns).  kAcc32 = false: u64 sums of the 32-bit products (exact for any
+// q; one IMAD.WIDE and one unpack instruction per element).  kAcc32 = true (q a power of two): u32 sums that wrap mod 2^32 --
+// exact mod q because q | 2^32 -- of products that keep the neighbouring column's bits above bit 15 (no mask: the low 16
+// bits of u * s depend only on the low 16 bits of u), i.e. one IMAD per element and one shift per pair: half the issue slots.
+template <bool kAcc32> struct ColAcc;
+template <> struct ColAcc<false> {
+    typedef unsigned long long T;
+    static __device__ __forceinline__ void mad(T &acc, uint32_t x, uint32_t y) { asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc) : "r"(x), "r"(y)); }
+    static __device__ __forceinline__ void row(T (&a)[8], const uint4 &u, uint32_t sj)
+    {
+        mad(a[0], u.x & 0xffffu, sj); mad(a[1], u.x >> 16, sj);
+        mad(a[2], u.y & 0xffffu, sj); mad(a[3], u.y >> 16, sj);
+        mad(a[4], u.z & 0xffffu, sj); mad(a[5], u.z >> 16, sj);
+        mad(a[6], u.w & 0xffffu, sj); mad(a[7], u.w >> 16, sj);
+    }
+};
+template <> struct ColAcc<true> {
+    typedef uint32_t T;
+    static __device__ __forceinline__ void row(T (&a)[8], const uint4 &u, uint32_t sj)
+    {
+        a[0] += u.x * sj; a[1] += (u.x >> 16) * sj; a[2] += u.y * sj; a[3] += (u.y >> 16) * sj;
+        a[4] += u.z * sj; a[5] += (u.z >> 16) * sj; a[6] += u.w * sj; a[7] += (u.w >> 16) * sj;
+    }
+};
 
-__device__ __forceinline__ void accumulate_row(unsigned long long (&a)[8], const uint4 &u, uint32_t sj)
-{
-    mad_wide(a[0], u.x & 0xffffu, sj); mad_wide(a[1], u.x >> 16, sj);
-    mad_wide(a[2], u.y & 0xffffu, sj); mad_wide(a[3], u.y >> 16, sj);
-    mad_wide(a[4], u.z & 0xffffu, sj); mad_wide(a[5], u.z >> 16, sj);
-    mad_wide(a[6], u.w & 0xffffu, sj); mad_wide(a[7], u.w >> 16, sj);
-}
-
+template <bool kAcc32>
 __global__ void __launch_bounds__(kDecThreads)
 decaps_kernel(const uint16_t *__restrict__ U, const uint16_t *__restrict__ v, const uint16_t *__restrict__ s,
               uint8_t *__restrict__ out, unsigned long long *__restrict__ acc, unsigned int *__restrict__ tickets,
               uint32_t n, uint32_t k, ModQ mq)
 {
+    typedef typename ColAcc<kAcc32>::T AccT;
     __shared__ uint32_t sLast;
     pdl_trigger();
     pdl_wait();
@@ -50,48 +63,66 @@ decaps_kernel(const uint16_t *__restrict__ U, const uint16_t *__restrict__ v, co
     const uint16_t *Ut = U + (size_t)t * n * k;
     const uint16_t *st = s + (size_t)t * n;
 
-    unsigned long long a[8];
+    AccT a[8];
 #pragma unroll
     for (int x = 0; x < 8; x++) a[x] = 0;
     if (active) {
-        // a CTA streams one contiguous range of rows; 8 independent 16-byte loads in flight per thread: the pass is
-        // HBM-bound (2nk bytes of U) only with ~100 KB in flight per SM (4 loads per thread left it latency-bound at
-        // 4.2 TB/s: ncu, round 2)
-        constexpr int kUnroll = 8;
+        // A CTA streams one contiguous range of rows, software-pipelined in registers: the loads of the next batch of
+        // kUnroll rows are issued before the current batch is consumed, so every thread has 4-8 independent 16-byte loads
+        // in flight at all times (the pass is HBM-bound -- 2nk bytes of U -- only with ~100 KB in flight per SM; with
+        // load-then-consume batches the kernel sat at 4.4 TB/s, a pure load loop of the same shape reaches 6.4).  Every
+        // batch is a full one: a row past the end of the range re-reads the instance's first row (a valid address) with
+        // s = 0, so that no thread ever walks a tail of single, latency-bound loads.
+        constexpr int kUnroll = 4;
         const uint32_t per_cta = ((n + gridDim.x - 1) / gridDim.x + rows_per_iter - 1) / rows_per_iter * rows_per_iter;
         const uint32_t jbeg = blockIdx.x * per_cta, jend = min(n, jbeg + per_cta);
         const size_t row_u4 = k / 8;                      // uint4 per row
         uint32_t j = jbeg + rslot;
         const uint4 *up = reinterpret_cast<const uint4 *>(Ut) + (size_t)j * row_u4 + cg;
         const size_t ustep = (size_t)rows_per_iter * row_u4;
-        for (; j + (kUnroll - 1) * rows_per_iter < jend; j += kUnroll * rows_per_iter, up += kUnroll * ustep) {
-            uint4 u[kUnroll];
-            uint32_t sj[kUnroll];
+        const uint32_t jstep = kUnroll * rows_per_iter;
+        uint4 u0[kUnroll], u1[kUnroll];
+        uint32_t s0[kUnroll], s1[kUnroll];
+        auto load = [&](uint4 (&uu)[kUnroll], uint32_t (&ss)[kUnroll]) {
 #pragma unroll
             for (int r = 0; r < kUnroll; r++) {
-                u[r] = ldg_stream16(up + r * ustep);
-                sj[r] = __ldg(st + j + r * rows_per_iter);
+                const bool in = j + r * rows_per_iter < jend;
+                uu[r] = ldg_stream16(in ? up + r * ustep : reinterpret_cast<const uint4 *>(Ut) + cg);
+                ss[r] = in ? (uint32_t)__ldg(st + j + r * rows_per_iter) : 0u;
             }
+            j += jstep;
+            up += kUnroll * ustep;
+        };
+        if (j < jend) {
+            load(u0, s0);
+            for (;;) {
+                const bool more1 = j < jend;
+                if (more1) load(u1, s1);
 #pragma unroll
-            for (int r = 0; r < kUnroll; r++) accumulate_row(a, u[r], sj[r]);
+                for (int r = 0; r < kUnroll; r++) ColAcc<kAcc32>::row(a, u0[r], s0[r]);
+                if (!more1) break;
+                const bool more0 = j < jend;
+                if (more0) load(u0, s0);
+#pragma unroll
+                for (int r = 0; r < kUnroll; r++) ColAcc<kAcc32>::row(a, u1[r], s1[r]);
+                if (!more0) break;
+            }
         }
-        for (; j < jend; j += rows_per_iter, up += ustep) accumulate_row(a, ldg_stream16(up), __ldg(st + j));
     }
     // sum the row slots of the CTA in shared memory, then one atomic per column per CTA.  Staged [row slot][column]:
-    // a thread stores its 8 columns as 64 contiguous bytes and thread c then reads column c of every slot -- consecutive
-    // 8-byte words across a warp in both phases (the earlier [x][thread] layout read 8 lanes from one bank: 660 k
+    // a thread stores its 8 columns contiguously and thread c then reads column c of every slot -- consecutive
+    // words across a warp in both phases (the earlier [x][thread] layout read 8 lanes from one bank: 660 k
     // conflicts per launch at C4, ncu)
-    __shared__ __align__(16) unsigned long long sCol[kDecThreads * 8];
-    {
-        ulonglong2 *dst = reinterpret_cast<ulonglong2 *>(sCol + (size_t)threadIdx.x * 8);   // = [rslot][cg * 8 + x]
-        dst[0] = make_ulonglong2(a[0], a[1]); dst[1] = make_ulonglong2(a[2], a[3]);
-        dst[2] = make_ulonglong2(a[4], a[5]); dst[3] = make_ulonglong2(a[6], a[7]);
-    }
+    __shared__ __align__(16) AccT sCol[kDecThreads * 8];
+#pragma unroll
+    for (int x = 0; x < 8; x++) sCol[(size_t)threadIdx.x * 8 + x] = a[x];   // = [rslot][cg * 8 + x], vectorised by the compiler
     __syncthreads();
     for (uint32_t c = threadIdx.x; c < k; c += kDecThreads) {
-        unsigned long long sum = 0;
+        AccT sum = 0;
         for (uint32_t rs = 0; rs < rows_per_iter; rs++) sum += sCol[(size_t)rs * k + c];
-        if (sum) atomicAdd(acc + (size_t)t * k + c, sum);
+        // u32 sums (q | 2^32) are added into the low word of the u64 accumulator: a carry into the high word is harmless,
+        // the finalize step reduces mod q
+        if (sum) atomicAdd(acc + (size_t)t * k + c, (unsigned long long)sum);
     }
     __threadfence();
     __syncthreads();
@@ -121,15 +152,16 @@ decaps_kernel(const uint16_t *__restrict__ U, const uint16_t *__restrict__ v, co
     if (threadIdx.x == 0) tickets[t] = 0;
 }
 
-cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
-                          uint8_t *d_out, uint32_t batch, cudaStream_t st)
+template <bool kAcc32>
+static cudaError_t launch_decaps_t(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
+                                   uint8_t *d_out, uint32_t batch, cudaStream_t st)
 {
     const uint32_t n = c->p.n, k = c->p.k;
     const uint32_t rows_per_iter = kDecThreads / (k / 8);
     // exactly one wave of resident CTAs (a second, partial wave was the tail: 1184 CTAs on 740 slots ran at
     // 0.54 of HBM): as many row splits per instance as fit the SMs at the kernel's occupancy
     int per_sm = 1;
-    cudaError_t perr = kernel_prepare(c, decaps_kernel, 0, kDecThreads, &per_sm);
+    cudaError_t perr = kernel_prepare(c, decaps_kernel<kAcc32>, 0, kDecThreads, &per_sm);
     if (perr != cudaSuccess) return perr;
     uint32_t splits = (uint32_t)(per_sm * c->sm_count) / batch;
     uint32_t max_splits = (n + 4 * rows_per_iter - 1) / (4 * rows_per_iter);       // >= 4 row groups per CTA
@@ -137,7 +169,14 @@ cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, cons
     if (splits < 1) splits = 1;
     dim3 grid(splits, batch);
     ProfScope prof(c, LWE_K_DECAPS, st);
-    return launch_k(c, decaps_kernel, grid, kDecThreads, 0, st, d_U, d_v, d_s, d_out, c->d_dacc, c->d_counters + 8, n, k, c->mq);
+    return launch_k(c, decaps_kernel<kAcc32>, grid, kDecThreads, 0, st, d_U, d_v, d_s, d_out, c->d_dacc, c->d_counters + 8, n, k, c->mq);
+}
+
+cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
+                          uint8_t *d_out, uint32_t batch, cudaStream_t st)
+{
+    return c->mq.pow2 ? launch_decaps_t<true>(c, d_U, d_v, d_s, d_out, batch, st)
+                      : launch_decaps_t<false>(c, d_U, d_v, d_s, d_out, batch, st);
 }
 
 // FO verdict (Alg.5 l.4): ok[t] = 1 iff the re-encrypted ciphertext equals the received one, i.e. no
