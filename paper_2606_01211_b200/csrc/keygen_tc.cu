@@ -37,10 +37,9 @@ using namespace tc;
 
 constexpr uint32_t kTileM = 128;          // rows of A per strip
 constexpr uint32_t kTileK = 128;          // bytes of k' per stage (= 64 columns of A)
-constexpr uint32_t kBytesA = kTileM * kTileK;
 constexpr uint32_t kThreads = 192;
 constexpr uint32_t kMaxStages = 8;
-constexpr uint32_t kSmemBudget = 200 * 1024;
+constexpr uint32_t kSmemBudget = 208 * 1024;      // ring; + one A tile of slack + alignment + barriers <= 227 KB
 
 __global__ void __launch_bounds__(256)
 keygen_prep_kernel(const uint16_t *__restrict__ s, uint16_t *__restrict__ Sx, uint32_t n, uint32_t batch,
@@ -121,11 +120,15 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     uint16_t *b = static_cast<uint16_t *>(b_);
     const int8_t *e8 = static_cast<const int8_t *>(e_);
     uint32_t *b32 = static_cast<uint32_t *>(b_);
-    // rps = rows of A per strip (<= 128, a multiple of 8; the TMA box of A has rps rows).  The MMA is always
-    // M = 128: rows rps..127 of the accumulator come from stale shared memory and are never read back.
+    // rps = rows of A per strip (<= 128, a multiple of 8; the TMA box of A has rps rows) and an A slab of the ring
+    // holds exactly those rows (rps * 128 bytes = whole 1 KB swizzle atoms).  The MMA is always M = 128: rows rps..127 of
+    // the accumulator are computed from whatever follows the slab in shared memory (the next slab, the S tiles, the next
+    // stage; the allocation ends with one A tile of slack for the last stage) and are never read back.  The ring is latency-bound (a stage is released only when its MMAs have completed), so what
+    // a short strip does not use buys more stages: 6 instead of 4 at the wide n = 8192 shape (56-row strips).
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t base = (raw + 1023u) & ~1023u;
+    const uint32_t kBytesA = rps * kTileK;
     const uint32_t bytes_slab = kBytesA + N * kTileK;
     const uint32_t bytes_stage = SLABS * bytes_slab;
     const uint32_t tx_stage = SLABS * (rps * kTileK + N * kTileK);          // bytes TMA delivers per stage
@@ -236,6 +239,18 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
                 epre[x] = (row_ok && x < batch) ? (kWide ? (uint32_t)(int)__ldg(e8 + (size_t)x * m + i)
                                                          : (uint32_t)__ldg(e + (size_t)x * m + i)) : 0u;
             const uint32_t exc = (kWide && row_ok) ? min(__ldg(wd.row_cnt + i), wd.cap) : 0u;
+            if (kWide) {
+                // the 2^16-weighted elements of this row (about one row in eight has one): their secrets are folded into
+                // the prefetched e here, 32 independent loads per exception, while the main loop still runs.  Inside the
+                // instance loop below the same sum was a dependent load chain per instance (~0.7 us each with nothing to
+                // hide it: 58 us for 32 instances against 32 us for 8, ncu)
+                for (uint32_t y = 0; y < exc; y++) {
+                    const uint32_t col = __ldg(wd.row_cols + (size_t)i * wd.cap + y);
+#pragma unroll
+                    for (uint32_t x = 0; x < 32; x++)
+                        if (x < batch) epre[x] -= wd.delta * (uint32_t)(int)__ldg(wd.s + (size_t)x * n + col);
+                }
+            }
             mbar_wait(tfull_bar(acc), acc_phase);
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((quarter * 32) << 16) + acc * acc_cols;
@@ -251,9 +266,14 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
                         const uint32_t inst = i0 + x;
                         if (inst < batch) {
                             if (kWide) {
-                                int ei = (i0 < 32) ? (int)epre[(i0 + x) & 31] : (int)e8[(size_t)inst * m + i];
-                                for (uint32_t y = 0; y < exc; y++)         // elements >= 2^16 of this row: rare
-                                    ei -= (int)wd.delta * (int)wd.s[(size_t)inst * n + wd.row_cols[(size_t)i * wd.cap + y]];
+                                int ei;
+                                if (i0 < 32) {
+                                    ei = (int)epre[(i0 + x) & 31];           // e minus the exception terms, prefetched
+                                } else {
+                                    ei = (int)e8[(size_t)inst * m + i];
+                                    for (uint32_t y = 0; y < exc; y++)     // elements >= 2^16 of this row: rare
+                                        ei -= (int)wd.delta * (int)wd.s[(size_t)inst * n + wd.row_cols[(size_t)i * wd.cap + y]];
+                                }
                                 // three 32-bit Barrett steps on biased (non-negative) values; a 64-bit remainder per
                                 // element (~150 instructions) made this epilogue, not HBM, the kernel's limit
                                 // (ncu: 67 us for 136 MB, DRAM 25 %)
@@ -298,6 +318,19 @@ uint32_t cols_per_inst(const lwe_params &p)
 // 8 instances per epilogue step and 16-column MMA granularity: whole groups of 8 instances
 uint32_t padded_cols(uint32_t batch, uint32_t cpi) { return (((batch + 7u) & ~7u) * cpi + 15u) & ~15u; }
 
+// Ring shape for strips of rps rows and N operand columns: slabs per stage as wide as leaves >= 3 stages in flight,
+// then as many stages as fit.  Returns the dynamic shared-memory size (ring + the slack an M = 128 MMA may read past a
+// short last slab + alignment + barriers).
+uint32_t ring_shape(uint32_t rps, uint32_t N, uint32_t *slabs, uint32_t *stages)
+{
+    const uint32_t bytes_slab = rps * kTileK + N * kTileK;
+    *slabs = (3 * 2 * bytes_slab <= kSmemBudget) ? 2 : 1;
+    const uint32_t bytes_stage = *slabs * bytes_slab;
+    *stages = kSmemBudget / bytes_stage;
+    if (*stages > kMaxStages) *stages = kMaxStages;
+    return *stages * bytes_stage + kTileM * kTileK + 1024 + 256;
+}
+
 }  // namespace
 
 size_t keygen_tc_workspace_bytes(const lwe_params &p)
@@ -340,13 +373,8 @@ cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, c
     if (rps < 8) rps = 8;
     if (!make_map_u8(c, &mapA, d_A, 2ull * p.n, p.m, rps)) return cudaErrorInvalidValue;
     if (!make_map_u8(c, &mapS, c->d_Sx, 2ull * p.n, N, N)) return cudaErrorInvalidValue;
-    // slabs per stage: as wide as leaves >= 3 stages in flight
-    const uint32_t bytes_slab = kBytesA + N * kTileK;
-    const uint32_t slabs = (3 * 2 * bytes_slab <= kSmemBudget) ? 2 : 1;
-    const uint32_t bytes_stage = slabs * bytes_slab;
-    uint32_t stages = kSmemBudget / bytes_stage;
-    if (stages > kMaxStages) stages = kMaxStages;
-    const uint32_t smem = stages * bytes_stage + 1024 + 256;
+    uint32_t slabs, stages;
+    const uint32_t smem = ring_shape(rps, N, &slabs, &stages);
     typedef void (*Kern)(const CUtensorMap, const CUtensorMap, const void *, void *, uint32_t, uint32_t, uint32_t,
                          uint32_t, uint32_t, ModQ, uint32_t, KgWide);
     static const Kern table[3][2] = {{keygen_tc_kernel<2, 1>, keygen_tc_kernel<2, 2>},
@@ -387,12 +415,8 @@ cudaError_t launch_wide_keygen_tc(Ctx *c, const int8_t *d_s, const int8_t *d_e, 
     if (rps < 8) rps = 8;
     if (!make_map_u8(c, &mapA, c->d_A16, 2ull * p.n, p.m, rps)) return cudaErrorInvalidValue;
     if (!make_map_u8(c, &mapS, c->d_Sx, 2ull * p.n, N, N)) return cudaErrorInvalidValue;
-    const uint32_t bytes_slab = kBytesA + N * kTileK;
-    const uint32_t slabs = (3 * 2 * bytes_slab <= kSmemBudget) ? 2 : 1;
-    const uint32_t bytes_stage = slabs * bytes_slab;
-    uint32_t stages = kSmemBudget / bytes_stage;
-    if (stages > kMaxStages) stages = kMaxStages;
-    const uint32_t smem = stages * bytes_stage + 1024 + 256;
+    uint32_t slabs, stages;
+    const uint32_t smem = ring_shape(rps, N, &slabs, &stages);
     auto kern = slabs == 2 ? keygen_tc_kernel<2, 2, true> : keygen_tc_kernel<2, 1, true>;
     cudaError_t perr = kernel_prepare(c, kern, smem);
     if (perr != cudaSuccess) return perr;
