@@ -101,6 +101,63 @@ keygen_gemv_kernel(const uint16_t *__restrict__ A, const __grid_constant__ AesKe
     for (uint32_t t = 0; t < batch; t++) {
         if (t) __syncthreads();
         pack_s_to_smem(sS, s + (size_t)t * n, n);
+        if (!kRegen && TPR == 32) {
+            // Stored A, a warp per row: software-pipelined in registers over the warp's whole sequence of (row, batch)
+            // positions -- the loads of the next batch (of this row or of the warp's next row) are issued before the
+            // current batch is consumed, so a lane always has UNR..2 UNR independent 16-byte loads in flight.  With
+            // load-then-consume batches the pass sat at 5.4 TB/s; a pure load loop of the same shape reaches 6.4.
+            uint4 a0[UNR], a1[UNR];
+            auto load = [&](uint4 (&a)[UNR], uint32_t i, uint32_t c0) {
+                const uint4 *Arow = reinterpret_cast<const uint4 *>(A + (size_t)i * n);
+#pragma unroll
+                for (int u = 0; u < UNR; u++) {
+                    const uint32_t c = c0 + u * TPR;
+                    if (c < chunks) a[u] = ldg_stream(Arow + c);
+                    else a[u] = make_uint4(0, 0, 0, 0);
+                }
+            };
+            uint64_t sum_lo = 0, sum_hi = 0;
+            uint32_t lo = 0, hi = 0, since = 0;
+            // consumes the batch at (i, c0); `last` = it is the row's last batch: reduce and write b[i]
+            auto consume = [&](const uint4 (&a)[UNR], uint32_t i, uint32_t c0, bool last) {
+#pragma unroll
+                for (int u = 0; u < UNR; u++) {
+                    const uint32_t c = c0 + u * TPR;
+                    const uint4 sw = (c < chunks) ? sS4[c] : make_uint4(0, 0, 0, 0);
+                    dot8(a[u], sw, lo, hi);
+                }
+                since += UNR;
+                if (!mq.pow2 && (since >= kFlushEvery || last)) {
+                    sum_lo += lo; sum_hi += hi; lo = 0; hi = 0; since = 0;
+                }
+                if (!last) return;
+                uint64_t total = mq.pow2 ? (uint64_t)(lo + (hi << 8)) : sum_lo + (sum_hi << 8);   // pow2: exact mod 2^32, q | 2^32
+                total = team_reduce<TPR, NT>(total, sRed);
+                if (tl == 0) {
+                    const uint32_t ei = e[(size_t)t * m + i];
+                    const uint32_t r = mq.pow2 ? (((uint32_t)total + ei) & mq.mask) : mod_u64(total + ei, mq);
+                    b[(size_t)t * m + i] = (uint16_t)r;
+                }
+                sum_lo = sum_hi = 0; lo = hi = 0; since = 0;
+            };
+            constexpr uint32_t kStep = UNR * TPR;
+            uint32_t ci = row0, cc = tl;                     // current position; the next one follows below
+            if (ci < m) load(a0, ci, cc);
+            while (ci < m) {
+                uint32_t ni = ci, nc = cc + kStep;
+                if (nc >= chunks) { ni = ci + row_step; nc = tl; }
+                if (ni < m) load(a1, ni, nc);
+                consume(a0, ci, cc, ni != ci);
+                if (ni >= m) break;
+                ci = ni; cc = nc;
+                ni = ci; nc = cc + kStep;
+                if (nc >= chunks) { ni = ci + row_step; nc = tl; }
+                if (ni < m) load(a0, ni, nc);
+                consume(a1, ci, cc, ni != ci);
+                ci = ni; cc = nc;
+            }
+            continue;
+        }
         // rows are visited team-uniformly; TPR == CTA needs every thread in the loop
         for (uint32_t i = row0; i < m; i += row_step) {
             uint64_t sum_lo = 0, sum_hi = 0;
