@@ -360,9 +360,147 @@ prep_R_pv_and_v_kernel(const uint16_t *__restrict__ tvec, const int8_t *__restri
     if (threadIdx.x == 0) tickets[t] = 0;
 }
 
+// v alone (the GEMM reads R in place, nothing to copy): a pure stream over the int8 R of every instance -- 16 columns
+// (one 16-byte load) per thread, rows split over the CTAs of an instance, register-pipelined like decaps_kernel (the
+// next four rows' loads are issued before the current four are consumed), s32 column sums per thread (|t_i r| < 2^24,
+// the host keeps a thread's share below 96 rows), u64 partial sums across CTAs, last CTA of the instance finalizes.
+// The one-word-per-thread loop above ran this pass at 0.9 TB/s (73 us for the 64 MB of Table 1's n = 8192 row).
+// TT = uint16_t (narrow contexts) or uint32_t (wide contexts): type of t and v.
+__device__ __forceinline__ uint4 ldg_stream16_aux(const uint4 *p)
+{
+    uint4 r;
+    asm("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void pv_row(int (&a)[16], const uint4 &u, int ti)
+{
+    const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+    for (int y = 0; y < 4; y++)
+#pragma unroll
+        for (int x = 0; x < 4; x++) a[4 * y + x] += ti * (int)(int8_t)(w[y] >> (8 * x));
+}
+
+template <class TT>
+__global__ void __launch_bounds__(kAuxThreads)
+pv_v_stream_kernel(const TT *__restrict__ tvec, const int8_t *__restrict__ R, const int8_t *__restrict__ e2,
+                   const uint8_t *__restrict__ mubits, TT *__restrict__ v, unsigned long long *__restrict__ acc,
+                   unsigned int *__restrict__ tickets, uint32_t m, uint32_t k, uint32_t q)
+{
+    __shared__ uint32_t sLast;
+    __shared__ __align__(16) int sCol[kAuxThreads * 16];
+    pdl_trigger();
+    pdl_wait();
+    const uint32_t t = blockIdx.y;
+    const uint32_t tpr = k / 16;                         // threads per row: a power of two <= 256 (host)
+    const uint32_t rpi = kAuxThreads / tpr;
+    const uint32_t rslot = threadIdx.x / tpr, cg = threadIdx.x % tpr;
+    const uint4 *Rt = reinterpret_cast<const uint4 *>(R + (size_t)t * m * k);
+    const TT *tt = tvec + (size_t)t * m;
+    int a[16];
+#pragma unroll
+    for (int x = 0; x < 16; x++) a[x] = 0;
+    {
+        constexpr int kUnroll = 4;
+        const uint32_t per_cta = ((m + gridDim.x - 1) / gridDim.x + rpi - 1) / rpi * rpi;
+        const uint32_t ibeg = blockIdx.x * per_cta, iend = min(m, ibeg + per_cta);
+        uint32_t i = ibeg + rslot;
+        const uint4 *up = Rt + (size_t)i * tpr + cg;
+        const size_t ustep = (size_t)rpi * tpr;
+        uint4 u0[kUnroll], u1[kUnroll];
+        int t0[kUnroll], t1[kUnroll];
+        auto load = [&](uint4 (&uu)[kUnroll], int (&ts)[kUnroll]) {
+#pragma unroll
+            for (int r = 0; r < kUnroll; r++) {
+                const bool in = i + r * rpi < iend;          // a row past the range: a valid address, t = 0
+                uu[r] = ldg_stream16_aux(in ? up + r * ustep : Rt + cg);
+                ts[r] = in ? (int)__ldg(tt + i + r * rpi) : 0;
+            }
+            i += kUnroll * rpi;
+            up += kUnroll * ustep;
+        };
+        if (i < iend) {
+            load(u0, t0);
+            for (;;) {
+                const bool more1 = i < iend;
+                if (more1) load(u1, t1);
+#pragma unroll
+                for (int r = 0; r < kUnroll; r++) pv_row(a, u0[r], t0[r]);
+                if (!more1) break;
+                const bool more0 = i < iend;
+                if (more0) load(u0, t0);
+#pragma unroll
+                for (int r = 0; r < kUnroll; r++) pv_row(a, u1[r], t1[r]);
+                if (!more0) break;
+            }
+        }
+    }
+    // [row slot][column]: a thread stores its 16 columns contiguously, thread c then reads column c of every slot
+#pragma unroll
+    for (int x = 0; x < 16; x++) sCol[(size_t)threadIdx.x * 16 + x] = a[x];
+    __syncthreads();
+    for (uint32_t c = threadIdx.x; c < k; c += kAuxThreads) {
+        long long sum = 0;
+        for (uint32_t rs = 0; rs < rpi; rs++) sum += (long long)sCol[(size_t)rs * k + c];
+        if (sum) atomicAdd(acc + (size_t)t * k + c, (unsigned long long)sum);     // two's complement: u64 adds
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) sLast = (atomicAdd(tickets + t, 1u) == gridDim.x - 1) ? 1u : 0u;
+    __syncthreads();
+    if (!sLast) return;
+    __threadfence();
+    for (uint32_t c = threadIdx.x; c < k; c += kAuxThreads) {
+        const long long sum = (long long)__ldcg(acc + (size_t)t * k + c);
+        acc[(size_t)t * k + c] = 0;
+        const uint32_t mu = (mubits[(size_t)t * (k / 8) + c / 8] >> (c % 8)) & 1u;
+        long long r = (sum + (long long)e2[(size_t)t * k + c] + (long long)mu * (q / 2)) % (long long)q;
+        if (r < 0) r += q;
+        v[(size_t)t * k + c] = (TT)r;
+    }
+    if (threadIdx.x == 0) tickets[t] = 0;
+}
+
+bool pv_v_stream_supported(const Ctx *c)
+{
+    const uint32_t tpr = c->p.k / 16;
+    return c->p.k % 16 == 0 && tpr >= 1 && tpr <= (uint32_t)kAuxThreads && (tpr & (tpr - 1)) == 0;
+}
+
+template <class TT>
+static cudaError_t launch_pv_v_stream_t(Ctx *c, const TT *d_t, const int8_t *d_R, const int8_t *d_e2, const uint8_t *d_mubits,
+                                        TT *d_v, uint32_t batch, cudaStream_t st)
+{
+    const uint32_t m = c->p.m, k = c->p.k;
+    const uint32_t rpi = kAuxThreads / (k / 16);
+    int per_sm = 1;
+    cudaError_t perr = kernel_prepare(c, pv_v_stream_kernel<TT>, 0, kAuxThreads, &per_sm);
+    if (perr != cudaSuccess) return perr;
+    uint32_t splits = (uint32_t)(per_sm * c->sm_count) / batch;            // one wave of resident CTAs
+    const uint32_t max_splits = (m + 4 * rpi - 1) / (4 * rpi);           // >= 4 row groups per CTA
+    const uint32_t min_splits = (m + 96 * rpi - 1) / (96 * rpi);         // <= 96 rows per thread: s32 sums cannot overflow
+    if (splits > max_splits) splits = max_splits;
+    if (splits < min_splits) splits = min_splits;
+    if (splits < 1) splits = 1;
+    ProfScope prof(c, LWE_K_PREP_R_PV, st);
+    return launch_k(c, pv_v_stream_kernel<TT>, dim3(splits, batch), kAuxThreads, 0, st, d_t, d_R, d_e2, d_mubits, d_v, c->d_vacc,
+                    c->d_counters + 8 + c->p.max_batch, m, k, c->p.q);
+}
+
+cudaError_t launch_pv_v_stream(Ctx *c, const void *d_t, bool wide, const int8_t *d_R, const int8_t *d_e2, const uint8_t *d_mubits,
+                               void *d_v, uint32_t batch, cudaStream_t st)
+{
+    if (wide)
+        return launch_pv_v_stream_t<uint32_t>(c, static_cast<const uint32_t *>(d_t), d_R, d_e2, d_mubits,
+                                              static_cast<uint32_t *>(d_v), batch, st);
+    return launch_pv_v_stream_t<uint16_t>(c, static_cast<const uint16_t *>(d_t), d_R, d_e2, d_mubits,
+                                          static_cast<uint16_t *>(d_v), batch, st);
+}
+
 cudaError_t launch_prep_R_pv_and_v(Ctx *c, const uint16_t *d_t, const int8_t *d_R, const int8_t *d_e2,
                                    const uint8_t *d_mubits, uint16_t *d_v, uint32_t batch, bool write_Rexp, cudaStream_t st)
 {
+    if (!write_Rexp && pv_v_stream_supported(c)) return launch_pv_v_stream(c, d_t, false, d_R, d_e2, d_mubits, d_v, batch, st);
     const uint32_t m = c->p.m, k = c->p.k;
     const uint32_t wpr = k / 4;
     const uint32_t rows_per_iter = kAuxThreads / wpr ? kAuxThreads / wpr : 1;

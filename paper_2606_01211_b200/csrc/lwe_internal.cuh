@@ -267,6 +267,10 @@ cudaError_t launch_sample_cuniform(Ctx *c, int8_t *d_out, uint64_t first, uint64
                                    uint32_t inst0, uint32_t n_inst, uint32_t bound, cudaStream_t st);
 cudaError_t launch_prep_R_pv_and_v(Ctx *c, const uint16_t *d_t, const int8_t *d_R, const int8_t *d_e2,
                                    const uint8_t *d_mubits, uint16_t *d_v, uint32_t batch, bool write_Rexp, cudaStream_t st);
+// v alone for the int8 R (no operand copy), as a 16-byte-per-thread stream; wide: t, v are uint32 (else uint16)
+bool pv_v_stream_supported(const Ctx *c);
+cudaError_t launch_pv_v_stream(Ctx *c, const void *d_t, bool wide, const int8_t *d_R, const int8_t *d_e2, const uint8_t *d_mubits,
+                               void *d_v, uint32_t batch, cudaStream_t st);
 // d_R != NULL (needs k % 128 == 0): the B operand is read in place from the caller's int8 R [batch][m][k]; NULL: from
 // the operand copy in c->d_Rexp
 bool encaps_tc2_r_inplace_supported(const Ctx *c, uint32_t batch);

@@ -350,6 +350,7 @@ cudaError_t launch_wide_keygen_simt(Ctx *c, const int8_t *d_s, const int8_t *d_e
 cudaError_t launch_wide_v(Ctx *c, const uint32_t *d_t, const int8_t *d_R, const int8_t *d_e2, const uint8_t *d_mubits,
                           uint32_t *d_v, uint32_t batch, bool write_Rexp, cudaStream_t st)
 {
+    if (!write_Rexp && pv_v_stream_supported(c)) return launch_pv_v_stream(c, d_t, true, d_R, d_e2, d_mubits, d_v, batch, st);
     const uint32_t m = c->p.m, k = c->p.k;
     const uint32_t wpr = k / 4;
     const uint32_t rows_per_iter = kThreads / wpr ? kThreads / wpr : 1;
