@@ -107,22 +107,25 @@ keygen_gemv_kernel(const uint16_t *__restrict__ A, const __grid_constant__ AesKe
             // current batch is consumed, so a lane always has UNR..2 UNR independent 16-byte loads in flight.  With
             // load-then-consume batches the pass sat at 5.4 TB/s; a pure load loop of the same shape reaches 6.4.
             uint4 a0[UNR], a1[UNR];
-            auto load = [&](uint4 (&a)[UNR], uint32_t i, uint32_t c0) {
+            // positions are (row, first chunk of the batch) with the chunk base WARP-UNIFORM (lane tl adds tl + u * 32 and
+            // masks what lies past the row's end), so that all lanes move to the next row -- and meet in its shuffle
+            // reduction -- together, whatever n is
+            auto load = [&](uint4 (&a)[UNR], uint32_t i, uint32_t cb) {
                 const uint4 *Arow = reinterpret_cast<const uint4 *>(A + (size_t)i * n);
 #pragma unroll
                 for (int u = 0; u < UNR; u++) {
-                    const uint32_t c = c0 + u * TPR;
+                    const uint32_t c = cb + tl + u * TPR;
                     if (c < chunks) a[u] = ldg_stream(Arow + c);
                     else a[u] = make_uint4(0, 0, 0, 0);
                 }
             };
             uint64_t sum_lo = 0, sum_hi = 0;
             uint32_t lo = 0, hi = 0, since = 0;
-            // consumes the batch at (i, c0); `last` = it is the row's last batch: reduce and write b[i]
-            auto consume = [&](const uint4 (&a)[UNR], uint32_t i, uint32_t c0, bool last) {
+            // consumes the batch at (i, cb); `last` = it is the row's last batch: reduce and write b[i]
+            auto consume = [&](const uint4 (&a)[UNR], uint32_t i, uint32_t cb, bool last) {
 #pragma unroll
                 for (int u = 0; u < UNR; u++) {
-                    const uint32_t c = c0 + u * TPR;
+                    const uint32_t c = cb + tl + u * TPR;
                     const uint4 sw = (c < chunks) ? sS4[c] : make_uint4(0, 0, 0, 0);
                     dot8(a[u], sw, lo, hi);
                 }
@@ -141,20 +144,20 @@ keygen_gemv_kernel(const uint16_t *__restrict__ A, const __grid_constant__ AesKe
                 sum_lo = sum_hi = 0; lo = hi = 0; since = 0;
             };
             constexpr uint32_t kStep = UNR * TPR;
-            uint32_t ci = row0, cc = tl;                     // current position; the next one follows below
-            if (ci < m) load(a0, ci, cc);
+            uint32_t ci = row0, cb = 0;                      // current position; the next one follows below
+            if (ci < m) load(a0, ci, cb);
             while (ci < m) {
-                uint32_t ni = ci, nc = cc + kStep;
-                if (nc >= chunks) { ni = ci + row_step; nc = tl; }
-                if (ni < m) load(a1, ni, nc);
-                consume(a0, ci, cc, ni != ci);
+                uint32_t ni = ci, nb = cb + kStep;
+                if (nb >= chunks) { ni = ci + row_step; nb = 0; }
+                if (ni < m) load(a1, ni, nb);
+                consume(a0, ci, cb, ni != ci);
                 if (ni >= m) break;
-                ci = ni; cc = nc;
-                ni = ci; nc = cc + kStep;
-                if (nc >= chunks) { ni = ci + row_step; nc = tl; }
-                if (ni < m) load(a0, ni, nc);
-                consume(a1, ci, cc, ni != ci);
-                ci = ni; cc = nc;
+                ci = ni; cb = nb;
+                ni = ci; nb = cb + kStep;
+                if (nb >= chunks) { ni = ci + row_step; nb = 0; }
+                if (ni < m) load(a0, ni, nb);
+                consume(a1, ci, cb, ni != ci);
+                ci = ni; cb = nb;
             }
             continue;
         }
