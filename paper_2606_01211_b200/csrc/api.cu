@@ -98,6 +98,8 @@ void free_all(Ctx *c)
     if (c->s_out) cudaStreamDestroy(c->s_out);
     if (c->ev_entry) cudaEventDestroy(c->ev_entry);
     if (c->ev_out) cudaEventDestroy(c->ev_out);
+    if (c->ev_se) cudaEventDestroy(c->ev_se);
+    if (c->ev_kg) cudaEventDestroy(c->ev_kg);
     for (int i = 0; i < kHostChunks; i++) {
         if (c->ev_in[i]) cudaEventDestroy(c->ev_in[i]);
         if (c->ev_done[i]) cudaEventDestroy(c->ev_done[i]);
@@ -230,6 +232,8 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
     ok(cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
     ok(cudaEventCreateWithFlags(&c->ev_entry, cudaEventDisableTiming));
     ok(cudaEventCreateWithFlags(&c->ev_out, cudaEventDisableTiming));
+    ok(cudaEventCreateWithFlags(&c->ev_se, cudaEventDisableTiming));
+    ok(cudaEventCreateWithFlags(&c->ev_kg, cudaEventDisableTiming));
     for (int i = 0; i < kHostChunks; i++) {
         ok(cudaEventCreateWithFlags(&c->ev_in[i], cudaEventDisableTiming));
         ok(cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming));
@@ -790,56 +794,77 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint1
     const size_t n = c->p.n, m = c->p.m, k = c->p.k;
     cudaStream_t st = (cudaStream_t)stream;
     DeviceGuard guard(c->device);
-    // Software pipeline over chunks of instances: the copy-in stream runs ahead of the compute stream (the
-    // caller's), the copy-out stream behind it, so that the PCIe transfers of the ciphertexts (U dominates:
-    // 2nk bytes per instance) overlap the GEMM of the following chunks.  Chunks of >= 4 instances keep the
-    // tensor-core GEMM's tile count above one wave.
-    uint32_t nchunks = batch / 4;
-    if (nchunks > (uint32_t)kHostChunks) nchunks = kHostChunks;
-    if (nchunks < 1) nchunks = 1;
-    uint32_t per = (batch + nchunks - 1) / nchunks;
-    // every chunk must start on a 16-byte boundary of each staging buffer (the packed-bit rows are the
-    // narrow ones: k/8 bytes of mu, m*k/8 bytes of R per instance); otherwise one chunk
-    if (((size_t)per * (k / 8)) % 16 || ((size_t)per * (m * k / 8)) % 16) per = batch;
+    // Software pipeline: the copy-in stream runs ahead of the compute stream (the caller's), the copy-out stream
+    // behind it.  The call is bound by the copy-out of the ciphertexts (U: 2nk bytes per instance, 134 MB of the
+    // 135 MB at C4), so the plan is made to START that copy as early as possible and never let it wait:
+    //   * s, e and mu of every instance go in first (small), and KeyGen runs ONCE for the whole batch (A is read -- or
+    //     regenerated -- once, not once per chunk);
+    //   * Encrypt + Decrypt run chunk by chunk over R, with chunks of 1, 1, 2, 4, 8, ... instances: the first ciphertext
+    //     is on its way back after one single-instance GEMM, and every later chunk is computed while the previous,
+    //     smaller one is still on the bus.  (Equal chunks of 4 left the copy-out stream idle for the first chunk's
+    //     compute and starved it in between: 46 GB/s of the link's 57.)
+    // Chunk boundaries must be 16-byte aligned in every staging buffer (the packed-bit rows are the narrow ones: k/8
+    // bytes of mu per instance); otherwise, and for a regenerated A (every Encrypt call regenerates all of A), fewer,
+    // equal chunks are used.
+    uint32_t c_t0[kHostChunks], c_g[kHostChunks], nchunks = 0;
+    const bool row_aligned = ((k / 8) % 16 == 0) && ((m * k / 8) % 16 == 0);
+    if (row_aligned && d_A) {
+        uint32_t t0 = 0, g = 1;
+        while (t0 < batch) {
+            uint32_t take = (nchunks == (uint32_t)kHostChunks - 1) ? batch - t0 : (g < batch - t0 ? g : batch - t0);
+            c_t0[nchunks] = t0; c_g[nchunks] = take; nchunks++;
+            t0 += take;
+            if (nchunks >= 2) g *= 2;
+        }
+    } else {
+        uint32_t want = row_aligned ? (batch >= 16 ? 2u : 1u) : 1u;
+        uint32_t per = (batch + want - 1) / want;
+        if (((size_t)per * (k / 8)) % 16 || ((size_t)per * (m * k / 8)) % 16) per = batch;
+        for (uint32_t t0 = 0; t0 < batch; t0 += per) {
+            c_t0[nchunks] = t0; c_g[nchunks] = (batch - t0 < per) ? (batch - t0) : per; nchunks++;
+        }
+    }
     LWE_CUDA_TRY(c, cudaEventRecord(c->ev_entry, st));
     LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_in, c->ev_entry, 0));      // staging buffers are free again
     LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_out, c->ev_entry, 0));
-    uint32_t ci = 0;
-    for (uint32_t t0 = 0; t0 < batch; t0 += per, ci++) {
-        const size_t g = (batch - t0 < per) ? (batch - t0) : per;
-        LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hs + t0 * n, h_s + t0 * n, g * n * 2, cudaMemcpyHostToDevice, c->s_in));
-        LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_he + t0 * m, h_e + t0 * m, g * m * 2, cudaMemcpyHostToDevice, c->s_in));
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hs, h_s, (size_t)batch * n * 2, cudaMemcpyHostToDevice, c->s_in));
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_he, h_e, (size_t)batch * m * 2, cudaMemcpyHostToDevice, c->s_in));
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hmu, h_mubits, (size_t)batch * k / 8, cudaMemcpyHostToDevice, c->s_in));
+    LWE_CUDA_TRY(c, cudaEventRecord(c->ev_se, c->s_in));
+    for (uint32_t ci = 0; ci < nchunks; ci++) {
+        const size_t t0 = c_t0[ci], g = c_g[ci];
         LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hR + t0 * (m * k / 8), h_Rbits + t0 * (m * k / 8), g * m * k / 8,
-                                        cudaMemcpyHostToDevice, c->s_in));
-        LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hmu + t0 * (k / 8), h_mubits + t0 * (k / 8), g * k / 8,
                                         cudaMemcpyHostToDevice, c->s_in));
         LWE_CUDA_TRY(c, cudaEventRecord(c->ev_in[ci], c->s_in));
     }
-    ci = 0;
-    for (uint32_t t0 = 0; t0 < batch; t0 += per, ci++) {
-        const uint32_t g = (batch - t0 < per) ? (batch - t0) : per;
+    auto drain = [&]() { cudaStreamSynchronize(c->s_in); cudaStreamSynchronize(st); cudaStreamSynchronize(c->s_out); };
+    LWE_CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_se, 0));
+    int rc = lwe_keygen(ctx, d_A, seed_A, c->d_hs, c->d_he, c->d_hb, batch, stream);
+    if (rc != LWE_OK) { drain(); return rc; }
+    LWE_CUDA_TRY(c, cudaEventRecord(c->ev_kg, st));
+    LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_out, c->ev_kg, 0));
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_b, c->d_hb, (size_t)batch * m * 2, cudaMemcpyDeviceToHost, c->s_out));
+    for (uint32_t ci = 0; ci < nchunks; ci++) {
+        const size_t t0 = c_t0[ci];
+        const uint32_t g = c_g[ci];
         LWE_CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_in[ci], 0));
-        int rc = lwe_keygen(ctx, d_A, seed_A, c->d_hs + t0 * n, c->d_he + t0 * m, c->d_hb + t0 * m, g, stream);
-        if (rc == LWE_OK)
-            rc = lwe_encaps(ctx, d_A, seed_A, c->d_hb + t0 * m, c->d_hR + t0 * (m * k / 8), c->d_hmu + t0 * (k / 8),
-                            c->d_hU + t0 * n * k, c->d_hv + t0 * k, g, stream);
-        if (rc == LWE_OK)
-            rc = lwe_decaps(ctx, c->d_hU + t0 * n * k, c->d_hv + t0 * k, c->d_hs + t0 * n, c->d_hmuout + t0 * (k / 8), g,
-                            stream);
-        if (rc != LWE_OK) {
-            cudaStreamSynchronize(c->s_in); cudaStreamSynchronize(st); cudaStreamSynchronize(c->s_out);
-            return rc;
-        }
-        LWE_CUDA_TRY(c, cudaEventRecord(c->ev_done[ci], st));
+        rc = lwe_encaps(ctx, d_A, seed_A, c->d_hb + t0 * m, c->d_hR + t0 * (m * k / 8), c->d_hmu + t0 * (k / 8),
+                        c->d_hU + t0 * n * k, c->d_hv + t0 * k, g, stream);
+        if (rc != LWE_OK) { drain(); return rc; }
+        LWE_CUDA_TRY(c, cudaEventRecord(c->ev_done[ci], st));           // the chunk's ciphertext leaves before it is decrypted
         LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_out, c->ev_done[ci], 0));
-        LWE_CUDA_TRY(c, cudaMemcpyAsync(h_b + t0 * m, c->d_hb + t0 * m, (size_t)g * m * 2, cudaMemcpyDeviceToHost, c->s_out));
         if (h_U)
             LWE_CUDA_TRY(c, cudaMemcpyAsync(h_U + t0 * n * k, c->d_hU + t0 * n * k, (size_t)g * n * k * 2,
                                             cudaMemcpyDeviceToHost, c->s_out));
-        LWE_CUDA_TRY(c, cudaMemcpyAsync(h_v + t0 * k, c->d_hv + t0 * k, (size_t)g * k * 2, cudaMemcpyDeviceToHost, c->s_out));
-        LWE_CUDA_TRY(c, cudaMemcpyAsync(h_mubits_out + t0 * (k / 8), c->d_hmuout + t0 * (k / 8), (size_t)g * k / 8,
-                                        cudaMemcpyDeviceToHost, c->s_out));
+        rc = lwe_decaps(ctx, c->d_hU + t0 * n * k, c->d_hv + t0 * k, c->d_hs + t0 * n, c->d_hmuout + t0 * (k / 8), g, stream);
+        if (rc != LWE_OK) { drain(); return rc; }
     }
+    // the small outputs of every chunk in one copy each, behind the last chunk's Decrypt (a copy of a few hundred bytes
+    // costs the copy engine as much as a megabyte of U)
+    LWE_CUDA_TRY(c, cudaEventRecord(c->ev_kg, st));
+    LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_out, c->ev_kg, 0));
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_v, c->d_hv, (size_t)batch * k * 2, cudaMemcpyDeviceToHost, c->s_out));
+    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_mubits_out, c->d_hmuout, (size_t)batch * k / 8, cudaMemcpyDeviceToHost, c->s_out));
     LWE_CUDA_TRY(c, cudaEventRecord(c->ev_out, c->s_out));
     LWE_CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_out, 0));            // the caller's stream sees the whole call
     LWE_CUDA_TRY(c, cudaStreamSynchronize(st));

@@ -126,7 +126,7 @@ struct Ctx {
     // lwe_kem_host pipeline: copy-in / copy-out streams and the events that order them against the
     // caller's compute stream, one pair per chunk of instances
     cudaStream_t s_in, s_out;
-    cudaEvent_t ev_entry, ev_out, ev_in[kHostChunks], ev_done[kHostChunks];
+    cudaEvent_t ev_entry, ev_out, ev_se, ev_kg, ev_in[kHostChunks], ev_done[kHostChunks];
 
     // driver entry point for TMA descriptors (resolved at create; no link-time libcuda)
     void *encode_tiled;

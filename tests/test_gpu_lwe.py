@@ -610,14 +610,16 @@ def test_contexts_on_two_devices_in_one_process(H):
 
 @pytest.mark.parametrize("n,m,k,q,batch,regen", [
     (256, 512, 256, 65536, 1, False),      # one chunk
-    (192, 384, 256, 65521, 9, False),      # two chunks of 5 + 4 instances, prime q
-    (128, 264, 256, 65536, 32, False),     # eight chunks of 4 (the shape of bench.py's e2e leg), ragged K tail
+    (192, 384, 256, 65521, 9, False),      # chunks of 1, 1, 2, 4, 1 instances, prime q
+    (128, 264, 256, 65536, 32, False),     # chunks of 1, 1, 2, 4, 8, 16 (the shape of bench.py's e2e leg), ragged K tail
+    (64, 128, 256, 65536, 200, False),     # more instances than the chunk plan has doubling steps: the last chunk takes the rest
     (64, 128, 8, 17, 9, False),            # packed-bit rows narrower than 16 bytes: falls back to one chunk
-    (192, 384, 256, 65536, 9, True),       # A regenerated from its seed for keygen and encaps
+    (192, 384, 256, 65536, 9, True),       # A regenerated from its seed for keygen and encaps (one chunk)
+    (64, 128, 256, 65536, 20, True),       # regenerated A, two equal chunks
 ])
 def test_kem_host_pipeline_matches_oracle(H, n, m, k, q, batch, regen):
-    """lwe_kem_host (the e2e call bench.py times): pinned host buffers in, chunked copy/compute/copy-out
-    pipeline inside, every output compared with the oracle per instance."""
+    """lwe_kem_host (the e2e call bench.py times): pinned host buffers in, KeyGen once for the batch, then a chunked
+    copy / Encrypt + Decrypt / copy-out pipeline inside, every output compared with the oracle per instance."""
     import torch
     seed = 11
     A = O.sample_uniform(0, m * n, seed, O.TAG_A, 0, q).reshape(m, n)
