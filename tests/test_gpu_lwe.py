@@ -314,7 +314,9 @@ def test_encaps_fused_regenerated_A_matches_oracle(H, m, n, k, q, seed):
 
 @pytest.mark.parametrize("n,k,q,batch", [(256, 256, 65536, 1), (1000, 256, 65521, 3), (64, 8, 17, 2),
                                           (4096, 128, 65521, 2), (8192, 256, 65536, 4), (136, 512, 65521, 2),
-                                          (72, 384, 65536, 3), (8, 2048, 65536, 1)])
+                                          (72, 384, 65536, 3), (8, 2048, 65536, 1),
+                                          (520, 64, 4096, 3), (8192, 256, 2, 2),      # small powers of two: the u32 wrap-around sums
+                                          (16384, 256, 65521, 2)])                    # u64 sums, many rows per thread
 def test_decaps_matches_oracle(H, n, k, q, batch):
     U = W.random_u16((batch, n, k), q, 41)
     v = W.random_u16((batch, k), q, 42)
