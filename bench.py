@@ -567,6 +567,79 @@ def paper_variant_wide_phase(B, device: int) -> dict:
             "encaps_gemm_frac_of_nominal_4500": ops / (g_ms / g_cnt * 1e-3) / 1e12 / 4500.0 if g_cnt else None,
             "decaps_GBps": 4.0 * n * k * Bt / (t_d * 1e-3) / 1e9, "all_bits_recovered": ok}
 
+TABLE1_ROWS = [  # (n, q, sigma, e2 bound, instances per batch in this phase): P:L94-102; tests/golden/paper_table1_params.txt
+    (512, 3329, 2.3, 3, 32), (1024, 12289, 2.3, 3, 32), (2048, 12289, 2.3, 3, 32), (4096, 12289, 1.7, 3, 32),
+    (8192, 65537, 1.2, 2, 32), (16384, 65537, 1.2, 2, 32), (32768, 65537, 1.0, 2, 32), (65536, 65537, 1.0, 1, 16),
+    (131072, 65537, 1.0, 1, 8)]
+
+
+def paper_table1_phase(B, device: int) -> dict:
+    """N2 on ALL nine parameter sets of the paper's Table 1: square A, CBD-3 secret, Gaussian e, r, e1,
+    centred-uniform e2, every object drawn on the device from the seed; sample -> KeyGen -> Encrypt -> Decrypt for a
+    batch of instances sharing A (32; 16 and 8 on the two largest rows).  Rows n <= 4096 run on uint16 residues, rows
+    n >= 8192 (q = 65537) on the wide path (uint32 residues, A packed by lwe_wide_load_matrix_seeded: the uint32 matrix never
+    exists; n = 131072: KeyGen in two column passes, Encrypt in two row passes).  Per call: mean of 5 after 2 warm-ups."""
+    rows = {}
+    dev = torch.device("cuda", device)
+    k, seed = 256, 9
+    for n, q, sigma, bound, Bt in TABLE1_ROWS:
+        wide = q > 65536
+        res_t = torch.int32 if wide else torch.int16
+        s8 = dict(dtype=torch.int8, device=dev)
+        with B.Context(n, n, k, q, 3, Bt, device) as c:
+            if wide:
+                t0 = time.perf_counter()
+                c.wide_load_matrix_seeded(seed)
+                torch.cuda.synchronize()
+                t_load = (time.perf_counter() - t0) * 1e3
+                A = None
+            else:
+                A = torch.empty(n, n, dtype=torch.int16, device=dev)
+                c.sample_uniform(A, 0, n * n, seed, W.TAG_A)
+                t_load = None
+            s = torch.empty(Bt, n, **s8) if wide else torch.empty(Bt, n, dtype=torch.int16, device=dev)
+            e = torch.empty(Bt, n, **s8) if wide else torch.empty(Bt, n, dtype=torch.int16, device=dev)
+            t = torch.empty(Bt, n, dtype=res_t, device=dev)
+            R, E1, e2 = torch.empty(Bt, n, k, **s8), torch.empty(Bt, n, k, **s8), torch.empty(Bt, k, **s8)
+            mu = torch.empty(Bt, k // 8, dtype=torch.uint8, device=dev)
+            out = torch.empty(Bt, k // 8, dtype=torch.uint8, device=dev)
+            U, v = torch.empty(Bt, n, k, dtype=res_t, device=dev), torch.empty(Bt, k, dtype=res_t, device=dev)
+
+            def sample():
+                if wide:
+                    c.sample_cbd_s8(s, 0, n, seed, W.TAG_S, 0, Bt)
+                    c.sample_gauss_s8(e, 0, n, seed, W.TAG_E, 0, Bt, sigma)
+                else:
+                    c.sample_cbd(s, 0, n, seed, W.TAG_S, 0, Bt)
+                    c.sample_gauss_u16(e, 0, n, seed, W.TAG_E, 0, Bt, sigma)
+                c.sample_gauss_s8(R, 0, n * k, seed, W.TAG_RG, 0, Bt, sigma)
+                c.sample_gauss_s8(E1, 0, n * k, seed, W.TAG_E1, 0, Bt, sigma)
+                c.sample_cuniform_s8(e2, 0, k, seed, W.TAG_E2, 0, Bt, bound)
+                c.sample_bits(mu, 0, k, seed, W.TAG_MU, 0, Bt)
+
+            if wide:
+                keygen = lambda: c.wide_keygen(s, e, t, Bt)                               # noqa: E731
+                encaps = lambda: c.wide_encaps(t, R, E1, e2, mu, U, v, Bt)                # noqa: E731
+                decaps = lambda: c.wide_decaps(U, v, s, out, Bt)                          # noqa: E731
+            else:
+                keygen = lambda: c.keygen(A, 0, s, e, t, Bt)                              # noqa: E731
+                encaps = lambda: c.encaps_pv(A, t, R, E1, e2, mu, U, v, Bt)               # noqa: E731
+                decaps = lambda: c.decaps(U, v, s, out, Bt)                               # noqa: E731
+            t_s = time_call(sample, reps=5, warm=2)
+            t_k = time_call(keygen, reps=5, warm=2)
+            t_e = time_call(encaps, reps=5, warm=2)
+            t_d = time_call(decaps, reps=5, warm=2)
+            ok = bool(torch.equal(out, mu))
+        ops = 4.0 * n * n * k * Bt
+        rows[f"n{n}"] = {"q": q, "sigma": sigma, "e2_bound": bound, "instances": Bt, "residues": "uint32" if wide else "uint16",
+                         "load_matrix_seeded_ms_one_off": t_load, "sample_ms": t_s, "keygen_ms": t_k, "encaps_ms": t_e,
+                         "decaps_ms": t_d, "kem_per_s": Bt * 1e3 / (t_s + t_k + t_e + t_d),
+                         "kem_per_s_encaps_plus_decaps": Bt * 1e3 / (t_e + t_d),
+                         "encaps_int8_TOPs": ops / (t_e * 1e-3) / 1e12, "all_bits_recovered": ok}
+        del A, s, e, t, R, E1, e2, U, v
+        torch.cuda.empty_cache()
+    return rows
+
 
 def single_kem_phase(B, device: int) -> dict:
     """Single-instance latency of every call on the small configs C1-C3 (the paper's Table 2 range), per
@@ -747,7 +820,7 @@ def sustained_block(job: Job, seconds: float, ms_step_burst: float, peaks: dict)
 
 
 PHASES = {"paper_variant_n4096_B32": paper_variant_phase, "paper_variant_n8192_q65537_B32": paper_variant_wide_phase,
-          "single_kem_B1": single_kem_phase,
+          "single_kem_B1": single_kem_phase, "paper_table1_all_rows": paper_table1_phase,
           "large_kem_C5_B1": lambda B, device: large_kem_phase(B, device, measured_peaks()["hbm_gbs"])}
 
 
@@ -1038,6 +1111,7 @@ def run_ours(args):
     if not args.quick:
         side["paper_variant_n4096_B32"] = paper_variant_phase(job.B, local)
         side["paper_variant_n8192_q65537_B32"] = paper_variant_wide_phase(job.B, local)
+        side["paper_table1_all_rows"] = paper_table1_phase(job.B, local)
         side["single_kem_B1"] = single_kem_phase(job.B, local)
         side["large_kem_C5_B1"] = large_kem_phase(job.B, local, hbm)
     buf = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")

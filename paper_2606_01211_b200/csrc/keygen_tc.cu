@@ -90,6 +90,10 @@ struct KgWide {
     // 32-bit reduction of the signed sums: bias / ebias are multiples of q above |D| <= 255 * 128 * n and above
     // |e - delta * corr| (corr = sum of the secrets at the row's exceptions), delta = q - 2^16 (2^16 = -delta mod q)
     uint32_t bias, ebias, delta;
+    // n > 65536 (a signed byte-plane sum holds 255 * 128 * 65536 < 2^31): the columns of A are contracted in passes of
+    // <= 65536; this launch covers one pass (its `n` argument = the columns of the pass), n_full = the row length of s;
+    // from the second pass on (accum) the epilogue adds the residues already in t instead of e and the exception terms
+    uint32_t n_full, accum;
 };
 
 // 8 * CPI accumulator columns (= 8 instances) of this warp's 32 TMEM lanes
@@ -233,12 +237,13 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
             const bool row_ok = rin < rps && i < m;
             // e of the first 32 instances is fetched while the main loop of this strip still runs: with one strip
             // per CTA nothing else hides the epilogue, and 4 rounds of dependent global loads were ~4 us of 56
+            const bool accum = kWide && wd.accum;
             uint32_t epre[32];
 #pragma unroll
             for (uint32_t x = 0; x < 32; x++)
-                epre[x] = (row_ok && x < batch) ? (kWide ? (uint32_t)(int)__ldg(e8 + (size_t)x * m + i)
+                epre[x] = (row_ok && x < batch) ? (kWide ? (accum ? b32[(size_t)x * m + i] : (uint32_t)(int)__ldg(e8 + (size_t)x * m + i))
                                                          : (uint32_t)__ldg(e + (size_t)x * m + i)) : 0u;
-            const uint32_t exc = (kWide && row_ok) ? min(__ldg(wd.row_cnt + i), wd.cap) : 0u;
+            const uint32_t exc = (kWide && row_ok && !accum) ? min(__ldg(wd.row_cnt + i), wd.cap) : 0u;
             if (kWide) {
                 // the 2^16-weighted elements of this row (about one row in eight has one): their secrets are folded into
                 // the prefetched e here, 32 independent loads per exception, while the main loop still runs.  Inside the
@@ -248,7 +253,7 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
                     const uint32_t col = __ldg(wd.row_cols + (size_t)i * wd.cap + y);
 #pragma unroll
                     for (uint32_t x = 0; x < 32; x++)
-                        if (x < batch) epre[x] -= wd.delta * (uint32_t)(int)__ldg(wd.s + (size_t)x * n + col);
+                        if (x < batch) epre[x] -= wd.delta * (uint32_t)(int)__ldg(wd.s + (size_t)x * wd.n_full + col);
                 }
             }
             mbar_wait(tfull_bar(acc), acc_phase);
@@ -266,13 +271,20 @@ keygen_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
                         const uint32_t inst = i0 + x;
                         if (inst < batch) {
                             if (kWide) {
+                                if (accum) {                             // a later column pass: add to the residue in t
+                                    const uint32_t old = (i0 < 32) ? epre[(i0 + x) & 31] : b32[(size_t)inst * m + i];
+                                    const uint32_t add = mod_u32(mod_u32(r[2 * x] + wd.bias, mq) + 256u * mod_u32(r[2 * x + 1] + wd.bias, mq), mq);
+                                    const uint32_t sum = old + add;      // < 2q
+                                    b32[(size_t)inst * m + i] = sum >= mq.q ? sum - mq.q : sum;
+                                    continue;
+                                }
                                 int ei;
                                 if (i0 < 32) {
                                     ei = (int)epre[(i0 + x) & 31];           // e minus the exception terms, prefetched
                                 } else {
                                     ei = (int)e8[(size_t)inst * m + i];
                                     for (uint32_t y = 0; y < exc; y++)     // elements >= 2^16 of this row: rare
-                                        ei -= (int)wd.delta * (int)wd.s[(size_t)inst * n + wd.row_cols[(size_t)i * wd.cap + y]];
+                                        ei -= (int)wd.delta * (int)wd.s[(size_t)inst * wd.n_full + wd.row_cols[(size_t)i * wd.cap + y]];
                                 }
                                 // three 32-bit Barrett steps on biased (non-negative) values; a 64-bit remainder per
                                 // element (~150 instructions) made this epilogue, not HBM, the kernel's limit
@@ -337,7 +349,7 @@ size_t keygen_tc_workspace_bytes(const lwe_params &p)
 {
     if (p.q > 65536u) {                                                 // wide context: two signed columns per instance
         const uint32_t Nw = padded_cols(p.max_batch, 2);
-        return (p.n <= 65536 && Nw <= 256) ? (size_t)Nw * 2 * p.n : 0;
+        return (p.n <= 262144 && Nw <= 256) ? (size_t)Nw * 2 * p.n : 0;
     }
     const uint32_t N = padded_cols(p.max_batch, cols_per_inst(p));
     return (p.n <= 32768 && N <= 256) ? (size_t)N * 2 * p.n : 0;       // 0: the tensor-core keygen is not available
@@ -392,8 +404,8 @@ cudaError_t launch_keygen_tc(Ctx *c, const uint16_t *d_A, const uint16_t *d_s, c
 // ---- wide path: t = A s + e on uint32 residues, A = the context's packed matrix (wide.cu)
 bool wide_keygen_tc_supported(const Ctx *c, uint32_t batch)
 {
-    // |D| <= 255 * 128 * n < 2^31 for n <= 65536
-    return c->encode_tiled != nullptr && c->d_Sx != nullptr && c->p.n <= 65536 && padded_cols(batch, 2) <= 256 &&
+    // |D| <= 255 * 128 * n < 2^31 for n <= 65536: longer rows are contracted in column passes of 65536
+    return c->encode_tiled != nullptr && c->d_Sx != nullptr && c->p.n <= 262144 && padded_cols(batch, 2) <= 256 &&
            padded_cols(c->p.max_batch, 2) <= 256;
 }
 
@@ -408,13 +420,10 @@ cudaError_t launch_wide_keygen_tc(Ctx *c, const int8_t *d_s, const int8_t *d_e, 
                                    p.n, batch);
         if (err != cudaSuccess) return err;
     }
-    CUtensorMap mapA, mapS;
     const uint32_t waves = (p.m + kTileM * (uint32_t)c->sm_count - 1) / (kTileM * (uint32_t)c->sm_count);
     uint32_t rps = ((p.m + waves * (uint32_t)c->sm_count - 1) / (waves * (uint32_t)c->sm_count) + 7u) & ~7u;
     if (rps > kTileM) rps = kTileM;
     if (rps < 8) rps = 8;
-    if (!make_map_u8(c, &mapA, c->d_A16, 2ull * p.n, p.m, rps)) return cudaErrorInvalidValue;
-    if (!make_map_u8(c, &mapS, c->d_Sx, 2ull * p.n, N, N)) return cudaErrorInvalidValue;
     uint32_t slabs, stages;
     const uint32_t smem = ring_shape(rps, N, &slabs, &stages);
     auto kern = slabs == 2 ? keygen_tc_kernel<2, 2, true> : keygen_tc_kernel<2, 1, true>;
@@ -422,12 +431,25 @@ cudaError_t launch_wide_keygen_tc(Ctx *c, const int8_t *d_s, const int8_t *d_e, 
     if (perr != cudaSuccess) return perr;
     const uint32_t strips = (p.m + rps - 1) / rps;
     const uint32_t grid = strips < (uint32_t)c->sm_count ? strips : (uint32_t)c->sm_count;
-    ProfScope prof(c, LWE_K_KEYGEN_TC, st);
     const uint64_t q = p.q, delta = q - 65536u;
-    const uint64_t plane_max = 255ull * 128ull * p.n, e_max = 128ull + delta * 128ull * c->exc_cap_row;
-    const KgWide wd = {c->d_exc_row_cnt, c->d_exc_row_cols, c->exc_cap_row, d_s,
-                       (uint32_t)((plane_max + q - 1) / q * q), (uint32_t)((e_max + q - 1) / q * q), (uint32_t)delta};
-    return launch_k(c, kern, grid, kThreads, smem, st, mapA, mapS, d_e, d_t, p.m, p.n, batch, N, stages, c->mq, rps, wd);
+    // column passes of <= 65536 (Table 1's n = 131072 row: two): each a column range of A16 and of the operand rows,
+    // mapped with the full row pitch; the first adds e and the exception terms, the later ones add to t
+    const uint32_t step = p.n < 65536u ? p.n : 65536u;
+    for (uint32_t col0 = 0; col0 < p.n; col0 += step) {
+        const uint32_t cols = (p.n - col0 < step) ? (p.n - col0) : step;
+        CUtensorMap mapA, mapS;
+        if (!make_map_u8(c, &mapA, c->d_A16 + col0, 2ull * cols, p.m, rps, 2ull * p.n)) return cudaErrorInvalidValue;
+        if (!make_map_u8(c, &mapS, c->d_Sx + 2ull * col0, 2ull * cols, N, N, 2ull * p.n)) return cudaErrorInvalidValue;
+        const uint64_t plane_max = 255ull * 128ull * cols, e_max = 128ull + delta * 128ull * c->exc_cap_row;
+        const KgWide wd = {c->d_exc_row_cnt, c->d_exc_row_cols, c->exc_cap_row, d_s,
+                           (uint32_t)((plane_max + q - 1) / q * q), (uint32_t)((e_max + q - 1) / q * q), (uint32_t)delta,
+                           p.n, col0 ? 1u : 0u};
+        ProfScope prof(c, LWE_K_KEYGEN_TC, st);
+        cudaError_t err = launch_k(c, kern, grid, kThreads, smem, st, mapA, mapS, d_e, d_t, p.m, cols, batch, N, stages, c->mq,
+                                   rps, wd);
+        if (err != cudaSuccess) return err;
+    }
+    return cudaSuccess;
 }
 
 }  // namespace lwe

@@ -274,12 +274,13 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 // u8 matrix [rows][width] row-major, box {128 bytes, box_rows}, SWIZZLE_128B, out-of-bounds -> 0
+// pitch: bytes between rows (0 = width: a dense matrix); a larger pitch maps a column range of a wider matrix
 inline bool make_map_u8(const Ctx *c, CUtensorMap *map, const void *ptr, uint64_t width, uint64_t rows,
-                        uint32_t box_rows)
+                        uint32_t box_rows, uint64_t pitch = 0)
 {
     if (!c->encode_tiled) return false;
     cuuint64_t dims[2] = {width, rows};
-    cuuint64_t strides[1] = {width};
+    cuuint64_t strides[1] = {pitch ? pitch : width};
     cuuint32_t box[2] = {128, box_rows};
     cuuint32_t estr[2] = {1, 1};
     CUresult r = ((EncodeTiledFn)c->encode_tiled)(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(ptr), dims,

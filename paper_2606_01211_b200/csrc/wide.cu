@@ -60,7 +60,7 @@ wide_pack_kernel(const uint32_t *__restrict__ A, uint16_t *__restrict__ A16, uin
 
 // ------------------------------------------------------------------ KeyGen on CUDA cores (one warp per row)
 // t[b][i] = (sum_j A[i][j] s[b][j] + e[b][i]) mod q,  A[i][j] = A16[i][j] + 2^16 [j in exceptions of row i].
-// Any n (the tensor-core kernel holds n <= 65536: Table 1's n = 131072 row runs here); 16-byte loads of A16 (8 elements)
+// Any n; the cross-check of the tensor-core kernel (LWE_OPT_KEYGEN_PATH = 1) and the path for shapes it does not take; 16-byte loads of A16 (8 elements)
 // against 8 secrets, products accumulated in 32 bits (|a s| < 2^23) and flushed into 64 bits every 128 steps.
 __global__ void __launch_bounds__(kThreads)
 wide_keygen_simt_kernel(const uint16_t *__restrict__ A16, const uint32_t *__restrict__ row_cnt,

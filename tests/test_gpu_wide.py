@@ -274,26 +274,33 @@ def test_wide_encaps_more_than_65536_rows(path):
         assert np.all(host32(U[:1]) == (((m - 4) * 65535 + 4 * (q - 1)) * -127 - 128) % q)
 
 
-def test_wide_keygen_beyond_the_tensor_kernels_n():
-    """n = 131072 > 65536 (Table 1's last row): the skinny tensor-core GEMM's byte-plane sums do not hold it, KeyGen
-    runs on the CUDA cores (forcing the tensor path is refused); |s| = 127 puts the 32-bit partial sums at their bound"""
-    m, n, q, batch = 72, 131072, F4, 2
+@pytest.mark.parametrize("n", [131072, 65536 + 8192])
+def test_wide_keygen_column_passes_beyond_65536(n):
+    """n > 65536 (Table 1's last row: 131072): a signed byte-plane sum of the skinny tensor-core GEMM holds 65536 columns,
+    so KeyGen contracts the columns of A in passes of 65536 (the second pass adds to the residues of the first; the
+    exception terms of the whole row go in with the first).  Both the tcgen05 path and the CUDA-core kernel against the
+    oracle; |s| = 127 puts every partial sum at its bound, and the exceptions lie on both sides of the pass boundary."""
+    m, q, batch = 72, F4, 2
     rng = np.random.default_rng(7)
     A = random_A(m, n, q, 13, 200)
+    A[:8, 65535] = 65536                                   # the last column of the first pass and the first of the second
+    A[:8, 65536] = 65536                                   # (8 rows: a column's exception list holds 16)
     s = rng.integers(-3, 4, (batch, n)).astype(np.int8)
     s[1, :] = 127
     e = rng.integers(-12, 13, (batch, m)).astype(np.int8)
+    got = {}
     with B().Context(n, m, 256, q, 3, batch) as c:
         c.wide_load_matrix(dev32(A))
-        t = empty32(batch, m)
-        c.wide_keygen(dev8(s), dev8(e), t, batch)
-        g = host32(t)
-        c.set_option(B().OPT_KEYGEN_PATH, 2)
-        with pytest.raises(B().LweError) as ei:
+        for path in (0, 1, 2):                             # auto (= tensor cores), CUDA cores, tensor cores forced
+            c.set_option(B().OPT_KEYGEN_PATH, path)
+            t = empty32(batch, m)
+            t.fill_(-1)
             c.wide_keygen(dev8(s), dev8(e), t, batch)
-        assert ei.value.code == -5
+            got[path] = host32(t)
     for b in range(batch):
-        assert np.array_equal(g[b], O.keygen_w(A, s[b], e[b], q)), b
+        want = O.keygen_w(A, s[b], e[b], q)
+        for path in got:
+            assert np.array_equal(got[path][b], want), (path, b)
 
 
 # ---------------------------------------------------------------- Decrypt
@@ -466,7 +473,7 @@ def test_table1_rows_q65537_sampled_rows_identity_and_recovery(n, batch, seeded,
 
 def test_table1_last_row_n131072_sampled_rows():
     """Table 1 row 9 (n = 131072, q = 65537, sigma = 1.0, e2 in [-1, 1], eta = 3), one instance: A loaded from
-    its seed panel by panel (A16 = 32 GiB; the uint32 matrix, 64 GiB, never exists), KeyGen on the CUDA cores, Encrypt in two
+    its seed panel by panel (A16 = 32 GiB; the uint32 matrix, 64 GiB, never exists), KeyGen in two column passes, Encrypt in two
     row passes on tcgen05, Decrypt.  40 sampled rows of t and 24 sampled rows of U against the oracle, every bit recovered."""
     n, q, sigma, kappa, k, seed, inst = 131072, F4, 1.0, 1, 256, 8, 3
     rng = np.random.default_rng(n)
