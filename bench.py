@@ -494,13 +494,8 @@ def paper_variant_phase(B, device: int) -> dict:
         mu, out = torch.empty(Bt, k // 8, **u8), torch.empty(Bt, k // 8, **u8)
         U, v = torch.empty(Bt, n, k, **i16), torch.empty(Bt, k, **i16)
 
-        def sample():
-            c.sample_cbd(s, 0, n, seed, W.TAG_S, 0, Bt)
-            c.sample_gauss_u16(e, 0, n, seed, W.TAG_E, 0, Bt, sigma)
-            c.sample_gauss_s8(R, 0, n * k, seed, W.TAG_RG, 0, Bt, sigma)
-            c.sample_gauss_s8(E1, 0, n * k, seed, W.TAG_E1, 0, Bt, sigma)
-            c.sample_cuniform_s8(e2, 0, k, seed, W.TAG_E2, 0, Bt, bound)
-            c.sample_bits(mu, 0, k, seed, W.TAG_MU, 0, Bt)
+        def sample():                                    # s, e, R, E1, e2, mu of the batch in one launch
+            c.sample_pke(s, e, R, E1, e2, mu, seed, 0, Bt, sigma, bound)
 
         t_s = time_call(sample)
         t_k = time_call(lambda: c.keygen(A, 0, s, e, t, Bt))
@@ -539,13 +534,8 @@ def paper_variant_wide_phase(B, device: int) -> dict:
         mu, out = torch.empty(Bt, k // 8, **u8), torch.empty(Bt, k // 8, **u8)
         U, v = torch.empty(Bt, n, k, **i32), torch.empty(Bt, k, **i32)
 
-        def sample():
-            c.sample_cbd_s8(s, 0, n, seed, W.TAG_S, 0, Bt)
-            c.sample_gauss_s8(e, 0, n, seed, W.TAG_E, 0, Bt, sigma)
-            c.sample_gauss_s8(R, 0, n * k, seed, W.TAG_RG, 0, Bt, sigma)
-            c.sample_gauss_s8(E1, 0, n * k, seed, W.TAG_E1, 0, Bt, sigma)
-            c.sample_cuniform_s8(e2, 0, k, seed, W.TAG_E2, 0, Bt, bound)
-            c.sample_bits(mu, 0, k, seed, W.TAG_MU, 0, Bt)
+        def sample():                                    # s, e, R, E1, e2, mu of the batch in one launch
+            c.sample_pke(s, e, R, E1, e2, mu, seed, 0, Bt, sigma, bound)
 
         t_s = time_call(sample)
         t_k = time_call(lambda: c.wide_keygen(s, e, t, Bt))
@@ -605,17 +595,8 @@ def paper_table1_phase(B, device: int) -> dict:
             out = torch.empty(Bt, k // 8, dtype=torch.uint8, device=dev)
             U, v = torch.empty(Bt, n, k, dtype=res_t, device=dev), torch.empty(Bt, k, dtype=res_t, device=dev)
 
-            def sample():
-                if wide:
-                    c.sample_cbd_s8(s, 0, n, seed, W.TAG_S, 0, Bt)
-                    c.sample_gauss_s8(e, 0, n, seed, W.TAG_E, 0, Bt, sigma)
-                else:
-                    c.sample_cbd(s, 0, n, seed, W.TAG_S, 0, Bt)
-                    c.sample_gauss_u16(e, 0, n, seed, W.TAG_E, 0, Bt, sigma)
-                c.sample_gauss_s8(R, 0, n * k, seed, W.TAG_RG, 0, Bt, sigma)
-                c.sample_gauss_s8(E1, 0, n * k, seed, W.TAG_E1, 0, Bt, sigma)
-                c.sample_cuniform_s8(e2, 0, k, seed, W.TAG_E2, 0, Bt, bound)
-                c.sample_bits(mu, 0, k, seed, W.TAG_MU, 0, Bt)
+            def sample():                                # s, e, R, E1, e2, mu of the batch in one launch
+                c.sample_pke(s, e, R, E1, e2, mu, seed, 0, Bt, sigma, bound)
 
             if wide:
                 keygen = lambda: c.wide_keygen(s, e, t, Bt)                               # noqa: E731

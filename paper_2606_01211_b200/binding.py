@@ -29,13 +29,13 @@ OPT_V_PATH = 9
 OPT_PDL = 10
 KERNELS = ["rng_fill", "sample_uniform", "sample_cbd", "sample_bits", "keygen_stored", "keygen_regen",
            "expand_R_v", "encaps_tc", "encaps_simt", "decaps", "keygen_prep", "keygen_tc", "fo_verdict",
-           "sample_gauss", "sample_cuniform", "prep_R_pv", "encaps_regen_tc", "sample_kem", "wide_pack", "wide_keygen"]
+           "sample_gauss", "sample_cuniform", "prep_R_pv", "encaps_regen_tc", "sample_kem", "wide_pack", "wide_keygen", "sample_pke"]
 
 EXPORTS = [
     "lwe_create", "lwe_destroy", "lwe_strerror", "lwe_last_cuda_error", "lwe_launch_count",
     "lwe_rng_fill", "lwe_sample_uniform", "lwe_sample_cbd", "lwe_sample_bits", "lwe_sample_kem",
     "lwe_keygen", "lwe_encaps", "lwe_decaps", "lwe_decaps_fo", "lwe_kem_host",
-    "lwe_sample_gauss_s8", "lwe_sample_gauss_u16", "lwe_sample_cuniform_s8", "lwe_encaps_pv", "lwe_set_option",
+    "lwe_sample_gauss_s8", "lwe_sample_gauss_u16", "lwe_sample_cuniform_s8", "lwe_sample_pke", "lwe_encaps_pv", "lwe_set_option",
     "lwe_profile_read", "lwe_profile_reset",
     "lwe_sample_uniform_u32", "lwe_sample_cbd_s8", "lwe_wide_load_matrix", "lwe_wide_load_matrix_seeded", "lwe_wide_keygen",
     "lwe_wide_encaps", "lwe_wide_decaps",
@@ -87,6 +87,7 @@ def load_library() -> C.CDLL:
     for f in (lib.lwe_sample_gauss_s8, lib.lwe_sample_gauss_u16):
         f.argtypes = [vp, vp, u64, u64, u64, u32, u32, u32, C.c_double, vp]
     lib.lwe_sample_cuniform_s8.argtypes = [vp, vp, u64, u64, u64, u32, u32, u32, u32, vp]
+    lib.lwe_sample_pke.argtypes = [vp, vp, vp, vp, vp, vp, vp, u64, u32, u32, C.c_double, u32, vp]
     lib.lwe_encaps_pv.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
     lib.lwe_kem_host.argtypes = [vp, vp, u64, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
     for f in (lib.lwe_sample_uniform_u32, lib.lwe_sample_cbd_s8):
@@ -228,6 +229,11 @@ class Context:
                            stream=None):
         self._check(self._lib.lwe_sample_cuniform_s8(self._h, _ptr(d_out), first, count, seed, tag, inst0, n_inst,
                                                      bound, _stream(stream)), "lwe_sample_cuniform_s8")
+
+    def sample_pke(self, d_s, d_e, d_R, d_E1, d_e2, d_mubits, seed: int, inst0: int, n_inst: int, sigma: float, e2_bound: int,
+                   stream=None):
+        self._check(self._lib.lwe_sample_pke(self._h, _ptr(d_s), _ptr(d_e), _ptr(d_R), _ptr(d_E1), _ptr(d_e2), _ptr(d_mubits),
+                                             seed, inst0, n_inst, float(sigma), e2_bound, _stream(stream)), "lwe_sample_pke")
 
     def encaps_pv(self, d_A, d_t, d_R, d_E1, d_e2, d_mubits, d_U, d_v, batch: int = 1, stream=None):
         self._check(self._lib.lwe_encaps_pv(self._h, _ptr(d_A), _ptr(d_t), _ptr(d_R), _ptr(d_E1), _ptr(d_e2),

@@ -616,6 +616,23 @@ int lwe_sample_cuniform_s8(lwe_ctx *ctx, int8_t *d_out, uint64_t first, uint64_t
     return LWE_OK;
 }
 
+int lwe_sample_pke(lwe_ctx *ctx, void *d_s, void *d_e, int8_t *d_R, int8_t *d_E1, int8_t *d_e2, uint8_t *d_mubits,
+                   uint64_t seed, uint32_t inst0, uint32_t n_inst, double sigma, uint32_t e2_bound, void *stream)
+{
+    CHECK_CTX(ctx);
+    if (!(sigma >= 0.5 && sigma <= 2.8) || e2_bound < 1 || e2_bound > 127) return LWE_ERR_PARAM;
+    if ((uint64_t)inst0 + n_inst > (1ull << 32)) return LWE_ERR_PARAM;
+    if (n_inst == 0) return LWE_OK;
+    REQUIRE_PTR(d_s); REQUIRE_PTR(d_e); REQUIRE_PTR(d_R); REQUIRE_PTR(d_E1); REQUIRE_PTR(d_e2); REQUIRE_PTR(d_mubits);
+    REQUIRE_ALIGNED(d_s); REQUIRE_ALIGNED(d_e); REQUIRE_ALIGNED(d_R); REQUIRE_ALIGNED(d_E1); REQUIRE_ALIGNED(d_e2);
+    REQUIRE_ALIGNED(d_mubits);
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_sample_pke(c, d_s, d_e, d_R, d_E1, d_e2, d_mubits, seed_key_host(seed), inst0, n_inst, sigma, e2_bound,
+                                (cudaStream_t)stream));
+    return LWE_OK;
+}
+
 int lwe_encaps_pv(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_t, const int8_t *d_R, const int8_t *d_E1,
                   const int8_t *d_e2, const uint8_t *d_mubits, uint16_t *d_U, uint16_t *d_v, uint32_t batch, void *stream)
 {

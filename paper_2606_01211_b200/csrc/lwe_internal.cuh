@@ -263,6 +263,8 @@ cudaError_t launch_encaps_tc2(Ctx *c, const uint16_t *d_A, uint16_t *d_U, uint32
 // N2 (the paper's own PKE variant)
 cudaError_t launch_sample_gauss(Ctx *c, void *d_out, bool as_u16, uint64_t first, uint64_t count, const AesKey &key,
                                 uint32_t tag, uint32_t inst0, uint32_t n_inst, double sigma, cudaStream_t st);
+cudaError_t launch_sample_pke(Ctx *c, void *d_s, void *d_e, int8_t *d_R, int8_t *d_E1, int8_t *d_e2, uint8_t *d_mubits,
+                              const AesKey &key, uint32_t inst0, uint32_t n_inst, double sigma, uint32_t bound, cudaStream_t st);
 cudaError_t launch_sample_cuniform(Ctx *c, int8_t *d_out, uint64_t first, uint64_t count, const AesKey &key, uint32_t tag,
                                    uint32_t inst0, uint32_t n_inst, uint32_t bound, cudaStream_t st);
 cudaError_t launch_prep_R_pv_and_v(Ctx *c, const uint16_t *d_t, const int8_t *d_R, const int8_t *d_e2,

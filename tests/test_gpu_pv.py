@@ -57,6 +57,43 @@ def test_cuniform_sampler_matches_oracle(H, bound):
         assert np.array_equal(g[t], O.sample_cuniform(first, count, seed, O.TAG_E2, inst0 + t, bound)), t
 
 
+@pytest.mark.parametrize("n,m,k,q,sigma,bound,inst0,n_inst", [
+    (512, 512, 256, 3329, 2.3, 3, 0, 3), (264, 136, 128, 12289, 1.7, 2, 7, 2), (64, 64, 8, 65536, 0.5, 127, 1, 5),
+    (1024, 1024, 256, 65537, 1.2, 2, 4, 2), (200, 72, 384, 65539, 2.8, 1, 0, 3)])
+def test_sample_pke_equals_the_six_sampler_calls_and_the_oracle(H, n, m, k, q, sigma, bound, inst0, n_inst):
+    """lwe_sample_pke (one launch) writes exactly what the six sampler calls write -- s (CBD), e, R, E1 (Gaussian), e2
+    (centred uniform), mu (bits) -- on narrow (uint16 s, e) and wide (int8 s, e) contexts; each object against the
+    oracle's own draw (O5 / O5s, O12, O13, O6)."""
+    import torch
+    seed, eta = 23, 3
+    wide = q > 65536
+    with B().Context(n, m, k, q, eta, n_inst) as c:
+        s = empty_s8(n_inst, n) if wide else H.dev_empty_u16(n_inst, n)
+        e = empty_s8(n_inst, m) if wide else H.dev_empty_u16(n_inst, m)
+        R, E1, e2 = empty_s8(n_inst, m, k), empty_s8(n_inst, n, k), empty_s8(n_inst, k)
+        mu = H.dev_empty_u8(n_inst, k // 8)
+        for t_ in (s, e, R, E1, e2, mu):
+            t_.fill_(0x55)
+        c.sample_pke(s, e, R, E1, e2, mu, seed, inst0, n_inst, sigma, bound)
+        torch.cuda.synchronize()
+        as8 = lambda t_: t_.cpu().numpy().view(np.int8)  # noqa: E731
+        gs = as8(s) if wide else H.host_u16(s)
+        ge = as8(e) if wide else H.host_u16(e)
+        gR, gE1, ge2, gmu = as8(R), as8(E1), as8(e2), H.host_u8(mu)
+    for t in range(n_inst):
+        i = inst0 + t
+        if wide:
+            assert np.array_equal(gs[t], O.sample_cbd_s8(0, n, seed, O.TAG_S, i, eta)), ("s", t)
+            assert np.array_equal(ge[t], O.sample_gauss(0, m, seed, O.TAG_E, i, sigma)), ("e", t)
+        else:
+            assert np.array_equal(gs[t], O.sample_cbd(0, n, seed, O.TAG_S, i, q, eta)), ("s", t)
+            assert np.array_equal(ge[t], O.sample_gauss(0, m, seed, O.TAG_E, i, sigma, q)), ("e", t)
+        assert np.array_equal(gR[t].ravel(), O.sample_gauss(0, m * k, seed, O.TAG_RG, i, sigma)), ("R", t)
+        assert np.array_equal(gE1[t].ravel(), O.sample_gauss(0, n * k, seed, O.TAG_E1, i, sigma)), ("E1", t)
+        assert np.array_equal(ge2[t], O.sample_cuniform(0, k, seed, O.TAG_E2, i, bound)), ("e2", t)
+        assert np.array_equal(gmu[t], O.sample_bits(0, k, seed, O.TAG_MU, i)), ("mu", t)
+
+
 PV_SHAPES = [  # (n = m, k, q, batch)
     (256, 256, 3329, 1), (192, 256, 12289, 3), (200, 128, 12289, 3), (456, 256, 65521, 5), (1280, 256, 65536, 2),
     (64, 16, 3329, 2),
