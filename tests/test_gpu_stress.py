@@ -81,3 +81,50 @@ def test_random_shapes_all_paths_under_a_competing_stream(H, chunk):
                     for t in range(batch):
                         assert np.array_equal(gv[t], want[t][1]), (m, n, k, q, batch, path, panel, rep, t, "v")
                         assert np.array_equal(gU[t], want[t][0]), (m, n, k, q, batch, path, panel, rep, t, "U")
+
+
+@pytest.mark.parametrize("chunk", range(4))
+def test_random_shapes_streaming_kernels_back_to_back(H, chunk):
+    """The register-pipelined stream kernels (stored-A GEMV, batched tensor-core keygen, decaps: loads of the next batch in
+    flight while the current one is consumed, rows that end inside a batch, u32 / u64 column sums) on seeded random
+    shapes and moduli, launched back to back on reused buffers with programmatic dependent launch on and off, beside a
+    competing stream; every b and every recovered bit string against the oracle."""
+    import torch
+    Bd = B()
+    rng = np.random.default_rng(4000 + chunk)
+    side = torch.cuda.Stream()
+    noise = torch.empty(32 << 20, dtype=torch.uint8, device="cuda")
+    with Bd.Context(64, 64, 256, 65536, 4, 1) as filler:
+        for _ in range(6):
+            k = int(rng.choice([64, 128, 256, 256, 384, 512]))
+            q = int(rng.choice([65536, 65521, 4096, 3329]))
+            batch = int(rng.integers(1, 5))
+            n = 8 * int(rng.integers(1, 400))
+            m = 8 * int(rng.integers(1, 300))
+            seed = int(rng.integers(1, 1 << 30))
+            A = W.random_u16((m, n), q, seed)
+            s, e = W.random_u16((batch, n), q, seed + 1), W.random_u16((batch, m), q, seed + 2)
+            U, v = W.random_u16((batch, n, k), q, seed + 3), W.random_u16((batch, k), q, seed + 4)
+            want_b = [O.keygen(A, s[t], e[t], q) for t in range(batch)]
+            want_o = [O.decaps(U[t], v[t], s[t], q) for t in range(batch)]
+            with Bd.Context(n, m, k, q, 4, batch) as c:
+                dA, ds, de, dU, dv = H.dev(A), H.dev(s), H.dev(e), H.dev(U), H.dev(v)
+                b1, b2 = H.dev_empty_u16(batch, m), H.dev_empty_u16(batch, m)
+                out = H.dev_empty_u8(batch, k // 8)
+                for pdl in (1, 0):
+                    c.set_option(Bd.OPT_PDL, pdl)
+                    with torch.cuda.stream(side):
+                        filler.rng_fill(noise, 32 << 20, bytes(16), bytes(16), 0)
+                    for rep in range(3):                             # back to back, outputs overwritten each time
+                        b1.fill_(-1); b2.fill_(-1); out.fill_(0xEE)
+                        c.set_option(Bd.OPT_KEYGEN_PATH, 1)
+                        c.keygen(dA, 0, ds, de, b1, batch)           # one GEMV per instance
+                        c.set_option(Bd.OPT_KEYGEN_PATH, 0)
+                        c.keygen(dA, 0, ds, de, b2, batch)           # auto: the skinny tensor-core GEMM for batch >= 2
+                        c.decaps(dU, dv, ds, out, batch)
+                    torch.cuda.synchronize()
+                    g1, g2, go = H.host_u16(b1), H.host_u16(b2), H.host_u8(out)
+                    for t in range(batch):
+                        assert np.array_equal(g1[t], want_b[t]), (m, n, k, q, batch, pdl, t, "gemv")
+                        assert np.array_equal(g2[t], want_b[t]), (m, n, k, q, batch, pdl, t, "keygen auto")
+                        assert np.array_equal(go[t], want_o[t]), (m, n, k, q, batch, pdl, t, "decaps")
