@@ -188,3 +188,44 @@ def test_pv_full_path_from_seeds_matches_oracle_and_recovers_every_bit(H, n, q, 
         assert np.array_equal(gU[b], Uo) and np.array_equal(gv[b], vo)
         assert np.array_equal(gout[b], O.decaps(Uo, vo, so, q))
         assert np.array_equal(gout[b], muo), "not every bit recovered"
+
+
+@pytest.mark.parametrize("n,q,sigma,bound", [(4096, 12289, 1.7, 3), (8192, 65537, 1.2, 2)])
+def test_sample_pke_at_the_sizes_bench_times_equals_the_six_sampler_calls(H, n, q, sigma, bound):
+    """lwe_sample_pke in the launch configuration bench.py's N2 phases time (32 instances, Table 1 rows n = 4096 and
+    n = 8192): byte for byte what the six single-object sampler calls write -- each of which is compared with the oracle
+    in the tests above -- plus the oracle's own draw of one instance's s, e, e2, mu and of sampled blocks of R and E1."""
+    import torch
+    k, Bt, seed, eta = 256, 32, 9, 3
+    wide = q > 65536
+    with B().Context(n, n, k, q, eta, Bt) as c:
+        def bufs():
+            s = empty_s8(Bt, n) if wide else H.dev_empty_u16(Bt, n)
+            e = empty_s8(Bt, n) if wide else H.dev_empty_u16(Bt, n)
+            return s, e, empty_s8(Bt, n, k), empty_s8(Bt, n, k), empty_s8(Bt, k), H.dev_empty_u8(Bt, k // 8)
+        one, six = bufs(), bufs()
+        c.sample_pke(*one, seed, 0, Bt, sigma, bound)
+        s, e, R, E1, e2, mu = six
+        if wide:
+            c.sample_cbd_s8(s, 0, n, seed, W.TAG_S, 0, Bt)
+            c.sample_gauss_s8(e, 0, n, seed, W.TAG_E, 0, Bt, sigma)
+        else:
+            c.sample_cbd(s, 0, n, seed, W.TAG_S, 0, Bt)
+            c.sample_gauss_u16(e, 0, n, seed, W.TAG_E, 0, Bt, sigma)
+        c.sample_gauss_s8(R, 0, n * k, seed, W.TAG_RG, 0, Bt, sigma)
+        c.sample_gauss_s8(E1, 0, n * k, seed, W.TAG_E1, 0, Bt, sigma)
+        c.sample_cuniform_s8(e2, 0, k, seed, W.TAG_E2, 0, Bt, bound)
+        c.sample_bits(mu, 0, k, seed, W.TAG_MU, 0, Bt)
+        torch.cuda.synchronize()
+        for name, a, b in zip("s e R E1 e2 mu".split(), one, six):
+            assert torch.equal(a, b), name
+        t = 17                                               # one instance against the oracle's own draws
+        gR = one[2][t].cpu().numpy().view(np.int8).ravel()
+        gE1 = one[3][t].cpu().numpy().view(np.int8).ravel()
+        ge2 = one[4][t].cpu().numpy().view(np.int8)
+        gmu = one[5][t].cpu().numpy()
+    for first in (0, 8 * 1001, n * k - 4096):
+        assert np.array_equal(gR[first:first + 4096], O.sample_gauss(first, 4096, seed, O.TAG_RG, t, sigma)), first
+        assert np.array_equal(gE1[first:first + 4096], O.sample_gauss(first, 4096, seed, O.TAG_E1, t, sigma)), first
+    assert np.array_equal(ge2, O.sample_cuniform(0, k, seed, O.TAG_E2, t, bound))
+    assert np.array_equal(gmu, O.sample_bits(0, k, seed, O.TAG_MU, t))
