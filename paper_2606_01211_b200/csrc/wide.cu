@@ -252,21 +252,28 @@ wide_decaps_kernel(const uint32_t *__restrict__ U, const uint32_t *__restrict__ 
         uint32_t j = jbeg + rslot;
         const uint4 *up = reinterpret_cast<const uint4 *>(Ub) + (size_t)j * tpr + cg;
         const size_t ustep = (size_t)rows_per_iter * tpr;
-        // products < 2^17 * 2^7 = 2^24: a 32-bit partial holds 128 rows; flush into 64 bits every 32 unrolled steps
+        // products < 2^17 * 2^7 = 2^24: a 32-bit partial holds 128 rows; flushed into 64 bits every 120 rows.
+        // Register-pipelined as decaps_kernel: the loads of the next four rows are issued before the current four are
+        // consumed; a row past the end of the range re-reads a valid address with s = 0 (no tail of single loads).
         int p[4] = {0, 0, 0, 0};
         uint32_t since = 0;
-        for (; j + (kUnroll - 1) * rows_per_iter < jend; j += kUnroll * rows_per_iter, up += kUnroll * ustep) {
-            uint4 u[kUnroll];
-            int sj[kUnroll];
+        uint4 u0[kUnroll], u1[kUnroll];
+        int s0[kUnroll], s1[kUnroll];
+        auto load = [&](uint4 (&uu)[kUnroll], int (&ss)[kUnroll]) {
 #pragma unroll
             for (int r = 0; r < kUnroll; r++) {
-                u[r] = ldg_stream16(up + r * ustep);
-                sj[r] = (int)__ldg(sb + j + r * rows_per_iter);
+                const bool in = j + r * rows_per_iter < jend;
+                uu[r] = ldg_stream16(in ? up + r * ustep : reinterpret_cast<const uint4 *>(Ub) + cg);
+                ss[r] = in ? (int)__ldg(sb + j + r * rows_per_iter) : 0;
             }
+            j += kUnroll * rows_per_iter;
+            up += kUnroll * ustep;
+        };
+        auto consume = [&](const uint4 (&uu)[kUnroll], const int (&ss)[kUnroll]) {
 #pragma unroll
             for (int r = 0; r < kUnroll; r++) {
-                p[0] += (int)u[r].x * sj[r]; p[1] += (int)u[r].y * sj[r];
-                p[2] += (int)u[r].z * sj[r]; p[3] += (int)u[r].w * sj[r];
+                p[0] += (int)uu[r].x * ss[r]; p[1] += (int)uu[r].y * ss[r];
+                p[2] += (int)uu[r].z * ss[r]; p[3] += (int)uu[r].w * ss[r];
             }
             since += kUnroll;
             if (since >= 120) {
@@ -274,12 +281,19 @@ wide_decaps_kernel(const uint32_t *__restrict__ U, const uint32_t *__restrict__ 
                 for (int x = 0; x < 4; x++) { a[x] += p[x]; p[x] = 0; }
                 since = 0;
             }
-        }
-        for (; j < jend; j += rows_per_iter, up += ustep) {
-            const uint4 u = ldg_stream16(up);
-            const int sj = (int)__ldg(sb + j);
-            a[0] += (long long)((int)u.x * sj); a[1] += (long long)((int)u.y * sj);
-            a[2] += (long long)((int)u.z * sj); a[3] += (long long)((int)u.w * sj);
+        };
+        if (j < jend) {
+            load(u0, s0);
+            for (;;) {
+                const bool more1 = j < jend;
+                if (more1) load(u1, s1);
+                consume(u0, s0);
+                if (!more1) break;
+                const bool more0 = j < jend;
+                if (more0) load(u0, s0);
+                consume(u1, s1);
+                if (!more0) break;
+            }
         }
 #pragma unroll
         for (int x = 0; x < 4; x++) a[x] += p[x];
