@@ -715,3 +715,37 @@ def test_decaps_fo_matches_oracle_honest_and_tampered(H, path, n, m, k, q, batch
         assert int(g_ok[t]) == o_ok, (t, tampers[t % len(tampers)])
         assert np.array_equal(g_out[t], o_out), t
         assert o_ok == (1 if tampers[t % len(tampers)] == "honest" else 0)
+
+
+def test_kem_host_chunk_plan_over_many_batch_sizes(H):
+    """lwe_kem_host's chunk plan (1, 1, 2, 4, ... instances, the last chunk taking the rest) at every batch size from 1 to
+    40 on one context: every output of every instance against the oracle (tiny shape, so that the sweep stays cheap)."""
+    import torch
+    n, m, k, q, seed, Bmax = 64, 128, 256, 65536, 5, 40
+    A = O.sample_uniform(0, m * n, seed, O.TAG_A, 0, q).reshape(m, n)
+    s, e = W.random_u16((Bmax, n), q, 61), W.random_u16((Bmax, m), 5, 62)
+    Rbits = W.random_bytes(Bmax * m * k // 8, 63).reshape(Bmax, -1)
+    mubits = W.random_bytes(Bmax * k // 8, 64).reshape(Bmax, -1)
+    want = []
+    for t in range(Bmax):
+        b = O.keygen(A, s[t], e[t], q)
+        U, v = O.encaps(A, b, Rbits[t], mubits[t], k, q)
+        want.append((b, U, v, O.decaps(U, v, s[t], q)))
+
+    def pinned(a):
+        return torch.from_numpy(a.view(np.int16) if a.dtype == np.uint16 else a).pin_memory()
+
+    h_s, h_e, h_R, h_mu = pinned(s), pinned(e), pinned(Rbits), pinned(mubits)
+    with B().Context(n, m, k, q, 4, Bmax) as c:
+        dA = H.dev(A)
+        for batch in range(1, Bmax + 1):
+            h_b = torch.zeros(batch, m, dtype=torch.int16).pin_memory()
+            h_U = torch.zeros(batch, n, k, dtype=torch.int16).pin_memory()
+            h_v = torch.zeros(batch, k, dtype=torch.int16).pin_memory()
+            h_out = torch.zeros(batch, k // 8, dtype=torch.uint8).pin_memory()
+            c.kem_host(dA, seed, h_s, h_e, h_R, h_mu, h_b, h_U, h_v, h_out, batch)
+            gb, gU, gv, go = h_b.numpy().view(np.uint16), h_U.numpy().view(np.uint16), h_v.numpy().view(np.uint16), h_out.numpy()
+            for t in range(batch):
+                b, U, v, out = want[t]
+                assert np.array_equal(gb[t], b) and np.array_equal(gU[t], U) and np.array_equal(gv[t], v), (batch, t)
+                assert np.array_equal(go[t], out), (batch, t)
