@@ -39,7 +39,9 @@ EXPORTS = [
     "lwe_profile_read", "lwe_profile_reset",
     "lwe_sample_uniform_u32", "lwe_sample_cbd_s8", "lwe_wide_load_matrix", "lwe_wide_load_matrix_seeded", "lwe_wide_keygen",
     "lwe_wide_encaps", "lwe_wide_decaps",
+    "lwe_decaps_static",
 ]
+STATIC_MAX_COLS, STATIC_MAX_BATCH = 16384, 64                # LWE_STATIC_MAX_COLS / _BATCH of include/lwe.h
 
 
 class LweError(RuntimeError):
@@ -97,6 +99,7 @@ def load_library() -> C.CDLL:
     lib.lwe_wide_keygen.argtypes = [vp, vp, vp, vp, u32, vp]
     lib.lwe_wide_encaps.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
     lib.lwe_wide_decaps.argtypes = [vp, vp, vp, vp, vp, u32, vp]
+    lib.lwe_decaps_static.argtypes = [u32, u32, u32, vp, vp, vp, vp, u32, vp]
     _lib = lib
     return lib
 
@@ -115,6 +118,17 @@ def _stream(stream) -> int:
     if isinstance(stream, int):
         return stream
     return stream.cuda_stream
+
+
+def decaps_static(n: int, k: int, q: int, d_U, d_v, d_s, d_mubits_out, batch: int = 1, stream=None):
+    """lwe_decaps_static: Decaps without a context, for callers that may not allocate device memory (they are handed
+    buffers and a stream by a host framework whose allocator owns the device).  Nothing is allocated here or in the
+    library: the scratch is a fixed array inside liblwe_b200.so, shared by every call on the device, so calls must not
+    overlap on the GPU, and batch * k <= STATIC_MAX_COLS, batch <= STATIC_MAX_BATCH.  The tensors' device must be the
+    current device.  Make the first call on a device outside stream capture."""
+    rc = load_library().lwe_decaps_static(n, k, q, _ptr(d_U), _ptr(d_v), _ptr(d_s), _ptr(d_mubits_out), batch, _stream(stream))
+    if rc != LWE_OK:
+        raise LweError(rc, "lwe_decaps_static")
 
 
 class Context:

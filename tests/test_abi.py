@@ -81,3 +81,20 @@ def test_kernel_id_table_of_the_binding_matches_the_header():
     assert ids.pop("COUNT") == len(B.KERNELS) == len(ids)
     for name, i in ids.items():
         assert B.KERNELS[i].upper() == name, (i, name, B.KERNELS[i])
+
+
+def test_decaps_static_checks_its_limits_before_touching_cuda(lib):
+    """lwe_decaps_static (the entry point for callers that cannot allocate): argument and size-limit errors come back
+    without any CUDA call, so they can be checked on a box with no GPU; the limits are those of include/lwe.h."""
+    from paper_2606_01211_b200 import binding as B
+    header = (ROOT / "include" / "lwe.h").read_text()
+    assert int(re.search(r"#define LWE_STATIC_MAX_COLS (\d+)u", header).group(1)) == B.STATIC_MAX_COLS
+    assert int(re.search(r"#define LWE_STATIC_MAX_BATCH (\d+)u", header).group(1)) == B.STATIC_MAX_BATCH
+    f = B.load_library().lwe_decaps_static
+    p = 4096                                               # any non-NULL 16-byte aligned value: never dereferenced here
+    assert f(64, 256, 65536, p, p, p, p, B.STATIC_MAX_BATCH + 1, None) == -5
+    assert f(64, 2048, 65536, p, p, p, p, B.STATIC_MAX_COLS // 2048 + 1, None) == -5
+    assert f(64, 256, 65537, p, p, p, p, 1, None) == -1
+    assert f(64, 12, 65536, p, p, p, p, 1, None) == -1
+    assert f(64, 256, 65536, None, p, p, p, 1, None) == -3
+    assert f(64, 256, 65536, p + 2, p, p, p, 1, None) == -2
