@@ -55,6 +55,10 @@ from paper_2606_01211_b200 import workloads as W  # noqa: E402
 
 METRIC = "encaps+decaps KEMs/sec at n=8192"
 UNIT = "KEM/s"
+# the same string in both arms' config.workload (the driver compares them)
+WORKLOAD = ("C4: n=8192 m=16384 q=65536 k=256 eta=4, 32 instances per step sharing one stored A (256 MiB); "
+            "step = sample s,e,R,mu + keygen + encaps + decaps")
+MAX_LINE_BYTES = 4096                    # the final stdout line must stay below this (round 2's 21.7 KB line was cut)
 SM_COUNT_B200 = 148
 INT8_OPS_PER_CLK_PER_SM = 16384          # 8192 u8 MACs per clock and SM (4.5 POP/s nominal at 1.86 GHz x 148 SMs)
 
@@ -342,7 +346,7 @@ def run_reference(args):
         "ms_per_step_is": "the MEASURED host time of one step's bounded sample",
         "extrapolated_ms_per_full_instance": sec_full * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "u16 mod q (u64 accumulate, % q per MAC)",
-        "data": "synthetic", "config": {"workload": "C4: n=8192 m=16384 q=65536 k=256 eta=4, 32 instances sharing one stored A",
+        "data": "synthetic", "config": {"workload": WORKLOAD,
                                         "note": "host cores only; value = 1 / (seconds per instance, extrapolated from the sample)"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": desc,
                          "host_cpus": os.cpu_count()},
@@ -748,6 +752,44 @@ def library_int8_gemm(seconds: float) -> dict:
         return {"unavailable": type(ex).__name__}
 
 
+def int8_pipe_probe(ctx, seconds: float) -> dict:
+    """lwe_probe_int8_pipe: every SM pair issues tcgen05.mma.cta_group::2.kind::i8 (the encaps GEMM's instruction and
+    shape) back to back on shared-memory-resident operands -- the int8 tensor pipe's own rate on THIS box, the
+    denominator S8(d) asks for.  Both operand kinds the product uses: u8 x {0,1} (binary R) and u8 x dense s8 (the
+    paper's own PKE).  burst: best of 5 launches of ~20 ms each; sustained (seconds > 0): ~20 ms launches back to back
+    for `seconds` with the NVML clock / power record, rate of the last quarter."""
+    out = {"instruction": "tcgen05.mma.cta_group::2.kind::i8 M=256 N=256 K=32, operands resident in smem, no TMA, no epilogue",
+           "pipe_nominal_TOPs_at_max_clock": SM_COUNT_B200 * INT8_OPS_PER_CLK_PER_SM * 1965e6 / 1e12}
+    for label, signed in (("u8_x_bits", False), ("u8_x_s8", True)):
+        ops0 = ctx.probe_int8_pipe(2000, signed)
+        t0 = time_call(lambda: ctx.probe_int8_pipe(2000, signed), reps=1, warm=1)
+        iters = max(2000, int(2000 * 20.0 / t0))
+        ops = ctx.probe_int8_pipe(iters, signed)
+        with ClockSampler(torch.cuda.current_device(), 0.002) as clk:
+            best = min(time_call(lambda: ctx.probe_int8_pipe(iters, signed), reps=1, warm=0) for _ in range(5))
+        entry = {"iters_per_pair": iters, "ops_per_launch": ops, "burst_ms": best, "burst_TOPs": ops / (best * 1e-3) / 1e12,
+                 "burst_clocks": clk.summary()}
+        mhz = entry["burst_clocks"].get("sm_mhz")
+        if mhz:
+            entry["burst_frac_of_148x16384xclock"] = ops / (best * 1e-3) / (SM_COUNT_B200 * INT8_OPS_PER_CLK_PER_SM * mhz * 1e6)
+        if seconds > 0:
+            reps = max(20, int(seconds * 1e3 / best))
+            with ClockSampler(torch.cuda.current_device(), 0.005) as clk:
+                t = time_call(lambda: ctx.probe_int8_pipe(iters, signed), reps=reps, warm=0)
+                t_tail = time_call(lambda: ctx.probe_int8_pipe(iters, signed), reps=max(5, reps // 4), warm=0)
+            entry.update({"sustained_TOPs": ops / (t_tail * 1e-3) / 1e12, "whole_loop_TOPs": ops / (t * 1e-3) / 1e12,
+                          "sustained_seconds": (t * reps + t_tail * max(5, reps // 4)) / 1e3,
+                          "sustained_clocks": clk.summary(detail=True)})
+        out[label] = entry
+        del ops0
+    return out
+
+
+def int8_pipe_peak_phase(B, device: int) -> dict:
+    with B.Context(W.C4.n, W.C4.m, W.C4.k, W.C4.q, W.C4.eta, 1, device) as ctx:
+        return int8_pipe_probe(ctx, 3.0)
+
+
 def sustained_block(job: Job, seconds: float, ms_step_burst: float, peaks: dict) -> dict:
     """The SAME step looped back to back for >= `seconds` (the power controller needs ~1 s to respond): per-step
     event times, the GEMM's own event times (LWE_OPT_PROFILE on that kernel only), NVML samples every 5 ms, results
@@ -802,7 +844,8 @@ def sustained_block(job: Job, seconds: float, ms_step_burst: float, peaks: dict)
 
 PHASES = {"paper_variant_n4096_B32": paper_variant_phase, "paper_variant_n8192_q65537_B32": paper_variant_wide_phase,
           "single_kem_B1": single_kem_phase, "paper_table1_all_rows": paper_table1_phase,
-          "large_kem_C5_B1": lambda B, device: large_kem_phase(B, device, measured_peaks()["hbm_gbs"])}
+          "large_kem_C5_B1": lambda B, device: large_kem_phase(B, device, measured_peaks()["hbm_gbs"]),
+          "int8_pipe_peak": int8_pipe_peak_phase}
 
 
 def pipelined_phase(job: Job, steps: int, sustained_s: float = 0.0) -> dict:
@@ -890,6 +933,102 @@ def pipelined_phase(job: Job, steps: int, sustained_s: float = 0.0) -> dict:
     finally:
         j1.ctx.close()
     return out
+
+
+def _r(x, nd=6):
+    """floats rounded for the compact line (6 significant digits are more than any figure here carries)"""
+    if isinstance(x, float):
+        return float(f"{x:.{nd}g}")
+    if isinstance(x, dict):
+        return {k2: _r(v2, nd) for k2, v2 in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_r(v2, nd) for v2 in x]
+    return x
+
+
+def _get(d, *path):
+    for key in path:
+        if not isinstance(d, dict) or d.get(key) is None:
+            return None
+        d = d[key]
+    return d
+
+
+COMPACT_KEYS = ["metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "gpu_launches", "config", "clocks", "roofline", "cpu_baseline", "e2e"]
+
+
+def compact_line(full: dict) -> dict:
+    """The ONE line the driver parses: the contract keys plus a dozen scalars, well under MAX_LINE_BYTES.  Everything
+    else of `full` (phases, per-kernel table, sustained block, per-config CPU baselines) goes to earlier stdout lines
+    and to bench_details.json (print_details)."""
+    out = {k2: full.get(k2) for k2 in COMPACT_KEYS[:13]}
+    cfg = full.get("config") or {}
+    out["config"] = {k2: cfg.get(k2) for k2 in ("workload", "instances_per_step_per_gpu", "parallelism", "l2", "regime",
+                                                "all_bits_recovered") if k2 in cfg}
+    clk = full.get("clocks") or {}
+    out["clocks"] = {k2: clk.get(k2) for k2 in ("sm_mhz", "sm_max_mhz", "reasons", "samples")}
+    rf = full.get("roofline")
+    if rf:
+        out["roofline"] = {k2: rf.get(k2) for k2 in ("kernel", "bound", "achieved", "peak", "unit", "frac", "traffic",
+                                                      "ms_per_launch", "peak_kind", "frac_of_measured_int8_pipe",
+                                                      "measured_int8_pipe_TOPs", "frac_of_nominal_4500") if k2 in rf}
+    else:
+        out["roofline"] = None
+    cb = full.get("cpu_baseline")
+    out["cpu_baseline"] = ({k2: cb.get(k2) for k2 in ("value", "unit", "cores", "kind", "sample")} if cb else None)
+    e2e = full.get("e2e") or {}
+    out["e2e"] = {k2: e2e.get(k2) for k2 in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "ms_per_step", "api")}
+    ph = full.get("phases") or {}
+    scalars = {
+        "dominant_kernel_share_of_step": full.get("dominant_kernel_share_of_step"),
+        "modular_GOPs": full.get("modular_GOPs"),
+        "sustained_value": _get(full, "sustained", "value_settled"),
+        "sustained_gemm_TOPs": _get(full, "sustained", "gemm", "int8_TOPs"),
+        "sustained_gemm_frac_of_measured_int8_pipe": _get(full, "sustained", "gemm", "frac_of_measured_int8_pipe"),
+        "pipelined_two_streams_value": _get(ph, "pipelined_B32", "value"),
+        "keygen_gemv_frac_hbm": _get(ph, "keygen_stored_B1", "back_to_back", "frac_hbm"),
+        "keygen_gemv_frac_hbm_per_call": _get(ph, "keygen_stored_B1", "frac_hbm"),
+        "keygen_B32_frac_hbm": _get(ph, "keygen_stored_B32", "back_to_back", "frac_hbm"),
+        "decaps_frac_hbm": _get(ph, "decaps_B32", "back_to_back", "frac_hbm"),
+        "aes_GBps": _get(ph, "rng_fill_1GiB", "GBps"),
+        "e2e_value_without_reading_U_back": _get(e2e, "without_reading_U_back", "value"),
+        "details": full.get("details"),
+    }
+    out.update({k2: v2 for k2, v2 in scalars.items() if v2 is not None})
+    return _r(out)
+
+
+def dumps_compact(full: dict) -> str:
+    line = json.dumps(compact_line(full), separators=(",", ":"))
+    if len(line) >= MAX_LINE_BYTES:                        # never print a line the driver would cut: drop the extras
+        small = compact_line({k2: v2 for k2, v2 in full.items() if k2 in COMPACT_KEYS})
+        line = json.dumps(small, separators=(",", ":"))
+    assert len(line) < MAX_LINE_BYTES, len(line)
+    return line
+
+
+def print_details(full: dict) -> str:
+    """Everything measured, away from the last line: one stdout line per phase / block (each short enough to read),
+    and the whole object as a file.  Returns the file's path relative to the repository."""
+    blocks = [("kernels", full.get("kernels")), ("sustained", full.get("sustained")), ("peaks", full.get("peaks")),
+              ("roofline", full.get("roofline")), ("e2e", full.get("e2e")), ("clocks", full.get("clocks"))]
+    blocks += [(f"cpu_baseline.{name}", cfg) for name, cfg in (_get(full, "cpu_baseline", "configs") or {}).items()]
+    for name, res in (full.get("phases") or {}).items():
+        if isinstance(res, dict) and name in ("paper_table1_all_rows", "single_kem_B1"):
+            blocks += [(f"phase.{name}.{sub}", val) for sub, val in res.items()]
+        else:
+            blocks.append((f"phase.{name}", res))
+    for name, res in blocks:
+        if res is not None:
+            print(json.dumps({"detail": name, "result": _r(res)}, separators=(",", ":")), flush=True)
+    rel = Path("gpurun_out") / "bench_details.json"
+    try:
+        (ROOT / rel).parent.mkdir(exist_ok=True)
+        (ROOT / rel).write_text(json.dumps(full, indent=1))
+    except OSError:
+        return "stdout lines above (file not writable)"
+    return str(rel)
 
 
 def run_dry(args):
@@ -1105,15 +1244,26 @@ def run_ours(args):
 
     # ---- LAST on the device (everything above is burst-regime; these loops leave the chip power-capped and warm for
     # seconds): the same step for >= 3 s with its clock / power record, then the library's int8 GEMM burst + sustained
+    probe = int8_pipe_probe(ctx, 0.0)                       # burst figures, before the long loops below
     if not args.quick:
         lib_burst = library_int8_gemm(0.0)
         side_sustained = sustained_block(job, 3.0, ms_total / args.steps, peaks)
         side_sustained["pipelined_two_streams"] = pipelined_phase(pipelined_job, 10, sustained_s=3.0).get("step_sustained")
         lib = library_int8_gemm(3.0)
         lib["burst_TOPs"] = lib_burst.get("burst_TOPs")           # the burst figure taken BEFORE the long loops
+        probe_sus = int8_pipe_probe(ctx, 3.0)
+        for kind in ("u8_x_bits", "u8_x_s8"):
+            probe[kind].update({k2: v2 for k2, v2 in probe_sus[kind].items() if k2.startswith(("sustained", "whole_loop"))})
+        if side_sustained.get("gemm") and probe["u8_x_bits"].get("sustained_TOPs"):
+            side_sustained["gemm"]["measured_int8_pipe_sustained_TOPs"] = probe["u8_x_bits"]["sustained_TOPs"]
+            side_sustained["gemm"]["frac_of_measured_int8_pipe"] = (side_sustained["gemm"]["int8_TOPs"] /
+                                                                    probe["u8_x_bits"]["sustained_TOPs"])
     else:
         side_sustained, lib = None, library_int8_gemm(0.0)
     if roofline is not None:
+        roofline["int8_pipe_probe"] = probe
+        roofline["measured_int8_pipe_TOPs"] = probe["u8_x_bits"]["burst_TOPs"]
+        roofline["frac_of_measured_int8_pipe"] = roofline["achieved"] / probe["u8_x_bits"]["burst_TOPs"]
         roofline["library_int8_gemm"] = lib
         if lib.get("burst_TOPs"):
             roofline["frac_of_library_int8_gemm_burst"] = roofline["achieved"] / lib["burst_TOPs"]
@@ -1127,8 +1277,7 @@ def run_ours(args):
         "ms_per_step": ms_step, "ms_per_step_stats_rank0": stats_ms(per_step),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u16 mod q (u8 x u8 -> s32 tensor, u32/u64 integer)", "data": "synthetic",
-        "config": {"workload": "C4: n=8192 m=16384 q=65536 k=256 eta=4, 32 instances per GPU per step sharing one "
-                               "stored A (256 MiB); step = sample s,e,R,mu + keygen + encaps + decaps",
+        "config": {"workload": WORKLOAD,
                    "instances_per_step_per_gpu": Bt, "parallelism": f"instances x{world} (no collective)",
                    "l2": "inputs larger than L2 (A 256 MiB read twice + U 128 MiB written and read per step); no flush",
                    "regime": "burst (K steps back to back, tens of ms; see `sustained` for the power-capped regime)",
@@ -1155,7 +1304,8 @@ def run_ours(args):
                   "int8_tops_burst_est": int8_peak_burst, "source": peaks["source"],
                   "note": "int8 estimates = 2 x the measured bf16 figures (nominal ratio 4.5 : 2.25)"},
     }
-    print(json.dumps(line), flush=True)
+    line["details"] = print_details(line)
+    print(dumps_compact(line), flush=True)                 # LAST line of stdout: the one the driver parses
     if world > 1:
         dist.destroy_process_group()
 

@@ -39,7 +39,7 @@ EXPORTS = [
     "lwe_profile_read", "lwe_profile_reset",
     "lwe_sample_uniform_u32", "lwe_sample_cbd_s8", "lwe_wide_load_matrix", "lwe_wide_load_matrix_seeded", "lwe_wide_keygen",
     "lwe_wide_encaps", "lwe_wide_decaps",
-    "lwe_decaps_static",
+    "lwe_decaps_static", "lwe_probe_int8_pipe",
 ]
 STATIC_MAX_COLS, STATIC_MAX_BATCH = 16384, 64                # LWE_STATIC_MAX_COLS / _BATCH of include/lwe.h
 
@@ -99,6 +99,7 @@ def load_library() -> C.CDLL:
     lib.lwe_wide_keygen.argtypes = [vp, vp, vp, vp, u32, vp]
     lib.lwe_wide_encaps.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, u32, vp]
     lib.lwe_wide_decaps.argtypes = [vp, vp, vp, vp, vp, u32, vp]
+    lib.lwe_probe_int8_pipe.argtypes = [vp, u32, C.c_int, C.POINTER(u64), vp]
     lib.lwe_decaps_static.argtypes = [u32, u32, u32, vp, vp, vp, vp, u32, vp]
     _lib = lib
     return lib
@@ -171,6 +172,13 @@ class Context:
 
     def set_option(self, option: int, value: int):
         self._check(self._lib.lwe_set_option(self._h, option, value), "lwe_set_option")
+
+    def probe_int8_pipe(self, iters: int, signed_dense_b: bool = False, stream=None) -> int:
+        """one launch of the tensor-pipe probe; returns the int8 operations it performs (time it with events)"""
+        ops = C.c_uint64(0)
+        self._check(self._lib.lwe_probe_int8_pipe(self._h, iters, int(signed_dense_b), C.byref(ops), _stream(stream)),
+                    "lwe_probe_int8_pipe")
+        return ops.value
 
     def profile_reset(self):
         self._check(self._lib.lwe_profile_reset(self._h), "lwe_profile_reset")

@@ -297,6 +297,8 @@ cudaError_t launch_wide_decaps(Ctx *c, const uint32_t *d_U, const uint32_t *d_v,
                                uint32_t batch, cudaStream_t st);
 cudaError_t launch_fo_verdict(Ctx *c, const uint16_t *d_v, const uint16_t *d_vprime, const uint32_t *d_flags,
                               uint8_t *d_ok, uint32_t batch, cudaStream_t st);
+// measurement hook (probe_int8.cu): back-to-back tcgen05.mma kind::i8 on shared-memory-resident operands
+cudaError_t launch_probe_int8(Ctx *c, uint32_t iters, int signed_dense_b, uint64_t *ops, cudaStream_t st);
 cudaError_t launch_decaps(Ctx *c, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
                           uint8_t *d_out, uint32_t batch, cudaStream_t st);
 
