@@ -204,6 +204,7 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
         // panels made the 32-instance encaps at C4 1.80 ms, of which only 0.36 ms is the generator and 1.0 ms the GEMM
         size_t rows = ((size_t)256 << 20) / (2 * n) / 128 * 128;
         if (rows < 128) rows = 128;
+        if (rows > 65536) rows = 65536;          // one tensor-core pass holds at most 65536 rows (32-bit byte-plane sums)
         if (rows > m) rows = m;
         c->panel_rows = c->panel_rows_alloc = (uint32_t)rows;
         ok(dev_alloc(&c->d_Apanel, rows * n));
@@ -329,6 +330,16 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
         return LWE_OK;
     }
     return LWE_ERR_PARAM;
+}
+
+int lwe_probe_int8_pipe(lwe_ctx *ctx, uint32_t iters, int signed_dense_b, uint64_t *h_ops, void *stream)
+{
+    CHECK_CTX(ctx);
+    if (iters == 0 || iters > (1u << 24) || (signed_dense_b != 0 && signed_dense_b != 1)) return LWE_ERR_PARAM;
+    Ctx *c = &ctx->c;
+    DeviceGuard guard(c->device);
+    LAUNCH(c, launch_probe_int8(c, iters, signed_dense_b, h_ops, (cudaStream_t)stream));
+    return LWE_OK;
 }
 
 int lwe_profile_reset(lwe_ctx *ctx)
@@ -488,7 +499,9 @@ static int encaps_core(Ctx *c, const uint16_t *d_A, uint64_t seed_A, const uint1
     // accumulated mod q).  d_A == NULL: A is regenerated from seed_A one row panel at a
     // time into the context's panel buffer (rows of A are contiguous ranges of the counter-indexed
     // stream) and the contraction is accumulated over the panels; A is never held in full.
-    const uint32_t m = c->p.m, step = d_A ? (m < 65536u ? m : 65536u) : c->panel_rows;
+    // Either way a pass is at most 65536 rows: the tcgen05 epilogue recombines lo + (hi << 8) in 32 bits, and a byte-plane
+    // sum over more rows would wrap for a modulus that is not a power of two.
+    const uint32_t m = c->p.m, cap = d_A ? m : c->panel_rows, step = cap < 65536u ? cap : 65536u;
     const AesKey keyA = d_A ? AesKey() : seed_key_host(seed_A);
     for (uint32_t row0 = 0; row0 < m; row0 += step) {
         const uint32_t rows = (m - row0 < step) ? (m - row0) : step;

@@ -212,6 +212,30 @@ def test_encaps_more_than_65536_rows_worst_case(H, path):
         assert np.array_equal(v[1], (ones * (q - 1) + q // 2) % q)
 
 
+@pytest.mark.parametrize("path", **ENCAPS_PATHS)
+def test_encaps_regenerated_A_more_than_65536_rows(H, path):
+    """d_A = NULL with m = 131072 and a small n: the row panel the context could hold (256 MiB / 2n) is far more than
+    65536 rows, but one tensor-core pass may not be (a byte-plane sum over more rows, recombined as lo + (hi << 8),
+    leaves 32 bits for a prime modulus).  R = all ones, so every U[j][c] is the column sum of the regenerated A: with a
+    uniform A the recombined value of a 131072-row pass is ~2^32 and wraps in about half the columns.  Expected values
+    from the ORACLE's own draw of A."""
+    m, n, k, q, seed = 131072, 64, 256, 65521, 77
+    A = O.sample_uniform(0, m * n, seed, O.TAG_A, 0, q).reshape(m, n)
+    b = W.random_u16((1, m), q, 22)
+    Rbits = np.full((1, m * k // 8), 0xFF, np.uint8)
+    mubits = np.zeros((1, k // 8), np.uint8)
+    with B().Context(n, m, k, q, 4, 1) as c:
+        set_encaps_path(c, path)
+        c.set_option(B().OPT_REGEN_PATH, 1)              # row panels through the GEMM (the fused kernel is bounded by m <= 65536 itself)
+        U, v = H.dev_empty_u16(1, n, k), H.dev_empty_u16(1, k)
+        U.fill_(-1)
+        c.encaps(None, seed, H.dev(b), H.dev(Rbits), H.dev(mubits), U, v, 1)
+        U, v = H.host_u16(U), H.host_u16(v)
+    colsum = (A.astype(np.uint64).sum(axis=0) % q).astype(np.uint16)
+    assert np.array_equal(U[0], np.broadcast_to(colsum[:, None], (n, k)))
+    assert np.all(v[0] == int(b[0].astype(np.uint64).sum() % q))
+
+
 @pytest.mark.parametrize("path", [3, 2], ids=["tcgen05_pair", "tcgen05"])
 def test_encaps_one_hot_R_picks_a_row_of_A(H, path):
     m, n, k, q = 256, 128, 256, 65521
