@@ -579,11 +579,23 @@ static cudaError_t launch_pair(Ctx *c, const uint16_t *d_A, void *d_U, uint32_t 
     const uint32_t tiles = ((2 * p.n + kPairM - 1) / kPairM) * ((ncols + kTileN - 1) / kTileN);
     uint32_t pairs = (uint32_t)c->sm_count / 2;
     if (pairs > tiles) pairs = tiles;
-    // tile order: with the expanded operand, groups of 8 n-tiles keep the group's R panels in L2 while A is
-    // re-streamed once per group; with the bit operand R is 16x smaller and stays in L2 by itself, so all n-tiles of
-    // an A strip run together and A crosses HBM once (ncu at C4: 1.14 GB -> 0.30 GB read per launch)
+    // tile order: groups of gw n-tiles run over every A strip before the next group starts, so A is re-streamed once per
+    // group while the group's slice of the B operand stays in L2.  Bit operand: R is 16x smaller and stays in L2 by
+    // itself, so all n-tiles of an A strip run together and A crosses HBM once (ncu at C4: 1.14 GB -> 0.30 GB read per
+    // launch).  Byte operand (expanded u8, or the int8 R read in place): as many n-tiles as keep the group's slice at or
+    // below 32 MiB, at least 8.  Measured on the signed-R GEMM, 32 instances (gw = 8 / 16 / 32): n = 8192, q = 65537
+    // 0.644 / 0.630 / 0.673 ms (the whole 64 MB R beside 134 MB of A, 64 MB of E1 and 268 MB of U does not stay
+    // resident), n = 4096 0.1587 / 0.1577 / 0.1559 ms.  The gain is small because that kernel is paced by the power cap,
+    // not by HBM: the dense signed operand holds the chip at ~1.6 GHz (bench.py --phase int8_pipe_peak: u8 x s8
+    // sustains 3.79 POP/s where u8 x {0,1} sustains 4.61).
     const uint32_t n_tiles_all = (ncols + kTileN - 1) / kTileN;
-    const uint32_t gw = kBitsB ? n_tiles_all : 8u;
+    uint32_t gw = n_tiles_all;
+    if (!kBitsB) {
+        const uint64_t slice = (uint64_t)rows * kTileN;                    // bytes of the B operand under one n-tile
+        gw = (uint32_t)(((uint64_t)32 << 20) / (slice ? slice : 1));
+        if (gw < 8u) gw = 8u;
+        if (gw > n_tiles_all) gw = n_tiles_all;
+    }
     ProfScope prof(c, LWE_K_ENCAPS_TC, st);
     // signed byte-plane sums of the N2 variant: |plane| <= 255 * 128 * rows; bias = the next multiple of q, so that
     // plane + bias is the same residue in [0, 2 bias] < 2^32 (rows <= 65536).  e1 (and, wide, e1 - delta * corr with
