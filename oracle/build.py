@@ -32,7 +32,41 @@ def needs_build() -> bool:
     return any(p.stat().st_mtime > t for p in SRC)
 
 
+SAN_LIB = HERE / "liblwe_oracle_san.so"
+SAN_FLAGS = ["-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer", "-g", "-O1"]
+
+
+def build_sanitized(force: bool = False) -> Path:
+    """The same source under AddressSanitizer + UndefinedBehaviorSanitizer (the only sanitizer that can
+    run on this pool guards the checker every parity claim rests on).  No OpenMP (its runtime's own allocations
+    only add noise); -fno-sanitize-recover makes any undefined behaviour abort instead of printing and going on.
+    A process that loads this library must start with libasan preloaded -- tests/test_oracle_sanitized.py runs its
+    checks in such a child process."""
+    if not force and SAN_LIB.exists() and all(p.stat().st_mtime <= SAN_LIB.stat().st_mtime for p in SRC):
+        return SAN_LIB
+    errors = []
+    for cc in _compilers():
+        cmd = [cc, *SAN_FLAGS, "-std=c11", "-Wall", "-Wextra", "-fPIC", "-shared", "-o", str(SAN_LIB), str(SRC[0]), "-lm"]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode == 0:
+            return SAN_LIB
+        errors.append(f"{' '.join(cmd)}\n{r.stderr}")
+    raise RuntimeError("could not build the sanitized oracle:\n" + "\n".join(errors))
+
+
+def asan_runtime() -> str:
+    """path of libasan.so for LD_PRELOAD (the sanitized library is loaded into an uninstrumented python)"""
+    for cc in _compilers():
+        r = subprocess.run([cc, "-print-file-name=libasan.so"], capture_output=True, text=True)
+        path = r.stdout.strip()
+        if r.returncode == 0 and os.path.isabs(path) and os.path.exists(path):
+            return os.path.realpath(path)
+    raise RuntimeError("libasan.so not found")
+
+
 def build(force: bool = False) -> Path:
+    if os.environ.get("LWE_ORACLE_SANITIZE") == "1":          # set by the sanitizer test's child process only
+        return build_sanitized(force)
     if not force and not needs_build():
         return LIB
     errors = []
@@ -48,4 +82,5 @@ def build(force: bool = False) -> Path:
 
 
 if __name__ == "__main__":
-    print(build(force=True))
+    import sys
+    print(build_sanitized(force=True) if "--sanitize" in sys.argv else build(force=True))
