@@ -213,10 +213,18 @@ def test_wide_encaps_matches_oracle(path, n, k, q, batch, big):
 
 @pytest.mark.parametrize("path", [0, 1], ids=["tcgen05_pair", "simt"])
 def test_wide_encaps_extreme_accumulators(path):
-    """|R| = 127, A's low half = 65535, m = 65536 (the path's limit): both signed byte-plane accumulators at
-    +/- 255*127*65536, every column with exceptions, the two- and three-reduction recombinations at their bounds"""
+    """|R| = 127, A's low half = 65535, m = the most rows ONE pass of the path takes for that modulus: both signed byte-plane
+    accumulators at +/- 255*127*m, every column with exceptions, the two- and three-reduction recombinations at their
+    bounds.  m = 65536 is the pass limit of the tensor path (F4 and 65539 run there).  For q = 66560, the largest
+    modulus of a wide context, lwe_create itself caps m: the exception lists hold 4x the expected number of elements
+    >= 2^16 per column of a uniform A (+16, rounded up to a power of two) and at most 1024 slots (lwe.h, lwe_params),
+    i.e. 4 * m * 1024 / 66560 + 16 <= 1024, m <= 16384 -- so 16384 IS that modulus's limit, and the test checks that a
+    larger m is refused rather than run.  Expected values: the closed form and the oracle."""
     n_small, k, batch = 64, 256, 1
-    for q, m in ((F4, 65536), (65539, 65536), (66560, 8192)):
+    with pytest.raises(B().LweError) as ei:                  # the cap stated above is enforced, not assumed
+        B().Context(n_small, 65536, k, 66560, 3, batch)
+    assert ei.value.code == -5
+    for q, m in ((F4, 65536), (65539, 65536), (66560, 16384)):
         for sign in (1, -1):
             A = np.full((m, n_small), 65535, np.uint32)
             for x in range(5):                               # five elements >= 2^16 in every column, one per row
@@ -235,6 +243,8 @@ def test_wide_encaps_extreme_accumulators(path):
             e1 = -128 if sign < 0 else 127
             assert np.all(gU == (((m - 5) * 65535 + 5 * (q - 1)) * 127 * sign + e1) % q), (q, sign)
             assert np.all(gv == (m * (q - 1) * 127 * sign + 3 * sign + q // 2) % q), (q, sign)
+            Uo, vo = O.encaps_pv_w(A, t[0], R[0], E1[0], e2[0], mubits[0], q)
+            assert np.array_equal(gU[0], Uo) and np.array_equal(gv[0], vo), (q, sign, "oracle")
 
 
 @pytest.mark.parametrize("path", [0, 1], ids=["tcgen05_pair", "simt"])
