@@ -8,6 +8,15 @@
 
 using namespace lwe;
 
+#include <nvtx3/nvToolsExt.h>
+
+// NVTX range around every entry point (the paper's own tooling: Nsight Systems timelines with NVTX).
+// Header-only NVTX3: without a tool attached a push / pop is one load and a branch.
+struct NvtxScope {
+    explicit NvtxScope(const char *name) { nvtxRangePushA(name); }
+    ~NvtxScope() { nvtxRangePop(); }
+};
+
 struct lwe_ctx {
     Ctx c;
 };
@@ -32,10 +41,22 @@ cudaError_t kernel_prepare(Ctx *c, const void *fn, size_t smem, int threads, int
         // kernels that need a large dynamic shared memory are launched with the SM's maximal shared-memory carve-out:
         // the driver's default sized the generator kernels (2 x 64 KB per SM wanted) for ONE resident CTA (ncu:
         // launch__occupancy_limit_shared_mem = 1)
+        // (decided by the first launch's request: every kernel here asks for the same order of dynamic shared memory on
+        // all its launches; the small-smem streaming kernels keep the default carve-out and their L1)
         if (smem > 48 * 1024)
             cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
         if ((int)smem > limit && (int)smem > 48 * 1024) return cudaErrorInvalidValue;
-        if (c->n_kcfg >= kMaxKernelCfg) return occ ? cudaErrorInvalidValue : cudaSuccess;   // table full: still configured
+        if (c->n_kcfg >= kMaxKernelCfg) {
+            // table full (more distinct kernels than kMaxKernelCfg: raise it): the function is configured, only the
+            // cache is missing -- answer an occupancy question with an uncached query instead of failing
+            if (occ) {
+                int q = 0;
+                err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&q, fn, threads, smem);
+                if (err != cudaSuccess) return err;
+                *occ = q < 1 ? 1 : q;
+            }
+            return cudaSuccess;
+        }
         k = &c->kcfg[c->n_kcfg++];
         k->fn = fn;
         k->occ_threads = 0;
@@ -162,6 +183,7 @@ const char *lwe_strerror(int code)
 
 int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
 {
+    NvtxScope nvtx_("lwe_create");
     if (!out || !p) return LWE_ERR_NULLPTR;
     *out = nullptr;
     if (p->n == 0 || p->m == 0 || p->k == 0 || p->n % 8 || p->m % 8 || p->k % 8) return LWE_ERR_PARAM;
@@ -266,6 +288,7 @@ int lwe_create(lwe_ctx **out, const lwe_params *p, int device)
 
 void lwe_destroy(lwe_ctx *ctx)
 {
+    NvtxScope nvtx_("lwe_destroy");
     if (!ctx) return;
     DeviceGuard guard(ctx->c.device);
     cudaDeviceSynchronize();
@@ -334,6 +357,7 @@ int lwe_set_option(lwe_ctx *ctx, int option, int64_t value)
 
 int lwe_probe_int8_pipe(lwe_ctx *ctx, uint32_t iters, int signed_dense_b, uint64_t *h_ops, void *stream)
 {
+    NvtxScope nvtx_("lwe_probe_int8_pipe");
     CHECK_CTX(ctx);
     if (iters == 0 || iters > (1u << 24) || (signed_dense_b != 0 && signed_dense_b != 1)) return LWE_ERR_PARAM;
     Ctx *c = &ctx->c;
@@ -373,6 +397,7 @@ int lwe_profile_read(lwe_ctx *ctx, int kernel_id, double *h_total_ms, uint64_t *
 int lwe_rng_fill(lwe_ctx *ctx, void *d_out, size_t nbytes, const uint8_t key[16], const uint8_t iv[16],
                  uint64_t byte_offset, void *stream)
 {
+    NvtxScope nvtx_("lwe_rng_fill");
     CHECK_CTX(ctx);
     REQUIRE_PTR(key); REQUIRE_PTR(iv);
     if (nbytes == 0) return LWE_OK;
@@ -402,6 +427,7 @@ static int sampler_args(lwe_ctx *ctx, const void *d_out, uint64_t first, uint64_
 int lwe_sample_uniform(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count, uint64_t seed,
                        uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream)
 {
+    NvtxScope nvtx_("lwe_sample_uniform");
     int rc = sampler_args(ctx, d_out, first, count, tag, inst0, n_inst);
     if (rc != LWE_OK) return rc;
     REQUIRE_NARROW(ctx);
@@ -415,6 +441,7 @@ int lwe_sample_uniform(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t c
 int lwe_sample_cbd(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count, uint64_t seed,
                    uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream)
 {
+    NvtxScope nvtx_("lwe_sample_cbd");
     int rc = sampler_args(ctx, d_out, first, count, tag, inst0, n_inst);
     if (rc != LWE_OK) return rc;
     REQUIRE_NARROW(ctx);
@@ -428,6 +455,7 @@ int lwe_sample_cbd(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count
 int lwe_sample_bits(lwe_ctx *ctx, uint8_t *d_out, uint64_t first_bit, uint64_t nbits, uint64_t seed,
                     uint32_t tag, uint32_t inst0, uint32_t n_inst, void *stream)
 {
+    NvtxScope nvtx_("lwe_sample_bits");
     int rc = sampler_args(ctx, d_out, first_bit, nbits, tag, inst0, n_inst);
     if (rc != LWE_OK || nbits == 0 || n_inst == 0) return rc;
     Ctx *c = &ctx->c;
@@ -439,6 +467,7 @@ int lwe_sample_bits(lwe_ctx *ctx, uint8_t *d_out, uint64_t first_bit, uint64_t n
 int lwe_sample_kem(lwe_ctx *ctx, uint16_t *d_s, uint16_t *d_e, uint8_t *d_Rbits, uint8_t *d_mubits, uint64_t seed,
                    uint32_t inst0, uint32_t n_inst, void *stream)
 {
+    NvtxScope nvtx_("lwe_sample_kem");
     CHECK_CTX(ctx);
     REQUIRE_NARROW(ctx);
     if ((uint64_t)inst0 + n_inst > (1ull << 32)) return LWE_ERR_PARAM;
@@ -454,6 +483,7 @@ int lwe_sample_kem(lwe_ctx *ctx, uint16_t *d_s, uint16_t *d_e, uint8_t *d_Rbits,
 int lwe_keygen(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_t *d_s, const uint16_t *d_e,
                uint16_t *d_b, uint32_t batch, void *stream)
 {
+    NvtxScope nvtx_("lwe_keygen");
     CHECK_CTX(ctx);
     REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
@@ -526,6 +556,7 @@ static int encaps_core(Ctx *c, const uint16_t *d_A, uint64_t seed_A, const uint1
 int lwe_encaps(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint16_t *d_b, const uint8_t *d_Rbits,
                const uint8_t *d_mubits, uint16_t *d_U, uint16_t *d_v, uint32_t batch, void *stream)
 {
+    NvtxScope nvtx_("lwe_encaps");
     CHECK_CTX(ctx);
     REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
@@ -541,6 +572,7 @@ int lwe_decaps_fo(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_b, const 
                   const uint16_t *d_s, const uint8_t *d_Rbits, uint8_t *d_mubits_out, uint8_t *d_ok, uint32_t batch,
                   void *stream)
 {
+    NvtxScope nvtx_("lwe_decaps_fo");
     CHECK_CTX(ctx);
     REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
@@ -568,6 +600,7 @@ int lwe_decaps_fo(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_b, const 
 int lwe_decaps(lwe_ctx *ctx, const uint16_t *d_U, const uint16_t *d_v, const uint16_t *d_s,
                uint8_t *d_mubits_out, uint32_t batch, void *stream)
 {
+    NvtxScope nvtx_("lwe_decaps");
     CHECK_CTX(ctx);
     REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
@@ -591,6 +624,7 @@ static int gauss_args(lwe_ctx *ctx, const void *d_out, uint64_t first, uint64_t 
 int lwe_sample_gauss_s8(lwe_ctx *ctx, int8_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
                         uint32_t inst0, uint32_t n_inst, double sigma, void *stream)
 {
+    NvtxScope nvtx_("lwe_sample_gauss_s8");
     int rc = gauss_args(ctx, d_out, first, count, tag, inst0, n_inst, sigma);
     if (rc != LWE_OK || count == 0 || n_inst == 0) return rc;
     Ctx *c = &ctx->c;
@@ -603,6 +637,7 @@ int lwe_sample_gauss_s8(lwe_ctx *ctx, int8_t *d_out, uint64_t first, uint64_t co
 int lwe_sample_gauss_u16(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
                          uint32_t inst0, uint32_t n_inst, double sigma, void *stream)
 {
+    NvtxScope nvtx_("lwe_sample_gauss_u16");
     int rc = gauss_args(ctx, d_out, first, count, tag, inst0, n_inst, sigma);
     if (rc != LWE_OK) return rc;
     REQUIRE_NARROW(ctx);
@@ -617,6 +652,7 @@ int lwe_sample_gauss_u16(lwe_ctx *ctx, uint16_t *d_out, uint64_t first, uint64_t
 int lwe_sample_cuniform_s8(lwe_ctx *ctx, int8_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
                            uint32_t inst0, uint32_t n_inst, uint32_t bound, void *stream)
 {
+    NvtxScope nvtx_("lwe_sample_cuniform_s8");
     CHECK_CTX(ctx);
     if (tag == 0 || tag > 255 || bound < 1 || bound > 127) return LWE_ERR_PARAM;
     if ((uint64_t)inst0 + n_inst > (1ull << 32)) return LWE_ERR_PARAM;
@@ -632,6 +668,7 @@ int lwe_sample_cuniform_s8(lwe_ctx *ctx, int8_t *d_out, uint64_t first, uint64_t
 int lwe_sample_pke(lwe_ctx *ctx, void *d_s, void *d_e, int8_t *d_R, int8_t *d_E1, int8_t *d_e2, uint8_t *d_mubits,
                    uint64_t seed, uint32_t inst0, uint32_t n_inst, double sigma, uint32_t e2_bound, void *stream)
 {
+    NvtxScope nvtx_("lwe_sample_pke");
     CHECK_CTX(ctx);
     if (!(sigma >= 0.5 && sigma <= 2.8) || e2_bound < 1 || e2_bound > 127) return LWE_ERR_PARAM;
     if ((uint64_t)inst0 + n_inst > (1ull << 32)) return LWE_ERR_PARAM;
@@ -649,6 +686,7 @@ int lwe_sample_pke(lwe_ctx *ctx, void *d_s, void *d_e, int8_t *d_R, int8_t *d_E1
 int lwe_encaps_pv(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_t, const int8_t *d_R, const int8_t *d_E1,
                   const int8_t *d_e2, const uint8_t *d_mubits, uint16_t *d_U, uint16_t *d_v, uint32_t batch, void *stream)
 {
+    NvtxScope nvtx_("lwe_encaps_pv");
     CHECK_CTX(ctx);
     REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
@@ -675,6 +713,7 @@ int lwe_encaps_pv(lwe_ctx *ctx, const uint16_t *d_A, const uint16_t *d_t, const 
 int lwe_sample_uniform_u32(lwe_ctx *ctx, uint32_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
                            uint32_t inst0, uint32_t n_inst, void *stream)
 {
+    NvtxScope nvtx_("lwe_sample_uniform_u32");
     CHECK_CTX(ctx);
     REQUIRE_WIDE(ctx);
     if (tag == 0 || tag > 255) return LWE_ERR_PARAM;
@@ -691,6 +730,7 @@ int lwe_sample_uniform_u32(lwe_ctx *ctx, uint32_t *d_out, uint64_t first, uint64
 int lwe_sample_cbd_s8(lwe_ctx *ctx, int8_t *d_out, uint64_t first, uint64_t count, uint64_t seed, uint32_t tag,
                       uint32_t inst0, uint32_t n_inst, void *stream)
 {
+    NvtxScope nvtx_("lwe_sample_cbd_s8");
     int rc = sampler_args(ctx, d_out, first, count, tag, inst0, n_inst);
     if (rc != LWE_OK || count == 0 || n_inst == 0) return rc;
     Ctx *c = &ctx->c;
@@ -720,6 +760,7 @@ static int wide_begin_load(Ctx *c, cudaStream_t st)
 
 int lwe_wide_load_matrix(lwe_ctx *ctx, const uint32_t *d_A, void *stream)
 {
+    NvtxScope nvtx_("lwe_wide_load_matrix");
     CHECK_CTX(ctx);
     REQUIRE_WIDE(ctx);
     REQUIRE_PTR(d_A); REQUIRE_ALIGNED(d_A);
@@ -734,6 +775,7 @@ int lwe_wide_load_matrix(lwe_ctx *ctx, const uint32_t *d_A, void *stream)
 
 int lwe_wide_load_matrix_seeded(lwe_ctx *ctx, uint64_t seed_A, void *stream)
 {
+    NvtxScope nvtx_("lwe_wide_load_matrix_seeded");
     CHECK_CTX(ctx);
     REQUIRE_WIDE(ctx);
     Ctx *c = &ctx->c;
@@ -756,6 +798,7 @@ int lwe_wide_load_matrix_seeded(lwe_ctx *ctx, uint64_t seed_A, void *stream)
 
 int lwe_wide_keygen(lwe_ctx *ctx, const int8_t *d_s, const int8_t *d_e, uint32_t *d_t, uint32_t batch, void *stream)
 {
+    NvtxScope nvtx_("lwe_wide_keygen");
     CHECK_CTX(ctx);
     REQUIRE_WIDE(ctx);
     Ctx *c = &ctx->c;
@@ -774,6 +817,7 @@ int lwe_wide_keygen(lwe_ctx *ctx, const int8_t *d_s, const int8_t *d_e, uint32_t
 int lwe_wide_encaps(lwe_ctx *ctx, const uint32_t *d_t, const int8_t *d_R, const int8_t *d_E1, const int8_t *d_e2,
                     const uint8_t *d_mubits, uint32_t *d_U, uint32_t *d_v, uint32_t batch, void *stream)
 {
+    NvtxScope nvtx_("lwe_wide_encaps");
     CHECK_CTX(ctx);
     REQUIRE_WIDE(ctx);
     Ctx *c = &ctx->c;
@@ -797,6 +841,7 @@ int lwe_wide_encaps(lwe_ctx *ctx, const uint32_t *d_t, const int8_t *d_R, const 
 int lwe_wide_decaps(lwe_ctx *ctx, const uint32_t *d_U, const uint32_t *d_v, const int8_t *d_s, uint8_t *d_mubits_out,
                     uint32_t batch, void *stream)
 {
+    NvtxScope nvtx_("lwe_wide_decaps");
     CHECK_CTX(ctx);
     REQUIRE_WIDE(ctx);
     Ctx *c = &ctx->c;
@@ -812,6 +857,7 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint1
                  const uint8_t *h_Rbits, const uint8_t *h_mubits, uint16_t *h_b, uint16_t *h_U, uint16_t *h_v,
                  uint8_t *h_mubits_out, uint32_t batch, void *stream)
 {
+    NvtxScope nvtx_("lwe_kem_host");
     CHECK_CTX(ctx);
     REQUIRE_NARROW(ctx);
     Ctx *c = &ctx->c;
@@ -854,51 +900,59 @@ int lwe_kem_host(lwe_ctx *ctx, const uint16_t *d_A, uint64_t seed_A, const uint1
             c_t0[nchunks] = t0; c_g[nchunks] = (batch - t0 < per) ? (batch - t0) : per; nchunks++;
         }
     }
-    LWE_CUDA_TRY(c, cudaEventRecord(c->ev_entry, st));
-    LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_in, c->ev_entry, 0));      // staging buffers are free again
-    LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_out, c->ev_entry, 0));
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hs, h_s, (size_t)batch * n * 2, cudaMemcpyHostToDevice, c->s_in));
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_he, h_e, (size_t)batch * m * 2, cudaMemcpyHostToDevice, c->s_in));
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hmu, h_mubits, (size_t)batch * k / 8, cudaMemcpyHostToDevice, c->s_in));
-    LWE_CUDA_TRY(c, cudaEventRecord(c->ev_se, c->s_in));
+    // Every failure from here on drains the three streams before returning: no copy to or from the caller's host
+    // buffers may still be in flight when the call hands them back (lwe.h).
+    auto drain = [&]() { cudaStreamSynchronize(c->s_in); cudaStreamSynchronize(st); cudaStreamSynchronize(c->s_out); };
+#define KEM_HOST_TRY(expr)                                                                        \
+    do {                                                                                          \
+        cudaError_t _e = (expr);                                                                  \
+        if (_e != cudaSuccess) { c->last_cuda_error = (int)_e; drain(); return LWE_ERR_CUDA; }    \
+    } while (0)
+    KEM_HOST_TRY(cudaEventRecord(c->ev_entry, st));
+    KEM_HOST_TRY(cudaStreamWaitEvent(c->s_in, c->ev_entry, 0));      // staging buffers are free again
+    KEM_HOST_TRY(cudaStreamWaitEvent(c->s_out, c->ev_entry, 0));
+    KEM_HOST_TRY(cudaMemcpyAsync(c->d_hs, h_s, (size_t)batch * n * 2, cudaMemcpyHostToDevice, c->s_in));
+    KEM_HOST_TRY(cudaMemcpyAsync(c->d_he, h_e, (size_t)batch * m * 2, cudaMemcpyHostToDevice, c->s_in));
+    KEM_HOST_TRY(cudaMemcpyAsync(c->d_hmu, h_mubits, (size_t)batch * k / 8, cudaMemcpyHostToDevice, c->s_in));
+    KEM_HOST_TRY(cudaEventRecord(c->ev_se, c->s_in));
     for (uint32_t ci = 0; ci < nchunks; ci++) {
         const size_t t0 = c_t0[ci], g = c_g[ci];
-        LWE_CUDA_TRY(c, cudaMemcpyAsync(c->d_hR + t0 * (m * k / 8), h_Rbits + t0 * (m * k / 8), g * m * k / 8,
+        KEM_HOST_TRY(cudaMemcpyAsync(c->d_hR + t0 * (m * k / 8), h_Rbits + t0 * (m * k / 8), g * m * k / 8,
                                         cudaMemcpyHostToDevice, c->s_in));
-        LWE_CUDA_TRY(c, cudaEventRecord(c->ev_in[ci], c->s_in));
+        KEM_HOST_TRY(cudaEventRecord(c->ev_in[ci], c->s_in));
     }
-    auto drain = [&]() { cudaStreamSynchronize(c->s_in); cudaStreamSynchronize(st); cudaStreamSynchronize(c->s_out); };
-    LWE_CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_se, 0));
+    KEM_HOST_TRY(cudaStreamWaitEvent(st, c->ev_se, 0));
     int rc = lwe_keygen(ctx, d_A, seed_A, c->d_hs, c->d_he, c->d_hb, batch, stream);
     if (rc != LWE_OK) { drain(); return rc; }
-    LWE_CUDA_TRY(c, cudaEventRecord(c->ev_kg, st));
-    LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_out, c->ev_kg, 0));
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_b, c->d_hb, (size_t)batch * m * 2, cudaMemcpyDeviceToHost, c->s_out));
+    KEM_HOST_TRY(cudaEventRecord(c->ev_kg, st));
+    KEM_HOST_TRY(cudaStreamWaitEvent(c->s_out, c->ev_kg, 0));
+    KEM_HOST_TRY(cudaMemcpyAsync(h_b, c->d_hb, (size_t)batch * m * 2, cudaMemcpyDeviceToHost, c->s_out));
     for (uint32_t ci = 0; ci < nchunks; ci++) {
         const size_t t0 = c_t0[ci];
         const uint32_t g = c_g[ci];
-        LWE_CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_in[ci], 0));
+        KEM_HOST_TRY(cudaStreamWaitEvent(st, c->ev_in[ci], 0));
         rc = lwe_encaps(ctx, d_A, seed_A, c->d_hb + t0 * m, c->d_hR + t0 * (m * k / 8), c->d_hmu + t0 * (k / 8),
                         c->d_hU + t0 * n * k, c->d_hv + t0 * k, g, stream);
         if (rc != LWE_OK) { drain(); return rc; }
-        LWE_CUDA_TRY(c, cudaEventRecord(c->ev_done[ci], st));           // the chunk's ciphertext leaves before it is decrypted
-        LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_out, c->ev_done[ci], 0));
+        KEM_HOST_TRY(cudaEventRecord(c->ev_done[ci], st));           // the chunk's ciphertext leaves before it is decrypted
+        KEM_HOST_TRY(cudaStreamWaitEvent(c->s_out, c->ev_done[ci], 0));
         if (h_U)
-            LWE_CUDA_TRY(c, cudaMemcpyAsync(h_U + t0 * n * k, c->d_hU + t0 * n * k, (size_t)g * n * k * 2,
+            KEM_HOST_TRY(cudaMemcpyAsync(h_U + t0 * n * k, c->d_hU + t0 * n * k, (size_t)g * n * k * 2,
                                             cudaMemcpyDeviceToHost, c->s_out));
         rc = lwe_decaps(ctx, c->d_hU + t0 * n * k, c->d_hv + t0 * k, c->d_hs + t0 * n, c->d_hmuout + t0 * (k / 8), g, stream);
         if (rc != LWE_OK) { drain(); return rc; }
     }
     // the small outputs of every chunk in one copy each, behind the last chunk's Decrypt (a copy of a few hundred bytes
     // costs the copy engine as much as a megabyte of U)
-    LWE_CUDA_TRY(c, cudaEventRecord(c->ev_kg, st));
-    LWE_CUDA_TRY(c, cudaStreamWaitEvent(c->s_out, c->ev_kg, 0));
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_v, c->d_hv, (size_t)batch * k * 2, cudaMemcpyDeviceToHost, c->s_out));
-    LWE_CUDA_TRY(c, cudaMemcpyAsync(h_mubits_out, c->d_hmuout, (size_t)batch * k / 8, cudaMemcpyDeviceToHost, c->s_out));
-    LWE_CUDA_TRY(c, cudaEventRecord(c->ev_out, c->s_out));
-    LWE_CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_out, 0));            // the caller's stream sees the whole call
-    LWE_CUDA_TRY(c, cudaStreamSynchronize(st));
+    KEM_HOST_TRY(cudaEventRecord(c->ev_kg, st));
+    KEM_HOST_TRY(cudaStreamWaitEvent(c->s_out, c->ev_kg, 0));
+    KEM_HOST_TRY(cudaMemcpyAsync(h_v, c->d_hv, (size_t)batch * k * 2, cudaMemcpyDeviceToHost, c->s_out));
+    KEM_HOST_TRY(cudaMemcpyAsync(h_mubits_out, c->d_hmuout, (size_t)batch * k / 8, cudaMemcpyDeviceToHost, c->s_out));
+    KEM_HOST_TRY(cudaEventRecord(c->ev_out, c->s_out));
+    KEM_HOST_TRY(cudaStreamWaitEvent(st, c->ev_out, 0));            // the caller's stream sees the whole call
+    KEM_HOST_TRY(cudaStreamSynchronize(st));
     return LWE_OK;
 }
+#undef KEM_HOST_TRY
 
 }  // extern "C"

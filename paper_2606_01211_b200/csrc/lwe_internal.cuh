@@ -189,6 +189,12 @@ inline cudaError_t kernel_prepare(Ctx *c, K fn, size_t smem, int threads = 0, in
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
+// CONTRACT of launch_k: it attaches programmatic stream serialisation, so a kernel launched through it may START
+// before its predecessor in the stream has finished.  Such a kernel MUST call pdl_wait() before its first access to
+// global memory that any other kernel writes (or that it writes and another kernel reads) -- all of them do so right
+// after their prologue -- and should call pdl_trigger() early.  A kernel without pdl_wait() must be launched with plain
+// <<<>>> (full stream order), never moved to launch_k.  tests/test_gpu_stress.py runs the streaming kernels back to
+// back with PDL on and off on reused buffers; the test cannot prove the absence of a race, the rule above does.
 template <class... KArgs, class... Args>
 inline cudaError_t launch_k(Ctx *c, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args)
 {

@@ -98,3 +98,15 @@ def test_decaps_static_checks_its_limits_before_touching_cuda(lib):
     assert f(64, 12, 65536, p, p, p, p, 1, None) == -1
     assert f(64, 256, 65536, None, p, p, p, 1, None) == -3
     assert f(64, 256, 65536, p + 2, p, p, p, 1, None) == -2
+
+
+def test_every_enqueueing_entry_point_opens_an_nvtx_range():
+    """SURVEY section 5 row 1 (the paper profiles with Nsight Systems + NVTX): each lwe_* call that
+    enqueues device work is bracketed by an NVTX range named after it."""
+    src = (ROOT / "paper_2606_01211_b200" / "csrc" / "api.cu").read_text()
+    bodies = re.findall(r"^(?:int|void) (lwe_[a-z0-9_]+)\([^{;]*\)\n\{\n(.*?)^\}", src, flags=re.M | re.S)
+    assert len(bodies) >= 25
+    quiet = {"lwe_last_cuda_error", "lwe_set_option", "lwe_profile_reset", "lwe_profile_read"}
+    for name, body in bodies:
+        if name not in quiet:
+            assert f'NvtxScope nvtx_("{name}");' in body, name
